@@ -1,0 +1,223 @@
+/*
+ * mlmd_ref.c -- FP64 CPU ORACLE for the domain-batched real-time Kohn-Sham step.
+ *
+ * TEST INFRASTRUCTURE ONLY.  This file is the slow, plain, obviously-correct statement of
+ * what the hot path computes.  It shares no code, header, table or constant with the CUDA
+ * library under paper_2509_00966_b200/csrc/ and is never linked into or called from it.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may load it.
+ *
+ * What it computes (citations: PAPER.md line / equation; BASELINE.json north_star; DESIGN.md
+ * reading numbers D1..D26 which restate SURVEY.md section 8(c)):
+ *
+ *   H = 1/2 (-i grad + A)^2 + V_loc + V_NL                     PAPER.md Eq. (3); a.u. (D6)
+ *     = -1/2 D2  - i A.D1  + 1/2 |A|^2  + V_loc(r)  +  dv * B diag(D) B^H       (D5, D10)
+ *   D2, D1: independent 4th-order central differences, periodic in x,y,z       north_star; D3, D26
+ *       c2 = [-1/12, 4/3, -5/2, 4/3, -1/12] / h^2 ,  c1 = [1/12, -2/3, 0, 2/3, -1/12] / h
+ *   V_NL psi = sum_p beta_p D_p <beta_p|psi>,  <a|b> = dv * sum_r conj(a) b     north_star; D4, D10
+ *   one step:  psi <- sum_{m=0..4} (-i dt H)^m / m!  psi,  H frozen at A[n] = A(t_n + dt/2)
+ *                                                              north_star; Eq. (2) L138 midpoint (D1, D2, D7)
+ *   rho(r) = sum_n f_n |psi_n(r)|^2 after every step           north_star; D13
+ *   overlap S = dv * Phi^H Psi                                 PAPER.md L283 (CGEMM(1)), L132
+ *
+ * Layout: psi[dom][ix][iy][iz][n] complex128 (orbital index fastest, D12);
+ * grid point index r = (ix*ny + iy)*nz + iz; beta[dom][r][p] complex128; D[dom][p];
+ * vloc[dom][r]; occ[dom][n]; A[step][a_ndom][3] with a_ndom in {1, ndom} (D8).
+ *
+ * Parallelism: OpenMP over grid points only; reductions are summed in a fixed order so a
+ * run is reproducible for a fixed thread count.  No blocking, fusion or reordering beyond
+ * the definition above.
+ *
+ * Pins (tests/test_oracle_pins.py): plane-wave closed form, dense Kronecker H, dense
+ * eigen-polynomial and expm on 16^3, Hermiticity, exact Taylor-4 norm identity, rank-1
+ * projector closed form, Eq. (5) special case, density sum rule, batch independence,
+ * Horner == term sum, brute force on an anisotropic 6x5x7 grid, 4th-order convergence.
+ * Absolute values printed by the paper: none exist (the paper prints no psi/rho numbers).
+ */
+#include <complex.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double complex zc;
+
+#define MLMD_REF_NO_KINETIC 1 /* oracle-internal switch for pin P6: drop -1/2 D2 - iA.D1 + 1/2|A|^2 */
+#define MLMD_REF_HORNER 2     /* pin P10: evaluate the same polynomial in Horner form */
+
+static const double C2[5] = {-1.0 / 12.0, 4.0 / 3.0, -5.0 / 2.0, 4.0 / 3.0, -1.0 / 12.0};
+static const double C1[5] = {1.0 / 12.0, -2.0 / 3.0, 0.0, 2.0 / 3.0, -1.0 / 12.0};
+
+static int wrap(int i, int n) {
+    i %= n;
+    return i < 0 ? i + n : i;
+}
+
+int mlmd_ref_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* out = H u for ONE domain.  u, out: [ngrid][norb]; beta: [ngrid][nproj]; D: [nproj]. */
+int mlmd_ref_apply_h(int nx, int ny, int nz, double hx, double hy, double hz, int norb, int nproj,
+                     const zc *u, zc *out, const double *vloc, const zc *beta, const double *D,
+                     const double *A, int flags) {
+    const int n3[3] = {nx, ny, nz};
+    const double h[3] = {hx, hy, hz};
+    const long ngrid = (long)nx * ny * nz;
+    const double dv = hx * hy * hz;
+    const double A2 = A[0] * A[0] + A[1] * A[1] + A[2] * A[2];
+    const int kinetic = !(flags & MLMD_REF_NO_KINETIC);
+
+    /* local part: -1/2 D2 u - i A.D1 u + (V_loc + 1/2|A|^2) u */
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int ix = 0; ix < nx; ++ix)
+        for (int iy = 0; iy < ny; ++iy)
+            for (int iz = 0; iz < nz; ++iz) {
+                const int i3[3] = {ix, iy, iz};
+                const long r = ((long)ix * ny + iy) * nz + iz;
+                const double vr = vloc[r] + (kinetic ? 0.5 * A2 : 0.0);
+                for (int n = 0; n < norb; ++n) out[r * norb + n] = vr * u[r * norb + n];
+                if (!kinetic) continue;
+                for (int d = 0; d < 3; ++d)
+                    for (int j = -2; j <= 2; ++j) {
+                        int q3[3] = {i3[0], i3[1], i3[2]};
+                        q3[d] = wrap(i3[d] + j, n3[d]);
+                        const long rr = ((long)q3[0] * ny + q3[1]) * nz + q3[2];
+                        const zc coef = -0.5 * C2[j + 2] / (h[d] * h[d]) - I * A[d] * C1[j + 2] / h[d];
+                        for (int n = 0; n < norb; ++n) out[r * norb + n] += coef * u[rr * norb + n];
+                    }
+            }
+    if (nproj <= 0) return 0;
+
+    /* nonlocal part: C[p][n] = sum_r conj(beta[r][p]) u[r][n]; out[r][n] += sum_p beta[r][p] D_p dv C[p][n] */
+    const int nt = mlmd_ref_num_threads();
+    zc *part = (zc *)calloc((size_t)nt * nproj * norb, sizeof(zc));
+    zc *C = (zc *)calloc((size_t)nproj * norb, sizeof(zc));
+    if (!part || !C) {
+        free(part);
+        free(C);
+        return 5;
+    }
+#pragma omp parallel num_threads(nt)
+    {
+#ifdef _OPENMP
+        zc *mine = part + (size_t)omp_get_thread_num() * nproj * norb;
+#else
+        zc *mine = part;
+#endif
+#pragma omp for schedule(static)
+        for (long r = 0; r < ngrid; ++r)
+            for (int p = 0; p < nproj; ++p) {
+                const zc b = conj(beta[r * nproj + p]);
+                for (int n = 0; n < norb; ++n) mine[(size_t)p * norb + n] += b * u[r * norb + n];
+            }
+    }
+    for (int t = 0; t < nt; ++t) /* fixed order */
+        for (long k = 0; k < (long)nproj * norb; ++k) C[k] += part[(size_t)t * nproj * norb + k];
+#pragma omp parallel for schedule(static)
+    for (long r = 0; r < ngrid; ++r)
+        for (int p = 0; p < nproj; ++p) {
+            const zc bd = beta[r * nproj + p] * (D[p] * dv);
+            for (int n = 0; n < norb; ++n) out[r * norb + n] += bd * C[(size_t)p * norb + n];
+        }
+    free(part);
+    free(C);
+    return 0;
+}
+
+/* rho[dom][r] = sum_n occ[dom][n] |psi[dom][r][n]|^2 */
+int mlmd_ref_density(int ndom, long ngrid, int norb, const zc *psi, const double *occ, double *rho) {
+    for (int dom = 0; dom < ndom; ++dom) {
+        const zc *p = psi + (size_t)dom * ngrid * norb;
+#pragma omp parallel for schedule(static)
+        for (long r = 0; r < ngrid; ++r) {
+            double s = 0.0;
+            for (int n = 0; n < norb; ++n) {
+                const zc v = p[r * norb + n];
+                s += occ[(size_t)dom * norb + n] * (creal(v) * creal(v) + cimag(v) * cimag(v));
+            }
+            rho[(size_t)dom * ngrid + r] = s;
+        }
+    }
+    return 0;
+}
+
+/* S[dom][m][n] = dv * sum_r conj(phi[dom][r][m]) psi[dom][r][n] */
+int mlmd_ref_overlap(int ndom, long ngrid, int norb, double dv, const zc *phi, const zc *psi, zc *S) {
+    for (int dom = 0; dom < ndom; ++dom) {
+        const zc *a = phi + (size_t)dom * ngrid * norb;
+        const zc *b = psi + (size_t)dom * ngrid * norb;
+        zc *s = S + (size_t)dom * norb * norb;
+#pragma omp parallel for schedule(static)
+        for (int m = 0; m < norb; ++m)
+            for (int n = 0; n < norb; ++n) {
+                zc acc = 0.0;
+                for (long r = 0; r < ngrid; ++r) acc += conj(a[r * norb + m]) * b[r * norb + n];
+                s[(size_t)m * norb + n] = dv * acc;
+            }
+    }
+    return 0;
+}
+
+/* nsteps Taylor-4 steps on every domain, in place; rho (may be NULL) from the last step. */
+int mlmd_ref_propagate(int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int norb,
+                       int nproj, zc *psi, const double *occ, const double *vloc, const zc *beta,
+                       const double *D, int nsteps, double dt, const double *A, int a_ndom,
+                       double *rho, int flags) {
+    const long ngrid = (long)nx * ny * nz;
+    const size_t ne = (size_t)ngrid * norb;
+    zc *phi = (zc *)malloc(ne * sizeof(zc));
+    zc *hphi = (zc *)malloc(ne * sizeof(zc));
+    zc *acc = (zc *)malloc(ne * sizeof(zc));
+    if (!phi || !hphi || !acc) {
+        free(phi);
+        free(hphi);
+        free(acc);
+        return 5;
+    }
+    int rc = 0;
+    for (int dom = 0; dom < ndom && !rc; ++dom) {
+        zc *p = psi + (size_t)dom * ne;
+        const double *v = vloc + (size_t)dom * ngrid;
+        const zc *b = beta ? beta + (size_t)dom * ngrid * nproj : NULL;
+        const double *d = D ? D + (size_t)dom * nproj : NULL;
+        for (int step = 0; step < nsteps && !rc; ++step) {
+            const double *Av = A + ((size_t)step * a_ndom + (a_ndom == 1 ? 0 : dom)) * 3;
+            if (flags & MLMD_REF_HORNER) {
+                /* w_4 = psi; w_{k-1} = psi + (-i dt/k) H w_k; psi_new = w_0 */
+                memcpy(phi, p, ne * sizeof(zc));
+                for (int k = 4; k >= 1 && !rc; --k) {
+                    rc = mlmd_ref_apply_h(nx, ny, nz, hx, hy, hz, norb, nproj, phi, hphi, v, b, d, Av, flags);
+                    const zc f = -I * dt / (double)k;
+                    for (size_t e = 0; e < ne; ++e) phi[e] = p[e] + f * hphi[e];
+                }
+                memcpy(p, phi, ne * sizeof(zc));
+            } else {
+                /* phi_0 = psi; phi_m = (-i dt/m) H phi_{m-1}; psi_new = sum_{m=0..4} phi_m */
+                memcpy(phi, p, ne * sizeof(zc));
+                memcpy(acc, p, ne * sizeof(zc));
+                for (int m = 1; m <= 4 && !rc; ++m) {
+                    rc = mlmd_ref_apply_h(nx, ny, nz, hx, hy, hz, norb, nproj, phi, hphi, v, b, d, Av, flags);
+                    const zc f = -I * dt / (double)m;
+                    for (size_t e = 0; e < ne; ++e) {
+                        phi[e] = f * hphi[e];
+                        acc[e] += phi[e];
+                    }
+                }
+                memcpy(p, acc, ne * sizeof(zc));
+            }
+            if (rho) mlmd_ref_density(1, ngrid, norb, p, occ + (size_t)dom * norb, rho + (size_t)dom * ngrid);
+        }
+        if (rho && nsteps == 0)
+            mlmd_ref_density(1, ngrid, norb, p, occ + (size_t)dom * norb, rho + (size_t)dom * ngrid);
+    }
+    free(phi);
+    free(hphi);
+    free(acc);
+    return rc;
+}
