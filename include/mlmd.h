@@ -1,0 +1,126 @@
+/*
+ * mlmd.h -- C ABI of libmlmd: the domain-batched real-time Kohn-Sham step on one B200 (sm_100a).
+ *
+ * One handle = a batch of `ndom` same-shaped, independent divide-and-conquer domains
+ * (PAPER.md L126, L298).  Orbitals psi_n on a periodic real-space grid are advanced by
+ *
+ *     psi <- sum_{m=0..4} (-i dt H)^m / m!  psi,       H = 1/2 (-i grad + A)^2 + V_loc + V_NL
+ *
+ * (Eq. (2) L138 and Eq. (3); BASELINE.json north_star: 4th-order Taylor propagator,
+ * 4th-order central finite differences, Kleinman-Bylander projectors
+ * V_NL psi = sum_p beta_p D_p <beta_p|psi>, <a|b> = dv * sum_r conj(a) b), and every step ends
+ * with rho(r) = sum_n f_n |psi_n(r)|^2.  Hartree atomic units; `A` means (e/c)A of Eq. (3).
+ * The readings of the paper that fix the details (D1..D26) are listed in DESIGN.md.
+ *
+ * Conventions
+ *   layout     psi[dom][ix][iy][iz][n] complex64 (re,im interleaved), orbital index n fastest
+ *              (PAPER.md L170); grid point index r = (ix*ny + iy)*nz + iz; beta[dom][r][p];
+ *              vloc[dom][r]; rho[dom][r]; D[dom][p]; occ[dom][n]; S[dom][m][n].
+ *   where      every data pointer comes with MLMD_HOST or MLMD_DEVICE saying where it lives
+ *              (device = the CUDA device current at mlmd_domain_create).
+ *   ownership  the caller owns every buffer it passes, including the workspace, which must stay
+ *              alive and untouched until mlmd_domain_destroy.  set_* calls copy their inputs
+ *              into the workspace.  The library allocates no device memory after create.
+ *   stream     all work is enqueued on the stream given at create.  Calls are asynchronous
+ *              w.r.t. the host except: any call with a MLMD_HOST pointer (synchronises the stream
+ *              before returning), mlmd_set_vloc (reads back max|V|), and mlmd_propagate when the
+ *              handle was created with MLMD_CHECK_FINITE.
+ *   errors     every call returns a status; on error nothing is written to caller buffers and
+ *              mlmd_last_error() describes the failure.  Nothing throws or aborts.
+ *   threading  one handle is not re-entrant; distinct handles are independent.
+ *   device     requires compute capability 10.x; anything else -> MLMD_ERR_CUDA.  There is no
+ *              CPU fallback.
+ */
+#ifndef MLMD_H
+#define MLMD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mlmd_domain mlmd_domain_t;
+
+enum {
+    MLMD_OK = 0,
+    MLMD_ERR_ARG = 1,       /* NULL pointer, bad enum, negative size */
+    MLMD_ERR_SHAPE = 2,     /* grid axis < 5, nproj > nproj_max, workspace too small, ... */
+    MLMD_ERR_STATE = 3,     /* e.g. propagate before set_orbitals / set_vloc */
+    MLMD_ERR_CUDA = 4,      /* CUDA runtime error or unsupported device */
+    MLMD_ERR_NOMEM = 5,
+    MLMD_ERR_NONFINITE = 6, /* MLMD_CHECK_FINITE found NaN/Inf in psi after propagate */
+    MLMD_WARN_UNSTABLE = 7  /* work done, but the a-priori Taylor-4 stability bound is exceeded */
+};
+enum { MLMD_HOST = 0, MLMD_DEVICE = 1 };
+enum { MLMD_BETA_REAL32 = 0, MLMD_BETA_COMPLEX64 = 1 };
+enum {
+    MLMD_GEMM_FP32GRADE = 0, /* default: 3xTF32 on tcgen05 tensor cores, FP32 accumulate          */
+    MLMD_GEMM_FP64 = 1,      /* FP64 accumulation of exact FP32 products (CUDA cores; slow, check) */
+    MLMD_GEMM_LOWP_BF16 = 2, /* opt-in: BF16 operands, FP32 accumulate      */
+    MLMD_GEMM_TF32X1 = 3,    /* optional rung: single TF32 product, FP32 accumulate               */
+    MLMD_GEMM_FP32_SIMT = 4  /* plain FP32 FMA on CUDA cores (portable fallback, any shape)       */
+};
+enum {
+    MLMD_KEEP_PSI0 = 1u,    /* snapshot Psi(0) at mlmd_set_orbitals for mlmd_overlap(which=1)     */
+    MLMD_CHECK_FINITE = 2u  /* scan psi for NaN/Inf at the end of every mlmd_propagate            */
+};
+
+/* Bytes of device workspace mlmd_domain_create needs for this shape (0 on invalid arguments).
+ * Holds Psi, two Psi-sized stage buffers (Horner form of the Taylor sum), optional Psi(0),
+ * V_loc, beta (and its split copies), D, occupations, rho, projection scratch. */
+size_t mlmd_workspace_bytes(int ndom, int nx, int ny, int nz, int norb, int nproj_max, unsigned flags);
+
+/* Create a batch of ndom periodic domains of nx*ny*nz points (each axis >= 5: the five radius-2
+ * periodic neighbours must be distinct), spacings hx,hy,hz (bohr), norb orbitals, at most
+ * nproj_max projectors (complex projectors count once).  workspace_dev: device memory, 256-byte
+ * aligned, >= mlmd_workspace_bytes(...).  cuda_stream: a cudaStream_t passed as void*
+ * (NULL = legacy default stream). */
+int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, double hx, double hy,
+                       double hz, int norb, int nproj_max, void *workspace_dev, size_t workspace_bytes,
+                       void *cuda_stream, unsigned flags);
+int mlmd_domain_destroy(mlmd_domain_t *h);
+
+/* Psi(t=0) and occupations f_n >= 0 (occ may be NULL = keep previous / all 2.0).
+ * psi: complex64 [ndom][nx][ny][nz][norb] at `where`; occ: double [ndom][norb], HOST. */
+int mlmd_set_orbitals(mlmd_domain_t *h, const void *psi_c64, const double *occ, int where);
+int mlmd_get_orbitals(mlmd_domain_t *h, void *psi_c64, int where);
+
+/* Local potential v_loc(r) of Eq. (3) in Hartree, float [ndom][nx][ny][nz]; frozen during a
+ * propagate call (only Delta v_loc is passed once per MD step; reading D25). */
+int mlmd_set_vloc(mlmd_domain_t *h, const float *vloc, int where);
+
+/* Nonlocal operator V_NL = dv * B diag(D) B^H (north_star; Eq. (5) L199 is the case
+ * B = Psi(0)).  beta: [ndom][ngrid][nproj], float (MLMD_BETA_REAL32) or complex64
+ * (MLMD_BETA_COMPLEX64) at `where`; D: double [ndom][nproj] in Hartree, HOST.
+ * nproj = 0 switches V_NL off (beta, D may be NULL). */
+int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_dtype, const double *D,
+                        int where);
+
+int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode);
+
+/* nsteps Taylor-4 steps of size dt.  A: double [nsteps][a_ndom][3], HOST; A[n] is the vector
+ * potential at the step midpoint t_n + dt/2 (Eq. (2)), uniform inside a domain;
+ * a_ndom = 1 (same field for every domain) or ndom.  The density of the final state is kept
+ * for mlmd_density.  Returns MLMD_WARN_UNSTABLE (work still done) if
+ * dt * [ (8/3) sum_d 1/h_d^2 + 1.3722 sum_d |A_d|/h_d + |A|^2/2 + max|V_loc| + max|D| ] > 2 sqrt(2). */
+int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
+
+/* rho(r) = sum_n f_n |psi_n(r)|^2 of the current state, float [ndom][nx][ny][nz] at `where`. */
+int mlmd_density(mlmd_domain_t *h, float *rho, int where);
+
+/* S[dom] = dv * Phi^H Psi(t), complex64 [ndom][norb][norb] at `where` (CGEMM(1)):
+ * which = 0: Phi = Psi(t) (Gram matrix); which = 1: Phi = Psi(0) (needs MLMD_KEEP_PSI0).
+ * Always evaluated in the FP32-grade (or FP64) GEMM mode: it is a measurement. */
+int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
+
+/* Number of kernels the library launched on this handle since create (bench.py's gpu_launches). */
+long long mlmd_launch_count(const mlmd_domain_t *h);
+
+/* Thread-local description of the last failure in this thread; never NULL. */
+const char *mlmd_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MLMD_H */

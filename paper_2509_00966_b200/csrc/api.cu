@@ -1,0 +1,399 @@
+// C ABI of libmlmd (include/mlmd.h): argument checking, workspace carving, and the step scheduler
+// that strings the kernels into four Horner stages + density per time step.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "mlmd_internal.h"
+
+using namespace mlmd;
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+#define CU(call)                                                                                    \
+    do {                                                                                            \
+        cudaError_t e__ = (call);                                                                   \
+        if (e__ != cudaSuccess)                                                                     \
+            return fail(MLMD_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    } while (0)
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static int round_up_i(int x, int a) { return (x + a - 1) / a * a; }
+
+struct Plan {
+    int ld, ldp_max, prows, nsplit;
+    long ngrid;
+    Workspace off;
+};
+
+static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max, unsigned flags, Plan *pl) {
+    if (ndom < 1 || nx < 5 || ny < 5 || nz < 5 || norb < 1 || nproj_max < 0) return false;
+    if ((double)ndom * nx * ny * nz > 2.0e9) return false;
+    pl->ld = round_up_i(norb, 8);
+    pl->ngrid = (long)nx * ny * nz;
+    pl->ldp_max = round_up_i(std::max(nproj_max, 1), 4);
+    pl->prows = std::max(pl->ldp_max, 2 * pl->ld);
+    const long tiles = (long)((2 * pl->ld + 63) / 64) * std::max(1, (nproj_max + 63) / 64) * ndom;
+    long ns = (592 + tiles - 1) / tiles;
+    ns = std::min<long>(ns, std::min<long>(kMaxSplit, pl->ngrid / 64));
+    pl->nsplit = (int)std::max<long>(ns, 1);
+    const size_t npts = (size_t)ndom * pl->ngrid;
+    const size_t psi_b = npts * pl->ld * sizeof(float2);
+    size_t o = 0;
+    auto take = [&](size_t bytes) {
+        size_t at = o;
+        o = align_up(o + bytes, 256);
+        return at;
+    };
+    Workspace &w = pl->off;
+    w.psi = take(psi_b);
+    w.ua = take(psi_b);
+    w.ub = take(psi_b);
+    w.psi0 = take((flags & MLMD_KEEP_PSI0) ? psi_b : 0);
+    w.vloc = take(npts * sizeof(float));
+    w.beta = take(npts * pl->ldp_max * sizeof(float));
+    w.beta_lo = take(npts * pl->ldp_max * sizeof(float));
+    w.dprime = take((size_t)ndom * pl->ldp_max * sizeof(float));
+    w.occ = take((size_t)ndom * pl->ld * sizeof(float));
+    w.rho = take(npts * sizeof(float));
+    const size_t zb = (size_t)ndom * pl->prows * 2 * pl->ld * sizeof(float);
+    w.z = take(zb);
+    w.what = take(zb);
+    w.zpart = take(zb * pl->nsplit);
+    w.coef = take((size_t)kCoefCapacity * ndom * sizeof(StepCoef));
+    w.flag = take(256);
+    w.total = o;
+    return true;
+}
+
+extern "C" {
+
+const char *mlmd_last_error(void) { return g_err; }
+
+size_t mlmd_workspace_bytes(int ndom, int nx, int ny, int nz, int norb, int nproj_max, unsigned flags) {
+    Plan pl;
+    if (!make_plan(ndom, nx, ny, nz, norb, nproj_max, flags, &pl)) return 0;
+    return pl.off.total;
+}
+
+int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, double hx, double hy,
+                       double hz, int norb, int nproj_max, void *workspace_dev, size_t workspace_bytes,
+                       void *cuda_stream, unsigned flags) {
+    if (!out) return fail(MLMD_ERR_ARG, "mlmd_domain_create: out is NULL");
+    *out = nullptr;
+    if (!workspace_dev) return fail(MLMD_ERR_ARG, "mlmd_domain_create: workspace is NULL");
+    if (!(hx > 0) || !(hy > 0) || !(hz > 0)) return fail(MLMD_ERR_ARG, "mlmd_domain_create: grid spacings must be > 0");
+    if (flags & ~(MLMD_KEEP_PSI0 | MLMD_CHECK_FINITE)) return fail(MLMD_ERR_ARG, "mlmd_domain_create: unknown flags 0x%x", flags);
+    Plan pl;
+    if (!make_plan(ndom, nx, ny, nz, norb, nproj_max, flags, &pl))
+        return fail(MLMD_ERR_SHAPE, "mlmd_domain_create: bad shape ndom=%d grid=%dx%dx%d norb=%d nproj_max=%d "
+                    "(every grid axis must be >= 5)", ndom, nx, ny, nz, norb, nproj_max);
+    if (workspace_bytes < pl.off.total)
+        return fail(MLMD_ERR_SHAPE, "mlmd_domain_create: workspace has %zu bytes, needs %zu", workspace_bytes, pl.off.total);
+    if (((uintptr_t)workspace_dev) % 256) return fail(MLMD_ERR_ARG, "mlmd_domain_create: workspace must be 256-byte aligned");
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10)
+        return fail(MLMD_ERR_CUDA, "mlmd_domain_create: device '%s' is sm_%d%d; this library is built for sm_100a only "
+                    "and has no fallback", prop.name, prop.major, prop.minor);
+    mlmd_domain *h = new (std::nothrow) mlmd_domain();
+    if (!h) return fail(MLMD_ERR_NOMEM, "mlmd_domain_create: out of host memory");
+    h->ndom = ndom; h->nx = nx; h->ny = ny; h->nz = nz; h->norb = norb; h->nproj_max = nproj_max;
+    h->ld = pl.ld; h->ngrid = pl.ngrid;
+    h->hx = hx; h->hy = hy; h->hz = hz; h->dv = hx * hy * hz;
+    h->flags = flags;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->ws = (char *)workspace_dev; h->ws_bytes = workspace_bytes; h->off = pl.off;
+    h->nproj = 0; h->beta_complex = 0; h->P = 0; h->ldp = pl.ldp_max; h->prows = pl.prows; h->nsplit = pl.nsplit;
+    h->gemm_mode = MLMD_GEMM_FP32GRADE;
+    h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
+    h->vmax = h->dmax = 0.0; h->launches = 0;
+    h->coef_host = nullptr; h->flag_host = nullptr;
+    cudaError_t e = cudaMallocHost((void **)&h->coef_host, (size_t)kCoefCapacity * ndom * sizeof(StepCoef));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&h->flag_host, 256);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->occ(), 0, (size_t)ndom * h->ld * sizeof(float), h->stream);
+    if (e != cudaSuccess) {
+        if (h->coef_host) cudaFreeHost(h->coef_host);
+        if (h->flag_host) cudaFreeHost(h->flag_host);
+        delete h;
+        return fail(MLMD_ERR_CUDA, "mlmd_domain_create: %s", cudaGetErrorString(e));
+    }
+    *out = h;
+    return MLMD_OK;
+}
+
+int mlmd_domain_destroy(mlmd_domain_t *h) {
+    if (!h) return MLMD_OK;
+    cudaStreamSynchronize(h->stream);
+    if (h->coef_host) cudaFreeHost(h->coef_host);
+    if (h->flag_host) cudaFreeHost(h->flag_host);
+    delete h;
+    return MLMD_OK;
+}
+
+long long mlmd_launch_count(const mlmd_domain_t *h) { return h ? h->launches : 0; }
+
+static cudaMemcpyKind kind_in(int where) { return where == MLMD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice; }
+static cudaMemcpyKind kind_out(int where) { return where == MLMD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice; }
+static bool bad_where(int where) { return where != MLMD_HOST && where != MLMD_DEVICE; }
+
+int mlmd_set_orbitals(mlmd_domain_t *h, const void *psi, const double *occ, int where) {
+    if (!h || !psi) return fail(MLMD_ERR_ARG, "mlmd_set_orbitals: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_set_orbitals: bad where=%d", where);
+    const size_t rows = (size_t)h->ndom * h->ngrid;
+    if (occ) {
+        std::vector<float> f((size_t)h->ndom * h->ld, 0.f);
+        for (int d = 0; d < h->ndom; ++d)
+            for (int n = 0; n < h->norb; ++n) {
+                const double v = occ[(size_t)d * h->norb + n];
+                if (!(v >= 0.0)) return fail(MLMD_ERR_ARG, "mlmd_set_orbitals: occ[%d][%d]=%g is not >= 0", d, n, v);
+                f[(size_t)d * h->ld + n] = (float)v;
+            }
+        CU(cudaMemcpyAsync(h->occ(), f.data(), f.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaStreamSynchronize(h->stream));   // f is a temporary
+        h->have_occ = true;
+    } else if (!h->have_occ) {
+        std::vector<float> f((size_t)h->ndom * h->ld, 0.f);
+        for (int d = 0; d < h->ndom; ++d)
+            for (int n = 0; n < h->norb; ++n) f[(size_t)d * h->ld + n] = 2.f;
+        CU(cudaMemcpyAsync(h->occ(), f.data(), f.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        h->have_occ = true;
+    }
+    if (h->ld != h->norb) CU(cudaMemsetAsync(h->psi(), 0, rows * h->ld * sizeof(float2), h->stream));
+    CU(cudaMemcpy2DAsync(h->psi(), (size_t)h->ld * sizeof(float2), psi, (size_t)h->norb * sizeof(float2),
+                         (size_t)h->norb * sizeof(float2), rows, kind_in(where), h->stream));
+    if (h->flags & MLMD_KEEP_PSI0)
+        CU(cudaMemcpyAsync(h->psi0(), h->psi(), rows * h->ld * sizeof(float2), cudaMemcpyDeviceToDevice, h->stream));
+    if (where == MLMD_HOST) CU(cudaStreamSynchronize(h->stream));
+    h->have_psi = true;
+    h->rho_valid = false;
+    return MLMD_OK;
+}
+
+int mlmd_get_orbitals(mlmd_domain_t *h, void *psi, int where) {
+    if (!h || !psi) return fail(MLMD_ERR_ARG, "mlmd_get_orbitals: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_get_orbitals: bad where=%d", where);
+    if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_get_orbitals: no orbitals set");
+    const size_t rows = (size_t)h->ndom * h->ngrid;
+    CU(cudaMemcpy2DAsync(psi, (size_t)h->norb * sizeof(float2), h->psi(), (size_t)h->ld * sizeof(float2),
+                         (size_t)h->norb * sizeof(float2), rows, kind_out(where), h->stream));
+    if (where == MLMD_HOST) CU(cudaStreamSynchronize(h->stream));
+    return MLMD_OK;
+}
+
+int mlmd_set_vloc(mlmd_domain_t *h, const float *vloc, int where) {
+    if (!h || !vloc) return fail(MLMD_ERR_ARG, "mlmd_set_vloc: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_set_vloc: bad where=%d", where);
+    const size_t n = (size_t)h->ndom * h->ngrid;
+    int nl = 0;
+    CU(cudaMemcpyAsync(h->vloc(), vloc, n * sizeof(float), kind_in(where), h->stream));
+    CU(launch_max_abs(h->stream, h->vloc(), n, h->flag(), &nl));
+    CU(cudaMemcpyAsync(h->flag_host, h->flag(), sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    h->launches += nl;
+    float vm;
+    memcpy(&vm, h->flag_host, sizeof(float));
+    if (!(vm < INFINITY)) return fail(MLMD_ERR_NONFINITE, "mlmd_set_vloc: V_loc contains NaN/Inf");
+    h->vmax = vm;
+    h->have_vloc = true;
+    return MLMD_OK;
+}
+
+int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_dtype, const double *D, int where) {
+    if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: NULL handle");
+    if (nproj < 0) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: nproj=%d", nproj);
+    if (nproj == 0) {
+        h->nproj = h->P = 0;
+        h->dmax = 0.0;
+        return MLMD_OK;
+    }
+    if (!beta || !D) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: NULL beta or D");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: bad where=%d", where);
+    if (beta_dtype != MLMD_BETA_REAL32 && beta_dtype != MLMD_BETA_COMPLEX64)
+        return fail(MLMD_ERR_ARG, "mlmd_set_projectors: bad beta_dtype=%d", beta_dtype);
+    const int cplx = beta_dtype == MLMD_BETA_COMPLEX64;
+    const int P = cplx ? 2 * nproj : nproj;
+    if (P > h->nproj_max)
+        return fail(MLMD_ERR_SHAPE, "mlmd_set_projectors: %d %s projectors need %d real rows, handle was created with "
+                    "nproj_max=%d", nproj, cplx ? "complex" : "real", P, h->nproj_max);
+    const size_t rows = (size_t)h->ndom * h->ngrid;
+    const int ldp = round_up_i(P, 4);
+    std::vector<float> dp((size_t)h->ndom * nproj);
+    double dmax = 0.0;
+    for (size_t i = 0; i < dp.size(); ++i) {
+        if (!std::isfinite(D[i])) return fail(MLMD_ERR_NONFINITE, "mlmd_set_projectors: D[%zu] is not finite", i);
+        dp[i] = (float)(D[i] * h->dv);
+        dmax = std::max(dmax, fabs(D[i]));
+    }
+    CU(cudaMemcpyAsync(h->dprime(), dp.data(), dp.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    if (ldp != P) CU(cudaMemsetAsync(h->beta(), 0, rows * ldp * sizeof(float), h->stream));
+    CU(cudaMemcpy2DAsync(h->beta(), (size_t)ldp * sizeof(float), beta, (size_t)P * sizeof(float), (size_t)P * sizeof(float),
+                         rows, kind_in(where), h->stream));
+    int nl = 0;
+    CU(launch_split_tf32_lo(h->stream, h->beta(), h->beta_lo(), rows * ldp, &nl));
+    h->launches += nl;
+    CU(cudaStreamSynchronize(h->stream));   // dp is a temporary; host beta may be reused by the caller
+    h->nproj = nproj; h->beta_complex = cplx; h->P = P; h->ldp = ldp; h->dmax = dmax;
+    return MLMD_OK;
+}
+
+int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
+    if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: NULL handle");
+    if (mode < MLMD_GEMM_FP32GRADE || mode > MLMD_GEMM_FP32_SIMT) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: bad mode %d", mode);
+    h->gemm_mode = mode;
+    return MLMD_OK;
+}
+
+// ---- the step --------------------------------------------------------------------------------
+static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
+    // SURVEY.md 8(a) S1; weights of the 4th-order central differences (north_star)
+    static const double c2[2] = {4.0 / 3.0, -1.0 / 12.0};   // j = 1, 2  (symmetric)
+    static const double c1[2] = {2.0 / 3.0, -1.0 / 12.0};   // j = +1, +2 (antisymmetric)
+    const double hh[3] = {h->hx, h->hy, h->hz};
+    double centre = 0.5 * (A3[0] * A3[0] + A3[1] * A3[1] + A3[2] * A3[2]);
+    for (int d = 0; d < 3; ++d) {
+        centre += -0.5 * (-5.0 / 2.0) / (hh[d] * hh[d]);
+        for (int j = 0; j < 2; ++j) {
+            c->p[d][j] = (float)(-0.5 * c2[j] / (hh[d] * hh[d]));
+            c->q[d][j] = (float)(A3[d] * c1[j] / hh[d]);
+        }
+    }
+    c->centre = (float)centre;
+    c->pad = 0.f;
+}
+
+static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl) {
+    // S2a + S2b: What = (-i tau) D' (beta^H w)
+    const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
+    CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, (const float *)w, 2 * h->ld, 2 * h->ld,
+                        h->zpart(), h->prows, h->nsplit, fp64, nl));
+    CU(launch_reduce_scale(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, h->nsplit, h->zpart(),
+                           h->dprime(), tau, h->what(), nl));
+    return MLMD_OK;
+}
+
+static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl) {
+    const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
+    CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, h->what(), (float *)out, 2 * h->ld,
+                        2 * h->ld, h->prows, fp64, nl));
+    return MLMD_OK;
+}
+
+int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom) {
+    if (!h) return fail(MLMD_ERR_ARG, "mlmd_propagate: NULL handle");
+    if (nsteps < 0 || !(dt == dt) || std::isinf(dt)) return fail(MLMD_ERR_ARG, "mlmd_propagate: nsteps=%d dt=%g", nsteps, dt);
+    if (nsteps > 0 && !A) return fail(MLMD_ERR_ARG, "mlmd_propagate: A is NULL");
+    if (a_ndom != 1 && a_ndom != h->ndom) return fail(MLMD_ERR_ARG, "mlmd_propagate: a_ndom=%d must be 1 or ndom=%d", a_ndom, h->ndom);
+    if (!h->have_psi || !h->have_vloc) return fail(MLMD_ERR_STATE, "mlmd_propagate: call mlmd_set_orbitals and mlmd_set_vloc first");
+    // a-priori stability bound of Taylor-4 (reading D14): dt * |lambda|max(H) <= 2 sqrt(2)
+    bool yz = false;
+    double bound = 0.0;
+    for (size_t i = 0; i < (size_t)nsteps * a_ndom; ++i) {
+        const double *a = A + 3 * i;
+        if (!std::isfinite(a[0]) || !std::isfinite(a[1]) || !std::isfinite(a[2]))
+            return fail(MLMD_ERR_NONFINITE, "mlmd_propagate: A[%zu] is not finite", i);
+        yz = yz || a[1] != 0.0 || a[2] != 0.0;
+        const double b = (8.0 / 3.0) * (1 / (h->hx * h->hx) + 1 / (h->hy * h->hy) + 1 / (h->hz * h->hz)) +
+                         1.3722 * (fabs(a[0]) / h->hx + fabs(a[1]) / h->hy + fabs(a[2]) / h->hz) +
+                         0.5 * (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) + h->vmax + (h->nproj ? h->dmax : 0.0);
+        bound = std::max(bound, b);
+    }
+    h->field_yz = yz;
+    int nl = 0;
+    for (int s0 = 0; s0 < nsteps; s0 += kCoefCapacity) {
+        const int ns = std::min(kCoefCapacity, nsteps - s0);
+        if (s0 > 0) CU(cudaStreamSynchronize(h->stream));   // the pinned staging buffer is reused
+        for (int s = 0; s < ns; ++s)
+            for (int d = 0; d < h->ndom; ++d)
+                fill_coef(h, A + ((size_t)(s0 + s) * a_ndom + (a_ndom == 1 ? 0 : d)) * 3, &h->coef_host[(size_t)s * h->ndom + d]);
+        CU(cudaMemcpyAsync(h->coef(), h->coef_host, (size_t)ns * h->ndom * sizeof(StepCoef), cudaMemcpyHostToDevice, h->stream));
+        for (int s = 0; s < ns; ++s) {
+            const StepCoef *coef = h->coef() + (size_t)s * h->ndom;
+            // Horner form of sum_{m<=4} (-i dt H)^m/m!: w4 = psi, w_{k-1} = psi + (-i dt/k) H w_k (S2)
+            const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
+            float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
+            for (int i = 0; i < 4; ++i) {
+                const float tau = (float)(dt / (4 - i));
+                if (h->nproj > 0) {
+                    int rc = nonlocal_project(h, src[i], tau, &nl);
+                    if (rc) return rc;
+                }
+                CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, tau, &nl));
+                if (h->nproj > 0) {
+                    int rc = nonlocal_back(h, dst[i], &nl);
+                    if (rc) return rc;
+                }
+            }
+            CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), &nl));
+        }
+    }
+    h->launches += nl;
+    if (nsteps > 0) h->rho_valid = true;
+    if (h->flags & MLMD_CHECK_FINITE) {
+        int n2 = 0;
+        CU(launch_check_finite(h->stream, (const float *)h->psi(), (size_t)h->ndom * h->ngrid * h->ld * 2, h->flag(), &n2));
+        h->launches += n2;
+        CU(cudaMemcpyAsync(h->flag_host, h->flag(), sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        if (*h->flag_host) return fail(MLMD_ERR_NONFINITE, "mlmd_propagate: psi contains NaN/Inf after %d steps", nsteps);
+    }
+    if (dt * bound > 2.0 * sqrt(2.0)) {
+        fail(MLMD_WARN_UNSTABLE, "mlmd_propagate: dt*|H|max bound = %.3f > 2 sqrt(2): Taylor-4 may be unstable", dt * bound);
+        return MLMD_WARN_UNSTABLE;
+    }
+    return MLMD_OK;
+}
+
+int mlmd_density(mlmd_domain_t *h, float *rho, int where) {
+    if (!h || !rho) return fail(MLMD_ERR_ARG, "mlmd_density: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_density: bad where=%d", where);
+    if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_density: no orbitals set");
+    if (!h->rho_valid) {
+        int nl = 0;
+        CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), &nl));
+        h->launches += nl;
+        h->rho_valid = true;
+    }
+    CU(cudaMemcpyAsync(rho, h->rho(), (size_t)h->ndom * h->ngrid * sizeof(float), kind_out(where), h->stream));
+    if (where == MLMD_HOST) CU(cudaStreamSynchronize(h->stream));
+    return MLMD_OK;
+}
+
+int mlmd_overlap(mlmd_domain_t *h, int which, void *S, int where) {
+    if (!h || !S) return fail(MLMD_ERR_ARG, "mlmd_overlap: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_overlap: bad where=%d", where);
+    if (which != 0 && which != 1) return fail(MLMD_ERR_ARG, "mlmd_overlap: which=%d", which);
+    if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_overlap: no orbitals set");
+    if (which == 1 && !(h->flags & MLMD_KEEP_PSI0)) return fail(MLMD_ERR_STATE, "mlmd_overlap: which=1 needs MLMD_KEEP_PSI0 at create");
+    const float2 *phi = which == 0 ? h->psi() : h->psi0();
+    int nl = 0;
+    const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
+    // projection GEMM with B := float view of Phi (2*ld real rows), S4 of SURVEY.md 8(a)
+    CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, (const float *)phi, 2 * h->ld, 2 * h->ld, (const float *)h->psi(),
+                        2 * h->ld, 2 * h->ld, h->zpart(), h->prows, h->nsplit, fp64, &nl));
+    float2 *sdev = where == MLMD_DEVICE ? (float2 *)S : (float2 *)h->z();
+    CU(launch_overlap_epilogue(h->stream, h->ndom, h->norb, h->ld, h->prows, h->nsplit, h->zpart(), (float)h->dv, sdev, &nl));
+    h->launches += nl;
+    if (where == MLMD_HOST) {
+        CU(cudaMemcpyAsync(S, sdev, (size_t)h->ndom * h->norb * h->norb * sizeof(float2), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    return MLMD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,166 @@
+// Small kernels around the GEMMs and the stencil: split-K reduction + projector scaling (S2b),
+// density (S3), overlap epilogue (S4), operand preparation and checks.
+#include "mlmd_internal.h"
+
+namespace mlmd {
+
+// S2b.  C[p][n] = sum over split slices (fixed order: bit-reproducible, reading D22) of the
+// projection, combined to the complex coefficient for complex projectors; then
+//   W[p][n] = (-i tau) * D'_p * C[p][n],  D' = D * dv (reading D10)
+// written in the real-GEMM form the back-application consumes:
+//   real beta:    What[p][2n] = Re W, What[p][2n+1] = Im W
+//   complex beta: rows 2p, 2p+1 hold the 2x2 real representation of W.
+__global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int prows, int nsplit,
+                                    const float *__restrict__ zpart, const float *__restrict__ dprime, float tau,
+                                    float *__restrict__ what) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.y, dom = blockIdx.z;
+    if (n >= ld) return;
+    const int N = 2 * ld;
+    const float *zp = zpart + (size_t)dom * nsplit * prows * N;
+    const size_t slice = (size_t)prows * N;
+    float cre = 0.f, cim = 0.f;
+    if (!beta_complex) {
+        for (int s = 0; s < nsplit; ++s) {
+            const float2 v = *(const float2 *)(zp + s * slice + (size_t)p * N + 2 * n);
+            cre += v.x;
+            cim += v.y;
+        }
+    } else {
+        for (int s = 0; s < nsplit; ++s) {
+            const float2 a = *(const float2 *)(zp + s * slice + (size_t)(2 * p) * N + 2 * n);      // Re(beta) row
+            const float2 b = *(const float2 *)(zp + s * slice + (size_t)(2 * p + 1) * N + 2 * n);  // Im(beta) row
+            cre += a.x + b.y;   // conj(beta) psi
+            cim += a.y - b.x;
+        }
+    }
+    const float f = tau * dprime[(size_t)dom * nproj + p];
+    const float wre = f * cim, wim = -f * cre;   // (-i f)(cre + i cim)
+    float *wd = what + (size_t)dom * prows * N;
+    if (!beta_complex) {
+        *(float2 *)(wd + (size_t)p * N + 2 * n) = make_float2(wre, wim);
+    } else {
+        *(float2 *)(wd + (size_t)(2 * p) * N + 2 * n) = make_float2(wre, wim);
+        *(float2 *)(wd + (size_t)(2 * p + 1) * N + 2 * n) = make_float2(-wim, wre);
+    }
+}
+
+cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows,
+                                int nsplit, const float *zpart, const float *dprime, float tau,
+                                float *what, int *nlaunch) {
+    dim3 grid((ld + 127) / 128, nproj, ndom);
+    ++*nlaunch;
+    reduce_scale_kernel<<<grid, 128, 0, st>>>(nproj, beta_complex, ld, prows, nsplit, zpart, dprime, tau, what);
+    return cudaGetLastError();
+}
+
+// S3: one warp per grid point; lanes stride over the orbital row with 128-bit loads and reduce
+// with shuffles (north_star kernel 4).
+__global__ void __launch_bounds__(256)
+density_kernel(long npoints, long ngrid, int lanes, const float4 *__restrict__ psi, const float *__restrict__ occ,
+               float *__restrict__ rho) {
+    const long pt = (long)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
+    if (pt >= npoints) return;
+    const int lane = threadIdx.x % 32;
+    const int dom = (int)(pt / ngrid);
+    const float4 *row = psi + pt * lanes;
+    const float2 *f = (const float2 *)(occ + (size_t)dom * lanes * 2);
+    float s = 0.f;
+    for (int l = lane; l < lanes; l += 32) {
+        const float4 v = __ldg(row + l);
+        const float2 ff = __ldg(f + l);
+        s = fmaf(ff.x, fmaf(v.x, v.x, v.y * v.y), s);
+        s = fmaf(ff.y, fmaf(v.z, v.z, v.w * v.w), s);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) rho[pt] = s;
+}
+
+cudaError_t launch_density(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, const float *occ,
+                           float *rho, int *nlaunch) {
+    const long npoints = (long)ndom * ngrid;
+    ++*nlaunch;
+    density_kernel<<<(unsigned)((npoints + 7) / 8), 256, 0, st>>>(npoints, ngrid, ld / 2, (const float4 *)psi, occ,
+                                                                 rho);
+    return cudaGetLastError();
+}
+
+// S4 epilogue: projection run with B := float view of Phi (rows 2m = Re, 2m+1 = Im):
+//   S[m][n] = dv * sum_r conj(Phi[r,m]) Psi[r,n]
+__global__ void overlap_epilogue_kernel(int norb, int ld, int prows, int nsplit, const float *__restrict__ zpart,
+                                        float dv, float2 *__restrict__ S) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    const int m = blockIdx.y, dom = blockIdx.z;
+    if (n >= norb) return;
+    const int N = 2 * ld;
+    const float *zp = zpart + (size_t)dom * nsplit * prows * N;
+    const size_t slice = (size_t)prows * N;
+    float sre = 0.f, sim = 0.f;
+    for (int s = 0; s < nsplit; ++s) {
+        const float2 a = *(const float2 *)(zp + s * slice + (size_t)(2 * m) * N + 2 * n);
+        const float2 b = *(const float2 *)(zp + s * slice + (size_t)(2 * m + 1) * N + 2 * n);
+        sre += a.x + b.y;
+        sim += a.y - b.x;
+    }
+    S[((size_t)dom * norb + m) * norb + n] = make_float2(dv * sre, dv * sim);
+}
+
+cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld, int prows, int nsplit,
+                                    const float *zpart, float dv, float2 *S, int *nlaunch) {
+    dim3 grid((norb + 127) / 128, norb, ndom);
+    ++*nlaunch;
+    overlap_epilogue_kernel<<<grid, 128, 0, st>>>(norb, ld, prows, nsplit, zpart, dv, S);
+    return cudaGetLastError();
+}
+
+// lo = x - hi with hi = x with the low 13 mantissa bits cleared (what a TF32 operand keeps); exact.
+__global__ void split_tf32_lo_kernel(const float *__restrict__ src, float *__restrict__ lo, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float x = src[i];
+        lo[i] = x - __uint_as_float(__float_as_uint(x) & 0xffffe000u);
+    }
+}
+cudaError_t launch_split_tf32_lo(cudaStream_t st, const float *src, float *lo, size_t n, int *nlaunch) {
+    ++*nlaunch;
+    split_tf32_lo_kernel<<<2368, 256, 0, st>>>(src, lo, n);
+    return cudaGetLastError();
+}
+
+// max |x| as the bit pattern of a non-negative float (atomicMax on ints orders them correctly)
+__global__ void max_abs_kernel(const float *__restrict__ x, size_t n, int *out) {
+    float m = 0.f;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float a = fabsf(x[i]);
+        m = (a > m || a != a) ? a : m;   // NaN propagates as a large bit pattern
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float other = __shfl_xor_sync(0xffffffffu, m, o);
+        m = (other > m || other != other) ? other : m;
+    }
+    if (threadIdx.x % 32 == 0) atomicMax(out, __float_as_int(m));
+}
+cudaError_t launch_max_abs(cudaStream_t st, const float *x, size_t n, int *flag_bits, int *nlaunch) {
+    ++*nlaunch;
+    cudaError_t e = cudaMemsetAsync(flag_bits, 0, sizeof(int), st);
+    if (e != cudaSuccess) return e;
+    max_abs_kernel<<<592, 256, 0, st>>>(x, n, flag_bits);
+    return cudaGetLastError();
+}
+
+__global__ void check_finite_kernel(const float *__restrict__ x, size_t n, int *flag) {
+    bool bad = false;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        bad |= !isfinite(x[i]);
+    if (__any_sync(0xffffffffu, bad) && threadIdx.x % 32 == 0) atomicOr(flag, 1);
+}
+cudaError_t launch_check_finite(cudaStream_t st, const float *x, size_t n, int *flag, int *nlaunch) {
+    ++*nlaunch;
+    cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int), st);
+    if (e != cudaSuccess) return e;
+    check_finite_kernel<<<1184, 256, 0, st>>>(x, n, flag);
+    return cudaGetLastError();
+}
+
+}  // namespace mlmd

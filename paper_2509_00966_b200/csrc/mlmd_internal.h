@@ -1,0 +1,110 @@
+// Internal declarations of libmlmd (not part of the C ABI; see include/mlmd.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/mlmd.h"
+
+namespace mlmd {
+
+// Per-(step, domain) stencil coefficients, computed in FP64 on the host and
+// rounded once.  For axis d and offset +-j (j = 1, 2):
+//   a_{d,+-j} = p[d][j-1] -+ i q[d][j-1],  p = -1/2 c2_j / h_d^2,  q = A_d c1_{+j} / h_d
+// centre (real): c0 + 1/2|A|^2 + V_loc(r).
+struct StepCoef {
+    float p[3][2];
+    float q[3][2];
+    float centre;   // c0 + 1/2 |A|^2
+    float pad;
+};
+static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
+
+struct Workspace {              // byte offsets into the caller's workspace
+    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, zpart, coef, flag, total;
+};
+
+constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
+constexpr int kMaxSplit = 64;        // split-K slices of the projection GEMM
+
+}  // namespace mlmd
+
+struct mlmd_domain {
+    int ndom, nx, ny, nz, norb, nproj_max;
+    int ld;                     // padded orbital count (row pitch of psi in complex elements)
+    long ngrid;
+    double hx, hy, hz, dv;
+    unsigned flags;
+    cudaStream_t stream;
+    char *ws;
+    size_t ws_bytes;
+    mlmd::Workspace off;
+    // state
+    int nproj;                  // projectors currently set (complex ones count once)
+    int beta_complex;           // 1: beta is complex64 -> real GEMM row count P = 2*nproj
+    int P;                      // real projector rows
+    int ldp;                    // padded P (pitch of beta rows / rows of Z, What)
+    int prows;                  // rows allocated for Z/What/zpart = max(ldp(nproj_max), 2*ld)
+    int nsplit;                 // split-K factor of the projection
+    int gemm_mode;
+    bool have_psi, have_vloc, have_occ, rho_valid;
+    bool field_yz;              // any A_y or A_z non-zero in the current propagate call
+    double vmax, dmax;
+    long long launches;
+    mlmd::StepCoef *coef_host;  // pinned, kCoefCapacity * ndom
+    int *flag_host;             // pinned
+    // typed views
+    float2 *psi() const { return (float2 *)(ws + off.psi); }
+    float2 *ua() const { return (float2 *)(ws + off.ua); }
+    float2 *ub() const { return (float2 *)(ws + off.ub); }
+    float2 *psi0() const { return (float2 *)(ws + off.psi0); }
+    float *vloc() const { return (float *)(ws + off.vloc); }
+    float *beta() const { return (float *)(ws + off.beta); }
+    float *beta_lo() const { return (float *)(ws + off.beta_lo); }
+    float *dprime() const { return (float *)(ws + off.dprime); }
+    float *occ() const { return (float *)(ws + off.occ); }
+    float *rho() const { return (float *)(ws + off.rho); }
+    float *z() const { return (float *)(ws + off.z); }
+    float *what() const { return (float *)(ws + off.what); }
+    float *zpart() const { return (float *)(ws + off.zpart); }
+    mlmd::StepCoef *coef() const { return (mlmd::StepCoef *)(ws + off.coef); }
+    int *flag() const { return (int *)(ws + off.flag); }
+};
+
+namespace mlmd {
+
+// ---- stencil.cu ------------------------------------------------------------------------------
+// One Horner stage without the nonlocal term:
+//   out(r,n) = psi(r,n) + (-i tau) [ sum_{d,j} a_{d,j} w(r + j e_d, n) + (centre + V(r)) w(r,n) ]
+// w, psi, out: [ndom][ngrid][ld] complex64; coef: [ndom] for this step; out may alias psi.
+cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
+                                 const StepCoef *coef, float tau, int *nlaunch);
+
+// ---- gemm_simt.cu ----------------------------------------------------------------------------
+// Projection (S2a): zpart[dom][s][p][c] = sum_{r in slice s} B[dom][r][p] * Y[dom][r][c]
+//   B: [ndom][ngrid][ldb] float (p fastest), Y: [ndom][ngrid][ldy] float, P rows, N columns used.
+cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float *B, int ldb, int P,
+                             const float *Y, int ldy, int N, float *zpart, int prows, int nsplit,
+                             bool fp64, int *nlaunch);
+// Back-application (S2d): Y[dom][r][c] += sum_p B[dom][r][p] * What[dom][p][c]
+cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float *B, int ldb, int P,
+                             const float *What, float *Y, int ldy, int N, int prows, bool fp64,
+                             int *nlaunch);
+
+// ---- glue.cu ---------------------------------------------------------------------------------
+// S2b: reduce split-K partials in fixed order and build What = (-i tau) D' C in real-GEMM form.
+cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows,
+                                int nsplit, const float *zpart, const float *dprime, float tau,
+                                float *what, int *nlaunch);
+// S3: rho[dom][r] = sum_n occ[dom][n] |psi[dom][r][n]|^2
+cudaError_t launch_density(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, const float *occ,
+                           float *rho, int *nlaunch);
+// S4 epilogue: S[dom][m][n] = dv * (sum over splits of the complex combination of Z)
+cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld, int prows, int nsplit,
+                                    const float *zpart, float dv, float2 *S, int *nlaunch);
+// lo = x - trunc_tf32(x): the part of x a TF32 tensor-core operand drops (exact in FP32)
+cudaError_t launch_split_tf32_lo(cudaStream_t st, const float *src, float *lo, size_t n, int *nlaunch);
+cudaError_t launch_max_abs(cudaStream_t st, const float *x, size_t n, int *flag_bits, int *nlaunch);
+cudaError_t launch_check_finite(cudaStream_t st, const float *x, size_t n, int *flag, int *nlaunch);
+
+}  // namespace mlmd
