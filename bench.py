@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py -- electron-steps/s of the domain-batched real-time Kohn-Sham step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--gemm-mode M] [--impl reference]
+
+A "step" is one Taylor-4 time step of EVERY domain of the config: four Horner stages (projection
+GEMM, fused stencil pass, back-application GEMM) plus the density.  The default
+workload is BASELINE.json configs[3] (64 PbTiO3-shaped domains, 48^3 grid, 224 orbitals, 240
+projectors: the "throughput at HBM fill" config the metric is quoted on).  One JSON line is printed
+by rank 0.  See DESIGN.md "Measurement" for the roofline arithmetic.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+PAPER_CONTEXT = {
+    "t2s_s_per_electron_step": 1.11e-7, "sustained_eflops": 1.87, "gpus": 60000,
+    "note": "PAPER.md L38-39, L298, L302: Aurora, 1,024-orbital domains of unstated mesh size; context only",
+}
+MODE_NAMES = {"fp32grade": 0, "fp64": 1, "bf16": 2, "tf32x1": 3, "simt": 4}
+# tensor peak as a multiple of the measured dense BF16 peak (B200_PROFILING.md nominal ratios:
+# tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
+TENSOR_RATIO = {"fp32grade": 0.5 / 3.0, "tf32x1": 0.5, "bf16": 1.0}
+FP32_ALU_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FMA lanes x 2 flop x max SM clock
+FP64_ALU_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12    # nominal 64 DFMA lanes per SM (guide: ~40 TF)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"hbm_gbs": p["hbm_gbs"], "bf16_burst": p["bf16_tflops"],
+                "bf16_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [x.strip() for x in out.strip().split(",")]
+                if len(parts) == 7:
+                    self.rows.append(parts)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.2)
+
+    def summary(self):
+        self.stop_flag.set()
+        self.join(timeout=6)
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[3 + k] == "Active" for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "samples": len(sm),
+                "power_w_max": max(float(r[2]) for r in self.rows), "reasons": reasons}
+
+
+def algorithmic(c, gemm_real=True):
+    """Algorithmic bytes and flops per step of the whole batch."""
+    elems = c.ndom * c.ngrid * c.norb
+    stage_bytes = [16, 24, 24, 24]
+    bytes_step = elems * (sum(stage_bytes) + 8) + c.ndom * c.ngrid * (4 * 4 + 4)
+    gemm_flops_each = (2 if gemm_real else 4) * 2.0 * c.ndom * c.ngrid * c.nproj * c.norb   # one GEMM batch
+    return {"elems": elems, "bytes_step": bytes_step, "stencil_bytes": [elems * b for b in stage_bytes],
+            "density_bytes": elems * 8, "gemm_flops_each": gemm_flops_each, "gemm_flops_step": 8 * gemm_flops_each}
+
+
+def sample_for_oracle(c, d, norb_sample):
+    """Domain 0, first norb_sample orbitals: the bounded sample the oracle is timed on."""
+    n = min(norb_sample, c.norb)
+    return {"psi": np.ascontiguousarray(d["psi"][:1, ..., :n]), "occ": np.ascontiguousarray(d["occ"][:1, :n]),
+            "vloc": d["vloc"][:1], "beta": d["beta"][:1], "D": d["D"][:1]}
+
+
+def time_oracle(c, s, A, steps, warmup):
+    from oracle import ref
+    for _ in range(warmup):
+        ref.propagate(s["psi"], s["occ"], s["vloc"], s["beta"], s["D"], A[:1], c.dt, c.h)
+    t0 = time.perf_counter()
+    psi = s["psi"]
+    for k in range(steps):
+        psi, _ = ref.propagate(psi, s["occ"], s["vloc"], s["beta"], s["D"], A[k:k + 1], c.dt, c.h)
+    dt = time.perf_counter() - t0
+    electrons = float(s["occ"].sum())
+    return electrons * steps / dt, dt / steps, ref.num_threads(), electrons
+
+
+def run_reference(args):
+    """--impl reference: the FP64 oracle, as it stands, on the host cores, on a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    c = W.get_config(args.config)
+    d1 = W.generate_domain(c, 0)
+    d = {k: d1[k][None] for k in ("psi", "occ", "vloc", "beta", "D")}
+    A = W.laser_samples(c, nsteps=max(args.steps, 1))
+    s = sample_for_oracle(c, d, args.oracle_orbitals)
+    value, sec_step, cores, electrons = time_oracle(c, s, A, args.steps, args.warmup)
+    sample = "domain 0 of configs[%d], first %d of %d orbitals (%g electrons), all %d projectors, 1 Taylor-4 step per bench step" % (
+        c.cfg, s["psi"].shape[-1], c.norb, electrons, c.nproj)
+    line = {
+        "impl": "reference", "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(c, args),
+        "cpu_baseline": {"value": value, "unit": "electron-steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "electron-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def workload_config(c, args):
+    return {"workload": "configs[%d] %s: %d domains x %dx%dx%d grid x %d orbitals x %d projectors, dt=%g" % (
+        c.cfg, c.name, c.ndom, *c.grid, c.norb, c.nproj, c.dt),
+        "ndom_per_gpu": c.ndom, "gemm_mode": args.gemm_mode, "gemm_path": getattr(args, "gemm_path", None), "parallelism": "domains sharded, no collective",
+        "l2": "working set (3 x %.1f GB psi buffers + beta) exceeds the 126 MB L2; no flush needed" % (
+            c.ndom * c.ngrid * c.norb * 8 / 1e9) if c.ndom * c.ngrid * c.norb * 8 > 4e8 else
+        "working set may fit L2: a 256 MB buffer is written between timed repetitions"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--ndom", type=int, default=0, help="override the number of domains (debug)")
+    ap.add_argument("--gemm-mode", default="fp32grade", choices=sorted(MODE_NAMES))
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--oracle-orbitals", type=int, default=32)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2509_00966_b200 as M
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libmlmd has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    c = W.get_config(args.config)
+    if args.ndom:
+        c = W.get_config(args.config, ndom=args.ndom)
+    K, Wm = args.steps, args.warmup
+    alg = algorithmic(c)
+    peaks = load_peaks()
+
+    # ---- inputs: seeded per (config, global domain index); generated in a thread pool, staged per domain
+    dev = torch.device("cuda", local)
+    psi_dev = torch.empty((c.ndom, *c.grid, c.norb), dtype=torch.complex64, device=dev)
+    beta_dev = torch.empty((c.ndom, c.ngrid, c.nproj), dtype=torch.float32, device=dev)
+    vloc = np.empty((c.ndom, *c.grid), dtype=np.float32)
+    occ = np.empty((c.ndom, c.norb))
+    D = np.empty((c.ndom, c.nproj))
+    first = {}
+    from concurrent.futures import ThreadPoolExecutor
+    workers = max(1, min(8, (os.cpu_count() or 2) // (2 * max(1, min(world, 8)))))
+    t_gen = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=workers) as ex:
+        for i, dd in enumerate(ex.map(lambda k: W.generate_domain(c, rank * c.ndom + k), range(c.ndom))):
+            psi_dev[i].copy_(torch.from_numpy(dd["psi"]))
+            beta_dev[i].copy_(torch.from_numpy(dd["beta"]))
+            vloc[i], occ[i], D[i] = dd["vloc"], dd["occ"], dd["D"]
+            if i == 0:
+                first = {k: dd[k][None] for k in ("psi", "occ", "vloc", "beta", "D")}
+    t_gen = time.perf_counter() - t_gen
+    A = W.laser_samples(c, nsteps=max(K, Wm, 1), t0=0.9)   # around the pulse maximum: A != 0 in every step
+
+    dom = M.Domain(c.ndom, c.grid, c.h, c.norb, c.nproj, device=str(dev))
+    dom.set_gemm_mode(MODE_NAMES[args.gemm_mode])
+    dom.set_vloc(vloc)
+    dom.set_projectors(beta_dev, D)
+    dom.set_orbitals(psi_dev, occ)
+    del beta_dev
+    stream = dom.stream
+    flush = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device=dev) if alg["elems"] * 8 < 4e8 else None
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up (W steps), then EXACTLY K timed steps in one mlmd_propagate call
+    if Wm > 0:
+        dom.propagate(Wm, c.dt, A)
+    dom.set_orbitals(psi_dev, occ)         # state reset: timed steps start from Psi(0)
+    if flush is not None:
+        flush.fill_(1.0)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    launches0 = dom.launch_count()
+    dom.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    dom.propagate(K, c.dt, A)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    dom.profile(False)
+    launches = dom.launch_count() - launches0
+    gemm_path = dom.gemm_path()
+    args.gemm_path = gemm_path
+    kern = dom.profile_read()
+    clocks = sampler.summary() if sampler else None
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    electrons = c.ndom * c.electrons_per_domain * world
+    value = electrons * K / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: per step the host sends V_loc (PAPER.md L145:
+    # only Delta v_loc goes to the GPU per MD step; Psi stays resident) and A, and reads rho back.
+    e2e = None
+    if not args.no_e2e:
+        vpin = torch.from_numpy(vloc).pin_memory()
+        rpin = torch.empty((c.ndom, *c.grid), dtype=torch.float32).pin_memory()
+        vnp, rnp = vpin.numpy(), rpin.numpy()
+        dom.set_orbitals(psi_dev, occ)
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(K):
+            dom.set_vloc(vnp)
+            dom.propagate(1, c.dt, A[k:k + 1])
+            dom.density(rnp)
+        torch.cuda.synchronize()
+        sec = time.perf_counter() - t0
+        tt = torch.tensor([sec], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        sec = float(tt.item())
+        e2e = {"value": electrons * K / sec, "unit": "electron-steps/s", "h2d_bytes_per_step": int(vnp.nbytes + 24),
+               "d2h_bytes_per_step": int(rnp.nbytes), "ms_per_step": sec / K * 1e3,
+               "what": "per step: mlmd_set_vloc(host pinned) + mlmd_propagate(1, A host) + mlmd_density(host pinned); "
+                       "Psi stays device-resident as in the paper's shadow dynamics (L130-132, L145)"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel class and of the whole step
+    mode = args.gemm_mode
+    tensor_peak_sus = peaks["bf16_sustained"] * TENSOR_RATIO.get(mode, TENSOR_RATIO["fp32grade"])
+    tensor_peak_burst = peaks["bf16_burst"] * TENSOR_RATIO.get(mode, TENSOR_RATIO["fp32grade"])
+    per_class = {}
+    total_kernel_ms = sum(v[0] for v in kern.values()) or 1.0
+    for name, (kms, n) in kern.items():
+        avg = kms / n
+        entry = {"ms_total": kms, "launches": n, "ms_avg": avg, "share": kms / total_kernel_ms}
+        if name == "stencil":
+            b = sum(alg["stencil_bytes"]) / 4.0
+            entry.update(bound="hbm", achieved=b / (avg * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
+        elif name == "density":
+            entry.update(bound="hbm", achieved=alg["density_bytes"] / (avg * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
+        elif name in ("proj", "back", "nlp"):
+            fl = alg["gemm_flops_each"] * (2 if name == "nlp" else 1)
+            if gemm_path == "simt":
+                pk = FP64_ALU_TFLOPS if mode == "fp64" else FP32_ALU_TFLOPS
+                entry.update(bound="alu", achieved=fl / (avg * 1e-3) / 1e12, peak=pk, unit="TFLOP/s")
+            else:
+                entry.update(bound="tensor", achieved=fl / (avg * 1e-3) / 1e12, peak=tensor_peak_sus, unit="TFLOP/s")
+        if "achieved" in entry:
+            entry["frac"] = entry["achieved"] / entry["peak"]
+        per_class[name] = entry
+    top = max((n for n in per_class if "achieved" in per_class[n]), key=lambda n: per_class[n]["ms_total"])
+    roof = {k: per_class[top][k] for k in ("bound", "achieved", "peak", "unit", "frac")}
+    roof.update(kernel=top, traffic=None, peak_source="%s (%s)" % (
+        "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
+        "hbm copy" if roof["bound"] == "hbm" else
+        "sustained bf16 x nominal ratio for the mode" if roof["bound"] == "tensor" else "derived FP32/FP64 ALU peak, DESIGN.md"))
+    t_hbm = alg["bytes_step"] / (peaks["hbm_gbs"] * 1e9) * 1e3
+    t_tc = alg["gemm_flops_step"] / (tensor_peak_sus * 1e12) * 1e3
+    t_roof = max(t_hbm, t_tc)
+    step_roof = {"t_hbm_ms": t_hbm, "t_tensor_ms": t_tc, "t_roof_ms": t_roof, "bound": "tensor" if t_tc > t_hbm else "hbm",
+                 "frac": t_roof / (ms / K), "tensor_peak_tflops": tensor_peak_sus, "tensor_peak_burst_tflops": tensor_peak_burst,
+                 "hbm_peak_gbs": peaks["hbm_gbs"], "bytes_step": alg["bytes_step"], "gemm_flops_step": alg["gemm_flops_step"],
+                 "definition": "max(stencil+density bytes / HBM peak, real-beta GEMM flops / tensor peak of the GEMM mode)"}
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        s = sample_for_oracle(c, first, args.oracle_orbitals)
+        v, sec_step, cores, el = time_oracle(c, s, A, steps=2, warmup=1)
+        cpu = {"value": v, "unit": "electron-steps/s", "cores": cores, "kind": "oracle", "s_per_step": sec_step,
+               "sample": "domain 0, first %d of %d orbitals (%g electrons), all %d projectors, 2 timed Taylor-4 steps" % (
+                   s["psi"].shape[-1], c.norb, el, c.nproj)}
+
+    line = {
+        "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "complex64",
+        "data": "synthetic", "config": workload_config(c, args), "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+        "roofline": roof, "cpu_baseline": cpu, "step_roofline": step_roof, "kernels": per_class,
+        "orbital_steps_per_s": c.ndom * c.norb * world * K / (ms * 1e-3), "input_generation_s": t_gen,
+        "paper_context": PAPER_CONTEXT,
+    }
+    print(json.dumps(line))
+    dom.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

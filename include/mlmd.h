@@ -114,6 +114,19 @@ int mlmd_density(mlmd_domain_t *h, float *rho, int where);
  * Always evaluated in the FP32-grade (or FP64) GEMM mode: it is a measurement. */
 int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
 
+/* Per-kernel-class timing of mlmd_propagate with CUDA events on the handle's stream (bench.py's
+ * roofline numbers).  mlmd_profile(h, 1) starts recording (and clears earlier records),
+ * mlmd_profile(h, 0) stops.  mlmd_profile_read synchronises the stream and returns the summed
+ * device time in milliseconds and the number of launches of class `kind` recorded so far. */
+enum { MLMD_K_STENCIL = 0, MLMD_K_PROJ = 1, MLMD_K_BACK = 2, MLMD_K_GLUE = 3, MLMD_K_DENSITY = 4,
+       MLMD_K_NLP = 5 /* fused back-application + projection */, MLMD_K_COUNT = 6 };
+int mlmd_profile(mlmd_domain_t *h, int enable);
+int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *launches);
+
+/* Which kernels run the nonlocal GEMMs for the current mode and shape: 0 = CUDA cores (SIMT),
+ * 1 = tcgen05 tensor cores. */
+int mlmd_gemm_path(const mlmd_domain_t *h);
+
 /* Number of kernels the library launched on this handle since create (bench.py's gpu_launches). */
 long long mlmd_launch_count(const mlmd_domain_t *h);
 

@@ -21,6 +21,9 @@ from .api import (  # noqa: F401
     mlmd_density,
     mlmd_overlap,
     mlmd_launch_count,
+    mlmd_profile,
+    mlmd_profile_read,
+    KERNEL_CLASSES,
     mlmd_last_error,
     EXPORTED_SYMBOLS,
     HOST, DEVICE, BETA_REAL32, BETA_COMPLEX64,

@@ -24,8 +24,10 @@ KEEP_PSI0, CHECK_FINITE = 1, 2
 EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",
     "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_propagate",
-    "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error",
+    "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
 ]
+K_STENCIL, K_PROJ, K_BACK, K_GLUE, K_DENSITY, K_NLP = range(6)
+KERNEL_CLASSES = ["stencil", "proj", "back", "glue", "density", "nlp"]
 
 
 class MlmdError(RuntimeError):
@@ -58,11 +60,14 @@ def lib() -> ctypes.CDLL:
         L.mlmd_propagate.argtypes = [p, i, d, p, i]
         L.mlmd_density.argtypes = [p, p, i]
         L.mlmd_overlap.argtypes = [p, i, p, i]
+        L.mlmd_profile.argtypes = [p, i]
+        L.mlmd_profile_read.argtypes = [p, i, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)]
         L.mlmd_launch_count.argtypes = [p]
+        L.mlmd_gemm_path.argtypes = [p]
         L.mlmd_launch_count.restype = ctypes.c_longlong
         L.mlmd_last_error.restype = ctypes.c_char_p
         for name in EXPORTED_SYMBOLS:
-            if name not in ("mlmd_workspace_bytes", "mlmd_launch_count", "mlmd_last_error"):
+            if name not in ("mlmd_workspace_bytes", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile_read"):
                 getattr(L, name).restype = i
         _lib = L
     return _lib
@@ -175,6 +180,17 @@ def mlmd_overlap(h, which, out):
     return out
 
 
+def mlmd_profile(h, enable: bool):
+    _check(lib().mlmd_profile(h, 1 if enable else 0))
+
+
+def mlmd_profile_read(h, kind: int):
+    """(milliseconds summed over launches, number of launches) of kernel class `kind`."""
+    ms, n = ctypes.c_double(), ctypes.c_longlong()
+    _check(lib().mlmd_profile_read(h, kind, ctypes.byref(ms), ctypes.byref(n)))
+    return ms.value, n.value
+
+
 def mlmd_launch_count(h) -> int:
     return int(lib().mlmd_launch_count(h))
 
@@ -242,6 +258,21 @@ class Domain:
         if out is None:
             out = np.empty((self.ndom, self.norb, self.norb), dtype=np.complex64)
         return mlmd_overlap(self.handle, which, out)
+
+    def profile(self, enable=True):
+        mlmd_profile(self.handle, enable)
+
+    def profile_read(self):
+        """{class name: (ms_total, launches)} for the classes that ran."""
+        out = {}
+        for k, name in enumerate(KERNEL_CLASSES):
+            ms, n = mlmd_profile_read(self.handle, k)
+            if n:
+                out[name] = (ms, n)
+        return out
+
+    def gemm_path(self):
+        return "tcgen05" if lib().mlmd_gemm_path(self.handle) else "simt"
 
     def launch_count(self):
         return mlmd_launch_count(self.handle)

@@ -122,7 +122,7 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
-    h->coef_host = nullptr; h->flag_host = nullptr;
+    h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
     cudaError_t e = cudaMallocHost((void **)&h->coef_host, (size_t)kCoefCapacity * ndom * sizeof(StepCoef));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&h->flag_host, 256);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->occ(), 0, (size_t)ndom * h->ld * sizeof(float), h->stream);
@@ -141,11 +141,44 @@ int mlmd_domain_destroy(mlmd_domain_t *h) {
     cudaStreamSynchronize(h->stream);
     if (h->coef_host) cudaFreeHost(h->coef_host);
     if (h->flag_host) cudaFreeHost(h->flag_host);
+    for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
     delete h;
     return MLMD_OK;
 }
 
+int mlmd_profile(mlmd_domain_t *h, int enable) {
+    if (!h) return fail(MLMD_ERR_ARG, "mlmd_profile: NULL handle");
+    h->prof_on = enable != 0;
+    if (enable) h->prof_recs.clear();
+    return MLMD_OK;
+}
+
+int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *launches) {
+    if (!h || !ms_total || !launches) return fail(MLMD_ERR_ARG, "mlmd_profile_read: NULL argument");
+    if (kind < 0 || kind >= MLMD_K_COUNT) return fail(MLMD_ERR_ARG, "mlmd_profile_read: kind=%d", kind);
+    CU(cudaStreamSynchronize(h->stream));
+    double ms = 0.0;
+    long long n = 0;
+    for (const auto &r : h->prof_recs) {
+        if (r.kind != kind) continue;
+        float t = 0.f;
+        CU(cudaEventElapsedTime(&t, h->prof_pool[r.e0], h->prof_pool[r.e1]));
+        ms += t;
+        ++n;
+    }
+    *ms_total = ms;
+    *launches = n;
+    return MLMD_OK;
+}
+
 long long mlmd_launch_count(const mlmd_domain_t *h) { return h ? h->launches : 0; }
+
+static bool use_tensor_cores(const mlmd_domain *h) {
+    (void)h;
+    return false;   // the tcgen05 GEMM path is selected here once it exists
+}
+
+int mlmd_gemm_path(const mlmd_domain_t *h) { return (h && use_tensor_cores(h)) ? 1 : 0; }
 
 static cudaMemcpyKind kind_in(int where) { return where == MLMD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice; }
 static cudaMemcpyKind kind_out(int where) { return where == MLMD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice; }
@@ -260,6 +293,27 @@ int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
 }
 
 // ---- the step --------------------------------------------------------------------------------
+// RAII pair of events around one kernel launch when mlmd_profile is on.
+struct ProfScope {
+    mlmd_domain *h;
+    int rec;
+    ProfScope(mlmd_domain *hh, int kind) : h(hh), rec(-1) {
+        if (!h->prof_on || h->prof_recs.size() >= (1u << 16)) return;
+        const size_t need = 2 * (h->prof_recs.size() + 1);
+        while (h->prof_pool.size() < need) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return;
+            h->prof_pool.push_back(e);
+        }
+        rec = (int)h->prof_recs.size();
+        h->prof_recs.push_back({kind, 2 * rec, 2 * rec + 1});
+        cudaEventRecord(h->prof_pool[2 * rec], h->stream);
+    }
+    ~ProfScope() {
+        if (rec >= 0) cudaEventRecord(h->prof_pool[2 * rec + 1], h->stream);
+    }
+};
+
 static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
     // SURVEY.md 8(a) S1; weights of the 4th-order central differences (north_star)
     static const double c2[2] = {4.0 / 3.0, -1.0 / 12.0};   // j = 1, 2  (symmetric)
@@ -280,8 +334,12 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
 static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl) {
     // S2a + S2b: What = (-i tau) D' (beta^H w)
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
-    CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, (const float *)w, 2 * h->ld, 2 * h->ld,
-                        h->zpart(), h->prows, h->nsplit, fp64, nl));
+    {
+        ProfScope ps(h, MLMD_K_PROJ);
+        CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, (const float *)w, 2 * h->ld, 2 * h->ld,
+                            h->zpart(), h->prows, h->nsplit, fp64, nl));
+    }
+    ProfScope ps(h, MLMD_K_GLUE);
     CU(launch_reduce_scale(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, h->nsplit, h->zpart(),
                            h->dprime(), tau, h->what(), nl));
     return MLMD_OK;
@@ -289,6 +347,7 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl)
 
 static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl) {
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
+    ProfScope ps(h, MLMD_K_BACK);
     CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, h->what(), (float *)out, 2 * h->ld,
                         2 * h->ld, h->prows, fp64, nl));
     return MLMD_OK;
@@ -333,12 +392,16 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
                     int rc = nonlocal_project(h, src[i], tau, &nl);
                     if (rc) return rc;
                 }
-                CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, tau, &nl));
+                {
+                    ProfScope ps(h, MLMD_K_STENCIL);
+                    CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, tau, &nl));
+                }
                 if (h->nproj > 0) {
                     int rc = nonlocal_back(h, dst[i], &nl);
                     if (rc) return rc;
                 }
             }
+            ProfScope ps(h, MLMD_K_DENSITY);
             CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), &nl));
         }
     }

@@ -4,6 +4,8 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/mlmd.h"
 
 namespace mlmd {
@@ -51,6 +53,11 @@ struct mlmd_domain {
     bool field_yz;              // any A_y or A_z non-zero in the current propagate call
     double vmax, dmax;
     long long launches;
+    // per-kernel-class CUDA-event records (mlmd_profile)
+    bool prof_on;
+    std::vector<cudaEvent_t> prof_pool;
+    struct ProfRec { int kind; int e0, e1; };
+    std::vector<ProfRec> prof_recs;
     mlmd::StepCoef *coef_host;  // pinned, kCoefCapacity * ndom
     int *flag_host;             // pinned
     // typed views

@@ -1,0 +1,81 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/mlmd.h declares,
+sizes workspaces sanely and fails loudly (no fallback) when there is no B200."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def M():
+    from paper_2509_00966_b200 import build
+    build.build()
+    import paper_2509_00966_b200 as M
+    return M
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "mlmd.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mlmd_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(M):
+    L = ctypes.CDLL(M.api.LIB_PATH)
+    names = declared_functions()
+    assert len(names) >= 13
+    for n in names:
+        assert hasattr(L, n), n
+    assert sorted(M.EXPORTED_SYMBOLS) == names
+
+
+def test_workspace_bytes(M):
+    wb = M.mlmd_workspace_bytes
+    assert wb(1, 4, 16, 16, 8, 8) == 0 and wb(0, 16, 16, 16, 8, 8) == 0 and wb(1, 16, 16, 16, 0, 8) == 0
+    small = wb(1, 16, 16, 16, 8, 8)
+    assert small >= 3 * 4096 * 8 * 8
+    assert wb(2, 16, 16, 16, 8, 8) > small and wb(1, 16, 16, 16, 8, 8, M.KEEP_PSI0) >= small + 4096 * 8 * 8
+    # configs[3] and configs[4] fit one B200's 180 GB
+    assert wb(64, 48, 48, 48, 224, 240) < 100e9 and wb(4, 64, 64, 64, 696, 810) < 100e9
+    psi3 = 64 * 48 ** 3 * 224 * 8
+    assert wb(64, 48, 48, 48, 224, 240) >= 3 * psi3
+
+
+def test_no_cpu_fallback(M):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(M.MlmdError) as e:
+        M.mlmd_domain_create(1, 16, 16, 16, 0.5, 0.5, 0.5, 8, 8, 256, 10 ** 9)
+    assert e.value.code == M.api.ERR_CUDA
+    with pytest.raises(M.MlmdError):
+        M.Domain(1, (16, 16, 16), (0.5, 0.5, 0.5), 8, 8)
+
+
+def test_argument_errors_without_gpu(M):
+    L = M.lib()
+    assert L.mlmd_propagate(None, 1, 0.02, None, 1) == M.api.ERR_ARG
+    assert b"NULL" in L.mlmd_last_error()
+    h = ctypes.c_void_p()
+    assert L.mlmd_domain_create(ctypes.byref(h), 1, 16, 16, 16, 0.5, 0.5, 0.5, 8, 8, None, 0, None, 0) == M.api.ERR_ARG
+    assert L.mlmd_domain_create(ctypes.byref(h), 1, 16, 16, 3, 0.5, 0.5, 0.5, 8, 8, ctypes.c_void_p(256), 1 << 30, None, 0) == M.api.ERR_SHAPE
+    assert L.mlmd_domain_destroy(None) == M.api.OK
+    assert M.mlmd_launch_count(None) == 0
+
+
+def test_product_does_not_import_oracle():
+    """The oracle is test infrastructure: nothing under the package may import or load it."""
+    pkg = os.path.join(ROOT, "paper_2509_00966_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh", ".cpp")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in text and "mlmd_ref" not in text, os.path.join(dirpath, f)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2509_00966_b200 import" not in text and "libmlmd.so" not in text

@@ -17,6 +17,7 @@ from dataclasses import dataclass, replace
 from typing import Dict, Optional, Tuple
 
 import numpy as np
+import scipy.linalg
 
 SEED_ROOT = 966
 A_LATTICE = 7.4  # bohr, cubic perovskite cell (BASELINE.json configs[2])
@@ -189,7 +190,10 @@ def _orbitals(c: DomainConfig, dom: int):
         mask = (KX * KX + KY * KY + KZ * KZ) <= c.smooth_kcut ** 2
         gk *= mask[..., None]
         g = np.fft.ifftn(gk, axes=(0, 1, 2)).reshape(c.ngrid, c.norb)
-    q, _ = np.linalg.qr(g)
+    # thin QR with positive-diagonal R, computed through the Cholesky factor of the Gram matrix
+    # (same Q as Householder QR up to rounding; ~10x faster for these well-conditioned tall matrices)
+    low = np.linalg.cholesky(g.conj().T @ g)
+    q = scipy.linalg.solve_triangular(low, g.conj().T, lower=True, overwrite_b=True, check_finite=False).conj().T
     return q / np.sqrt(c.dv)
 
 
@@ -226,9 +230,16 @@ def generate_domain(c: DomainConfig, dom: int) -> Dict[str, np.ndarray]:
     }
 
 
-def generate(c: DomainConfig) -> Dict[str, np.ndarray]:
-    """Stack ``generate_domain`` over all ``c.ndom`` domains and add the laser samples."""
-    doms = [generate_domain(c, d) for d in range(c.ndom)]
+def generate(c: DomainConfig, workers: int = 1) -> Dict[str, np.ndarray]:
+    """Stack ``generate_domain`` over all ``c.ndom`` domains and add the laser samples.
+    ``workers`` > 1 builds domains in a thread pool (numpy's RNG, BLAS and LAPACK release the GIL);
+    the result does not depend on it because every domain has its own seed."""
+    if workers > 1 and c.ndom > 1:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=workers) as ex:
+            doms = list(ex.map(lambda d: generate_domain(c, d), range(c.ndom)))
+    else:
+        doms = [generate_domain(c, d) for d in range(c.ndom)]
     out = {k: np.stack([d[k] for d in doms], axis=0) for k in ("psi", "occ", "vloc", "beta", "D")}
     out["A"] = laser_samples(c)
     return out
