@@ -33,7 +33,7 @@ static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 static int round_up_i(int x, int a) { return (x + a - 1) / a * a; }
 
 struct Plan {
-    int ld, ldp_max, prows, nsplit;
+    int ld, ldp_max, prows, nsplit, nsplit_tc, nsplit_tc_ovl;
     long ngrid;
     Workspace off;
 };
@@ -41,14 +41,16 @@ struct Plan {
 static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max, unsigned flags, Plan *pl) {
     if (ndom < 1 || nx < 5 || ny < 5 || nz < 5 || norb < 1 || nproj_max < 0) return false;
     if ((double)ndom * nx * ny * nz > 2.0e9) return false;
-    pl->ld = round_up_i(norb, 8);
+    pl->ld = round_up_i(norb, 16);      // 2*ld floats per row = whole 128-byte TMA chunks
     pl->ngrid = (long)nx * ny * nz;
-    pl->ldp_max = round_up_i(std::max(nproj_max, 1), 4);
+    pl->ldp_max = round_up_i(std::max(nproj_max, 1), 8);
     pl->prows = std::max(pl->ldp_max, 2 * pl->ld);
     const long tiles = (long)((2 * pl->ld + 63) / 64) * std::max(1, (nproj_max + 63) / 64) * ndom;
     long ns = (592 + tiles - 1) / tiles;
     ns = std::min<long>(ns, std::min<long>(kMaxSplit, pl->ngrid / 64));
     pl->nsplit = (int)std::max<long>(ns, 1);
+    pl->nsplit_tc = tc_choose_nsplit(ndom, pl->ngrid, pl->ldp_max, 2 * pl->ld);
+    pl->nsplit_tc_ovl = tc_choose_nsplit(ndom, pl->ngrid, 2 * pl->ld, 2 * pl->ld);
     const size_t npts = (size_t)ndom * pl->ngrid;
     const size_t psi_b = npts * pl->ld * sizeof(float2);
     size_t o = 0;
@@ -63,15 +65,17 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.ub = take(psi_b);
     w.psi0 = take((flags & MLMD_KEEP_PSI0) ? psi_b : 0);
     w.vloc = take(npts * sizeof(float));
-    w.beta = take(npts * pl->ldp_max * sizeof(float));
-    w.beta_lo = take(npts * pl->ldp_max * sizeof(float));
+    // + slack: the last 32-column TMA chunk of a row may read up to 128 B past the row
+    w.beta = take(npts * pl->ldp_max * sizeof(float) + 256);
+    w.beta_lo = take(npts * pl->ldp_max * sizeof(float) + 256);
     w.dprime = take((size_t)ndom * pl->ldp_max * sizeof(float));
     w.occ = take((size_t)ndom * pl->ld * sizeof(float));
     w.rho = take(npts * sizeof(float));
     const size_t zb = (size_t)ndom * pl->prows * 2 * pl->ld * sizeof(float);
     w.z = take(zb);
     w.what = take(zb);
-    w.zpart = take(zb * pl->nsplit);
+    w.what_lo = take(zb);
+    w.zpart = take(zb * std::max(pl->nsplit, std::max(pl->nsplit_tc, pl->nsplit_tc_ovl)));
     w.coef = take((size_t)kCoefCapacity * ndom * sizeof(StepCoef));
     w.flag = take(256);
     w.total = o;
@@ -119,6 +123,11 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->stream = (cudaStream_t)cuda_stream;
     h->ws = (char *)workspace_dev; h->ws_bytes = workspace_bytes; h->off = pl.off;
     h->nproj = 0; h->beta_complex = 0; h->P = 0; h->ldp = pl.ldp_max; h->prows = pl.prows; h->nsplit = pl.nsplit;
+    h->nsplit_tc = pl.nsplit_tc; h->nsplit_tc_ovl = pl.nsplit_tc_ovl;
+    {
+        const char *force = getenv("MLMD_GEMM_PATH");   // "simt": keep the GEMMs on CUDA cores (A/B checks)
+        h->tc_ok = tc_available() && pl.ngrid % 128 == 0 && !(force && strcmp(force, "simt") == 0);
+    }
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
@@ -126,6 +135,8 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     cudaError_t e = cudaMallocHost((void **)&h->coef_host, (size_t)kCoefCapacity * ndom * sizeof(StepCoef));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&h->flag_host, 256);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->occ(), 0, (size_t)ndom * h->ld * sizeof(float), h->stream);
+    // rows >= P of W are read (times zero columns of beta) by the K = 8 slabs of the back-application
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->what(), 0, 2 * (pl.off.what_lo - pl.off.what), h->stream);
     if (e != cudaSuccess) {
         if (h->coef_host) cudaFreeHost(h->coef_host);
         if (h->flag_host) cudaFreeHost(h->flag_host);
@@ -174,8 +185,7 @@ int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *l
 long long mlmd_launch_count(const mlmd_domain_t *h) { return h ? h->launches : 0; }
 
 static bool use_tensor_cores(const mlmd_domain *h) {
-    (void)h;
-    return false;   // the tcgen05 GEMM path is selected here once it exists
+    return h->tc_ok && (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_TF32X1);
 }
 
 int mlmd_gemm_path(const mlmd_domain_t *h) { return (h && use_tensor_cores(h)) ? 1 : 0; }
@@ -265,7 +275,7 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
         return fail(MLMD_ERR_SHAPE, "mlmd_set_projectors: %d %s projectors need %d real rows, handle was created with "
                     "nproj_max=%d", nproj, cplx ? "complex" : "real", P, h->nproj_max);
     const size_t rows = (size_t)h->ndom * h->ngrid;
-    const int ldp = round_up_i(P, 4);
+    const int ldp = round_up_i(P, 8);
     std::vector<float> dp((size_t)h->ndom * nproj);
     double dmax = 0.0;
     for (size_t i = 0; i < dp.size(); ++i) {
@@ -278,7 +288,7 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
     CU(cudaMemcpy2DAsync(h->beta(), (size_t)ldp * sizeof(float), beta, (size_t)P * sizeof(float), (size_t)P * sizeof(float),
                          rows, kind_in(where), h->stream));
     int nl = 0;
-    CU(launch_split_tf32_lo(h->stream, h->beta(), h->beta_lo(), rows * ldp, &nl));
+    CU(launch_split_tf32(h->stream, h->beta(), h->beta_lo(), rows * ldp, &nl));
     h->launches += nl;
     CU(cudaStreamSynchronize(h->stream));   // dp is a temporary; host beta may be reused by the caller
     h->nproj = nproj; h->beta_complex = cplx; h->P = P; h->ldp = ldp; h->dmax = dmax;
@@ -334,22 +344,32 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
 static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl) {
     // S2a + S2b: What = (-i tau) D' (beta^H w)
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
+    const bool tc = use_tensor_cores(h);
+    const int nsplit = tc ? h->nsplit_tc : h->nsplit;
     {
         ProfScope ps(h, MLMD_K_PROJ);
-        CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, (const float *)w, 2 * h->ld, 2 * h->ld,
-                            h->zpart(), h->prows, h->nsplit, fp64, nl));
+        if (tc)
+            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, h->gemm_mode == MLMD_GEMM_TF32X1 ? 1 : 3, nl));
+        else
+            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
+                                2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
     }
     ProfScope ps(h, MLMD_K_GLUE);
-    CU(launch_reduce_scale(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, h->nsplit, h->zpart(),
-                           h->dprime(), tau, h->what(), nl));
+    CU(launch_reduce_scale(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, nsplit, h->zpart(),
+                           h->dprime(), tau, h->what(), h->what_lo(), nl));
     return MLMD_OK;
 }
 
 static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl) {
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     ProfScope ps(h, MLMD_K_BACK);
-    CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, h->what(), (float *)out, 2 * h->ld,
-                        2 * h->ld, h->prows, fp64, nl));
+    if (use_tensor_cores(h))
+        CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
+                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, h->gemm_mode == MLMD_GEMM_TF32X1 ? 1 : 3, nl));
+    else
+        CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
+                            (float *)out, 2 * h->ld, 2 * h->ld, h->prows, fp64, nl));
     return MLMD_OK;
 }
 
@@ -446,11 +466,18 @@ int mlmd_overlap(mlmd_domain_t *h, int which, void *S, int where) {
     const float2 *phi = which == 0 ? h->psi() : h->psi0();
     int nl = 0;
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
-    // projection GEMM with B := float view of Phi (2*ld real rows), S4 of SURVEY.md 8(a)
-    CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, (const float *)phi, 2 * h->ld, 2 * h->ld, (const float *)h->psi(),
-                        2 * h->ld, 2 * h->ld, h->zpart(), h->prows, h->nsplit, fp64, &nl));
+    // projection GEMM with B := float view of Phi (2*ld real rows), S4 of SURVEY.md 8(a); always
+    // FP32-grade (3xTF32 on tensor cores, or the CUDA-core path): it is a measurement
+    const bool tc = h->tc_ok && h->gemm_mode != MLMD_GEMM_FP64 && h->gemm_mode != MLMD_GEMM_FP32_SIMT;
+    const int nsplit = tc ? h->nsplit_tc_ovl : h->nsplit;
+    if (tc)
+        CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, (const float *)phi, nullptr, 2 * h->ld, 2 * h->ld,
+                          (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, 3, &nl));
+    else
+        CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, (const float *)phi, nullptr, 2 * h->ld, 2 * h->ld,
+                            (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, &nl));
     float2 *sdev = where == MLMD_DEVICE ? (float2 *)S : (float2 *)h->z();
-    CU(launch_overlap_epilogue(h->stream, h->ndom, h->norb, h->ld, h->prows, h->nsplit, h->zpart(), (float)h->dv, sdev, &nl));
+    CU(launch_overlap_epilogue(h->stream, h->ndom, h->norb, h->ld, h->prows, nsplit, h->zpart(), (float)h->dv, sdev, &nl));
     h->launches += nl;
     if (where == MLMD_HOST) {
         CU(cudaMemcpyAsync(S, sdev, (size_t)h->ndom * h->norb * h->norb * sizeof(float2), cudaMemcpyDeviceToHost, h->stream));

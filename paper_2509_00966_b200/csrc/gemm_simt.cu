@@ -16,14 +16,15 @@ constexpr int TM = 64, TN = 64, TK = 16;
 
 template <typename Acc>
 __global__ void __launch_bounds__(256)
-proj_simt_kernel(long ngrid, const float *__restrict__ B, int ldb, int P, const float *__restrict__ Y, int ldy,
-                 int N, float *__restrict__ zpart, int prows, int nsplit) {
+proj_simt_kernel(long ngrid, const float *__restrict__ B, const float *__restrict__ Blo, int ldb, int P,
+                 const float *__restrict__ Y, int ldy, int N, float *__restrict__ zpart, int prows, int nsplit) {
     __shared__ float Bs[TK][TM + 4];
     __shared__ float Ys[TK][TN + 4];
     const int dom = blockIdx.z / nsplit, split = blockIdx.z % nsplit;
     const int p0 = blockIdx.y * TM, c0 = blockIdx.x * TN;
     const long rlo = ngrid * split / nsplit, rhi = ngrid * (split + 1) / nsplit;
     const float *Bd = B + (size_t)dom * ngrid * ldb;
+    const float *Bl = Blo ? Blo + (size_t)dom * ngrid * ldb : nullptr;   // B = hi + lo (exact)
     const float *Yd = Y + (size_t)dom * ngrid * ldy;
     const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
     Acc acc[4][4];
@@ -39,7 +40,7 @@ proj_simt_kernel(long ngrid, const float *__restrict__ B, int ldb, int P, const 
             const int kk = idx / 64, cc = idx % 64;
             const long r = r0 + kk;
             const bool rok = r < rhi;
-            Bs[kk][cc] = (rok && p0 + cc < P) ? Bd[r * ldb + p0 + cc] : 0.f;
+            Bs[kk][cc] = (rok && p0 + cc < P) ? (Bl ? Bd[r * ldb + p0 + cc] + Bl[r * ldb + p0 + cc] : Bd[r * ldb + p0 + cc]) : 0.f;
             Ys[kk][cc] = (rok && c0 + cc < N) ? Yd[r * ldy + c0 + cc] : 0.f;
         }
         __syncthreads();
@@ -72,15 +73,18 @@ proj_simt_kernel(long ngrid, const float *__restrict__ B, int ldb, int P, const 
 
 template <typename Acc>
 __global__ void __launch_bounds__(256)
-back_simt_kernel(long ngrid, const float *__restrict__ B, int ldb, int P, const float *__restrict__ What,
-                 float *__restrict__ Y, int ldy, int N, int prows) {
+back_simt_kernel(long ngrid, const float *__restrict__ B, const float *__restrict__ Blo, int ldb, int P,
+                 const float *__restrict__ What, const float *__restrict__ Wlo, float *__restrict__ Y, int ldy, int N,
+                 int prows) {
     __shared__ float As[TK][TM + 4];   // As[k][r]
     __shared__ float Ws[TK][TN + 4];
     const int dom = blockIdx.z;
     const long r0 = (long)blockIdx.y * TM;
     const int c0 = blockIdx.x * TN;
     const float *Bd = B + (size_t)dom * ngrid * ldb;
+    const float *Bl = Blo + (size_t)dom * ngrid * ldb;     // operands are stored as exact hi + lo pairs
     const float *Wd = What + (size_t)dom * prows * N;
+    const float *Wl = Wlo + (size_t)dom * prows * N;
     float *Yd = Y + (size_t)dom * ngrid * ldy;
     const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
     Acc acc[4][4];
@@ -95,11 +99,11 @@ back_simt_kernel(long ngrid, const float *__restrict__ B, int ldb, int P, const 
             {   // A tile: 64 rows x 16 k; consecutive threads walk k (contiguous in memory)
                 const int rr = idx / 16, kk = idx % 16;
                 const long r = r0 + rr;
-                As[kk][rr] = (r < ngrid && k0 + kk < P) ? Bd[r * ldb + k0 + kk] : 0.f;
+                As[kk][rr] = (r < ngrid && k0 + kk < P) ? Bd[r * ldb + k0 + kk] + Bl[r * ldb + k0 + kk] : 0.f;
             }
             {
                 const int kk = idx / 64, cc = idx % 64;
-                Ws[kk][cc] = (k0 + kk < P && c0 + cc < N) ? Wd[(size_t)(k0 + kk) * N + c0 + cc] : 0.f;
+                Ws[kk][cc] = (k0 + kk < P && c0 + cc < N) ? Wd[(size_t)(k0 + kk) * N + c0 + cc] + Wl[(size_t)(k0 + kk) * N + c0 + cc] : 0.f;
             }
         }
         __syncthreads();
@@ -129,27 +133,27 @@ back_simt_kernel(long ngrid, const float *__restrict__ B, int ldb, int P, const 
     }
 }
 
-cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float *B, int ldb, int P,
+cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
                              const float *Y, int ldy, int N, float *zpart, int prows, int nsplit,
                              bool fp64, int *nlaunch) {
     dim3 grid((N + TN - 1) / TN, (P + TM - 1) / TM, ndom * nsplit);
     ++*nlaunch;
     if (fp64)
-        proj_simt_kernel<double><<<grid, 256, 0, st>>>(ngrid, B, ldb, P, Y, ldy, N, zpart, prows, nsplit);
+        proj_simt_kernel<double><<<grid, 256, 0, st>>>(ngrid, B, Blo, ldb, P, Y, ldy, N, zpart, prows, nsplit);
     else
-        proj_simt_kernel<float><<<grid, 256, 0, st>>>(ngrid, B, ldb, P, Y, ldy, N, zpart, prows, nsplit);
+        proj_simt_kernel<float><<<grid, 256, 0, st>>>(ngrid, B, Blo, ldb, P, Y, ldy, N, zpart, prows, nsplit);
     return cudaGetLastError();
 }
 
-cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float *B, int ldb, int P,
-                             const float *What, float *Y, int ldy, int N, int prows, bool fp64,
+cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
+                             const float *What, const float *Wlo, float *Y, int ldy, int N, int prows, bool fp64,
                              int *nlaunch) {
     dim3 grid((N + TN - 1) / TN, (unsigned)((ngrid + TM - 1) / TM), ndom);
     ++*nlaunch;
     if (fp64)
-        back_simt_kernel<double><<<grid, 256, 0, st>>>(ngrid, B, ldb, P, What, Y, ldy, N, prows);
+        back_simt_kernel<double><<<grid, 256, 0, st>>>(ngrid, B, Blo, ldb, P, What, Wlo, Y, ldy, N, prows);
     else
-        back_simt_kernel<float><<<grid, 256, 0, st>>>(ngrid, B, ldb, P, What, Y, ldy, N, prows);
+        back_simt_kernel<float><<<grid, 256, 0, st>>>(ngrid, B, Blo, ldb, P, What, Wlo, Y, ldy, N, prows);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,535 @@
+// tcgen05 tensor-core GEMMs of the nonlocal operator (north_star kernel 3).
+//
+// Complex GEMMs run as REAL GEMMs on the interleaved storage:
+//   projection        Z[p][c]  = sum_r B[r][p] * Y[r][c]        K = grid points   (PAPER.md L283 CGEMM(1))
+//   back-application  Y[r][c] += sum_p B[r][p] * W[p][c]        K = projector rows (PAPER.md L283 CGEMM(2))
+// with Y the float view [ngrid][2*ld] of a psi-like buffer and B the float view of beta.
+//
+// Operands are staged by TMA (cp.async.bulk.tensor, SWIZZLE_128B_ATOM_32B) straight from their natural
+// row-major HBM layouts: a [rows x 32 floats] box IS one column-chunk of the canonical UMMA
+// MN-major SWIZZLE_128B_BASE32B layout (K = rows), so neither GEMM needs a transposed copy of psi or beta.
+// Accumulators live in TMEM; one thread issues tcgen05.mma; warp roles: 0 = TMA producer,
+// 1 = MMA issuer (+ TMEM allocation), the rest convert (hi/lo split) and run the epilogue.
+//
+// FP32-grade accuracy = 3xTF32 (PAPER.md L239 describes the same idea as BF16x3):
+//   a*b ~= a_hi*b_hi + a_lo*b_hi + a_hi*b_lo,  x_hi = x with the 13 low mantissa bits cleared (what
+// a kind::tf32 operand keeps), x_lo = x - x_hi (exact in FP32); FP32 accumulation in TMEM.
+// beta_hi / beta_lo are split once at mlmd_set_projectors; psi-side lo tiles are produced in shared
+// memory by the converter warps; W hi/lo are written by the glue kernel.
+#include <stdio.h>
+#include <stdlib.h>
+
+#include "mlmd_internal.h"
+#include "tc_ptx.cuh"
+
+namespace mlmd {
+
+using namespace ptx;
+
+namespace {
+
+// ---- tensor maps --------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// Column-chunked view of a row-major float matrix [rows][pitch]: dims (32 floats, rows, chunks of 32
+// columns); a box (32, box_rows, box_chunks) lands in shared memory as box_chunks consecutive
+// [box_rows x 128 B] regions in the 128B-span / 32B-atom swizzle = UMMA MN-major SWIZZLE_128B_BASE32B
+// atoms (4 K-rows x 32 MN-elements each; the only MN-major layout tcgen05 takes for TF32 operands).
+bool make_chunk_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t pitch, uint64_t nchunk, uint32_t box_rows,
+                    uint32_t box_chunks) {
+    EncodeTiledFn f = encode_fn();
+    if (!f) return false;
+    cuuint64_t dims[3] = {32, rows, nchunk};
+    cuuint64_t strides[2] = {pitch * sizeof(float), 32 * sizeof(float)};
+    cuuint32_t box[3] = {32, box_rows, box_chunks};
+    cuuint32_t es[3] = {1, 1, 1};
+    return f(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Plain 2-D view (cols, rows) with a (8 floats = 32 B, box_rows) box and the 32-byte swizzle = UMMA
+// K-major SWIZZLE_32B layout of one K = 8 slab.
+bool make_k8_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch, uint32_t box_rows) {
+    EncodeTiledFn f = encode_fn();
+    if (!f) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {pitch * sizeof(float)};
+    cuuint32_t box[2] = {8, box_rows};
+    cuuint32_t es[2] = {1, 1};
+    return f(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+// in place: v -> hi (TF32-representable), returns lo = v - hi (exact)
+__device__ __forceinline__ float4 split4(float4 &v) {
+    const float4 h = make_float4(tf32_hi(v.x), tf32_hi(v.y), tf32_hi(v.z), tf32_hi(v.w));
+    const float4 l = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
+    v = h;
+    return l;
+}
+
+// =================================================================================================
+// Projection: Z[p][c] = sum_r A[r][p] * Y[r][c] over one K slice; FP32 partials per slice.
+// CTA tile: up to 256 rows p (two M = 128 UMMA blocks) x BN <= 224 columns; K pipeline of 16 rows.
+// =================================================================================================
+constexpr int PJ_BK = 16;               // grid points per pipeline stage (two K = 8 UMMA steps)
+constexpr int PJ_STAGES = 3;
+constexpr int PJ_MAXBN = 224;
+constexpr int PJ_A_BYTES = 8 * PJ_BK * 128;            // 8 chunks of 32 p  = 256 rows p
+constexpr int PJ_Y_BYTES = (PJ_MAXBN / 32) * PJ_BK * 128;
+constexpr int PJ_STAGE_BYTES = 2 * PJ_A_BYTES + 2 * PJ_Y_BYTES;
+constexpr int PJ_SMEM = PJ_STAGES * PJ_STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int PJ_THREADS = 192;          // warp 0 TMA, warp 1 MMA, warps 2-5 convert + epilogue
+
+struct ProjParams {
+    int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, debug;
+    float *zpart;
+};
+
+__global__ void __launch_bounds__(PJ_THREADS, 1)
+proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
+               const __grid_constant__ CUtensorMap map_y, const ProjParams q) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint64_t *bars = (uint64_t *)(smem + PJ_STAGES * PJ_STAGE_BYTES);
+    uint64_t *full = bars, *empty = bars + PJ_STAGES, *conv = bars + 2 * PJ_STAGES;
+    uint64_t *acc_full = bars + 3 * PJ_STAGES, *acc_empty = acc_full + 1;
+    uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < PJ_STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], 1);
+            mbar_init(&conv[s], 128);
+        }
+        mbar_init(acc_full, 1);
+        mbar_init(acc_empty, 128);
+        fence_barrier_init();
+        prefetch_tmap(&map_ahi);
+        prefetch_tmap(&map_alo);
+        prefetch_tmap(&map_y);
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const int nkb = q.ngrid / PJ_BK;
+    const int total = q.ndom * q.ntile_m * q.ntile_n * q.nsplit;
+    const bool need_lo = q.nprod == 3;
+    const bool load_alo = need_lo && !q.conv_a;
+    const uint32_t y_bytes = (uint32_t)(q.BN / 32) * PJ_BK * 128;
+    const uint32_t tx_bytes = PJ_A_BYTES * (load_alo ? 2u : 1u) + y_bytes;
+
+    auto decode = [&](int u, int &dom, int &mt, int &nt, int &kb0, int &kb1) {
+        nt = u % q.ntile_n;
+        u /= q.ntile_n;
+        const int sp = u % q.nsplit;
+        u /= q.nsplit;
+        mt = u % q.ntile_m;
+        dom = u / q.ntile_m;
+        kb0 = (int)((long)nkb * sp / q.nsplit);
+        kb1 = (int)((long)nkb * (sp + 1) / q.nsplit);
+    };
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int it = 0;
+            for (int u = blockIdx.x; u < total; u += gridDim.x) {
+                int dom, mt, nt, kb0, kb1;
+                decode(u, dom, mt, nt, kb0, kb1);
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    const int s = it % PJ_STAGES;
+                    mbar_wait(&empty[s], ((it / PJ_STAGES) & 1) ^ 1);
+                    uint8_t *st = smem + s * PJ_STAGE_BYTES;
+                    mbar_expect_tx(&full[s], tx_bytes);
+                    const int row = dom * q.ngrid + kb * PJ_BK;
+                    tma_load_3d(st, &map_ahi, &full[s], 0, row, mt * 8);
+                    if (load_alo) tma_load_3d(st + PJ_A_BYTES, &map_alo, &full[s], 0, row, mt * 8);
+                    tma_load_3d(st + 2 * PJ_A_BYTES, &map_y, &full[s], 0, row, nt * (q.BN / 32));
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            const uint32_t idesc = instr_desc(FMT_TF32, 1, 1, 128, (uint32_t)q.BN);
+            int it = 0, nu = 0;
+            for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
+                int dom, mt, nt, kb0, kb1;
+                decode(u, dom, mt, nt, kb0, kb1);
+                const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
+                mbar_wait(acc_empty, (nu & 1) ^ 1);
+                tc_fence_after();
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    const int s = it % PJ_STAGES;
+                    const uint32_t ph = (it / PJ_STAGES) & 1;
+                    mbar_wait(&full[s], ph);
+                    if (need_lo) mbar_wait(&conv[s], ph);
+                    tc_fence_after();
+                    const uint32_t st = smem_u32(smem + s * PJ_STAGE_BYTES);
+                    const uint32_t a_hi = st, a_lo = st + PJ_A_BYTES, y_hi = st + 2 * PJ_A_BYTES,
+                                   y_lo = st + 2 * PJ_A_BYTES + PJ_Y_BYTES;
+#pragma unroll
+                    for (int k8 = 0; k8 < PJ_BK / 8; ++k8) {
+                        const uint64_t dy = smem_desc(y_hi + k8 * 1024, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                        const uint64_t dyl = smem_desc(y_lo + k8 * 1024, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                        for (int mb = 0; mb < nblk; ++mb) {
+                            const uint32_t aoff = mb * 4 * (PJ_BK * 128) + k8 * 1024;
+                            const uint64_t da = smem_desc(a_hi + aoff, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                            const uint32_t d = tmem + mb * q.BN;
+                            umma_tf32(d, da, dy, idesc, (kb > kb0 || k8 > 0) ? 1u : 0u);
+                            if (need_lo) {
+                                const uint64_t dal = smem_desc(a_lo + aoff, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                                umma_tf32(d, dal, dy, idesc, 1u);
+                                umma_tf32(d, da, dyl, idesc, 1u);
+                            }
+                        }
+                    }
+                    umma_commit(&empty[s]);
+                }
+                umma_commit(acc_full);
+            }
+        }
+    } else {
+        const int t = threadIdx.x - 64;   // 0..127
+        const int quarter = warp % 4;
+        int it = 0, nu = 0;
+        for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
+            int dom, mt, nt, kb0, kb1;
+            decode(u, dom, mt, nt, kb0, kb1);
+            if (need_lo) {
+                const int ny4 = q.BN / 32 * PJ_BK * 8;    // float4 count of the Y tile
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    const int s = it % PJ_STAGES;
+                    mbar_wait(&full[s], (it / PJ_STAGES) & 1);
+                    uint8_t *st = smem + s * PJ_STAGE_BYTES;
+                    // elementwise on the swizzled image: the lo tile has the same layout as the hi tile
+                    float4 *ysrc = (float4 *)(st + 2 * PJ_A_BYTES);
+                    float4 *ydst = (float4 *)(st + 2 * PJ_A_BYTES + PJ_Y_BYTES);
+                    for (int i = t; i < ny4; i += 128) {
+                        float4 v = ysrc[i];
+                        ydst[i] = split4(v);
+                        ysrc[i] = v;
+                    }
+                    if (q.conv_a) {
+                        float4 *asrc = (float4 *)st;
+                        float4 *adst = (float4 *)(st + PJ_A_BYTES);
+                        for (int i = t; i < PJ_A_BYTES / 16; i += 128) {
+                            float4 v = asrc[i];
+                            adst[i] = split4(v);
+                            asrc[i] = v;
+                        }
+                    }
+                    fence_proxy_async_smem();
+                    mbar_arrive(&conv[s]);
+                }
+            }
+            // epilogue: TMEM -> partial sums of this K slice
+            mbar_wait(acc_full, nu & 1);
+            tc_fence_after();
+            const int sp = (u / q.ntile_n) % q.nsplit;
+            float *zd = q.zpart + ((size_t)dom * q.nsplit + sp) * q.prows * q.N;
+            const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
+            for (int mb = 0; mb < nblk; ++mb) {
+                const int p = mt * 256 + mb * 128 + quarter * 32 + lane;
+                for (int cb = 0; cb < q.BN / 32; ++cb) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + mb * q.BN + cb * 32, v);
+                    tmem_ld_wait();
+                    const int c0 = nt * q.BN + cb * 32;
+                    if (p < q.P && c0 < q.N) {
+                        float4 *dst = (float4 *)(zd + (size_t)p * q.N + c0);
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            dst[j] = make_float4(__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                                                 __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
+                    }
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(acc_empty);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc(tmem, 512);
+    }
+}
+
+// =================================================================================================
+// Back-application: Y[r][c] += sum_p A[r][p] * W[p][c].
+// CTA tile: 128 grid points x BN <= 448 columns (TMEM accumulator), K pipeline of 8 projector rows.
+// =================================================================================================
+constexpr int BK_STAGES = 5;
+constexpr int BK_MAXBN = 448;
+constexpr int BK_A_BYTES = 128 * 32;                    // [128 rows x 8 floats], SWIZZLE_32B
+constexpr int BK_W_BYTES = (BK_MAXBN / 32) * 1024;      // chunks of [8 rows x 128 B], SWIZZLE_128B
+constexpr int BK_STAGE_BYTES = 2 * BK_A_BYTES + 2 * BK_W_BYTES;
+constexpr int BK_SMEM = BK_STAGES * BK_STAGE_BYTES + 1024 + 256;
+constexpr int BK_EPI_WARPS = 8;
+constexpr int BK_THREADS = 64 + 32 * BK_EPI_WARPS;
+
+struct BackParams {
+    int ndom, ngrid, P, N, BN, ntile_n, prows, nprod, ldy;
+    float *Y;
+};
+
+__global__ void __launch_bounds__(BK_THREADS, 1)
+back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
+               const __grid_constant__ CUtensorMap map_whi, const __grid_constant__ CUtensorMap map_wlo,
+               const BackParams q) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint64_t *bars = (uint64_t *)(smem + BK_STAGES * BK_STAGE_BYTES);
+    uint64_t *full = bars, *empty = bars + BK_STAGES;
+    uint64_t *acc_full = bars + 2 * BK_STAGES, *acc_empty = acc_full + 1;
+    uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < BK_STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], 1);
+        }
+        mbar_init(acc_full, 1);
+        mbar_init(acc_empty, 32 * BK_EPI_WARPS);
+        fence_barrier_init();
+        prefetch_tmap(&map_ahi);
+        prefetch_tmap(&map_alo);
+        prefetch_tmap(&map_whi);
+        prefetch_tmap(&map_wlo);
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const int nrt = q.ngrid / 128;                 // row tiles per domain
+    const int total = q.ndom * nrt * q.ntile_n;
+    const int nk = (q.P + 7) / 8;
+    const bool need_lo = q.nprod == 3;
+    const uint32_t w_bytes = (uint32_t)(q.BN / 32) * 1024;
+    const uint32_t tx_bytes = (need_lo ? 2u : 1u) * (BK_A_BYTES + w_bytes);
+    const int ninstr = q.BN > 256 ? 2 : 1;
+    const int NI = q.BN / ninstr;                   // columns per UMMA instruction (multiple of 32)
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int it = 0;
+            for (int u = blockIdx.x; u < total; u += gridDim.x) {
+                const int nt = u % q.ntile_n, rt = (u / q.ntile_n) % nrt, dom = u / (q.ntile_n * nrt);
+                const int row = dom * q.ngrid + rt * 128;
+                for (int k = 0; k < nk; ++k, ++it) {
+                    const int s = it % BK_STAGES;
+                    mbar_wait(&empty[s], ((it / BK_STAGES) & 1) ^ 1);
+                    uint8_t *st = smem + s * BK_STAGE_BYTES;
+                    mbar_expect_tx(&full[s], tx_bytes);
+                    tma_load_2d(st, &map_ahi, &full[s], k * 8, row);
+                    tma_load_3d(st + 2 * BK_A_BYTES, &map_whi, &full[s], 0, dom * q.prows + k * 8, nt * (q.BN / 32));
+                    if (need_lo) {
+                        tma_load_2d(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
+                        tma_load_3d(st + 2 * BK_A_BYTES + BK_W_BYTES, &map_wlo, &full[s], 0, dom * q.prows + k * 8,
+                                    nt * (q.BN / 32));
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            const uint32_t idesc = instr_desc(FMT_TF32, 0, 1, 128, (uint32_t)NI);
+            int it = 0, nu = 0;
+            for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
+                mbar_wait(acc_empty, (nu & 1) ^ 1);
+                tc_fence_after();
+                for (int k = 0; k < nk; ++k, ++it) {
+                    const int s = it % BK_STAGES;
+                    mbar_wait(&full[s], (it / BK_STAGES) & 1);
+                    tc_fence_after();
+                    const uint32_t st = smem_u32(smem + s * BK_STAGE_BYTES);
+                    const uint64_t da = smem_desc(st, 16, 256, LAYOUT_SW32);
+                    const uint64_t dal = smem_desc(st + BK_A_BYTES, 16, 256, LAYOUT_SW32);
+                    for (int h = 0; h < ninstr; ++h) {
+                        const uint32_t woff = (uint32_t)h * (NI / 32) * 1024;
+                        const uint64_t dw = smem_desc(st + 2 * BK_A_BYTES + woff, 1024, 512, LAYOUT_SW128_32B);
+                        const uint32_t d = tmem + h * NI;
+                        umma_tf32(d, da, dw, idesc, k > 0 ? 1u : 0u);
+                        if (need_lo) {
+                            const uint64_t dwl = smem_desc(st + 2 * BK_A_BYTES + BK_W_BYTES + woff, 1024, 512, LAYOUT_SW128_32B);
+                            umma_tf32(d, dal, dw, idesc, 1u);
+                            umma_tf32(d, da, dwl, idesc, 1u);
+                        }
+                    }
+                    umma_commit(&empty[s]);
+                }
+                umma_commit(acc_full);
+            }
+        }
+    } else {
+        const int ew = warp - 2;                    // 0..7
+        const int quarter = warp % 4;
+        const int par = ew / 4;                     // which half of the column blocks this warp takes
+        int nu = 0;
+        for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
+            const int nt = u % q.ntile_n, rt = (u / q.ntile_n) % nrt, dom = u / (q.ntile_n * nrt);
+            const size_t r = (size_t)dom * q.ngrid + rt * 128 + quarter * 32 + lane;
+            mbar_wait(acc_full, nu & 1);
+            tc_fence_after();
+            for (int cb = par; cb < q.BN / 32; cb += BK_EPI_WARPS / 4) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
+                tmem_ld_wait();
+                const int c0 = nt * q.BN + cb * 32;
+                if (c0 < q.N) {
+                    float4 *dst = (float4 *)(q.Y + r * q.ldy + c0);
+                    float4 y[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) y[j] = dst[j];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        y[j].x += __uint_as_float(v[4 * j]);
+                        y[j].y += __uint_as_float(v[4 * j + 1]);
+                        y[j].z += __uint_as_float(v[4 * j + 2]);
+                        y[j].w += __uint_as_float(v[4 * j + 3]);
+                        dst[j] = y[j];
+                    }
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(acc_empty);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc(tmem, 512);
+    }
+}
+
+int g_num_sms = 0;
+int num_sms() {
+    if (!g_num_sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (g_num_sms <= 0) g_num_sms = 148;
+    }
+    return g_num_sms;
+}
+
+}  // namespace
+
+bool tc_available() { return encode_fn() != nullptr; }
+
+int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
+    const int ntile_m = (P + 255) / 256;
+    const int ntile_n = (N + PJ_MAXBN - 1) / PJ_MAXBN;
+    const long base = (long)ndom * ntile_m * ntile_n;
+    const int sms = 148;
+    const long nkb = ngrid / PJ_BK;
+    int best = 1;
+    double best_eff = 0.0;
+    for (int ns = 1; ns <= kMaxSplit && ns <= nkb / 8; ++ns) {
+        const long units = base * ns;
+        const double eff = (double)units / (double)(((units + sms - 1) / sms) * sms);
+        if (eff > best_eff + 1e-9) {
+            best_eff = eff;
+            best = ns;
+        }
+        if (eff >= 0.97) return ns;
+    }
+    return best;
+}
+
+cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
+                           const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
+                           int *nlaunch) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    ProjParams q;
+    q.ndom = ndom;
+    q.ngrid = (int)ngrid;
+    q.P = P;
+    q.N = N;
+    q.ntile_m = (P + 255) / 256;
+    q.ntile_n = (N + PJ_MAXBN - 1) / PJ_MAXBN;
+    q.BN = ((N + q.ntile_n - 1) / q.ntile_n + 31) / 32 * 32;
+    q.nsplit = nsplit;
+    q.prows = prows;
+    q.nprod = nprod;
+    q.conv_a = (nprod == 3 && A_lo == nullptr) ? 1 : 0;
+    q.zpart = zpart;
+    q.debug = getenv("MLMD_TC_DEBUG") ? 1 : 0;
+    const uint64_t rows = (uint64_t)ndom * ngrid;
+    CUtensorMap ma, mal, my;
+    if (!make_chunk_map(&ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(&mal, A_lo ? A_lo : A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(&my, Y, rows, ldy, N / 32, PJ_BK, q.BN / 32)) return cudaErrorInvalidValue;
+    const int total = ndom * q.ntile_m * q.ntile_n * nsplit;
+    const int grid = total < num_sms() ? total : num_sms();
+    ++*nlaunch;
+    proj_tc_kernel<<<grid, PJ_THREADS, PJ_SMEM, st>>>(ma, mal, my, q);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
+                           const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
+                           int *nlaunch) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(back_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, BK_SMEM);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    BackParams q;
+    q.ndom = ndom;
+    q.ngrid = (int)ngrid;
+    q.P = P;
+    q.N = N;
+    q.ntile_n = (N + BK_MAXBN - 1) / BK_MAXBN;
+    const int per = (N + q.ntile_n - 1) / q.ntile_n;
+    q.BN = per <= 256 ? (per + 31) / 32 * 32 : (per + 63) / 64 * 64;
+    q.prows = prows;
+    q.nprod = nprod;
+    q.ldy = ldy;
+    q.Y = Y;
+    const uint64_t rows = (uint64_t)ndom * ngrid;
+    CUtensorMap ma, mal, mw, mwl;
+    if (!make_k8_map(&ma, A_hi, rows, lda, lda, 128)) return cudaErrorInvalidValue;
+    if (!make_k8_map(&mal, A_lo, rows, lda, lda, 128)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(&mw, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, q.BN / 32)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(&mwl, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, q.BN / 32)) return cudaErrorInvalidValue;
+    const int total = ndom * (int)(ngrid / 128) * q.ntile_n;
+    const int grid = total < num_sms() ? total : num_sms();
+    ++*nlaunch;
+    back_tc_kernel<<<grid, BK_THREADS, BK_SMEM, st>>>(ma, mal, mw, mwl, q);
+    return cudaGetLastError();
+}
+
+}  // namespace mlmd

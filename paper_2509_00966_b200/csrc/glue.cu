@@ -4,6 +4,9 @@
 
 namespace mlmd {
 
+// x with the 13 low mantissa bits cleared: the part of x a kind::tf32 tensor-core operand keeps
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+
 // S2b.  C[p][n] = sum over split slices (fixed order: bit-reproducible, reading D22) of the
 // projection, combined to the complex coefficient for complex projectors; then
 //   W[p][n] = (-i tau) * D'_p * C[p][n],  D' = D * dv (reading D10)
@@ -12,7 +15,7 @@ namespace mlmd {
 //   complex beta: rows 2p, 2p+1 hold the 2x2 real representation of W.
 __global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int prows, int nsplit,
                                     const float *__restrict__ zpart, const float *__restrict__ dprime, float tau,
-                                    float *__restrict__ what) {
+                                    float *__restrict__ what, float *__restrict__ what_lo) {
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
     const int p = blockIdx.y, dom = blockIdx.z;
     if (n >= ld) return;
@@ -36,21 +39,28 @@ __global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int pro
     }
     const float f = tau * dprime[(size_t)dom * nproj + p];
     const float wre = f * cim, wim = -f * cre;   // (-i f)(cre + i cim)
+    // stored as TF32-representable hi part + exact FP32 remainder lo (hi + lo == W exactly)
+    const float wre_h = tf32_hi(wre), wim_h = tf32_hi(wim);
+    const float wre_l = wre - wre_h, wim_l = wim - wim_h;
     float *wd = what + (size_t)dom * prows * N;
+    float *wl = what_lo + (size_t)dom * prows * N;
     if (!beta_complex) {
-        *(float2 *)(wd + (size_t)p * N + 2 * n) = make_float2(wre, wim);
+        *(float2 *)(wd + (size_t)p * N + 2 * n) = make_float2(wre_h, wim_h);
+        *(float2 *)(wl + (size_t)p * N + 2 * n) = make_float2(wre_l, wim_l);
     } else {
-        *(float2 *)(wd + (size_t)(2 * p) * N + 2 * n) = make_float2(wre, wim);
-        *(float2 *)(wd + (size_t)(2 * p + 1) * N + 2 * n) = make_float2(-wim, wre);
+        *(float2 *)(wd + (size_t)(2 * p) * N + 2 * n) = make_float2(wre_h, wim_h);
+        *(float2 *)(wd + (size_t)(2 * p + 1) * N + 2 * n) = make_float2(-wim_h, wre_h);
+        *(float2 *)(wl + (size_t)(2 * p) * N + 2 * n) = make_float2(wre_l, wim_l);
+        *(float2 *)(wl + (size_t)(2 * p + 1) * N + 2 * n) = make_float2(-wim_l, wre_l);
     }
 }
 
 cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows,
                                 int nsplit, const float *zpart, const float *dprime, float tau,
-                                float *what, int *nlaunch) {
+                                float *what, float *what_lo, int *nlaunch) {
     dim3 grid((ld + 127) / 128, nproj, ndom);
     ++*nlaunch;
-    reduce_scale_kernel<<<grid, 128, 0, st>>>(nproj, beta_complex, ld, prows, nsplit, zpart, dprime, tau, what);
+    reduce_scale_kernel<<<grid, 128, 0, st>>>(nproj, beta_complex, ld, prows, nsplit, zpart, dprime, tau, what, what_lo);
     return cudaGetLastError();
 }
 
@@ -114,16 +124,19 @@ cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld,
     return cudaGetLastError();
 }
 
-// lo = x - hi with hi = x with the low 13 mantissa bits cleared (what a TF32 operand keeps); exact.
-__global__ void split_tf32_lo_kernel(const float *__restrict__ src, float *__restrict__ lo, size_t n) {
+// In place: x -> hi = x with the low 13 mantissa bits cleared (what a TF32 operand keeps), lo = x - hi
+// (exact in FP32, so hi + lo restores x bit for bit).
+__global__ void split_tf32_kernel(float *__restrict__ x, float *__restrict__ lo, size_t n) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const float x = src[i];
-        lo[i] = x - __uint_as_float(__float_as_uint(x) & 0xffffe000u);
+        const float v = x[i];
+        const float hi = tf32_hi(v);
+        x[i] = hi;
+        lo[i] = v - hi;
     }
 }
-cudaError_t launch_split_tf32_lo(cudaStream_t st, const float *src, float *lo, size_t n, int *nlaunch) {
+cudaError_t launch_split_tf32(cudaStream_t st, float *x, float *lo, size_t n, int *nlaunch) {
     ++*nlaunch;
-    split_tf32_lo_kernel<<<2368, 256, 0, st>>>(src, lo, n);
+    split_tf32_kernel<<<2368, 256, 0, st>>>(x, lo, n);
     return cudaGetLastError();
 }
 

@@ -23,7 +23,7 @@ struct StepCoef {
 static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
-    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, zpart, coef, flag, total;
+    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, flag, total;
 };
 
 constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
@@ -47,7 +47,9 @@ struct mlmd_domain {
     int P;                      // real projector rows
     int ldp;                    // padded P (pitch of beta rows / rows of Z, What)
     int prows;                  // rows allocated for Z/What/zpart = max(ldp(nproj_max), 2*ld)
-    int nsplit;                 // split-K factor of the projection
+    int nsplit;                 // split-K factor of the projection (CUDA-core path)
+    int nsplit_tc, nsplit_tc_ovl;   // split-K factors of the tcgen05 projection (beta rows / overlap)
+    bool tc_ok;                 // shape and device allow the tcgen05 GEMM kernels
     int gemm_mode;
     bool have_psi, have_vloc, have_occ, rho_valid;
     bool field_yz;              // any A_y or A_z non-zero in the current propagate call
@@ -73,6 +75,7 @@ struct mlmd_domain {
     float *rho() const { return (float *)(ws + off.rho); }
     float *z() const { return (float *)(ws + off.z); }
     float *what() const { return (float *)(ws + off.what); }
+    float *what_lo() const { return (float *)(ws + off.what_lo); }
     float *zpart() const { return (float *)(ws + off.zpart); }
     mlmd::StepCoef *coef() const { return (mlmd::StepCoef *)(ws + off.coef); }
     int *flag() const { return (int *)(ws + off.flag); }
@@ -90,27 +93,41 @@ cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const fl
 // ---- gemm_simt.cu ----------------------------------------------------------------------------
 // Projection (S2a): zpart[dom][s][p][c] = sum_{r in slice s} B[dom][r][p] * Y[dom][r][c]
 //   B: [ndom][ngrid][ldb] float (p fastest), Y: [ndom][ngrid][ldy] float, P rows, N columns used.
-cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float *B, int ldb, int P,
+//   Blo (may be NULL): B is stored as an exact hi + lo pair and summed on load.
+cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
                              const float *Y, int ldy, int N, float *zpart, int prows, int nsplit,
                              bool fp64, int *nlaunch);
-// Back-application (S2d): Y[dom][r][c] += sum_p B[dom][r][p] * What[dom][p][c]
-cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float *B, int ldb, int P,
-                             const float *What, float *Y, int ldy, int N, int prows, bool fp64,
+// Back-application (S2d): Y[dom][r][c] += sum_p B[dom][r][p] * What[dom][p][c]  (both stored as hi + lo)
+cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
+                             const float *What, const float *Wlo, float *Y, int ldy, int N, int prows, bool fp64,
                              int *nlaunch);
+
+// ---- gemm_tc.cu ------------------------------------------------------------------------------
+// The same two contractions on tcgen05 tensor cores, operands staged by TMA.  nprod = 3: 3xTF32
+// (FP32-grade), nprod = 1: single TF32 product.  A_lo == NULL with nprod == 3: the kernel splits A
+// itself (overlap, where A is a psi buffer).  Requires ngrid % 128 == 0, N % 32 == 0, lda % 8 == 0.
+bool tc_available();
+int tc_choose_nsplit(int ndom, long ngrid, int P, int N);
+cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
+                           const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
+                           int *nlaunch);
+cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
+                           const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
+                           int *nlaunch);
 
 // ---- glue.cu ---------------------------------------------------------------------------------
 // S2b: reduce split-K partials in fixed order and build What = (-i tau) D' C in real-GEMM form.
 cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows,
                                 int nsplit, const float *zpart, const float *dprime, float tau,
-                                float *what, int *nlaunch);
+                                float *what, float *what_lo, int *nlaunch);
 // S3: rho[dom][r] = sum_n occ[dom][n] |psi[dom][r][n]|^2
 cudaError_t launch_density(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, const float *occ,
                            float *rho, int *nlaunch);
 // S4 epilogue: S[dom][m][n] = dv * (sum over splits of the complex combination of Z)
 cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld, int prows, int nsplit,
                                     const float *zpart, float dv, float2 *S, int *nlaunch);
-// lo = x - trunc_tf32(x): the part of x a TF32 tensor-core operand drops (exact in FP32)
-cudaError_t launch_split_tf32_lo(cudaStream_t st, const float *src, float *lo, size_t n, int *nlaunch);
+// in place x -> hi (TF32-representable part), lo = x - hi (exact in FP32)
+cudaError_t launch_split_tf32(cudaStream_t st, float *x, float *lo, size_t n, int *nlaunch);
 cudaError_t launch_max_abs(cudaStream_t st, const float *x, size_t n, int *flag_bits, int *nlaunch);
 cudaError_t launch_check_finite(cudaStream_t st, const float *x, size_t n, int *flag, int *nlaunch);
 
