@@ -13,6 +13,10 @@
 
 using namespace mlmd;
 
+// TMEM accumulation chain lengths (16-row stages) of the tcgen05 projection: tensor-core FP32
+// accumulation truncates, so long chains drift by ~1 ulp per MMA.
+static const int kProjChain = 64, kOverlapChain = 4;
+
 static thread_local char g_err[512] = "";
 
 static int fail(int code, const char *fmt, ...) {
@@ -350,7 +354,7 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl)
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, h->gemm_mode == MLMD_GEMM_TF32X1 ? 1 : 3, nl));
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, h->gemm_mode == MLMD_GEMM_TF32X1 ? 1 : 3, kProjChain, nl));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
@@ -472,7 +476,7 @@ int mlmd_overlap(mlmd_domain_t *h, int which, void *S, int where) {
     const int nsplit = tc ? h->nsplit_tc_ovl : h->nsplit;
     if (tc)
         CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, (const float *)phi, nullptr, 2 * h->ld, 2 * h->ld,
-                          (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, 3, &nl));
+                          (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, 3, kOverlapChain, &nl));
     else
         CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, (const float *)phi, nullptr, 2 * h->ld, 2 * h->ld,
                             (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, &nl));

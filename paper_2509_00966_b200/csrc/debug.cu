@@ -9,11 +9,11 @@ extern "C" {
 // Z partials [ndom][nsplit][prows][N] = per-K-slice sums of A^T Y.  A_lo may be NULL (kernel splits A).
 // path: 0 = CUDA cores, 1 = tcgen05.  Returns a cudaError_t value.
 int mlmd_debug_proj(int path, void *stream, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
-                    const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod) {
+                    const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod, int chain) {
     int nl = 0;
     cudaError_t e;
     if (path == 1)
-        e = launch_proj_tc((cudaStream_t)stream, ndom, ngrid, A_hi, A_lo, lda, P, Y, ldy, N, zpart, prows, nsplit, nprod, &nl);
+        e = launch_proj_tc((cudaStream_t)stream, ndom, ngrid, A_hi, A_lo, lda, P, Y, ldy, N, zpart, prows, nsplit, nprod, chain, &nl);
     else
         e = launch_proj_simt((cudaStream_t)stream, ndom, ngrid, A_hi, A_lo, lda, P, Y, ldy, N, zpart, prows, nsplit, false, &nl);
     if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);

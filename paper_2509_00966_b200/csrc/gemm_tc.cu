@@ -99,7 +99,7 @@ constexpr int PJ_SMEM = PJ_STAGES * PJ_STAGE_BYTES + 1024 /*align*/ + 256 /*barr
 constexpr int PJ_THREADS = 192;          // warp 0 TMA, warp 1 MMA, warps 2-5 convert + epilogue
 
 struct ProjParams {
-    int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, debug;
+    int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, chain;
     float *zpart;
 };
 
@@ -172,14 +172,19 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     } else if (warp == 1) {
         if (lane == 0) {
             const uint32_t idesc = instr_desc(FMT_TF32, 1, 1, 128, (uint32_t)q.BN);
-            int it = 0, nu = 0;
-            for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
+            int it = 0, nd = 0;   // nd: accumulator hand-overs (drains) so far
+            for (int u = blockIdx.x; u < total; u += gridDim.x) {
                 int dom, mt, nt, kb0, kb1;
                 decode(u, dom, mt, nt, kb0, kb1);
                 const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
-                mbar_wait(acc_empty, (nu & 1) ^ 1);
-                tc_fence_after();
                 for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    // a chain = at most q.chain stages accumulated in TMEM before the epilogue warps add
+                    // it to the FP32 partial sums (tensor-core accumulation truncates)
+                    const bool first = (kb - kb0) % q.chain == 0;
+                    if (first) {
+                        mbar_wait(acc_empty, (nd & 1) ^ 1);
+                        tc_fence_after();
+                    }
                     const int s = it % PJ_STAGES;
                     const uint32_t ph = (it / PJ_STAGES) & 1;
                     mbar_wait(&full[s], ph);
@@ -196,7 +201,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                             const uint32_t aoff = mb * 4 * (PJ_BK * 128) + k8 * 1024;
                             const uint64_t da = smem_desc(a_hi + aoff, PJ_BK * 128, 512, LAYOUT_SW128_32B);
                             const uint32_t d = tmem + mb * q.BN;
-                            umma_tf32(d, da, dy, idesc, (kb > kb0 || k8 > 0) ? 1u : 0u);
+                            umma_tf32(d, da, dy, idesc, (!first || k8 > 0) ? 1u : 0u);
                             if (need_lo) {
                                 const uint64_t dal = smem_desc(a_lo + aoff, PJ_BK * 128, 512, LAYOUT_SW128_32B);
                                 umma_tf32(d, dal, dy, idesc, 1u);
@@ -205,68 +210,82 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         }
                     }
                     umma_commit(&empty[s]);
+                    if ((kb - kb0 + 1) % q.chain == 0 || kb + 1 == kb1) {
+                        umma_commit(acc_full);
+                        ++nd;
+                    }
                 }
-                umma_commit(acc_full);
             }
         }
     } else {
         const int t = threadIdx.x - 64;   // 0..127
         const int quarter = warp % 4;
-        int it = 0, nu = 0;
-        for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
+        int it = 0, nd = 0;
+        const int ny4 = q.BN / 32 * PJ_BK * 8;    // float4 count of the Y tile
+        for (int u = blockIdx.x; u < total; u += gridDim.x) {
             int dom, mt, nt, kb0, kb1;
             decode(u, dom, mt, nt, kb0, kb1);
-            if (need_lo) {
-                const int ny4 = q.BN / 32 * PJ_BK * 8;    // float4 count of the Y tile
-                for (int kb = kb0; kb < kb1; ++kb, ++it) {
-                    const int s = it % PJ_STAGES;
-                    mbar_wait(&full[s], (it / PJ_STAGES) & 1);
-                    uint8_t *st = smem + s * PJ_STAGE_BYTES;
-                    // elementwise on the swizzled image: the lo tile has the same layout as the hi tile
-                    float4 *ysrc = (float4 *)(st + 2 * PJ_A_BYTES);
-                    float4 *ydst = (float4 *)(st + 2 * PJ_A_BYTES + PJ_Y_BYTES);
-                    for (int i = t; i < ny4; i += 128) {
-                        float4 v = ysrc[i];
-                        ydst[i] = split4(v);
-                        ysrc[i] = v;
-                    }
-                    if (q.conv_a) {
-                        float4 *asrc = (float4 *)st;
-                        float4 *adst = (float4 *)(st + PJ_A_BYTES);
-                        for (int i = t; i < PJ_A_BYTES / 16; i += 128) {
-                            float4 v = asrc[i];
-                            adst[i] = split4(v);
-                            asrc[i] = v;
-                        }
-                    }
-                    fence_proxy_async_smem();
-                    mbar_arrive(&conv[s]);
-                }
-            }
-            // epilogue: TMEM -> partial sums of this K slice
-            mbar_wait(acc_full, nu & 1);
-            tc_fence_after();
             const int sp = (u / q.ntile_n) % q.nsplit;
             float *zd = q.zpart + ((size_t)dom * q.nsplit + sp) * q.prows * q.N;
             const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
-            for (int mb = 0; mb < nblk; ++mb) {
-                const int p = mt * 256 + mb * 128 + quarter * 32 + lane;
-                for (int cb = 0; cb < q.BN / 32; ++cb) {
-                    uint32_t v[32];
-                    tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + mb * q.BN + cb * 32, v);
-                    tmem_ld_wait();
-                    const int c0 = nt * q.BN + cb * 32;
-                    if (p < q.P && c0 < q.N) {
-                        float4 *dst = (float4 *)(zd + (size_t)p * q.N + c0);
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            dst[j] = make_float4(__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
-                                                 __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
+            for (int c0k = kb0; c0k < kb1; c0k += q.chain) {
+                const int c1k = min(c0k + q.chain, kb1);
+                if (need_lo) {
+                    for (int kb = c0k; kb < c1k; ++kb, ++it) {
+                        const int s = it % PJ_STAGES;
+                        mbar_wait(&full[s], (it / PJ_STAGES) & 1);
+                        uint8_t *st = smem + s * PJ_STAGE_BYTES;
+                        // elementwise on the swizzled image: the lo tile has the same layout as the hi tile
+                        float4 *ysrc = (float4 *)(st + 2 * PJ_A_BYTES);
+                        float4 *ydst = (float4 *)(st + 2 * PJ_A_BYTES + PJ_Y_BYTES);
+                        for (int i = t; i < ny4; i += 128) {
+                            float4 v = ysrc[i];
+                            ydst[i] = split4(v);
+                            ysrc[i] = v;
+                        }
+                        if (q.conv_a) {
+                            float4 *asrc = (float4 *)st;
+                            float4 *adst = (float4 *)(st + PJ_A_BYTES);
+                            for (int i = t; i < PJ_A_BYTES / 16; i += 128) {
+                                float4 v = asrc[i];
+                                adst[i] = split4(v);
+                                asrc[i] = v;
+                            }
+                        }
+                        fence_proxy_async_smem();
+                        mbar_arrive(&conv[s]);
                     }
                 }
+                // drain this chain: TMEM -> (+)= FP32 partial sums of this K slice (round-to-nearest adds)
+                mbar_wait(acc_full, nd & 1);
+                ++nd;
+                tc_fence_after();
+                const bool add = c0k > kb0;
+                for (int mb = 0; mb < nblk; ++mb) {
+                    const int p = mt * 256 + mb * 128 + quarter * 32 + lane;
+                    for (int cb = 0; cb < q.BN / 32; ++cb) {
+                        uint32_t v[32];
+                        tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + mb * q.BN + cb * 32, v);
+                        tmem_ld_wait();
+                        const int c0 = nt * q.BN + cb * 32;
+                        if (p < q.P && c0 < q.N) {
+                            float4 *dst = (float4 *)(zd + (size_t)p * q.N + c0);
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) {
+                                const float a = __uint_as_float(v[4 * j]), b = __uint_as_float(v[4 * j + 1]),
+                                            c = __uint_as_float(v[4 * j + 2]), d = __uint_as_float(v[4 * j + 3]);
+                                // every element has one owner thread, so the order of adds is fixed (reading D22)
+                                if (add)
+                                    red_add_v4((float *)(dst + j), a, b, c, d);
+                                else
+                                    dst[j] = make_float4(a, b, c, d);
+                            }
+                        }
+                    }
+                }
+                tc_fence_before();
+                mbar_arrive(acc_empty);
             }
-            tc_fence_before();
-            mbar_arrive(acc_empty);
         }
     }
     tc_fence_before();
@@ -402,18 +421,11 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 tmem_ld_wait();
                 const int c0 = nt * q.BN + cb * 32;
                 if (c0 < q.N) {
-                    float4 *dst = (float4 *)(q.Y + r * q.ldy + c0);
-                    float4 y[8];
+                    float *dst = q.Y + r * q.ldy + c0;
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) y[j] = dst[j];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        y[j].x += __uint_as_float(v[4 * j]);
-                        y[j].y += __uint_as_float(v[4 * j + 1]);
-                        y[j].z += __uint_as_float(v[4 * j + 2]);
-                        y[j].w += __uint_as_float(v[4 * j + 3]);
-                        dst[j] = y[j];
-                    }
+                    for (int j = 0; j < 8; ++j)
+                        red_add_v4(dst + 4 * j, __uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                                   __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
                 }
             }
             tc_fence_before();
@@ -465,7 +477,7 @@ int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
 
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
-                           int *nlaunch) {
+                           int chain, int *nlaunch) {
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
@@ -485,7 +497,7 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.nprod = nprod;
     q.conv_a = (nprod == 3 && A_lo == nullptr) ? 1 : 0;
     q.zpart = zpart;
-    q.debug = getenv("MLMD_TC_DEBUG") ? 1 : 0;
+    q.chain = chain > 0 ? chain : (1 << 30);
     const uint64_t rows = (uint64_t)ndom * ngrid;
     CUtensorMap ma, mal, my;
     if (!make_chunk_map(&ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;

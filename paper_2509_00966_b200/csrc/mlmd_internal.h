@@ -110,7 +110,7 @@ bool tc_available();
 int tc_choose_nsplit(int ndom, long ngrid, int P, int N);
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
-                           int *nlaunch);
+                           int chain /* 16-row stages per TMEM accumulation chain, 0 = whole slice */, int *nlaunch);
 cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
                            int *nlaunch);

@@ -110,6 +110,11 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// fire-and-forget FP32 vector add in L2 (round-to-nearest): *p += v, no value returned to the SM
+__device__ __forceinline__ void red_add_v4(float *p, float a, float b, float c, float d) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
 // ---- UMMA descriptors (bit layouts of the sm_100 shared-memory and instruction descriptors) -----
 // SW128_32B (32-byte chunks swizzled inside a 128-byte row, 4-row atoms) is the only swizzled layout the
 // hardware accepts for MN-major 32-bit (TF32) operands; verified on B200: plain SW128 yields zeros.
