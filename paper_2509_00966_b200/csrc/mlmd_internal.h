@@ -90,6 +90,12 @@ namespace mlmd {
 cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
                                  const StepCoef *coef, float tau, int *nlaunch);
 
+// ---- stencil_tma.cu ---------------------------------------------------------------------------
+// The same stage with TMA-staged x-planes (needs ny % 16 == 0, nz % 16 == 0).
+bool stencil_tma_supported(const mlmd_domain *h);
+cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
+                               float tau, int *nlaunch);
+
 // ---- gemm_simt.cu ----------------------------------------------------------------------------
 // Projection (S2a): zpart[dom][s][p][c] = sum_{r in slice s} B[dom][r][p] * Y[dom][r][c]
 //   B: [ndom][ngrid][ldb] float (p fastest), Y: [ndom][ngrid][ldy] float, P rows, N columns used.

@@ -190,7 +190,8 @@ cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const fl
     P.ny = h->ny;
     P.nz = h->nz;
     P.lanes = h->ld / 2;
-    const int variant = env_int("MLMD_STENCIL", 1);   // 0: simple (cross-check), 1: marching
+    const int variant = env_int("MLMD_STENCIL", 2);   // 0: simple (cross-check), 1: register marching, 2: TMA planes
+    if (variant == 2 && stencil_tma_supported(h)) return launch_stencil_tma(h, w, psi, out, coef, tau, nlaunch);
     const int xseg_env = env_int("MLMD_XSEG", 0);     // tuning override: planes per CTA
     ++*nlaunch;
     const bool tile_ok = (h->ny % 8 == 0) && (h->nz % 8 == 0);

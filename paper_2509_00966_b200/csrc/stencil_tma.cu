@@ -1,0 +1,297 @@
+// Fused kinetic stencil / local potential / Horner pass with TMA-staged planes (
+// north_star kernel 2).  Same arithmetic as stencil.cu:
+//
+//   out(r,n) = psi(r,n) + (-i tau) [ sum_{d,j} ( p_dj (w(r+j e_d) + w(r-j e_d)) - i q_dj (w(r+j e_d) - w(r-j e_d)) )
+//                                   + (centre + V_loc(r)) w(r,n) ]          (Eq. (3), 4th-order FD)
+//
+// Decomposition (orbital-fastest layout, orbital blocking, y-z planes concurrent):
+// one CTA owns a 16(y) x 16(z) patch of the y-z plane for a 64-byte orbital chunk (8 orbitals) and
+// marches along x.  Every x-plane of the patch -- centre box plus four 2-deep periodic halo strips --
+// is brought into shared memory ONCE by TMA (cp.async.bulk.tensor, 4-D tensor map over
+// [x*dom][y][z][orbital]) several planes ahead of the compute; the y/z taps are shared-memory reads, the
+// x taps are scattered into a five-deep ring of accumulators held in registers, so no plane is read
+// twice and the load latency is hidden by the asynchronous pipeline instead of by occupancy.
+#include "mlmd_internal.h"
+#include "tc_ptx.cuh"
+
+namespace mlmd {
+
+using namespace ptx;
+
+namespace {
+
+constexpr int SY = 16, SZ = 16, SL = 4;            // patch: 16 y x 16 z x 4 float4 lanes
+constexpr int S_CENTER = SY * SZ * 64;             // bytes
+constexpr int S_STRIP = 2 * 16 * 64;
+constexpr int S_PLANE = S_CENTER + 4 * S_STRIP;    // centre, z-lo, z-hi, y-lo, y-hi
+constexpr int S_NBUF = 6, S_PF = 4;
+constexpr int S_THREADS = SY * SZ * SL;            // 1024
+constexpr int S_SMEM = S_NBUF * S_PLANE + 1024 + 256;
+
+struct TmaStencilParams {
+    const float4 *psi;
+    float4 *out;
+    const float *vloc;
+    const StepCoef *coef;
+    float tau;
+    int nx, ny, nz, lanes;   // lanes = float4 per grid point
+    int xs, nxseg;           // planes per CTA, segments per domain
+    int nchunk;              // 64-byte chunks per grid point
+};
+
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, uint64_t *bar, int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+__device__ __forceinline__ float4 lds4(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+// acc += (p + s*i*q) * u for both complex numbers of the float4 (s = +1 or -1 folded into q)
+__device__ __forceinline__ void cmul_acc(float4 &acc, const float4 u, const float p, const float q) {
+    acc.x = fmaf(p, u.x, acc.x);
+    acc.x = fmaf(-q, u.y, acc.x);
+    acc.y = fmaf(p, u.y, acc.y);
+    acc.y = fmaf(q, u.x, acc.y);
+    acc.z = fmaf(p, u.z, acc.z);
+    acc.z = fmaf(-q, u.w, acc.z);
+    acc.w = fmaf(p, u.w, acc.w);
+    acc.w = fmaf(q, u.z, acc.w);
+}
+__device__ __forceinline__ void pair_acc(float4 &acc, const float4 a, const float4 b, const float p, const float q) {
+    acc.x = fmaf(p, a.x + b.x, acc.x);
+    acc.y = fmaf(p, a.y + b.y, acc.y);
+    acc.z = fmaf(p, a.z + b.z, acc.z);
+    acc.w = fmaf(p, a.w + b.w, acc.w);
+    acc.x = fmaf(q, a.y - b.y, acc.x);
+    acc.y = fmaf(-q, a.x - b.x, acc.y);
+    acc.z = fmaf(q, a.w - b.w, acc.z);
+    acc.w = fmaf(-q, a.z - b.z, acc.w);
+}
+__device__ __forceinline__ void pair_acc_real(float4 &acc, const float4 a, const float4 b, const float p) {
+    acc.x = fmaf(p, a.x + b.x, acc.x);
+    acc.y = fmaf(p, a.y + b.y, acc.y);
+    acc.z = fmaf(p, a.z + b.z, acc.z);
+    acc.w = fmaf(p, a.w + b.w, acc.w);
+}
+
+template <bool AYZ>
+__global__ void __launch_bounds__(S_THREADS, 1)
+stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_z,
+                   const __grid_constant__ CUtensorMap map_y, const TmaStencilParams P) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint64_t *full = (uint64_t *)(smem + S_NBUF * S_PLANE), *empty = full + S_NBUF;
+    const int tid = threadIdx.x;
+    const int l = tid % SL, tz = (tid / SL) % SZ, ty = tid / (SL * SZ);
+
+    // work item
+    int item = blockIdx.x;
+    const int seg = item % P.nxseg;
+    item /= P.nxseg;
+    const int nzt = P.nz / SZ, nyt = P.ny / SY;
+    const int zt = item % nzt;
+    item /= nzt;
+    const int yt = item % nyt;
+    item /= nyt;
+    const int chunk = item % P.nchunk;
+    const int dom = item / P.nchunk;
+    const int x0 = seg * P.xs;
+    const int x1 = min(x0 + P.xs, P.nx);
+    const int nplanes = (x1 - x0) + 4;
+    const int y0 = yt * SY, z0 = zt * SZ;
+
+    if (tid == 0) {
+        for (int b = 0; b < S_NBUF; ++b) {
+            mbar_init(&full[b], 1);
+            mbar_init(&empty[b], S_THREADS / 32);
+        }
+        fence_barrier_init();
+        prefetch_tmap(&map_c);
+        prefetch_tmap(&map_z);
+        prefetch_tmap(&map_y);
+    }
+    __syncthreads();
+
+    const int zlo = (z0 - 2 + P.nz) % P.nz, zhi = (z0 + SZ) % P.nz;
+    const int ylo = (y0 - 2 + P.ny) % P.ny, yhi = (y0 + SY) % P.ny;
+    auto issue = [&](int n) {   // plane n of this march: x = x0 - 2 + n (periodic)
+        const int b = n % S_NBUF;
+        int x = x0 - 2 + n;
+        x = x < 0 ? x + P.nx : (x >= P.nx ? x - P.nx : x);
+        const int xr = dom * P.nx + x;
+        uint8_t *buf = smem + b * S_PLANE;
+        mbar_expect_tx(&full[b], S_PLANE);
+        tma_load_4d(buf, &map_c, &full[b], chunk * 16, z0, y0, xr);
+        tma_load_4d(buf + S_CENTER, &map_z, &full[b], chunk * 16, zlo, y0, xr);
+        tma_load_4d(buf + S_CENTER + S_STRIP, &map_z, &full[b], chunk * 16, zhi, y0, xr);
+        tma_load_4d(buf + S_CENTER + 2 * S_STRIP, &map_y, &full[b], chunk * 16, z0, ylo, xr);
+        tma_load_4d(buf + S_CENTER + 3 * S_STRIP, &map_y, &full[b], chunk * 16, z0, yhi, xr);
+    };
+    if (tid == 0)
+        for (int n = 0; n < S_PF && n < nplanes; ++n) issue(n);
+
+    // byte offsets of the own point and the eight in-plane neighbours inside a plane buffer
+    const uint32_t own = (uint32_t)((ty * SZ + tz) * 64 + l * 16);
+    auto zoff = [&](int t) -> uint32_t {
+        if (t < 0) return (uint32_t)(S_CENTER + (ty * 2 + (t + 2)) * 64 + l * 16);
+        if (t >= SZ) return (uint32_t)(S_CENTER + S_STRIP + (ty * 2 + (t - SZ)) * 64 + l * 16);
+        return (uint32_t)((ty * SZ + t) * 64 + l * 16);
+    };
+    auto yoff = [&](int t) -> uint32_t {
+        if (t < 0) return (uint32_t)(S_CENTER + 2 * S_STRIP + ((t + 2) * SZ + tz) * 64 + l * 16);
+        if (t >= SY) return (uint32_t)(S_CENTER + 3 * S_STRIP + ((t - SY) * SZ + tz) * 64 + l * 16);
+        return (uint32_t)((t * SZ + tz) * 64 + l * 16);
+    };
+    const uint32_t ozp1 = zoff(tz + 1), ozm1 = zoff(tz - 1), ozp2 = zoff(tz + 2), ozm2 = zoff(tz - 2);
+    const uint32_t oyp1 = yoff(ty + 1), oym1 = yoff(ty - 1), oyp2 = yoff(ty + 2), oym2 = yoff(ty - 2);
+
+    const StepCoef c = P.coef[dom];
+    const long sz = P.lanes, sy = sz * P.nz, sx = sy * P.ny;
+    const long pbase = (long)dom * sx * P.nx + (long)(y0 + ty) * sy + (long)(z0 + tz) * sz + chunk * SL + l;
+    const float *vd = P.vloc + ((long)dom * P.nx * P.ny + (y0 + ty)) * P.nz + (z0 + tz);
+    const long vsx = (long)P.ny * P.nz;
+    const uint32_t sbase = smem_u32(smem);
+
+    float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0, a2 = a0, a3 = a0, a4 = a0;   // planes q-2 .. q+2
+    float4 ps = P.psi[pbase + (long)x0 * sx];   // Horner base of the first output plane
+
+    for (int n = 0; n < nplanes; ++n) {
+        const int b = n % S_NBUF;
+        if (tid == 0 && n + S_PF < nplanes) {
+            const int m = n + S_PF;
+            if (m >= S_NBUF) mbar_wait(&empty[m % S_NBUF], ((m / S_NBUF) - 1) & 1);
+            issue(m);
+        }
+        int xq = x0 - 2 + n;
+        xq = xq < 0 ? xq + P.nx : (xq >= P.nx ? xq - P.nx : xq);
+        const float vv = __ldg(vd + (long)xq * vsx);
+        // Horner base of the NEXT output plane (plane x0 + n - 3), prefetched one step ahead
+        const int pn = n - 3;
+        float4 psn = ps;
+        if (pn >= 1 && x0 + pn < x1) psn = P.psi[pbase + (long)(x0 + pn) * sx];
+
+        mbar_wait(&full[b], (n / S_NBUF) & 1);
+        const uint32_t buf = sbase + b * S_PLANE;
+        const float4 u = lds4(buf + own);
+        const float cen = c.centre + vv;
+        a2.x = fmaf(cen, u.x, a2.x);
+        a2.y = fmaf(cen, u.y, a2.y);
+        a2.z = fmaf(cen, u.z, a2.z);
+        a2.w = fmaf(cen, u.w, a2.w);
+        {
+            const float4 p1 = lds4(buf + oyp1), m1 = lds4(buf + oym1);
+            if (AYZ) pair_acc(a2, p1, m1, c.p[1][0], c.q[1][0]); else pair_acc_real(a2, p1, m1, c.p[1][0]);
+            const float4 p2 = lds4(buf + oyp2), m2 = lds4(buf + oym2);
+            if (AYZ) pair_acc(a2, p2, m2, c.p[1][1], c.q[1][1]); else pair_acc_real(a2, p2, m2, c.p[1][1]);
+        }
+        {
+            const float4 p1 = lds4(buf + ozp1), m1 = lds4(buf + ozm1);
+            if (AYZ) pair_acc(a2, p1, m1, c.p[2][0], c.q[2][0]); else pair_acc_real(a2, p1, m1, c.p[2][0]);
+            const float4 p2 = lds4(buf + ozp2), m2 = lds4(buf + ozm2);
+            if (AYZ) pair_acc(a2, p2, m2, c.p[2][1], c.q[2][1]); else pair_acc_real(a2, p2, m2, c.p[2][1]);
+        }
+        // x taps: u = w(plane q) is the +j neighbour of plane q-j (coefficient p_j - i q_j) and the -j
+        // neighbour of plane q+j (coefficient p_j + i q_j)
+        cmul_acc(a1, u, c.p[0][0], -c.q[0][0]);
+        cmul_acc(a3, u, c.p[0][0], c.q[0][0]);
+        cmul_acc(a0, u, c.p[0][1], -c.q[0][1]);
+        cmul_acc(a4, u, c.p[0][1], c.q[0][1]);
+        __syncwarp();
+        if (tid % 32 == 0) mbar_arrive(&empty[b]);
+        // plane q-2 is complete
+        const int po = n - 4;
+        if (po >= 0 && x0 + po < x1) {
+            const float4 o = make_float4(fmaf(P.tau, a0.y, ps.x), fmaf(-P.tau, a0.x, ps.y), fmaf(P.tau, a0.w, ps.z),
+                                         fmaf(-P.tau, a0.z, ps.w));
+            P.out[pbase + (long)(x0 + po) * sx] = o;
+        }
+        a0 = a1;
+        a1 = a2;
+        a2 = a3;
+        a3 = a4;
+        a4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        ps = psn;
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_fn2() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+bool make_plane_map(CUtensorMap *m, const float *base, int F, int nz, int ny, long nxd, int bz, int by) {
+    EncodeTiledFn f = encode_fn2();
+    if (!f) return false;
+    cuuint64_t dims[4] = {(cuuint64_t)F, (cuuint64_t)nz, (cuuint64_t)ny, (cuuint64_t)nxd};
+    cuuint64_t strides[3] = {(cuuint64_t)F * 4, (cuuint64_t)F * 4 * nz, (cuuint64_t)F * 4 * nz * ny};
+    cuuint32_t box[4] = {16, (cuuint32_t)bz, (cuuint32_t)by, 1};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    return f(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+bool stencil_tma_supported(const mlmd_domain *h) {
+    return encode_fn2() != nullptr && h->ny % SY == 0 && h->nz % SZ == 0 && h->nx >= 5 && h->ld % 8 == 0;
+}
+
+cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
+                               float tau, int *nlaunch) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(stencil_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int F = 2 * h->ld;
+    CUtensorMap mc, mz, my;
+    const long nxd = (long)h->nx * h->ndom;
+    if (!make_plane_map(&mc, (const float *)w, F, h->nz, h->ny, nxd, SZ, SY)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&mz, (const float *)w, F, h->nz, h->ny, nxd, 2, SY)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&my, (const float *)w, F, h->nz, h->ny, nxd, SZ, 2)) return cudaErrorInvalidValue;
+    TmaStencilParams P;
+    P.psi = (const float4 *)psi;
+    P.out = (float4 *)out;
+    P.vloc = h->vloc();
+    P.coef = coef;
+    P.tau = tau;
+    P.nx = h->nx;
+    P.ny = h->ny;
+    P.nz = h->nz;
+    P.lanes = h->ld / 2;
+    P.nchunk = h->ld / 8;
+    const long base = (long)h->ndom * P.nchunk * (h->ny / SY) * (h->nz / SZ);
+    int nxseg = 1;
+    while (base * nxseg < 2 * 148 && h->nx / (nxseg * 2) >= 8) nxseg *= 2;
+    const char *env = getenv("MLMD_XSEG");
+    if (env && atoi(env) > 0) nxseg = (h->nx + atoi(env) - 1) / atoi(env);
+    P.xs = (h->nx + nxseg - 1) / nxseg;
+    P.nxseg = (h->nx + P.xs - 1) / P.xs;
+    const long grid = base * P.nxseg;
+    ++*nlaunch;
+    if (h->field_yz)
+        stencil_tma_kernel<true><<<(unsigned)grid, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+    else
+        stencil_tma_kernel<false><<<(unsigned)grid, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+    return cudaGetLastError();
+}
+
+}  // namespace mlmd
