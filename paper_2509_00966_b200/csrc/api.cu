@@ -418,7 +418,7 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
                 }
                 {
                     ProfScope ps(h, MLMD_K_STENCIL);
-                    CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, tau, &nl));
+                    CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr, tau, &nl));
                 }
                 if (h->nproj > 0) {
                     int rc = nonlocal_back(h, dst[i], &nl);

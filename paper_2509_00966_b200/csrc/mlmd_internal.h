@@ -88,13 +88,15 @@ namespace mlmd {
 //   out(r,n) = psi(r,n) + (-i tau) [ sum_{d,j} a_{d,j} w(r + j e_d, n) + (centre + V(r)) w(r,n) ]
 // w, psi, out: [ndom][ngrid][ld] complex64; coef: [ndom] for this step; out may alias psi.
 cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
-                                 const StepCoef *coef, float tau, int *nlaunch);
+                                 const StepCoef *coef, const StepCoef *coef_host, float tau, int *nlaunch);
 
 // ---- stencil_tma.cu ---------------------------------------------------------------------------
 // The same stage with TMA-staged x-planes (needs ny % 16 == 0, nz % 16 == 0).
 bool stencil_tma_supported(const mlmd_domain *h);
+// coef_host: the one coefficient set of this step when every domain sees the same field (passed by
+// value through the constant bank), NULL when coef[dom] differs per domain.
 cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
-                               float tau, int *nlaunch);
+                               const StepCoef *coef_host, float tau, int *nlaunch);
 
 // ---- gemm_simt.cu ----------------------------------------------------------------------------
 // Projection (S2a): zpart[dom][s][p][c] = sum_{r in slice s} B[dom][r][p] * Y[dom][r][c]

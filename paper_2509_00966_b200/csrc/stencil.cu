@@ -178,7 +178,7 @@ static int env_int(const char *name, int dflt) {
 }
 
 cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
-                                 const StepCoef *coef, float tau, int *nlaunch) {
+                                 const StepCoef *coef, const StepCoef *coef_host, float tau, int *nlaunch) {
     StencilParams P;
     P.w = (const float4 *)w;
     P.psi = (const float4 *)psi;
@@ -191,7 +191,7 @@ cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const fl
     P.nz = h->nz;
     P.lanes = h->ld / 2;
     const int variant = env_int("MLMD_STENCIL", 2);   // 0: simple (cross-check), 1: register marching, 2: TMA planes
-    if (variant == 2 && stencil_tma_supported(h)) return launch_stencil_tma(h, w, psi, out, coef, tau, nlaunch);
+    if (variant == 2 && stencil_tma_supported(h)) return launch_stencil_tma(h, w, psi, out, coef, coef_host, tau, nlaunch);
     const int xseg_env = env_int("MLMD_XSEG", 0);     // tuning override: planes per CTA
     ++*nlaunch;
     const bool tile_ok = (h->ny % 8 == 0) && (h->nz % 8 == 0);

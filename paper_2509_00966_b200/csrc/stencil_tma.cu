@@ -24,15 +24,16 @@ constexpr int SY = 16, SZ = 16, SL = 4;            // patch: 16 y x 16 z x 4 flo
 constexpr int S_CENTER = SY * SZ * 64;             // bytes
 constexpr int S_STRIP = 2 * 16 * 64;
 constexpr int S_PLANE = S_CENTER + 4 * S_STRIP;    // centre, z-lo, z-hi, y-lo, y-hi
-constexpr int S_NBUF = 6, S_PF = 4;
-constexpr int S_THREADS = SY * SZ * SL;            // 1024
-constexpr int S_SMEM = S_NBUF * S_PLANE + 1024 + 256;
+constexpr int S_NBUF = 8, S_PF = 5;              // power of two: buffer index and phase by mask/shift
+constexpr int S_THREADS = SY * (SZ / 2) * SL;      // 512: every thread owns the points (y, z) and (y, z + 8)
+constexpr int S_SMEM = S_NBUF * S_PLANE + 256;
 
 struct TmaStencilParams {
     const float4 *psi;
     float4 *out;
     const float *vloc;
-    const StepCoef *coef;
+    const StepCoef *coef;    // per-domain coefficients (PERDOM variant)
+    StepCoef cval;           // the single coefficient set when the field is the same for every domain
     float tau;
     int nx, ny, nz, lanes;   // lanes = float4 per grid point
     int xs, nxseg;           // planes per CTA, segments per domain
@@ -78,15 +79,14 @@ __device__ __forceinline__ void pair_acc_real(float4 &acc, const float4 a, const
     acc.w = fmaf(p, a.w + b.w, acc.w);
 }
 
-template <bool AYZ>
+template <bool AYZ, bool PERDOM>
 __global__ void __launch_bounds__(S_THREADS, 1)
 stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_z,
                    const __grid_constant__ CUtensorMap map_y, const TmaStencilParams P) {
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t *full = (uint64_t *)(smem + S_NBUF * S_PLANE), *empty = full + S_NBUF;
     const int tid = threadIdx.x;
-    const int l = tid % SL, tz = (tid / SL) % SZ, ty = tid / (SL * SZ);
+    const int l = tid % SL, tz = (tid / SL) % (SZ / 2), ty = tid / (SL * SZ / 2);   // tz in 0..7
 
     // work item
     int item = blockIdx.x;
@@ -134,7 +134,9 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     if (tid == 0)
         for (int n = 0; n < S_PF && n < nplanes; ++n) issue(n);
 
-    // byte offsets of the own point and the eight in-plane neighbours inside a plane buffer
+    // Byte offsets inside a plane buffer.  Point A = (ty, tz), point B = (ty, tz + 8): B's centre and
+    // y-neighbour offsets are A's + 512; z-neighbours that stay inside the centre box are +-64/128 from
+    // the own offset, only A's z-1, z-2 and B's z+1, z+2 can fall into a halo strip.
     const uint32_t own = (uint32_t)((ty * SZ + tz) * 64 + l * 16);
     auto zoff = [&](int t) -> uint32_t {
         if (t < 0) return (uint32_t)(S_CENTER + (ty * 2 + (t + 2)) * 64 + l * 16);
@@ -146,75 +148,107 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         if (t >= SY) return (uint32_t)(S_CENTER + 3 * S_STRIP + ((t - SY) * SZ + tz) * 64 + l * 16);
         return (uint32_t)((t * SZ + tz) * 64 + l * 16);
     };
-    const uint32_t ozp1 = zoff(tz + 1), ozm1 = zoff(tz - 1), ozp2 = zoff(tz + 2), ozm2 = zoff(tz - 2);
+    const uint32_t oAzm1 = zoff(tz - 1), oAzm2 = zoff(tz - 2), oBzp1 = zoff(tz + 9), oBzp2 = zoff(tz + 10);
     const uint32_t oyp1 = yoff(ty + 1), oym1 = yoff(ty - 1), oyp2 = yoff(ty + 2), oym2 = yoff(ty - 2);
 
-    const StepCoef c = P.coef[dom];
+    const StepCoef c = PERDOM ? P.coef[dom] : P.cval;   // by-value copy lives in the constant bank: no registers
     const long sz = P.lanes, sy = sz * P.nz, sx = sy * P.ny;
     const long pbase = (long)dom * sx * P.nx + (long)(y0 + ty) * sy + (long)(z0 + tz) * sz + chunk * SL + l;
     const float *vd = P.vloc + ((long)dom * P.nx * P.ny + (y0 + ty)) * P.nz + (z0 + tz);
     const long vsx = (long)P.ny * P.nz;
     const uint32_t sbase = smem_u32(smem);
 
-    float4 a0 = make_float4(0.f, 0.f, 0.f, 0.f), a1 = a0, a2 = a0, a3 = a0, a4 = a0;   // planes q-2 .. q+2
-    float4 ps = P.psi[pbase + (long)x0 * sx];   // Horner base of the first output plane
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 a0 = zero4, a1 = zero4, a2 = zero4, a3 = zero4, a4 = zero4;   // point A, planes q-2 .. q+2
+    float4 b0 = zero4, b1 = zero4, b2 = zero4, b3 = zero4, b4 = zero4;   // point B
+    // running element offsets (no per-step 64-bit index arithmetic): Horner base / output of the plane
+    // being completed, V_loc of the plane being consumed.  B = A + 8 grid points along z.
+    const long dB = 8 * sz;
+    const float4 *psi_p = P.psi + pbase + (long)x0 * sx;
+    float4 *out_p = P.out + pbase + (long)x0 * sx;
+    float4 psA = psi_p[0], psB = psi_p[dB];   // Horner base of the first output plane
+    psi_p += sx;
+    int xq = x0 - 2;
+    xq = xq < 0 ? xq + P.nx : xq;
+    const float *vp = vd + (long)xq * vsx;
+    const long vwrap = (long)P.nx * vsx;
+    const int nout = x1 - x0;
 
-    for (int n = 0; n < nplanes; ++n) {
-        const int b = n % S_NBUF;
-        if (tid == 0 && n + S_PF < nplanes) {
-            const int m = n + S_PF;
-            if (m >= S_NBUF) mbar_wait(&empty[m % S_NBUF], ((m / S_NBUF) - 1) & 1);
-            issue(m);
-        }
-        int xq = x0 - 2 + n;
-        xq = xq < 0 ? xq + P.nx : (xq >= P.nx ? xq - P.nx : xq);
-        const float vv = __ldg(vd + (long)xq * vsx);
-        // Horner base of the NEXT output plane (plane x0 + n - 3), prefetched one step ahead
-        const int pn = n - 3;
-        float4 psn = ps;
-        if (pn >= 1 && x0 + pn < x1) psn = P.psi[pbase + (long)(x0 + pn) * sx];
-
-        mbar_wait(&full[b], (n / S_NBUF) & 1);
-        const uint32_t buf = sbase + b * S_PLANE;
-        const float4 u = lds4(buf + own);
-        const float cen = c.centre + vv;
-        a2.x = fmaf(cen, u.x, a2.x);
-        a2.y = fmaf(cen, u.y, a2.y);
-        a2.z = fmaf(cen, u.z, a2.z);
-        a2.w = fmaf(cen, u.w, a2.w);
+    auto point = [&](const uint32_t buf, const uint32_t o, const uint32_t ozm1, const uint32_t ozm2, const uint32_t ozp1,
+                     const uint32_t ozp2, const uint32_t dy, const float cen, float4 &A0, float4 &A1, float4 &A2,
+                     float4 &A3, float4 &A4) {
+        const float4 u = lds4(buf + o);
+        A2.x = fmaf(cen, u.x, A2.x);
+        A2.y = fmaf(cen, u.y, A2.y);
+        A2.z = fmaf(cen, u.z, A2.z);
+        A2.w = fmaf(cen, u.w, A2.w);
         {
-            const float4 p1 = lds4(buf + oyp1), m1 = lds4(buf + oym1);
-            if (AYZ) pair_acc(a2, p1, m1, c.p[1][0], c.q[1][0]); else pair_acc_real(a2, p1, m1, c.p[1][0]);
-            const float4 p2 = lds4(buf + oyp2), m2 = lds4(buf + oym2);
-            if (AYZ) pair_acc(a2, p2, m2, c.p[1][1], c.q[1][1]); else pair_acc_real(a2, p2, m2, c.p[1][1]);
+            const float4 p1 = lds4(buf + oyp1 + dy), m1 = lds4(buf + oym1 + dy);
+            if (AYZ) pair_acc(A2, p1, m1, c.p[1][0], c.q[1][0]); else pair_acc_real(A2, p1, m1, c.p[1][0]);
+            const float4 p2 = lds4(buf + oyp2 + dy), m2 = lds4(buf + oym2 + dy);
+            if (AYZ) pair_acc(A2, p2, m2, c.p[1][1], c.q[1][1]); else pair_acc_real(A2, p2, m2, c.p[1][1]);
         }
         {
             const float4 p1 = lds4(buf + ozp1), m1 = lds4(buf + ozm1);
-            if (AYZ) pair_acc(a2, p1, m1, c.p[2][0], c.q[2][0]); else pair_acc_real(a2, p1, m1, c.p[2][0]);
+            if (AYZ) pair_acc(A2, p1, m1, c.p[2][0], c.q[2][0]); else pair_acc_real(A2, p1, m1, c.p[2][0]);
             const float4 p2 = lds4(buf + ozp2), m2 = lds4(buf + ozm2);
-            if (AYZ) pair_acc(a2, p2, m2, c.p[2][1], c.q[2][1]); else pair_acc_real(a2, p2, m2, c.p[2][1]);
+            if (AYZ) pair_acc(A2, p2, m2, c.p[2][1], c.q[2][1]); else pair_acc_real(A2, p2, m2, c.p[2][1]);
         }
         // x taps: u = w(plane q) is the +j neighbour of plane q-j (coefficient p_j - i q_j) and the -j
         // neighbour of plane q+j (coefficient p_j + i q_j)
-        cmul_acc(a1, u, c.p[0][0], -c.q[0][0]);
-        cmul_acc(a3, u, c.p[0][0], c.q[0][0]);
-        cmul_acc(a0, u, c.p[0][1], -c.q[0][1]);
-        cmul_acc(a4, u, c.p[0][1], c.q[0][1]);
+        cmul_acc(A1, u, c.p[0][0], -c.q[0][0]);
+        cmul_acc(A3, u, c.p[0][0], c.q[0][0]);
+        cmul_acc(A0, u, c.p[0][1], -c.q[0][1]);
+        cmul_acc(A4, u, c.p[0][1], c.q[0][1]);
+    };
+    // One plane step.  A0..A4 / B0..B4 are the accumulators of planes q-2..q+2; the caller rotates the
+    // names, so the ring costs no register moves.
+    auto step = [&](const int n, float4 &A0, float4 &A1, float4 &A2, float4 &A3, float4 &A4, float4 &B0, float4 &B1,
+                    float4 &B2, float4 &B3, float4 &B4) {
+        const int b = n & (S_NBUF - 1);
+        if (tid == 0 && n + S_PF < nplanes) {
+            const int m = n + S_PF;
+            if (m >= S_NBUF) mbar_wait(&empty[m & (S_NBUF - 1)], ((m / S_NBUF) - 1) & 1);
+            issue(m);
+        }
+        const float vA = __ldg(vp), vB = __ldg(vp + 8);
+        vp += vsx;
+        if (++xq == P.nx) {
+            xq = 0;
+            vp -= vwrap;
+        }
+        // Horner base of the NEXT output plane (n - 3), prefetched one step ahead of its use
+        float4 pnA = psA, pnB = psB;
+        if (n >= 4 && n - 3 < nout) {
+            pnA = psi_p[0];
+            pnB = psi_p[dB];
+            psi_p += sx;
+        }
+        mbar_wait(&full[b], (n / S_NBUF) & 1);
+        const uint32_t buf = sbase + b * S_PLANE;
+        point(buf, own, oAzm1, oAzm2, own + 64, own + 128, 0u, c.centre + vA, A0, A1, A2, A3, A4);
+        point(buf, own + 512, own + 512 - 64, own + 512 - 128, oBzp1, oBzp2, 512u, c.centre + vB, B0, B1, B2, B3, B4);
         __syncwarp();
         if (tid % 32 == 0) mbar_arrive(&empty[b]);
-        // plane q-2 is complete
-        const int po = n - 4;
-        if (po >= 0 && x0 + po < x1) {
-            const float4 o = make_float4(fmaf(P.tau, a0.y, ps.x), fmaf(-P.tau, a0.x, ps.y), fmaf(P.tau, a0.w, ps.z),
-                                         fmaf(-P.tau, a0.z, ps.w));
-            P.out[pbase + (long)(x0 + po) * sx] = o;
+        // plane q-2 (output n - 4) is complete
+        if (n >= 4) {
+            out_p[0] = make_float4(fmaf(P.tau, A0.y, psA.x), fmaf(-P.tau, A0.x, psA.y), fmaf(P.tau, A0.w, psA.z),
+                                   fmaf(-P.tau, A0.z, psA.w));
+            out_p[dB] = make_float4(fmaf(P.tau, B0.y, psB.x), fmaf(-P.tau, B0.x, psB.y), fmaf(P.tau, B0.w, psB.z),
+                                    fmaf(-P.tau, B0.z, psB.w));
+            out_p += sx;
         }
-        a0 = a1;
-        a1 = a2;
-        a2 = a3;
-        a3 = a4;
-        a4 = make_float4(0.f, 0.f, 0.f, 0.f);
-        ps = psn;
+        A0 = zero4;
+        B0 = zero4;
+        psA = pnA;
+        psB = pnB;
+    };
+    for (int n = 0; n < nplanes; n += 5) {
+        step(n, a0, a1, a2, a3, a4, b0, b1, b2, b3, b4);
+        if (n + 1 < nplanes) step(n + 1, a1, a2, a3, a4, a0, b1, b2, b3, b4, b0);
+        if (n + 2 < nplanes) step(n + 2, a2, a3, a4, a0, a1, b2, b3, b4, b0, b1);
+        if (n + 3 < nplanes) step(n + 3, a3, a4, a0, a1, a2, b3, b4, b0, b1, b2);
+        if (n + 4 < nplanes) step(n + 4, a4, a0, a1, a2, a3, b4, b0, b1, b2, b3);
     }
 }
 
@@ -252,12 +286,13 @@ bool stencil_tma_supported(const mlmd_domain *h) {
 }
 
 cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
-                               float tau, int *nlaunch) {
+                               const StepCoef *coef_host, float tau, int *nlaunch) {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(stencil_tma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -287,10 +322,16 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
     P.nxseg = (h->nx + P.xs - 1) / P.xs;
     const long grid = base * P.nxseg;
     ++*nlaunch;
-    if (h->field_yz)
-        stencil_tma_kernel<true><<<(unsigned)grid, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
-    else
-        stencil_tma_kernel<false><<<(unsigned)grid, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+    const unsigned g = (unsigned)grid;
+    if (coef_host) {
+        P.cval = *coef_host;
+        if (h->field_yz) stencil_tma_kernel<true, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+        else stencil_tma_kernel<false, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+    } else {
+        P.cval = StepCoef();
+        if (h->field_yz) stencil_tma_kernel<true, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+        else stencil_tma_kernel<false, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+    }
     return cudaGetLastError();
 }
 
