@@ -23,13 +23,13 @@ namespace {
 constexpr int SY = 16, SZ = 16, SL = 4;            // patch: 16 y x 16 z x 4 float4 lanes
 constexpr int S_CENTER = SY * SZ * 64;             // bytes
 constexpr int S_STRIP = 2 * 16 * 64;
-constexpr int S_PLANE = S_CENTER + 4 * S_STRIP;    // centre, z-lo, z-hi, y-lo, y-hi
-constexpr int S_NBUF = 8, S_PF = 5;              // power of two: buffer index and phase by mask/shift
+constexpr int S_PLANE_W = S_CENTER + 4 * S_STRIP;  // w: centre, z-lo, z-hi, y-lo, y-hi
+constexpr int S_PLANE = S_PLANE_W + S_CENTER;      // + the Horner base psi of the plane completed by this step
+constexpr int S_NBUF = 5, S_PF = 3;                // NBUF = unroll factor of the march: buffer index is static
 constexpr int S_THREADS = SY * (SZ / 2) * SL;      // 512: every thread owns the points (y, z) and (y, z + 8)
 constexpr int S_SMEM = S_NBUF * S_PLANE + 256;
 
 struct TmaStencilParams {
-    const float4 *psi;
     float4 *out;
     const float *vloc;
     const StepCoef *coef;    // per-domain coefficients (PERDOM variant)
@@ -82,7 +82,8 @@ __device__ __forceinline__ void pair_acc_real(float4 &acc, const float4 a, const
 template <bool AYZ, bool PERDOM>
 __global__ void __launch_bounds__(S_THREADS, 1)
 stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_z,
-                   const __grid_constant__ CUtensorMap map_y, const TmaStencilParams P) {
+                   const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_p,
+                   const TmaStencilParams P) {
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t *full = (uint64_t *)(smem + S_NBUF * S_PLANE), *empty = full + S_NBUF;
     const int tid = threadIdx.x;
@@ -102,6 +103,7 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const int x0 = seg * P.xs;
     const int x1 = min(x0 + P.xs, P.nx);
     const int nplanes = (x1 - x0) + 4;
+    const int nout = x1 - x0;
     const int y0 = yt * SY, z0 = zt * SZ;
 
     if (tid == 0) {
@@ -113,6 +115,7 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         prefetch_tmap(&map_c);
         prefetch_tmap(&map_z);
         prefetch_tmap(&map_y);
+        prefetch_tmap(&map_p);
     }
     __syncthreads();
 
@@ -124,7 +127,10 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         x = x < 0 ? x + P.nx : (x >= P.nx ? x - P.nx : x);
         const int xr = dom * P.nx + x;
         uint8_t *buf = smem + b * S_PLANE;
-        mbar_expect_tx(&full[b], S_PLANE);
+        const int po = n - 4;   // output plane completed by step n: its Horner base travels with plane n
+        const bool with_psi = po >= 0 && po < nout;
+        mbar_expect_tx(&full[b], with_psi ? S_PLANE : S_PLANE_W);
+        if (with_psi) tma_load_4d(buf + S_PLANE_W, &map_p, &full[b], chunk * 16, z0, y0, dom * P.nx + x0 + po);
         tma_load_4d(buf, &map_c, &full[b], chunk * 16, z0, y0, xr);
         tma_load_4d(buf + S_CENTER, &map_z, &full[b], chunk * 16, zlo, y0, xr);
         tma_load_4d(buf + S_CENTER + S_STRIP, &map_z, &full[b], chunk * 16, zhi, y0, xr);
@@ -164,15 +170,11 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // running element offsets (no per-step 64-bit index arithmetic): Horner base / output of the plane
     // being completed, V_loc of the plane being consumed.  B = A + 8 grid points along z.
     const long dB = 8 * sz;
-    const float4 *psi_p = P.psi + pbase + (long)x0 * sx;
     float4 *out_p = P.out + pbase + (long)x0 * sx;
-    float4 psA = psi_p[0], psB = psi_p[dB];   // Horner base of the first output plane
-    psi_p += sx;
     int xq = x0 - 2;
     xq = xq < 0 ? xq + P.nx : xq;
     const float *vp = vd + (long)xq * vsx;
     const long vwrap = (long)P.nx * vsx;
-    const int nout = x1 - x0;
 
     auto point = [&](const uint32_t buf, const uint32_t o, const uint32_t ozm1, const uint32_t ozm2, const uint32_t ozp1,
                      const uint32_t ozp2, const uint32_t dy, const float cen, float4 &A0, float4 &A1, float4 &A2,
@@ -203,12 +205,12 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     };
     // One plane step.  A0..A4 / B0..B4 are the accumulators of planes q-2..q+2; the caller rotates the
     // names, so the ring costs no register moves.
-    auto step = [&](const int n, float4 &A0, float4 &A1, float4 &A2, float4 &A3, float4 &A4, float4 &B0, float4 &B1,
-                    float4 &B2, float4 &B3, float4 &B4) {
-        const int b = n & (S_NBUF - 1);
+    auto step = [&](const int n, const int k, const int it, float4 &A0, float4 &A1, float4 &A2, float4 &A3, float4 &A4,
+                    float4 &B0, float4 &B1, float4 &B2, float4 &B3, float4 &B4) {
+        // n = 5 it + k: plane n lives in buffer k; its barrier phase is it & 1
         if (tid == 0 && n + S_PF < nplanes) {
-            const int m = n + S_PF;
-            if (m >= S_NBUF) mbar_wait(&empty[m & (S_NBUF - 1)], ((m / S_NBUF) - 1) & 1);
+            const int m = n + S_PF, bm = (k + S_PF) % S_NBUF, um = it + (k + S_PF) / S_NBUF;   // um-th use of buffer bm
+            if (um >= 1) mbar_wait(&empty[bm], (um - 1) & 1);
             issue(m);
         }
         const float vA = __ldg(vp), vB = __ldg(vp + 8);
@@ -217,38 +219,30 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             xq = 0;
             vp -= vwrap;
         }
-        // Horner base of the NEXT output plane (n - 3), prefetched one step ahead of its use
-        float4 pnA = psA, pnB = psB;
-        if (n >= 4 && n - 3 < nout) {
-            pnA = psi_p[0];
-            pnB = psi_p[dB];
-            psi_p += sx;
-        }
-        mbar_wait(&full[b], (n / S_NBUF) & 1);
-        const uint32_t buf = sbase + b * S_PLANE;
+        mbar_wait(&full[k], it & 1);
+        const uint32_t buf = sbase + k * S_PLANE;
         point(buf, own, oAzm1, oAzm2, own + 64, own + 128, 0u, c.centre + vA, A0, A1, A2, A3, A4);
         point(buf, own + 512, own + 512 - 64, own + 512 - 128, oBzp1, oBzp2, 512u, c.centre + vB, B0, B1, B2, B3, B4);
-        __syncwarp();
-        if (tid % 32 == 0) mbar_arrive(&empty[b]);
-        // plane q-2 (output n - 4) is complete
+        // plane q-2 (output n - 4) is complete: out = psi + (-i tau) acc
         if (n >= 4) {
+            const float4 psA = lds4(buf + S_PLANE_W + own), psB = lds4(buf + S_PLANE_W + own + 512);
             out_p[0] = make_float4(fmaf(P.tau, A0.y, psA.x), fmaf(-P.tau, A0.x, psA.y), fmaf(P.tau, A0.w, psA.z),
                                    fmaf(-P.tau, A0.z, psA.w));
             out_p[dB] = make_float4(fmaf(P.tau, B0.y, psB.x), fmaf(-P.tau, B0.x, psB.y), fmaf(P.tau, B0.w, psB.z),
                                     fmaf(-P.tau, B0.z, psB.w));
             out_p += sx;
         }
+        __syncwarp();
+        if (tid % 32 == 0) mbar_arrive(&empty[k]);
         A0 = zero4;
         B0 = zero4;
-        psA = pnA;
-        psB = pnB;
     };
-    for (int n = 0; n < nplanes; n += 5) {
-        step(n, a0, a1, a2, a3, a4, b0, b1, b2, b3, b4);
-        if (n + 1 < nplanes) step(n + 1, a1, a2, a3, a4, a0, b1, b2, b3, b4, b0);
-        if (n + 2 < nplanes) step(n + 2, a2, a3, a4, a0, a1, b2, b3, b4, b0, b1);
-        if (n + 3 < nplanes) step(n + 3, a3, a4, a0, a1, a2, b3, b4, b0, b1, b2);
-        if (n + 4 < nplanes) step(n + 4, a4, a0, a1, a2, a3, b4, b0, b1, b2, b3);
+    for (int n = 0, it = 0; n < nplanes; n += 5, ++it) {
+        step(n, 0, it, a0, a1, a2, a3, a4, b0, b1, b2, b3, b4);
+        if (n + 1 < nplanes) step(n + 1, 1, it, a1, a2, a3, a4, a0, b1, b2, b3, b4, b0);
+        if (n + 2 < nplanes) step(n + 2, 2, it, a2, a3, a4, a0, a1, b2, b3, b4, b0, b1);
+        if (n + 3 < nplanes) step(n + 3, 3, it, a3, a4, a0, a1, a2, b3, b4, b0, b1, b2);
+        if (n + 4 < nplanes) step(n + 4, 4, it, a4, a0, a1, a2, a3, b4, b0, b1, b2, b3);
     }
 }
 
@@ -297,13 +291,13 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
         attr_set = true;
     }
     const int F = 2 * h->ld;
-    CUtensorMap mc, mz, my;
+    CUtensorMap mc, mz, my, mp;
     const long nxd = (long)h->nx * h->ndom;
     if (!make_plane_map(&mc, (const float *)w, F, h->nz, h->ny, nxd, SZ, SY)) return cudaErrorInvalidValue;
     if (!make_plane_map(&mz, (const float *)w, F, h->nz, h->ny, nxd, 2, SY)) return cudaErrorInvalidValue;
     if (!make_plane_map(&my, (const float *)w, F, h->nz, h->ny, nxd, SZ, 2)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&mp, (const float *)psi, F, h->nz, h->ny, nxd, SZ, SY)) return cudaErrorInvalidValue;
     TmaStencilParams P;
-    P.psi = (const float4 *)psi;
     P.out = (float4 *)out;
     P.vloc = h->vloc();
     P.coef = coef;
@@ -325,12 +319,12 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
     const unsigned g = (unsigned)grid;
     if (coef_host) {
         P.cval = *coef_host;
-        if (h->field_yz) stencil_tma_kernel<true, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
-        else stencil_tma_kernel<false, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+        if (h->field_yz) stencil_tma_kernel<true, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
     } else {
         P.cval = StepCoef();
-        if (h->field_yz) stencil_tma_kernel<true, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
-        else stencil_tma_kernel<false, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, P);
+        if (h->field_yz) stencil_tma_kernel<true, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
     }
     return cudaGetLastError();
 }
