@@ -48,7 +48,8 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     pl->ld = round_up_i(norb, 16);      // 2*ld floats per row = whole 128-byte TMA chunks
     pl->ngrid = (long)nx * ny * nz;
     pl->ldp_max = round_up_i(std::max(nproj_max, 1), 8);
-    pl->prows = std::max(pl->ldp_max, 2 * pl->ld);
+    // rows of Z / W per (domain, slice): whole 128-row accumulator blocks of the tcgen05 projection
+    pl->prows = round_up_i(std::max(pl->ldp_max, 2 * pl->ld), 128);
     const long tiles = (long)((2 * pl->ld + 63) / 64) * std::max(1, (nproj_max + 63) / 64) * ndom;
     long ns = (592 + tiles - 1) / tiles;
     ns = std::min<long>(ns, std::min<long>(kMaxSplit, pl->ngrid / 64));

@@ -76,6 +76,43 @@ bool make_k8_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols
              CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// (cols, rows) view with a [128 rows x 32 floats] box in the plain 128-byte swizzle: epilogue staging tiles
+bool make_out_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch) {
+    EncodeTiledFn f = encode_fn();
+    if (!f) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {pitch * sizeof(float)};
+    cuuint32_t box[2] = {32, 128};
+    cuuint32_t es[2] = {1, 1};
+    return f(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+constexpr int EPI_TILE_BYTES = 128 * 128;   // one staging tile: 128 rows x 32 floats
+constexpr int EPI_BAR = 1;                  // named barrier of the 128 epilogue threads
+
+// The 128 epilogue threads hand one [128 x 32] FP32 tile (thread r holds row r in v) to the TMA engine,
+// which stores it or adds it (L2 reduction, round-to-nearest) into global memory at (c0, row0).
+// Two staging tiles alternate; `slot` counts tiles issued so far by this group.
+__device__ __forceinline__ void epi_tile_out(uint8_t *stage, int &slot, const CUtensorMap *map, int c0, int row0,
+                                             const uint32_t (&v)[32], int r, bool add) {
+    uint8_t *buf = stage + (slot & 1) * EPI_TILE_BYTES;
+    if (r == 0) bulk_wait_read<1>();          // the tile issued two slots ago has left this buffer
+    named_bar_sync(EPI_BAR, 128);
+    const uint32_t rowaddr = smem_u32(buf) + r * 128;
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+        sts4(rowaddr + (((uint32_t)j ^ ((uint32_t)r & 7u)) << 4), v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+    fence_proxy_async_smem();
+    named_bar_sync(EPI_BAR, 128);
+    if (r == 0) {
+        if (add) tma_reduce_add_2d(map, buf, c0, row0);
+        else tma_store_2d(map, buf, c0, row0);
+        bulk_commit();
+    }
+    ++slot;
+}
+
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 // in place: v -> hi (TF32-representable), returns lo = v - hi (exact)
 __device__ __forceinline__ float4 split4(float4 &v) {
@@ -95,7 +132,7 @@ constexpr int PJ_MAXBN = 224;
 constexpr int PJ_A_BYTES = 8 * PJ_BK * 128;            // 8 chunks of 32 p  = 256 rows p
 constexpr int PJ_Y_BYTES = (PJ_MAXBN / 32) * PJ_BK * 128;
 constexpr int PJ_STAGE_BYTES = 2 * PJ_A_BYTES + 2 * PJ_Y_BYTES;
-constexpr int PJ_SMEM = PJ_STAGES * PJ_STAGE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int PJ_SMEM = PJ_STAGES * PJ_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int PJ_THREADS = 192;          // warp 0 TMA, warp 1 MMA, warps 2-5 convert + epilogue
 
 struct ProjParams {
@@ -105,10 +142,11 @@ struct ProjParams {
 
 __global__ void __launch_bounds__(PJ_THREADS, 1)
 proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
-               const __grid_constant__ CUtensorMap map_y, const ProjParams q) {
+               const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_z, const ProjParams q) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint64_t *bars = (uint64_t *)(smem + PJ_STAGES * PJ_STAGE_BYTES);
+    uint8_t *stage = smem + PJ_STAGES * PJ_STAGE_BYTES;
+    uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
     uint64_t *full = bars, *empty = bars + PJ_STAGES, *conv = bars + 2 * PJ_STAGES;
     uint64_t *acc_full = bars + 3 * PJ_STAGES, *acc_empty = acc_full + 1;
     uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
@@ -126,6 +164,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         prefetch_tmap(&map_ahi);
         prefetch_tmap(&map_alo);
         prefetch_tmap(&map_y);
+        prefetch_tmap(&map_z);
     }
     if (warp == 1) tmem_alloc(tmem_slot, 512);
     tc_fence_before();
@@ -220,13 +259,13 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     } else {
         const int t = threadIdx.x - 64;   // 0..127
         const int quarter = warp % 4;
-        int it = 0, nd = 0;
+        const int er = quarter * 32 + lane;   // TMEM lane = accumulator row of this thread; er == 0 leads the TMA stores
+        int it = 0, nd = 0, slot = 0;
         const int ny4 = q.BN / 32 * PJ_BK * 8;    // float4 count of the Y tile
         for (int u = blockIdx.x; u < total; u += gridDim.x) {
             int dom, mt, nt, kb0, kb1;
             decode(u, dom, mt, nt, kb0, kb1);
             const int sp = (u / q.ntile_n) % q.nsplit;
-            float *zd = q.zpart + ((size_t)dom * q.nsplit + sp) * q.prows * q.N;
             const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
             for (int c0k = kb0; c0k < kb1; c0k += q.chain) {
                 const int c1k = min(c0k + q.chain, kb1);
@@ -261,32 +300,23 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 ++nd;
                 tc_fence_after();
                 const bool add = c0k > kb0;
+                // the store of the slice's first chain must have landed before later chains add to it
+                if (add && c0k == kb0 + q.chain && er == 0) bulk_wait<0>();
+                const int zrow = (dom * q.nsplit + sp) * q.prows + mt * 256;
                 for (int mb = 0; mb < nblk; ++mb) {
-                    const int p = mt * 256 + mb * 128 + quarter * 32 + lane;
                     for (int cb = 0; cb < q.BN / 32; ++cb) {
                         uint32_t v[32];
                         tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + mb * q.BN + cb * 32, v);
                         tmem_ld_wait();
                         const int c0 = nt * q.BN + cb * 32;
-                        if (p < q.P && c0 < q.N) {
-                            float4 *dst = (float4 *)(zd + (size_t)p * q.N + c0);
-#pragma unroll
-                            for (int j = 0; j < 8; ++j) {
-                                const float a = __uint_as_float(v[4 * j]), b = __uint_as_float(v[4 * j + 1]),
-                                            c = __uint_as_float(v[4 * j + 2]), d = __uint_as_float(v[4 * j + 3]);
-                                // every element has one owner thread, so the order of adds is fixed (reading D22)
-                                if (add)
-                                    red_add_v4((float *)(dst + j), a, b, c, d);
-                                else
-                                    dst[j] = make_float4(a, b, c, d);
-                            }
-                        }
+                        if (c0 < q.N) epi_tile_out(stage, slot, &map_z, c0, zrow + mb * 128, v, er, add);
                     }
                 }
                 tc_fence_before();
                 mbar_arrive(acc_empty);
             }
         }
+        if (er == 0) bulk_wait<0>();
     }
     tc_fence_before();
     __syncthreads();
@@ -305,8 +335,8 @@ constexpr int BK_MAXBN = 448;
 constexpr int BK_A_BYTES = 128 * 32;                    // [128 rows x 8 floats], SWIZZLE_32B
 constexpr int BK_W_BYTES = (BK_MAXBN / 32) * 1024;      // chunks of [8 rows x 128 B], SWIZZLE_128B
 constexpr int BK_STAGE_BYTES = 2 * BK_A_BYTES + 2 * BK_W_BYTES;
-constexpr int BK_SMEM = BK_STAGES * BK_STAGE_BYTES + 1024 + 256;
-constexpr int BK_EPI_WARPS = 8;
+constexpr int BK_SMEM = BK_STAGES * BK_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 256;
+constexpr int BK_EPI_WARPS = 4;
 constexpr int BK_THREADS = 64 + 32 * BK_EPI_WARPS;
 
 struct BackParams {
@@ -317,10 +347,11 @@ struct BackParams {
 __global__ void __launch_bounds__(BK_THREADS, 1)
 back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
                const __grid_constant__ CUtensorMap map_whi, const __grid_constant__ CUtensorMap map_wlo,
-               const BackParams q) {
+               const __grid_constant__ CUtensorMap map_out, const BackParams q) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint64_t *bars = (uint64_t *)(smem + BK_STAGES * BK_STAGE_BYTES);
+    uint8_t *stage = smem + BK_STAGES * BK_STAGE_BYTES;
+    uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
     uint64_t *full = bars, *empty = bars + BK_STAGES;
     uint64_t *acc_full = bars + 2 * BK_STAGES, *acc_empty = acc_full + 1;
     uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
@@ -338,6 +369,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         prefetch_tmap(&map_alo);
         prefetch_tmap(&map_whi);
         prefetch_tmap(&map_wlo);
+        prefetch_tmap(&map_out);
     }
     if (warp == 1) tmem_alloc(tmem_slot, 512);
     tc_fence_before();
@@ -406,31 +438,26 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
             }
         }
     } else {
-        const int ew = warp - 2;                    // 0..7
         const int quarter = warp % 4;
-        const int par = ew / 4;                     // which half of the column blocks this warp takes
-        int nu = 0;
+        const int er = quarter * 32 + lane;         // accumulator row of this thread
+        int nu = 0, slot = 0;
         for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
             const int nt = u % q.ntile_n, rt = (u / q.ntile_n) % nrt, dom = u / (q.ntile_n * nrt);
-            const size_t r = (size_t)dom * q.ngrid + rt * 128 + quarter * 32 + lane;
+            const int row0 = dom * q.ngrid + rt * 128;
             mbar_wait(acc_full, nu & 1);
             tc_fence_after();
-            for (int cb = par; cb < q.BN / 32; cb += BK_EPI_WARPS / 4) {
+            for (int cb = 0; cb < q.BN / 32; ++cb) {
                 uint32_t v[32];
                 tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
                 tmem_ld_wait();
                 const int c0 = nt * q.BN + cb * 32;
-                if (c0 < q.N) {
-                    float *dst = q.Y + r * q.ldy + c0;
-#pragma unroll
-                    for (int j = 0; j < 8; ++j)
-                        red_add_v4(dst + 4 * j, __uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
-                                   __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
-                }
+                // Y += tile through the TMA engine: the add happens in L2, nothing is read back into the SM
+                if (c0 < q.N) epi_tile_out(stage, slot, &map_out, c0, row0, v, er, true);
             }
             tc_fence_before();
             mbar_arrive(acc_empty);
         }
+        if (er == 0) bulk_wait<0>();
     }
     tc_fence_before();
     __syncthreads();
@@ -503,10 +530,12 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     if (!make_chunk_map(&ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;
     if (!make_chunk_map(&mal, A_lo ? A_lo : A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;
     if (!make_chunk_map(&my, Y, rows, ldy, N / 32, PJ_BK, q.BN / 32)) return cudaErrorInvalidValue;
+    CUtensorMap mz;
+    if (!make_out_map(&mz, zpart, (uint64_t)ndom * nsplit * prows, N, N)) return cudaErrorInvalidValue;
     const int total = ndom * q.ntile_m * q.ntile_n * nsplit;
     const int grid = total < num_sms() ? total : num_sms();
     ++*nlaunch;
-    proj_tc_kernel<<<grid, PJ_THREADS, PJ_SMEM, st>>>(ma, mal, my, q);
+    proj_tc_kernel<<<grid, PJ_THREADS, PJ_SMEM, st>>>(ma, mal, my, mz, q);
     return cudaGetLastError();
 }
 
@@ -537,10 +566,12 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     if (!make_k8_map(&mal, A_lo, rows, lda, lda, 128)) return cudaErrorInvalidValue;
     if (!make_chunk_map(&mw, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, q.BN / 32)) return cudaErrorInvalidValue;
     if (!make_chunk_map(&mwl, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, q.BN / 32)) return cudaErrorInvalidValue;
+    CUtensorMap mo;
+    if (!make_out_map(&mo, Y, rows, N, ldy)) return cudaErrorInvalidValue;
     const int total = ndom * (int)(ngrid / 128) * q.ntile_n;
     const int grid = total < num_sms() ? total : num_sms();
     ++*nlaunch;
-    back_tc_kernel<<<grid, BK_THREADS, BK_SMEM, st>>>(ma, mal, mw, mwl, q);
+    back_tc_kernel<<<grid, BK_THREADS, BK_SMEM, st>>>(ma, mal, mw, mwl, mo, q);
     return cudaGetLastError();
 }
 
