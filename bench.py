@@ -91,6 +91,19 @@ def algorithmic(c, gemm_real=True):
             "density_bytes": elems * 8, "gemm_flops_each": gemm_flops_each, "gemm_flops_step": 8 * gemm_flops_each}
 
 
+def ncu_traffic(c, kernel_class):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the class's kernel from the committed
+    `ncu --set full` capture of the same workload (profiles/r1_traffic_cfg3.json), else None."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic_cfg3.json")
+    if c.cfg != 3 or c.ndom != 64 or not os.path.exists(path):
+        return None
+    with open(path) as f:
+        t = json.load(f)["dram_bytes_per_launch"]
+    pick = {"stencil": "stencil_tma_kernel<0, 0>", "proj": "proj_tc_kernel", "back": "back_tc_kernel",
+            "density": "density_kernel"}.get(kernel_class)
+    return t.get(pick)
+
+
 def sample_for_oracle(c, d, norb_sample):
     """Domain 0, first norb_sample orbitals: the bounded sample the oracle is timed on."""
     n = min(norb_sample, c.norb)
@@ -304,7 +317,7 @@ def main():
         per_class[name] = entry
     top = max((n for n in per_class if "achieved" in per_class[n]), key=lambda n: per_class[n]["ms_total"])
     roof = {k: per_class[top][k] for k in ("bound", "achieved", "peak", "unit", "frac")}
-    roof.update(kernel=top, traffic=None, peak_source="%s (%s)" % (
+    roof.update(kernel=top, traffic=ncu_traffic(c, top), peak_source="%s (%s)" % (
         "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
         "hbm copy" if roof["bound"] == "hbm" else
         "sustained bf16 x nominal ratio for the mode" if roof["bound"] == "tensor" else "derived FP32/FP64 ALU peak, DESIGN.md"))
