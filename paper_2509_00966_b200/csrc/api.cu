@@ -190,7 +190,12 @@ int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *l
 long long mlmd_launch_count(const mlmd_domain_t *h) { return h ? h->launches : 0; }
 
 static bool use_tensor_cores(const mlmd_domain *h) {
-    return h->tc_ok && (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_TF32X1);
+    return h->tc_ok && (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_TF32X1 ||
+                        h->gemm_mode == MLMD_GEMM_LOWP_BF16);
+}
+// products per MAC on the tensor-core path: 3 = 3xTF32, 1 = TF32x1, 0 = BF16-rounded operands x1
+static int tc_nprod(const mlmd_domain *h) {
+    return h->gemm_mode == MLMD_GEMM_TF32X1 ? 1 : (h->gemm_mode == MLMD_GEMM_LOWP_BF16 ? 0 : 3);
 }
 
 int mlmd_gemm_path(const mlmd_domain_t *h) { return (h && use_tensor_cores(h)) ? 1 : 0; }
@@ -355,14 +360,14 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl)
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, h->gemm_mode == MLMD_GEMM_TF32X1 ? 1 : 3, kProjChain, nl));
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, tc_nprod(h), kProjChain, nl));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
     }
     ProfScope ps(h, MLMD_K_GLUE);
     CU(launch_reduce_scale(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, nsplit, h->zpart(),
-                           h->dprime(), tau, h->what(), h->what_lo(), nl));
+                           h->dprime(), tau, h->what(), h->what_lo(), (tc && h->gemm_mode == MLMD_GEMM_LOWP_BF16) ? 1 : 0, nl));
     return MLMD_OK;
 }
 
@@ -371,7 +376,7 @@ static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl) {
     ProfScope ps(h, MLMD_K_BACK);
     if (use_tensor_cores(h))
         CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
-                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, h->gemm_mode == MLMD_GEMM_TF32X1 ? 1 : 3, nl));
+                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, tc_nprod(h), nl));
     else
         CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
                             (float *)out, 2 * h->ld, 2 * h->ld, h->prows, fp64, nl));

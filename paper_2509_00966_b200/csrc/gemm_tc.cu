@@ -122,6 +122,16 @@ __device__ __forceinline__ float4 split4(float4 &v) {
     return l;
 }
 
+// round-to-nearest-even to BF16 precision, kept in an FP32 container (every BF16 value is a TF32 value)
+__device__ __forceinline__ float bf16_round(float x) {
+    uint32_t u = __float_as_uint(x);
+    u += 0x7fffu + ((u >> 16) & 1u);
+    return __uint_as_float(u & 0xffff0000u);
+}
+__device__ __forceinline__ float4 bf16_round4(const float4 v) {
+    return make_float4(bf16_round(v.x), bf16_round(v.y), bf16_round(v.z), bf16_round(v.w));
+}
+
 // =================================================================================================
 // Projection: Z[p][c] = sum_r A[r][p] * Y[r][c] over one K slice; FP32 partials per slice.
 // CTA tile: up to 256 rows p (two M = 128 UMMA blocks) x BN <= 224 columns; K pipeline of 16 rows.
@@ -136,7 +146,7 @@ constexpr int PJ_SMEM = PJ_STAGES * PJ_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 /
 constexpr int PJ_THREADS = 192;          // warp 0 TMA, warp 1 MMA, warps 2-5 convert + epilogue
 
 struct ProjParams {
-    int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, chain;
+    int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, chain, lowp;
     float *zpart;
 };
 
@@ -175,6 +185,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     const int nkb = q.ngrid / PJ_BK;
     const int total = q.ndom * q.ntile_m * q.ntile_n * q.nsplit;
     const bool need_lo = q.nprod == 3;
+    const bool need_conv = need_lo || q.lowp;   // converter warps touch every stage
     const bool load_alo = need_lo && !q.conv_a;
     const uint32_t y_bytes = (uint32_t)(q.BN / 32) * PJ_BK * 128;
     const uint32_t tx_bytes = PJ_A_BYTES * (load_alo ? 2u : 1u) + y_bytes;
@@ -227,7 +238,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                     const int s = it % PJ_STAGES;
                     const uint32_t ph = (it / PJ_STAGES) & 1;
                     mbar_wait(&full[s], ph);
-                    if (need_lo) mbar_wait(&conv[s], ph);
+                    if (need_conv) mbar_wait(&conv[s], ph);
                     tc_fence_after();
                     const uint32_t st = smem_u32(smem + s * PJ_STAGE_BYTES);
                     const uint32_t a_hi = st, a_lo = st + PJ_A_BYTES, y_hi = st + 2 * PJ_A_BYTES,
@@ -269,7 +280,20 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
             const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
             for (int c0k = kb0; c0k < kb1; c0k += q.chain) {
                 const int c1k = min(c0k + q.chain, kb1);
-                if (need_lo) {
+                if (q.lowp) {
+                    // opt-in low precision (PAPER.md L207, L239 float_to_BF16): both operands rounded to BF16
+                    for (int kb = c0k; kb < c1k; ++kb, ++it) {
+                        const int s = it % PJ_STAGES;
+                        mbar_wait(&full[s], (it / PJ_STAGES) & 1);
+                        uint8_t *st = smem + s * PJ_STAGE_BYTES;
+                        float4 *y4 = (float4 *)(st + 2 * PJ_A_BYTES);
+                        for (int i = t; i < ny4; i += 128) y4[i] = bf16_round4(y4[i]);
+                        float4 *a4 = (float4 *)st;
+                        for (int i = t; i < PJ_A_BYTES / 16; i += 128) a4[i] = bf16_round4(a4[i]);
+                        fence_proxy_async_smem();
+                        mbar_arrive(&conv[s]);
+                    }
+                } else if (need_lo) {
                     for (int kb = c0k; kb < c1k; ++kb, ++it) {
                         const int s = it % PJ_STAGES;
                         mbar_wait(&full[s], (it / PJ_STAGES) & 1);
@@ -340,7 +364,7 @@ constexpr int BK_EPI_WARPS = 4;
 constexpr int BK_THREADS = 64 + 32 * BK_EPI_WARPS;
 
 struct BackParams {
-    int ndom, ngrid, P, N, BN, ntile_n, prows, nprod, ldy;
+    int ndom, ngrid, P, N, BN, ntile_n, prows, nprod, ldy, lowp;
     float *Y;
 };
 
@@ -352,8 +376,8 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *stage = smem + BK_STAGES * BK_STAGE_BYTES;
     uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
-    uint64_t *full = bars, *empty = bars + BK_STAGES;
-    uint64_t *acc_full = bars + 2 * BK_STAGES, *acc_empty = acc_full + 1;
+    uint64_t *full = bars, *empty = bars + BK_STAGES, *conv = bars + 2 * BK_STAGES;
+    uint64_t *acc_full = bars + 3 * BK_STAGES, *acc_empty = acc_full + 1;
     uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
 
@@ -361,6 +385,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         for (int s = 0; s < BK_STAGES; ++s) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], 1);
+            mbar_init(&conv[s], 32 * BK_EPI_WARPS);
         }
         mbar_init(acc_full, 1);
         mbar_init(acc_empty, 32 * BK_EPI_WARPS);
@@ -417,6 +442,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 for (int k = 0; k < nk; ++k, ++it) {
                     const int s = it % BK_STAGES;
                     mbar_wait(&full[s], (it / BK_STAGES) & 1);
+                    if (q.lowp) mbar_wait(&conv[s], (it / BK_STAGES) & 1);
                     tc_fence_after();
                     const uint32_t st = smem_u32(smem + s * BK_STAGE_BYTES);
                     const uint64_t da = smem_desc(st, 16, 256, LAYOUT_SW32);
@@ -440,10 +466,22 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     } else {
         const int quarter = warp % 4;
         const int er = quarter * 32 + lane;         // accumulator row of this thread
-        int nu = 0, slot = 0;
+        int nu = 0, slot = 0, it = 0;
         for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
             const int nt = u % q.ntile_n, rt = (u / q.ntile_n) % nrt, dom = u / (q.ntile_n * nrt);
             const int row0 = dom * q.ngrid + rt * 128;
+            if (q.lowp) {
+                // low-precision mode: the otherwise idle epilogue warps round the beta slab of every stage
+                // to BF16 in place (W was rounded by the glue kernel)
+                for (int k = 0; k < nk; ++k, ++it) {
+                    const int s = it % BK_STAGES;
+                    mbar_wait(&full[s], (it / BK_STAGES) & 1);
+                    float4 *a4 = (float4 *)(smem + s * BK_STAGE_BYTES);
+                    for (int i = er; i < BK_A_BYTES / 16; i += 32 * BK_EPI_WARPS) a4[i] = bf16_round4(a4[i]);
+                    fence_proxy_async_smem();
+                    mbar_arrive(&conv[s]);
+                }
+            }
             mbar_wait(acc_full, nu & 1);
             tc_fence_after();
             for (int cb = 0; cb < q.BN / 32; ++cb) {
@@ -525,6 +563,8 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.conv_a = (nprod == 3 && A_lo == nullptr) ? 1 : 0;
     q.zpart = zpart;
     q.chain = chain > 0 ? chain : (1 << 30);
+    q.lowp = nprod == 0 ? 1 : 0;     // nprod 0 = one product of BF16-rounded operands
+    if (q.lowp) q.nprod = 1;
     const uint64_t rows = (uint64_t)ndom * ngrid;
     CUtensorMap ma, mal, my;
     if (!make_chunk_map(&ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;
@@ -557,7 +597,8 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     const int per = (N + q.ntile_n - 1) / q.ntile_n;
     q.BN = per <= 256 ? (per + 31) / 32 * 32 : (per + 63) / 64 * 64;
     q.prows = prows;
-    q.nprod = nprod;
+    q.lowp = nprod == 0 ? 1 : 0;
+    q.nprod = nprod == 0 ? 1 : nprod;
     q.ldy = ldy;
     q.Y = Y;
     const uint64_t rows = (uint64_t)ndom * ngrid;

@@ -7,6 +7,12 @@ namespace mlmd {
 // x with the 13 low mantissa bits cleared: the part of x a kind::tf32 tensor-core operand keeps
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 
+__device__ __forceinline__ float bf16_rne(float x) {
+    unsigned u = __float_as_uint(x);
+    u += 0x7fffu + ((u >> 16) & 1u);
+    return __uint_as_float(u & 0xffff0000u);
+}
+
 // S2b.  C[p][n] = sum over split slices (fixed order: bit-reproducible, reading D22) of the
 // projection, combined to the complex coefficient for complex projectors; then
 //   W[p][n] = (-i tau) * D'_p * C[p][n],  D' = D * dv (reading D10)
@@ -15,7 +21,7 @@ __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__flo
 //   complex beta: rows 2p, 2p+1 hold the 2x2 real representation of W.
 __global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int prows, int nsplit,
                                     const float *__restrict__ zpart, const float *__restrict__ dprime, float tau,
-                                    float *__restrict__ what, float *__restrict__ what_lo) {
+                                    float *__restrict__ what, float *__restrict__ what_lo, int lowp) {
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
     const int p = blockIdx.y, dom = blockIdx.z;
     if (n >= ld) return;
@@ -40,8 +46,9 @@ __global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int pro
     const float f = tau * dprime[(size_t)dom * nproj + p];
     const float wre = f * cim, wim = -f * cre;   // (-i f)(cre + i cim)
     // stored as TF32-representable hi part + exact FP32 remainder lo (hi + lo == W exactly)
-    const float wre_h = tf32_hi(wre), wim_h = tf32_hi(wim);
-    const float wre_l = wre - wre_h, wim_l = wim - wim_h;
+    // low-precision mode: W rounded to BF16 (round-to-nearest-even), no remainder
+    const float wre_h = lowp ? bf16_rne(wre) : tf32_hi(wre), wim_h = lowp ? bf16_rne(wim) : tf32_hi(wim);
+    const float wre_l = lowp ? 0.f : wre - wre_h, wim_l = lowp ? 0.f : wim - wim_h;
     float *wd = what + (size_t)dom * prows * N;
     float *wl = what_lo + (size_t)dom * prows * N;
     if (!beta_complex) {
@@ -57,10 +64,10 @@ __global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int pro
 
 cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows,
                                 int nsplit, const float *zpart, const float *dprime, float tau,
-                                float *what, float *what_lo, int *nlaunch) {
+                                float *what, float *what_lo, int lowp, int *nlaunch) {
     dim3 grid((ld + 127) / 128, nproj, ndom);
     ++*nlaunch;
-    reduce_scale_kernel<<<grid, 128, 0, st>>>(nproj, beta_complex, ld, prows, nsplit, zpart, dprime, tau, what, what_lo);
+    reduce_scale_kernel<<<grid, 128, 0, st>>>(nproj, beta_complex, ld, prows, nsplit, zpart, dprime, tau, what, what_lo, lowp);
     return cudaGetLastError();
 }
 

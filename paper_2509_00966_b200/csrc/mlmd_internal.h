@@ -112,7 +112,8 @@ cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float 
 
 // ---- gemm_tc.cu ------------------------------------------------------------------------------
 // The same two contractions on tcgen05 tensor cores, operands staged by TMA.  nprod = 3: 3xTF32
-// (FP32-grade), nprod = 1: single TF32 product.  A_lo == NULL with nprod == 3: the kernel splits A
+// (FP32-grade), nprod = 1: single TF32 product, nprod = 0: single product of operands rounded to BF16
+// in shared memory (opt-in low precision).  A_lo == NULL with nprod == 3: the kernel splits A
 // itself (overlap, where A is a psi buffer).  Requires ngrid % 128 == 0, N % 32 == 0, lda % 8 == 0.
 bool tc_available();
 int tc_choose_nsplit(int ndom, long ngrid, int P, int N);
@@ -127,7 +128,7 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
 // S2b: reduce split-K partials in fixed order and build What = (-i tau) D' C in real-GEMM form.
 cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows,
                                 int nsplit, const float *zpart, const float *dprime, float tau,
-                                float *what, float *what_lo, int *nlaunch);
+                                float *what, float *what_lo, int lowp /* round W to BF16 */, int *nlaunch);
 // S3: rho[dom][r] = sum_n occ[dom][n] |psi[dom][r][n]|^2
 cudaError_t launch_density(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, const float *occ,
                            float *rho, int *nlaunch);
