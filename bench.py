@@ -208,7 +208,9 @@ def main():
     workers = max(1, min(8, (os.cpu_count() or 2) // (2 * max(1, min(world, 8)))))
     t_gen = time.perf_counter()
     with ThreadPoolExecutor(max_workers=workers) as ex:
-        for i, dd in enumerate(ex.map(lambda k: W.generate_domain(c, rank * c.ndom + k), range(c.ndom))):
+        from paper_2509_00966_b200.shard import weak_scaling_block
+        first_dom, last_dom = weak_scaling_block(c.ndom, rank)   # domains are the sharding unit: no collective
+        for i, dd in enumerate(ex.map(lambda k: W.generate_domain(c, k), range(first_dom, last_dom))):
             psi_dev[i].copy_(torch.from_numpy(dd["psi"]))
             beta_dev[i].copy_(torch.from_numpy(dd["beta"]))
             vloc[i], occ[i], D[i] = dd["vloc"], dd["occ"], dd["D"]
