@@ -93,11 +93,12 @@ constexpr int EPI_BAR = 1;                  // named barrier of the 128 epilogue
 
 // The 128 epilogue threads hand one [128 x 32] FP32 tile (thread r holds row r in v) to the TMA engine,
 // which stores it or adds it (L2 reduction, round-to-nearest) into global memory at (c0, row0).
-// Two staging tiles alternate; `slot` counts tiles issued so far by this group.
+// NB staging tiles rotate; `slot` counts tiles issued so far by this group.
+template <int NB>
 __device__ __forceinline__ void epi_tile_out(uint8_t *stage, int &slot, const CUtensorMap *map, int c0, int row0,
                                              const uint32_t (&v)[32], int r, bool add) {
-    uint8_t *buf = stage + (slot & 1) * EPI_TILE_BYTES;
-    if (r == 0) bulk_wait_read<1>();          // the tile issued two slots ago has left this buffer
+    uint8_t *buf = stage + (slot % NB) * EPI_TILE_BYTES;
+    if (r == 0) bulk_wait_read<NB - 1>();     // the tile issued NB slots ago has left this buffer
     named_bar_sync(EPI_BAR, 128);
     const uint32_t rowaddr = smem_u32(buf) + r * 128;
 #pragma unroll
@@ -333,7 +334,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + mb * q.BN + cb * 32, v);
                         tmem_ld_wait();
                         const int c0 = nt * q.BN + cb * 32;
-                        if (c0 < q.N) epi_tile_out(stage, slot, &map_z, c0, zrow + mb * 128, v, er, add);
+                        if (c0 < q.N) epi_tile_out<2>(stage, slot, &map_z, c0, zrow + mb * 128, v, er, add);
                     }
                 }
                 tc_fence_before();
@@ -353,13 +354,17 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
 // =================================================================================================
 // Back-application: Y[r][c] += sum_p A[r][p] * W[p][c].
 // CTA tile: 128 grid points x BN <= 448 columns (TMEM accumulator), K pipeline of 8 projector rows.
+// CTAs run as clusters of two on neighbouring row tiles: the W slab of a stage is the same for both, so
+// each CTA fetches half of it and TMA-multicasts it into both shared memories (the GEMM is otherwise
+// bound by L2->SM bandwidth, ~43 B/cycle/SM measured, not by the tensor pipe).
 // =================================================================================================
-constexpr int BK_STAGES = 5;
+constexpr int BK_STAGES = 4;
+constexpr int BK_EPI_NB = 5;                            // staging tiles of the epilogue in flight
 constexpr int BK_MAXBN = 448;
 constexpr int BK_A_BYTES = 128 * 32;                    // [128 rows x 8 floats], SWIZZLE_32B
 constexpr int BK_W_BYTES = (BK_MAXBN / 32) * 1024;      // chunks of [8 rows x 128 B], SWIZZLE_128B
 constexpr int BK_STAGE_BYTES = 2 * BK_A_BYTES + 2 * BK_W_BYTES;
-constexpr int BK_SMEM = BK_STAGES * BK_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 256;
+constexpr int BK_SMEM = BK_STAGES * BK_STAGE_BYTES + BK_EPI_NB * EPI_TILE_BYTES + 1024 + 256;
 constexpr int BK_EPI_WARPS = 4;
 constexpr int BK_THREADS = 64 + 32 * BK_EPI_WARPS;
 
@@ -368,14 +373,14 @@ struct BackParams {
     float *Y;
 };
 
-__global__ void __launch_bounds__(BK_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(BK_THREADS, 1)
 back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
                const __grid_constant__ CUtensorMap map_whi, const __grid_constant__ CUtensorMap map_wlo,
                const __grid_constant__ CUtensorMap map_out, const BackParams q) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *stage = smem + BK_STAGES * BK_STAGE_BYTES;
-    uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
+    uint64_t *bars = (uint64_t *)(stage + BK_EPI_NB * EPI_TILE_BYTES);
     uint64_t *full = bars, *empty = bars + BK_STAGES, *conv = bars + 2 * BK_STAGES;
     uint64_t *acc_full = bars + 3 * BK_STAGES, *acc_empty = acc_full + 1;
     uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
@@ -384,7 +389,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     if (threadIdx.x == 0) {
         for (int s = 0; s < BK_STAGES; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], 1);
+            mbar_init(&empty[s], 2);    // this CTA's MMAs and the peer's (its multicast half lands here too)
             mbar_init(&conv[s], 32 * BK_EPI_WARPS);
         }
         mbar_init(acc_full, 1);
@@ -398,15 +403,19 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     }
     if (warp == 1) tmem_alloc(tmem_slot, 512);
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();          // barrier inits visible to the peer before any remote arrive / multicast
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    const int crank = (int)cluster_ctarank();
 
     const int nrt = q.ngrid / 128;                 // row tiles per domain
-    const int total = q.ndom * nrt * q.ntile_n;
+    const int nrp = (nrt + 1) / 2;                 // pairs of row tiles: one per cluster unit
+    const int total = q.ndom * nrp * q.ntile_n;    // cluster units
+    const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
     const int nk = (q.P + 7) / 8;
     const bool need_lo = q.nprod == 3;
-    const uint32_t w_bytes = (uint32_t)(q.BN / 32) * 1024;
+    const int nchunk = q.BN / 32, chalf = (nchunk + 1) / 2;   // W chunks: this CTA fetches `chalf` of them
+    const uint32_t w_bytes = (uint32_t)(2 * chalf) * 1024;
     const uint32_t tx_bytes = (need_lo ? 2u : 1u) * (BK_A_BYTES + w_bytes);
     const int ninstr = q.BN > 256 ? 2 : 1;
     const int NI = q.BN / ninstr;                   // columns per UMMA instruction (multiple of 32)
@@ -414,8 +423,8 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     if (warp == 0) {
         if (lane == 0) {
             int it = 0;
-            for (int u = blockIdx.x; u < total; u += gridDim.x) {
-                const int nt = u % q.ntile_n, rt = (u / q.ntile_n) % nrt, dom = u / (q.ntile_n * nrt);
+            for (int u = cl; u < total; u += ncl) {
+                const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
                 const int row = dom * q.ngrid + rt * 128;
                 for (int k = 0; k < nk; ++k, ++it) {
                     const int s = it % BK_STAGES;
@@ -423,11 +432,12 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                     uint8_t *st = smem + s * BK_STAGE_BYTES;
                     mbar_expect_tx(&full[s], tx_bytes);
                     tma_load_2d(st, &map_ahi, &full[s], k * 8, row);
-                    tma_load_3d(st + 2 * BK_A_BYTES, &map_whi, &full[s], 0, dom * q.prows + k * 8, nt * (q.BN / 32));
+                    tma_load_3d_mc(st + 2 * BK_A_BYTES + crank * chalf * 1024, &map_whi, &full[s], 0, dom * q.prows + k * 8,
+                                   nt * nchunk + crank * chalf, (uint16_t)3);
                     if (need_lo) {
                         tma_load_2d(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
-                        tma_load_3d(st + 2 * BK_A_BYTES + BK_W_BYTES, &map_wlo, &full[s], 0, dom * q.prows + k * 8,
-                                    nt * (q.BN / 32));
+                        tma_load_3d_mc(st + 2 * BK_A_BYTES + BK_W_BYTES + crank * chalf * 1024, &map_wlo, &full[s], 0,
+                                       dom * q.prows + k * 8, nt * nchunk + crank * chalf, (uint16_t)3);
                     }
                 }
             }
@@ -436,7 +446,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         if (lane == 0) {
             const uint32_t idesc = instr_desc(FMT_TF32, 0, 1, 128, (uint32_t)NI);
             int it = 0, nu = 0;
-            for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
+            for (int u = cl; u < total; u += ncl, ++nu) {
                 mbar_wait(acc_empty, (nu & 1) ^ 1);
                 tc_fence_after();
                 for (int k = 0; k < nk; ++k, ++it) {
@@ -458,7 +468,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                             umma_tf32(d, da, dwl, idesc, 1u);
                         }
                     }
-                    umma_commit(&empty[s]);
+                    umma_commit_mc(&empty[s], (uint16_t)3);   // frees the stage in both CTAs of the cluster
                 }
                 umma_commit(acc_full);
             }
@@ -467,9 +477,10 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         const int quarter = warp % 4;
         const int er = quarter * 32 + lane;         // accumulator row of this thread
         int nu = 0, slot = 0, it = 0;
-        for (int u = blockIdx.x; u < total; u += gridDim.x, ++nu) {
-            const int nt = u % q.ntile_n, rt = (u / q.ntile_n) % nrt, dom = u / (q.ntile_n * nrt);
+        for (int u = cl; u < total; u += ncl, ++nu) {
+            const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
             const int row0 = dom * q.ngrid + rt * 128;
+            const bool live = rt < nrt;           // odd tile count: the last pair's second CTA only keeps the protocol going
             if (q.lowp) {
                 // low-precision mode: the otherwise idle epilogue warps round the beta slab of every stage
                 // to BF16 in place (W was rounded by the glue kernel)
@@ -490,7 +501,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 tmem_ld_wait();
                 const int c0 = nt * q.BN + cb * 32;
                 // Y += tile through the TMA engine: the add happens in L2, nothing is read back into the SM
-                if (c0 < q.N) epi_tile_out(stage, slot, &map_out, c0, row0, v, er, true);
+                if (c0 < q.N && live) epi_tile_out<BK_EPI_NB>(stage, slot, &map_out, c0, row0, v, er, true);
             }
             tc_fence_before();
             mbar_arrive(acc_empty);
@@ -499,6 +510,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     }
     tc_fence_before();
     __syncthreads();
+    cluster_sync_all();          // the peer may still multicast into / arrive on this CTA's shared memory
     if (warp == 1) {
         __syncwarp();
         tmem_dealloc(tmem, 512);
@@ -605,12 +617,13 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     CUtensorMap ma, mal, mw, mwl;
     if (!make_k8_map(&ma, A_hi, rows, lda, lda, 128)) return cudaErrorInvalidValue;
     if (!make_k8_map(&mal, A_lo, rows, lda, lda, 128)) return cudaErrorInvalidValue;
-    if (!make_chunk_map(&mw, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, q.BN / 32)) return cudaErrorInvalidValue;
-    if (!make_chunk_map(&mwl, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, q.BN / 32)) return cudaErrorInvalidValue;
+    const int chalf = (q.BN / 32 + 1) / 2;   // each CTA of a cluster fetches (and multicasts) half of the W chunks
+    if (!make_chunk_map(&mw, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, chalf)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(&mwl, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, chalf)) return cudaErrorInvalidValue;
     CUtensorMap mo;
     if (!make_out_map(&mo, Y, rows, N, ldy)) return cudaErrorInvalidValue;
-    const int total = ndom * (int)(ngrid / 128) * q.ntile_n;
-    const int grid = total < num_sms() ? total : num_sms();
+    const int total = ndom * (int)((ngrid / 128 + 1) / 2) * q.ntile_n;   // cluster units (pairs of row tiles)
+    const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
     back_tc_kernel<<<grid, BK_THREADS, BK_SMEM, st>>>(ma, mal, mw, mwl, mo, q);
     return cudaGetLastError();
