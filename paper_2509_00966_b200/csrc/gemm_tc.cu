@@ -136,6 +136,8 @@ __device__ __forceinline__ float4 bf16_round4(const float4 v) {
 // =================================================================================================
 // Projection: Z[p][c] = sum_r A[r][p] * Y[r][c] over one K slice; FP32 partials per slice.
 // CTA tile: up to 256 rows p (two M = 128 UMMA blocks) x BN <= 224 columns; K pipeline of 16 rows.
+// CTAs run as clusters of two on neighbouring column tiles of the same (domain, row tile, K slice): the
+// beta tile of a stage is the same for both, so each fetches half of its chunks and TMA-multicasts them.
 // =================================================================================================
 constexpr int PJ_BK = 16;               // grid points per pipeline stage (two K = 8 UMMA steps)
 constexpr int PJ_STAGES = 3;
@@ -151,7 +153,7 @@ struct ProjParams {
     float *zpart;
 };
 
-__global__ void __launch_bounds__(PJ_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PJ_THREADS, 1)
 proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
                const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_z, const ProjParams q) {
     extern __shared__ uint8_t smem_raw[];
@@ -166,7 +168,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     if (threadIdx.x == 0) {
         for (int s = 0; s < PJ_STAGES; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], 1);
+            mbar_init(&empty[s], 2);    // this CTA's MMAs and the peer's (its multicast half lands here too)
             mbar_init(&conv[s], 128);
         }
         mbar_init(acc_full, 1);
@@ -179,12 +181,15 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     }
     if (warp == 1) tmem_alloc(tmem_slot, 512);
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();          // barrier inits visible to the peer before any remote arrive / multicast
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    const int crank = (int)cluster_ctarank();
+    const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
 
     const int nkb = q.ngrid / PJ_BK;
-    const int total = q.ndom * q.ntile_m * q.ntile_n * q.nsplit;
+    const int nntp = (q.ntile_n + 1) / 2;          // pairs of column tiles: one per cluster unit
+    const int total = q.ndom * q.ntile_m * nntp * q.nsplit;   // cluster units
     const bool need_lo = q.nprod == 3;
     const bool need_conv = need_lo || q.lowp;   // converter warps touch every stage
     const bool load_alo = need_lo && !q.conv_a;
@@ -192,8 +197,8 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     const uint32_t tx_bytes = PJ_A_BYTES * (load_alo ? 2u : 1u) + y_bytes;
 
     auto decode = [&](int u, int &dom, int &mt, int &nt, int &kb0, int &kb1) {
-        nt = u % q.ntile_n;
-        u /= q.ntile_n;
+        nt = 2 * (u % nntp) + crank;   // may be == ntile_n (odd tile count): that CTA only keeps the protocol going
+        u /= nntp;
         const int sp = u % q.nsplit;
         u /= q.nsplit;
         mt = u % q.ntile_m;
@@ -205,7 +210,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     if (warp == 0) {
         if (lane == 0) {
             int it = 0;
-            for (int u = blockIdx.x; u < total; u += gridDim.x) {
+            for (int u = cl; u < total; u += ncl) {
                 int dom, mt, nt, kb0, kb1;
                 decode(u, dom, mt, nt, kb0, kb1);
                 for (int kb = kb0; kb < kb1; ++kb, ++it) {
@@ -214,8 +219,10 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                     uint8_t *st = smem + s * PJ_STAGE_BYTES;
                     mbar_expect_tx(&full[s], tx_bytes);
                     const int row = dom * q.ngrid + kb * PJ_BK;
-                    tma_load_3d(st, &map_ahi, &full[s], 0, row, mt * 8);
-                    if (load_alo) tma_load_3d(st + PJ_A_BYTES, &map_alo, &full[s], 0, row, mt * 8);
+                    const int ahalf = crank * 4 * (PJ_BK * 128);   // this CTA fetches 4 of the 8 beta chunks for both
+                    tma_load_3d_mc(st + ahalf, &map_ahi, &full[s], 0, row, mt * 8 + crank * 4, (uint16_t)3);
+                    if (load_alo)
+                        tma_load_3d_mc(st + PJ_A_BYTES + ahalf, &map_alo, &full[s], 0, row, mt * 8 + crank * 4, (uint16_t)3);
                     tma_load_3d(st + 2 * PJ_A_BYTES, &map_y, &full[s], 0, row, nt * (q.BN / 32));
                 }
             }
@@ -224,7 +231,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         if (lane == 0) {
             const uint32_t idesc = instr_desc(FMT_TF32, 1, 1, 128, (uint32_t)q.BN);
             int it = 0, nd = 0;   // nd: accumulator hand-overs (drains) so far
-            for (int u = blockIdx.x; u < total; u += gridDim.x) {
+            for (int u = cl; u < total; u += ncl) {
                 int dom, mt, nt, kb0, kb1;
                 decode(u, dom, mt, nt, kb0, kb1);
                 const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
@@ -260,7 +267,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                             }
                         }
                     }
-                    umma_commit(&empty[s]);
+                    umma_commit_mc(&empty[s], (uint16_t)3);   // frees the stage in both CTAs of the cluster
                     if ((kb - kb0 + 1) % q.chain == 0 || kb + 1 == kb1) {
                         umma_commit(acc_full);
                         ++nd;
@@ -274,10 +281,10 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         const int er = quarter * 32 + lane;   // TMEM lane = accumulator row of this thread; er == 0 leads the TMA stores
         int it = 0, nd = 0, slot = 0;
         const int ny4 = q.BN / 32 * PJ_BK * 8;    // float4 count of the Y tile
-        for (int u = blockIdx.x; u < total; u += gridDim.x) {
+        for (int u = cl; u < total; u += ncl) {
             int dom, mt, nt, kb0, kb1;
             decode(u, dom, mt, nt, kb0, kb1);
-            const int sp = (u / q.ntile_n) % q.nsplit;
+            const int sp = (u / nntp) % q.nsplit;
             const int nblk = (q.P - mt * 256 > 128) ? 2 : 1;
             for (int c0k = kb0; c0k < kb1; c0k += q.chain) {
                 const int c1k = min(c0k + q.chain, kb1);
@@ -334,7 +341,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + mb * q.BN + cb * 32, v);
                         tmem_ld_wait();
                         const int c0 = nt * q.BN + cb * 32;
-                        if (c0 < q.N) epi_tile_out<2>(stage, slot, &map_z, c0, zrow + mb * 128, v, er, add);
+                        if (c0 < q.N && nt < q.ntile_n) epi_tile_out<2>(stage, slot, &map_z, c0, zrow + mb * 128, v, er, add);
                     }
                 }
                 tc_fence_before();
@@ -345,6 +352,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     }
     tc_fence_before();
     __syncthreads();
+    cluster_sync_all();          // the peer may still multicast into / arrive on this CTA's shared memory
     if (warp == 1) {
         __syncwarp();
         tmem_dealloc(tmem, 512);
@@ -535,8 +543,8 @@ bool tc_available() { return encode_fn() != nullptr; }
 int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
     const int ntile_m = (P + 255) / 256;
     const int ntile_n = (N + PJ_MAXBN - 1) / PJ_MAXBN;
-    const long base = (long)ndom * ntile_m * ntile_n;
-    const int sms = 148;
+    const long base = (long)ndom * ntile_m * ((ntile_n + 1) / 2);   // cluster units per K slice
+    const int sms = 74;                                               // clusters of two CTAs
     const long nkb = ngrid / PJ_BK;
     int best = 1;
     double best_eff = 0.0;
@@ -579,13 +587,14 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     if (q.lowp) q.nprod = 1;
     const uint64_t rows = (uint64_t)ndom * ngrid;
     CUtensorMap ma, mal, my;
-    if (!make_chunk_map(&ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;
-    if (!make_chunk_map(&mal, A_lo ? A_lo : A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 8)) return cudaErrorInvalidValue;
+    // 4-chunk boxes: each CTA of a cluster fetches (and multicasts) half of the 8 beta chunks of a stage
+    if (!make_chunk_map(&ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(&mal, A_lo ? A_lo : A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
     if (!make_chunk_map(&my, Y, rows, ldy, N / 32, PJ_BK, q.BN / 32)) return cudaErrorInvalidValue;
     CUtensorMap mz;
     if (!make_out_map(&mz, zpart, (uint64_t)ndom * nsplit * prows, N, N)) return cudaErrorInvalidValue;
-    const int total = ndom * q.ntile_m * q.ntile_n * nsplit;
-    const int grid = total < num_sms() ? total : num_sms();
+    const int total = ndom * q.ntile_m * ((q.ntile_n + 1) / 2) * nsplit;   // cluster units
+    const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
     proj_tc_kernel<<<grid, PJ_THREADS, PJ_SMEM, st>>>(ma, mal, my, mz, q);
     return cudaGetLastError();
