@@ -525,6 +525,160 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     }
 }
 
+// =================================================================================================
+// Back-application on CTA PAIRS (tcgen05 cta_group::2): Y[r][c] += sum_p A[r][p] * W[p][c].
+// One UMMA spans two SMs: M = 256 grid points (128 per CTA, each CTA stages only its own beta slab)
+// and the W slab is split by columns between the two shared memories, so every operand byte is read
+// from shared memory once per pair instead of once per CTA.  With single-CTA UMMAs (M = 128) the
+// operand reads alone take ~98 of the 128 B/cycle of shared-memory bandwidth and, together with the
+// TMA fills, cap the tensor pipe near 75 % (measured); this is what cta_group::2 exists for.
+// Per CTA: 128 x BN accumulator in TMEM (BN <= 448, BN % 64 == 0), UMMA pieces of N = 256 and BN - 256.
+// =================================================================================================
+constexpr int B2_STAGES = 7;
+constexpr int B2_WH_BYTES = 7 * 1024;                  // this CTA's half of the W slab: <= 224 columns
+constexpr int B2_STAGE_BYTES = 2 * BK_A_BYTES + 2 * B2_WH_BYTES;
+constexpr int B2_SMEM = B2_STAGES * B2_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 256;
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(BK_THREADS, 1)
+back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
+                const __grid_constant__ CUtensorMap map_w0h, const __grid_constant__ CUtensorMap map_w0l,
+                const __grid_constant__ CUtensorMap map_w1h, const __grid_constant__ CUtensorMap map_w1l,
+                const __grid_constant__ CUtensorMap map_out, const BackParams q) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *stage = smem + B2_STAGES * B2_STAGE_BYTES;
+    uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
+    uint64_t *full = bars, *empty = bars + B2_STAGES;
+    uint64_t *acc_full = bars + 2 * B2_STAGES, *acc_empty = acc_full + 1;
+    uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const int crank = (int)cluster_ctarank();
+    const bool leader = crank == 0;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < B2_STAGES; ++s) {
+            mbar_init(&full[s], 1);     // used in the leader: its own expect_tx arrive; both CTAs' TMA bytes land on it
+            mbar_init(&empty[s], 1);    // the leader's tcgen05.commit, multicast to both CTAs
+        }
+        mbar_init(acc_full, 1);         // commit multicast
+        mbar_init(acc_empty, 2);        // one elected epilogue thread per CTA (remote arrive on the leader)
+        fence_barrier_init();
+        prefetch_tmap(&map_ahi);
+        prefetch_tmap(&map_alo);
+        prefetch_tmap(&map_w0h);
+        prefetch_tmap(&map_w0l);
+        prefetch_tmap(&map_out);
+    }
+    if (warp == 1) tmem_alloc_2cta(tmem_slot, 512);
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const int nrt = q.ngrid / 128, nrp = (nrt + 1) / 2;
+    const int total = q.ndom * nrp * q.ntile_n;    // cluster units: a pair of row tiles x one column tile
+    const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
+    const int nk = (q.P + 7) / 8;
+    const bool need_lo = q.nprod == 3;
+    const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;   // UMMA pieces (columns); per CTA n/2 of each
+    const int h0 = n0 / 64, h1 = n1 / 64;                      // this CTA's 32-column chunks of each piece
+    const uint32_t cta_bytes = (need_lo ? 2u : 1u) * (BK_A_BYTES + (uint32_t)(h0 + h1) * 1024);
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int it = 0;
+            for (int u = cl; u < total; u += ncl) {
+                const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
+                const int row = dom * q.ngrid + rt * 128;
+                const int ch0 = nt * (q.BN / 32) + crank * h0, ch1 = nt * (q.BN / 32) + n0 / 32 + crank * h1;
+                for (int k = 0; k < nk; ++k, ++it) {
+                    const int s = it % B2_STAGES;
+                    mbar_wait(&empty[s], ((it / B2_STAGES) & 1) ^ 1);
+                    uint8_t *st = smem + s * B2_STAGE_BYTES;
+                    if (leader) mbar_expect_tx(&full[s], 2 * cta_bytes);
+                    const int wrow = dom * q.prows + k * 8;
+                    tma_load_2d_2cta(st, &map_ahi, &full[s], k * 8, row);
+                    tma_load_3d_2cta(st + 2 * BK_A_BYTES, &map_w0h, &full[s], 0, wrow, ch0);
+                    if (h1) tma_load_3d_2cta(st + 2 * BK_A_BYTES + h0 * 1024, &map_w1h, &full[s], 0, wrow, ch1);
+                    if (need_lo) {
+                        tma_load_2d_2cta(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
+                        tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES, &map_w0l, &full[s], 0, wrow, ch0);
+                        if (h1)
+                            tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES + h0 * 1024, &map_w1l, &full[s], 0, wrow, ch1);
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0 && leader) {
+            const uint32_t id0 = instr_desc(FMT_TF32, 0, 1, 256, (uint32_t)n0);
+            const uint32_t id1 = instr_desc(FMT_TF32, 0, 1, 256, (uint32_t)(n1 ? n1 : 64));
+            int it = 0, nu = 0;
+            for (int u = cl; u < total; u += ncl, ++nu) {
+                mbar_wait(acc_empty, (nu & 1) ^ 1);
+                tc_fence_after();
+                for (int k = 0; k < nk; ++k, ++it) {
+                    const int s = it % B2_STAGES;
+                    mbar_wait(&full[s], (it / B2_STAGES) & 1);
+                    tc_fence_after();
+                    const uint32_t st = smem_u32(smem + s * B2_STAGE_BYTES);
+                    const uint64_t da = smem_desc(st, 16, 256, LAYOUT_SW32);
+                    const uint64_t dal = smem_desc(st + BK_A_BYTES, 16, 256, LAYOUT_SW32);
+                    const uint32_t wh = st + 2 * BK_A_BYTES, wl = wh + B2_WH_BYTES;
+                    const uint32_t acc = k > 0 ? 1u : 0u;
+                    {
+                        const uint64_t dw = smem_desc(wh, 1024, 512, LAYOUT_SW128_32B);
+                        umma_tf32_2cta(tmem, da, dw, id0, acc);
+                        if (need_lo) {
+                            umma_tf32_2cta(tmem, dal, dw, id0, 1u);
+                            umma_tf32_2cta(tmem, da, smem_desc(wl, 1024, 512, LAYOUT_SW128_32B), id0, 1u);
+                        }
+                    }
+                    if (h1) {
+                        const uint64_t dw = smem_desc(wh + h0 * 1024, 1024, 512, LAYOUT_SW128_32B);
+                        umma_tf32_2cta(tmem + n0, da, dw, id1, acc);
+                        if (need_lo) {
+                            umma_tf32_2cta(tmem + n0, dal, dw, id1, 1u);
+                            umma_tf32_2cta(tmem + n0, da, smem_desc(wl + h0 * 1024, 1024, 512, LAYOUT_SW128_32B), id1, 1u);
+                        }
+                    }
+                    umma_commit_2cta_mc(&empty[s], (uint16_t)3);
+                }
+                umma_commit_2cta_mc(acc_full, (uint16_t)3);
+            }
+        }
+    } else {
+        const int quarter = warp % 4;
+        const int er = quarter * 32 + lane;         // accumulator row of this thread
+        int nu = 0, slot = 0;
+        for (int u = cl; u < total; u += ncl, ++nu) {
+            const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
+            const int row0 = dom * q.ngrid + rt * 128;
+            const bool live = rt < nrt;
+            mbar_wait(acc_full, nu & 1);
+            tc_fence_after();
+            for (int cb = 0; cb < q.BN / 32; ++cb) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
+                tmem_ld_wait();
+                const int c0 = nt * q.BN + cb * 32;
+                if (c0 < q.N && live && q.dbg != 1) epi_tile_out<2>(stage, slot, &map_out, c0, row0, v, er, true, q.dbg);
+            }
+            tc_fence_before();
+            named_bar_sync(EPI_BAR, 128);
+            if (er == 0) mbar_arrive_remote(acc_empty, 0);   // this CTA's half of the accumulator is drained
+        }
+        if (er == 0) bulk_wait<0>();
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc_2cta(tmem, 512);
+    }
+}
+
 int g_num_sms = 0;
 int num_sms() {
     if (!g_num_sms) {
@@ -635,6 +789,23 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     const int total = ndom * (int)((ngrid / 128 + 1) / 2) * q.ntile_n;   // cluster units (pairs of row tiles)
     const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
+    const char *pair = getenv("MLMD_BACK_PAIR");   // "0": keep single-CTA UMMAs (A/B checks)
+    if (q.BN % 64 == 0 && !q.lowp && !(pair && pair[0] == '0')) {
+        static bool attr2 = false;
+        if (!attr2) {
+            cudaError_t e = cudaFuncSetAttribute(back2_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, B2_SMEM);
+            if (e != cudaSuccess) return e;
+            attr2 = true;
+        }
+        const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;
+        CUtensorMap w0h, w0l, w1h, w1l;
+        if (!make_chunk_map(&w0h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(&w0l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(&w1h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(&w1l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
+        back2_tc_kernel<<<grid, BK_THREADS, B2_SMEM, st>>>(ma, mal, w0h, w0l, w1h, w1l, mo, q);
+        return cudaGetLastError();
+    }
     back_tc_kernel<<<grid, BK_THREADS, BK_SMEM, st>>>(ma, mal, mw, mwl, mo, q);
     return cudaGetLastError();
 }
