@@ -34,7 +34,8 @@ MODE_NAMES = {"fp32grade": 0, "fp64": 1, "bf16": 2, "tf32x1": 3, "simt": 4}
 # tensor peak as a multiple of the measured dense BF16 peak (B200_PROFILING.md nominal ratios:
 # tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
 # the opt-in BF16-operand mode issues its single product on the TF32 pipe (BF16 values are TF32 values)
-TENSOR_RATIO = {"fp32grade": 0.5 / 3.0, "tf32x1": 0.5, "bf16": 0.5}
+TF32_OVER_BF16 = 1.1 / 2.25     # nominal dense peaks (B200_PROFILING.md): tf32 1.1 PF, bf16 2.25 PF
+TENSOR_RATIO = {"fp32grade": TF32_OVER_BF16 / 3.0, "tf32x1": TF32_OVER_BF16, "bf16": TF32_OVER_BF16}
 FP32_ALU_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FMA lanes x 2 flop x max SM clock
 FP64_ALU_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12    # nominal 64 DFMA lanes per SM (guide: ~40 TF)
 

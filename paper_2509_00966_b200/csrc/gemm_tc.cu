@@ -96,7 +96,7 @@ constexpr int EPI_BAR = 1;                  // named barrier of the 128 epilogue
 // NB staging tiles rotate; `slot` counts tiles issued so far by this group.
 template <int NB>
 __device__ __forceinline__ void epi_tile_out(uint8_t *stage, int &slot, const CUtensorMap *map, int c0, int row0,
-                                             const uint32_t (&v)[32], int r, bool add, int dbg = 0) {
+                                             const uint32_t (&v)[32], int r, bool add) {
     uint8_t *buf = stage + (slot % NB) * EPI_TILE_BYTES;
     if (r == 0) bulk_wait_read<NB - 1>();     // the tile issued NB slots ago has left this buffer
     named_bar_sync(EPI_BAR, 128);
@@ -106,8 +106,8 @@ __device__ __forceinline__ void epi_tile_out(uint8_t *stage, int &slot, const CU
         sts4(rowaddr + (((uint32_t)j ^ ((uint32_t)r & 7u)) << 4), v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
     fence_proxy_async_smem();
     named_bar_sync(EPI_BAR, 128);
-    if (r == 0 && dbg != 3) {
-        if (add && dbg != 2) tma_reduce_add_2d(map, buf, c0, row0);
+    if (r == 0) {
+        if (add) tma_reduce_add_2d(map, buf, c0, row0);
         else tma_store_2d(map, buf, c0, row0);
         bulk_commit();
     }
@@ -377,7 +377,7 @@ constexpr int BK_EPI_WARPS = 4;
 constexpr int BK_THREADS = 64 + 32 * BK_EPI_WARPS;
 
 struct BackParams {
-    int ndom, ngrid, P, N, BN, ntile_n, prows, nprod, ldy, lowp, dbg;
+    int ndom, ngrid, P, N, BN, ntile_n, prows, nprod, ldy, lowp;
     float *Y;
 };
 
@@ -509,7 +509,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 tmem_ld_wait();
                 const int c0 = nt * q.BN + cb * 32;
                 // Y += tile through the TMA engine: the add happens in L2, nothing is read back into the SM
-                if (c0 < q.N && live && q.dbg != 1) epi_tile_out<BK_EPI_NB>(stage, slot, &map_out, c0, row0, v, er, true, q.dbg);
+                if (c0 < q.N && live) epi_tile_out<BK_EPI_NB>(stage, slot, &map_out, c0, row0, v, er, true);
             }
             tc_fence_before();
             mbar_arrive(acc_empty);
@@ -662,7 +662,7 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
                 tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
                 tmem_ld_wait();
                 const int c0 = nt * q.BN + cb * 32;
-                if (c0 < q.N && live && q.dbg != 1) epi_tile_out<2>(stage, slot, &map_out, c0, row0, v, er, true, q.dbg);
+                if (c0 < q.N && live) epi_tile_out<2>(stage, slot, &map_out, c0, row0, v, er, true);
             }
             tc_fence_before();
             named_bar_sync(EPI_BAR, 128);
@@ -776,7 +776,6 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.nprod = nprod == 0 ? 1 : nprod;
     q.ldy = ldy;
     q.Y = Y;
-    q.dbg = getenv("MLMD_BACK_DBG") ? atoi(getenv("MLMD_BACK_DBG")) : 0;   // timing experiments only
     const uint64_t rows = (uint64_t)ndom * ngrid;
     CUtensorMap ma, mal, mw, mwl;
     if (!make_k8_map(&ma, A_hi, rows, lda, lda, 128)) return cudaErrorInvalidValue;
