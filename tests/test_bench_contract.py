@@ -1,0 +1,35 @@
+"""CPU-only checks of bench.py's contract: the reference arm (the oracle on the host cores) prints one
+JSON line with the agreed keys, and the roofline arithmetic of DESIGN.md section 6 is what bench.py uses."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_reference_arm_prints_one_json_line():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "0",
+                          "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr
+    lines = [l for l in out.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert j["impl"] == "reference" and j["metric"] == "electron-steps/s" and j["higher_is_better"] is True
+    assert j["value"] > 0 and j["steps"] == 2 and j["warmup"] == 1 and j["dtype"] == "f64"
+    assert j["cpu_baseline"]["kind"] == "oracle" and j["cpu_baseline"]["cores"] >= 1 and j["cpu_baseline"]["sample"]
+    assert j["e2e"] == {"value": j["value"], "unit": j["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert "workload" in j["config"] and "model" not in j["config"]
+
+
+def test_algorithmic_counts_match_design():
+    sys.path.insert(0, ROOT)
+    import bench
+    import workloads as W
+    c = W.get_config(3)
+    a = bench.algorithmic(c)
+    elems = 64 * 48 ** 3 * 224
+    assert a["elems"] == elems
+    assert a["bytes_step"] == elems * 96 + 64 * 48 ** 3 * 20           # 88 B stage passes + 8 B density
+    assert abs(a["gemm_flops_step"] - 8 * 4.0 * 64 * 48 ** 3 * 240 * 224) < 1.0   # real beta: 32 N_grid N_proj N_orb per domain
+    assert abs(bench.TENSOR_RATIO["fp32grade"] - (1.1 / 2.25) / 3) < 1e-12
