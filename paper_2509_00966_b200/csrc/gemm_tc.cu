@@ -679,6 +679,10 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
     }
 }
 
+// column tiles of the projection: <= 224 columns each.  (An odd count leaves one CTA of the last cluster
+// without a tile; rounding up to an even count of narrower tiles measured slower on configs[4].)
+int proj_ntile_n(int N) { return (N + PJ_MAXBN - 1) / PJ_MAXBN; }
+
 int g_num_sms = 0;
 int num_sms() {
     if (!g_num_sms) {
@@ -696,7 +700,7 @@ bool tc_available() { return encode_fn() != nullptr; }
 
 int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
     const int ntile_m = (P + 255) / 256;
-    const int ntile_n = (N + PJ_MAXBN - 1) / PJ_MAXBN;
+    const int ntile_n = proj_ntile_n(N);
     const long base = (long)ndom * ntile_m * ((ntile_n + 1) / 2);   // cluster units per K slice
     const int sms = 74;                                               // clusters of two CTAs
     const long nkb = ngrid / PJ_BK;
@@ -729,7 +733,7 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.P = P;
     q.N = N;
     q.ntile_m = (P + 255) / 256;
-    q.ntile_n = (N + PJ_MAXBN - 1) / PJ_MAXBN;
+    q.ntile_n = proj_ntile_n(N);
     q.BN = ((N + q.ntile_n - 1) / q.ntile_n + 31) / 32 * 32;
     q.nsplit = nsplit;
     q.prows = prows;

@@ -71,17 +71,54 @@ cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_c
     return cudaGetLastError();
 }
 
-// S3: one warp per grid point; lanes stride over the orbital row with 128-bit loads and reduce
-// with shuffles (north_star kernel 4).
+// S3: one warp per group of DP consecutive grid points; lanes stride over the orbital rows with 128-bit
+// loads (all DP rows are requested before any is reduced, so a warp keeps DP x 512 B per trip in flight)
+// and reduce with shuffles (north_star kernel 4).
+constexpr int DP = 4;
 __global__ void __launch_bounds__(256)
 density_kernel(long npoints, long ngrid, int lanes, const float4 *__restrict__ psi, const float *__restrict__ occ,
                float *__restrict__ rho) {
+    const long p0 = ((long)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32) * DP;
+    if (p0 >= npoints) return;
+    const int lane = threadIdx.x % 32;
+    float s[DP];
+#pragma unroll
+    for (int k = 0; k < DP; ++k) s[k] = 0.f;
+    // ngrid % DP == 0 is checked by the launcher, so the DP points share a domain
+    const float2 *f = (const float2 *)(occ + (size_t)(p0 / ngrid) * lanes * 2);
+    for (int l = lane; l < lanes; l += 32) {
+        float4 v[DP];
+#pragma unroll
+        for (int k = 0; k < DP; ++k) v[k] = p0 + k < npoints ? __ldcs(psi + (p0 + k) * lanes + l) : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float2 ff = __ldg(f + l);
+#pragma unroll
+        for (int k = 0; k < DP; ++k) {
+            s[k] = fmaf(ff.x, fmaf(v[k].x, v[k].x, v[k].y * v[k].y), s[k]);
+            s[k] = fmaf(ff.y, fmaf(v[k].z, v[k].z, v[k].w * v[k].w), s[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < DP; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s[k] += __shfl_xor_sync(0xffffffffu, s[k], o);
+    }
+    if (lane < DP && p0 + lane < npoints) {
+        float out = s[0];
+#pragma unroll
+        for (int k = 1; k < DP; ++k) out = lane == k ? s[k] : out;
+        rho[p0 + lane] = out;
+    }
+}
+
+// one point per warp: any ngrid
+__global__ void __launch_bounds__(256)
+density_kernel_1(long npoints, long ngrid, int lanes, const float4 *__restrict__ psi, const float *__restrict__ occ,
+                 float *__restrict__ rho) {
     const long pt = (long)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
     if (pt >= npoints) return;
     const int lane = threadIdx.x % 32;
-    const int dom = (int)(pt / ngrid);
     const float4 *row = psi + pt * lanes;
-    const float2 *f = (const float2 *)(occ + (size_t)dom * lanes * 2);
+    const float2 *f = (const float2 *)(occ + (size_t)(pt / ngrid) * lanes * 2);
     float s = 0.f;
     for (int l = lane; l < lanes; l += 32) {
         const float4 v = __ldg(row + l);
@@ -98,8 +135,12 @@ cudaError_t launch_density(cudaStream_t st, int ndom, long ngrid, int ld, const 
                            float *rho, int *nlaunch) {
     const long npoints = (long)ndom * ngrid;
     ++*nlaunch;
-    density_kernel<<<(unsigned)((npoints + 7) / 8), 256, 0, st>>>(npoints, ngrid, ld / 2, (const float4 *)psi, occ,
-                                                                 rho);
+    if (ngrid % DP == 0) {
+        const long nwarps = npoints / DP;
+        density_kernel<<<(unsigned)((nwarps + 7) / 8), 256, 0, st>>>(npoints, ngrid, ld / 2, (const float4 *)psi, occ, rho);
+    } else {
+        density_kernel_1<<<(unsigned)((npoints + 7) / 8), 256, 0, st>>>(npoints, ngrid, ld / 2, (const float4 *)psi, occ, rho);
+    }
     return cudaGetLastError();
 }
 
