@@ -721,11 +721,11 @@ int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
                            int chain, int *nlaunch) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
+    if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_set.mark();
     }
     ProjParams q;
     q.ndom = ndom;
@@ -761,11 +761,11 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
 cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
                            int *nlaunch) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_set;
+    if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(back_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, BK_SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_set.mark();
     }
     BackParams q;
     q.ndom = ndom;
@@ -794,11 +794,11 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     ++*nlaunch;
     const char *pair = getenv("MLMD_BACK_PAIR");   // "0": keep single-CTA UMMAs (A/B checks)
     if (q.BN % 64 == 0 && !q.lowp && !(pair && pair[0] == '0')) {
-        static bool attr2 = false;
-        if (!attr2) {
+        static DeviceOnce attr2;
+        if (!attr2.done()) {
             cudaError_t e = cudaFuncSetAttribute(back2_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, B2_SMEM);
             if (e != cudaSuccess) return e;
-            attr2 = true;
+            attr2.mark();
         }
         const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;
         CUtensorMap w0h, w0l, w1h, w1l;

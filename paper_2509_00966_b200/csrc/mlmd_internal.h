@@ -83,6 +83,18 @@ struct mlmd_domain {
 
 namespace mlmd {
 
+// One-time-per-device flag (function attributes such as the dynamic shared-memory limit are per device).
+struct DeviceOnce {
+    unsigned long long mask = 0;
+    static int dev() {
+        int d = 0;
+        cudaGetDevice(&d);
+        return d & 63;
+    }
+    bool done() const { return (mask >> dev()) & 1ull; }
+    void mark() { mask |= 1ull << dev(); }
+};
+
 // ---- stencil.cu ------------------------------------------------------------------------------
 // One Horner stage without the nonlocal term:
 //   out(r,n) = psi(r,n) + (-i tau) [ sum_{d,j} a_{d,j} w(r + j e_d, n) + (centre + V(r)) w(r,n) ]

@@ -281,14 +281,14 @@ bool stencil_tma_supported(const mlmd_domain *h) {
 
 cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
                                const StepCoef *coef_host, float tau, int *nlaunch) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
+    if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_set.mark();
     }
     const int F = 2 * h->ld;
     CUtensorMap mc, mz, my, mp;
