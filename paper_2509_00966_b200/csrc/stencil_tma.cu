@@ -175,6 +175,9 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     xq = xq < 0 ? xq + P.nx : xq;
     const float *vp = vd + (long)xq * vsx;
     const long vwrap = (long)P.nx * vsx;
+    // V_loc of the plane consumed by the NEXT step, loaded one step ahead so that its latency is off the
+    // critical path of the first FMA
+    float vAn = __ldg(vp), vBn = __ldg(vp + 8);
 
     auto point = [&](const uint32_t buf, const uint32_t o, const uint32_t ozm1, const uint32_t ozm2, const uint32_t ozp1,
                      const uint32_t ozp2, const uint32_t dy, const float cen, float4 &A0, float4 &A1, float4 &A2,
@@ -213,12 +216,14 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             if (um >= 1) mbar_wait(&empty[bm], (um - 1) & 1);
             issue(m);
         }
-        const float vA = __ldg(vp), vB = __ldg(vp + 8);
+        const float vA = vAn, vB = vBn;
         vp += vsx;
         if (++xq == P.nx) {
             xq = 0;
             vp -= vwrap;
         }
+        vAn = __ldg(vp);
+        vBn = __ldg(vp + 8);
         mbar_wait(&full[k], it & 1);
         const uint32_t buf = sbase + k * S_PLANE;
         point(buf, own, oAzm1, oAzm2, own + 64, own + 128, 0u, c.centre + vA, A0, A1, A2, A3, A4);
