@@ -311,8 +311,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         float4 *ydst = (float4 *)(st + 2 * PJ_A_BYTES + PJ_Y_BYTES);
                         for (int i = t; i < ny4; i += 128) {
                             float4 v = ysrc[i];
-                            ydst[i] = split4(v);
-                            ysrc[i] = v;
+                            ydst[i] = split4(v);   // the hi tile stays as loaded: kind::tf32 ignores the 13 low bits
                         }
                         if (q.conv_a) {
                             float4 *asrc = (float4 *)st;
@@ -320,7 +319,6 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                             for (int i = t; i < PJ_A_BYTES / 16; i += 128) {
                                 float4 v = asrc[i];
                                 adst[i] = split4(v);
-                                asrc[i] = v;
                             }
                         }
                         fence_proxy_async_smem();
