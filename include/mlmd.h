@@ -21,7 +21,8 @@
  *   ownership  the caller owns every buffer it passes, including the workspace, which must stay
  *              alive and untouched until mlmd_domain_destroy.  set_* calls copy their inputs
  *              into the workspace.  The library allocates no device memory after create.
- *   stream     all work is enqueued on the stream given at create.  Calls are asynchronous
+ *   stream     all work is ordered on the stream given at create (small batches replay a CUDA graph of
+ *              the step on an internal stream that is forked from and joined to that stream).  Calls are asynchronous
  *              w.r.t. the host except: any call with a MLMD_HOST pointer (synchronises the stream
  *              before returning), mlmd_set_vloc (reads back max|V|), and mlmd_propagate when the
  *              handle was created with MLMD_CHECK_FINITE.

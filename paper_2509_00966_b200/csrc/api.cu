@@ -82,6 +82,7 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.what_lo = take(zb);
     w.zpart = take(zb * std::max(pl->nsplit, std::max(pl->nsplit_tc, pl->nsplit_tc_ovl)));
     w.coef = take((size_t)kCoefCapacity * ndom * sizeof(StepCoef));
+    w.coef_cur = take((size_t)ndom * sizeof(StepCoef));
     w.flag = take(256);
     w.total = o;
     return true;
@@ -137,8 +138,15 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
     h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
+    h->coef_uploaded = nullptr; h->gexec = nullptr; h->gstream = nullptr; h->gfork = h->gjoin = nullptr;
+    h->g_launches = 0; h->g_dt = 0.0; h->g_yz = false;
+    {
+        const char *g = getenv("MLMD_GRAPH");   // "0": never capture the step into a CUDA graph
+        h->graph_allowed = !(g && g[0] == '0');
+    }
     cudaError_t e = cudaMallocHost((void **)&h->coef_host, (size_t)kCoefCapacity * ndom * sizeof(StepCoef));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&h->flag_host, 256);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->coef_uploaded, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->occ(), 0, (size_t)ndom * h->ld * sizeof(float), h->stream);
     // rows >= P of W are read (times zero columns of beta) by the K = 8 slabs of the back-application
     if (e == cudaSuccess) e = cudaMemsetAsync(h->what(), 0, 2 * (pl.off.what_lo - pl.off.what), h->stream);
@@ -157,6 +165,14 @@ int mlmd_domain_destroy(mlmd_domain_t *h) {
     cudaStreamSynchronize(h->stream);
     if (h->coef_host) cudaFreeHost(h->coef_host);
     if (h->flag_host) cudaFreeHost(h->flag_host);
+    if (h->coef_uploaded) cudaEventDestroy(h->coef_uploaded);
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    if (h->gstream) {
+        cudaStreamSynchronize(h->gstream);
+        cudaStreamDestroy(h->gstream);
+    }
+    if (h->gfork) cudaEventDestroy(h->gfork);
+    if (h->gjoin) cudaEventDestroy(h->gjoin);
     for (cudaEvent_t e : h->prof_pool) cudaEventDestroy(e);
     delete h;
     return MLMD_OK;
@@ -267,9 +283,19 @@ int mlmd_set_vloc(mlmd_domain_t *h, const float *vloc, int where) {
     return MLMD_OK;
 }
 
+// the captured step bakes in the projector count, the GEMM mode and dt: reconfiguration discards it
+static void drop_graph(mlmd_domain *h) {
+    if (h->gexec) {
+        cudaStreamSynchronize(h->gstream);
+        cudaGraphExecDestroy(h->gexec);
+        h->gexec = nullptr;
+    }
+}
+
 int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_dtype, const double *D, int where) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: NULL handle");
     if (nproj < 0) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: nproj=%d", nproj);
+    drop_graph(h);
     if (nproj == 0) {
         h->nproj = h->P = 0;
         h->dmax = 0.0;
@@ -307,6 +333,7 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
 
 int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: NULL handle");
+    drop_graph(h);
     if (mode < MLMD_GEMM_FP32GRADE || mode > MLMD_GEMM_FP32_SIMT) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: bad mode %d", mode);
     h->gemm_mode = mode;
     return MLMD_OK;
@@ -383,6 +410,69 @@ static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl) {
     return MLMD_OK;
 }
 
+// One Taylor-4 time step on h->stream: four Horner stages (projection, glue, fused stencil pass,
+// back-application) and the density.  coef: this step's device coefficients [ndom];
+// coef_host: the same set on the host when it is identical for all domains (constant-bank path), else NULL.
+static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, int *nl) {
+    // Horner form of sum_{m<=4} (-i dt H)^m/m!: w4 = psi, w_{k-1} = psi + (-i dt/k) H w_k
+    const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
+    float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
+    for (int i = 0; i < 4; ++i) {
+        const float tau = (float)(dt / (4 - i));
+        if (h->nproj > 0) {
+            int rc = nonlocal_project(h, src[i], tau, nl);
+            if (rc) return rc;
+        }
+        {
+            ProfScope ps(h, MLMD_K_STENCIL);
+            CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, coef_host, tau, nl));
+        }
+        if (h->nproj > 0) {
+            int rc = nonlocal_back(h, dst[i], nl);
+            if (rc) return rc;
+        }
+    }
+    ProfScope ps(h, MLMD_K_DENSITY);
+    CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), nl));
+    return MLMD_OK;
+}
+
+// Capture one step (coefficients taken from the device slot that advance_coef refills) into h->gexec.
+static int capture_step(mlmd_domain *h, double dt, bool yz) {
+    if (!h->gstream) {
+        CU(cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&h->gfork, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&h->gjoin, cudaEventDisableTiming));
+    }
+    cudaStream_t user = h->stream;
+    cudaGraph_t graph = nullptr;
+    int nl = 0;
+    CU(cudaStreamBeginCapture(h->gstream, cudaStreamCaptureModeThreadLocal));
+    h->stream = h->gstream;
+    cudaError_t e = launch_advance_coef(h->gstream, h->coef(), h->coef_cur(), h->step_counter(), h->ndom, &nl);
+    int rc = e == cudaSuccess ? enqueue_step(h, h->coef_cur(), nullptr, dt, &nl) : MLMD_ERR_CUDA;
+    h->stream = user;
+    cudaError_t e2 = cudaStreamEndCapture(h->gstream, &graph);
+    if (rc || e != cudaSuccess || e2 != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        h->graph_allowed = false;      // fall back to eager launches for the life of the handle
+        return MLMD_OK;
+    }
+    e = cudaGraphInstantiate(&h->gexec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {
+        h->gexec = nullptr;
+        cudaGetLastError();
+        h->graph_allowed = false;
+        return MLMD_OK;
+    }
+    h->g_launches = nl;
+    h->g_dt = dt;
+    h->g_yz = yz;
+    return MLMD_OK;
+}
+
 int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_propagate: NULL handle");
     if (nsteps < 0 || !(dt == dt) || std::isinf(dt)) return fail(MLMD_ERR_ARG, "mlmd_propagate: nsteps=%d dt=%g", nsteps, dt);
@@ -404,6 +494,12 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
     }
     h->field_yz = yz;
     int nl = 0;
+    // Small problems are launch-bound (17 launches per step): after one eager step the step is captured
+    // into a CUDA graph that reads its stencil coefficients from a device slot.
+    const bool want_graph = h->graph_allowed && !h->prof_on && nsteps >= 4 &&
+                            (double)h->ndom * (double)h->ngrid * h->ld <= (double)(1 << 23);
+    if (h->gexec && (h->g_dt != dt || h->g_yz != yz)) drop_graph(h);
+    CU(cudaEventSynchronize(h->coef_uploaded));   // an earlier call's upload has left the pinned staging buffer
     for (int s0 = 0; s0 < nsteps; s0 += kCoefCapacity) {
         const int ns = std::min(kCoefCapacity, nsteps - s0);
         if (s0 > 0) CU(cudaStreamSynchronize(h->stream));   // the pinned staging buffer is reused
@@ -411,28 +507,32 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
             for (int d = 0; d < h->ndom; ++d)
                 fill_coef(h, A + ((size_t)(s0 + s) * a_ndom + (a_ndom == 1 ? 0 : d)) * 3, &h->coef_host[(size_t)s * h->ndom + d]);
         CU(cudaMemcpyAsync(h->coef(), h->coef_host, (size_t)ns * h->ndom * sizeof(StepCoef), cudaMemcpyHostToDevice, h->stream));
-        for (int s = 0; s < ns; ++s) {
-            const StepCoef *coef = h->coef() + (size_t)s * h->ndom;
-            // Horner form of sum_{m<=4} (-i dt H)^m/m!: w4 = psi, w_{k-1} = psi + (-i dt/k) H w_k (S2)
-            const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
-            float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
-            for (int i = 0; i < 4; ++i) {
-                const float tau = (float)(dt / (4 - i));
-                if (h->nproj > 0) {
-                    int rc = nonlocal_project(h, src[i], tau, &nl);
-                    if (rc) return rc;
-                }
-                {
-                    ProfScope ps(h, MLMD_K_STENCIL);
-                    CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr, tau, &nl));
-                }
-                if (h->nproj > 0) {
-                    int rc = nonlocal_back(h, dst[i], &nl);
-                    if (rc) return rc;
-                }
+        CU(cudaEventRecord(h->coef_uploaded, h->stream));
+        int s = 0;
+        if (want_graph) {
+            if (!h->gexec) {
+                // one eager step first: it also sets the per-function attributes, which must not happen in a capture
+                int rc = enqueue_step(h, h->coef(), a_ndom == 1 ? &h->coef_host[0] : nullptr, dt, &nl);
+                if (rc) return rc;
+                s = 1;
+                rc = capture_step(h, dt, yz);
+                if (rc) return rc;
             }
-            ProfScope ps(h, MLMD_K_DENSITY);
-            CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), &nl));
+            if (h->gexec && s < ns) {
+                CU(cudaEventRecord(h->gfork, h->stream));
+                CU(cudaStreamWaitEvent(h->gstream, h->gfork, 0));
+                CU(launch_set_counter(h->gstream, h->step_counter(), s, &nl));
+                for (; s < ns; ++s) {
+                    CU(cudaGraphLaunch(h->gexec, h->gstream));
+                    nl += h->g_launches;
+                }
+                CU(cudaEventRecord(h->gjoin, h->gstream));
+                CU(cudaStreamWaitEvent(h->stream, h->gjoin, 0));
+            }
+        }
+        for (; s < ns; ++s) {
+            int rc = enqueue_step(h, h->coef() + (size_t)s * h->ndom, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr, dt, &nl);
+            if (rc) return rc;
         }
     }
     h->launches += nl;

@@ -224,4 +224,24 @@ cudaError_t launch_check_finite(cudaStream_t st, const float *x, size_t n, int *
     return cudaGetLastError();
 }
 
+// ---- CUDA-graph support: the captured step reads its stencil coefficients from a device slot that this
+// kernel refills from the uploaded table at the start of every graph launch
+__global__ void set_counter_kernel(int *counter, int value) { *counter = value; }
+__global__ void advance_coef_kernel(const StepCoef *__restrict__ all, StepCoef *__restrict__ cur, int *counter, int ndom) {
+    const int s = *counter;
+    for (int d = threadIdx.x; d < ndom; d += blockDim.x) cur[d] = all[(size_t)s * ndom + d];
+    __syncthreads();
+    if (threadIdx.x == 0) *counter = s + 1;
+}
+cudaError_t launch_set_counter(cudaStream_t st, int *counter, int value, int *nlaunch) {
+    ++*nlaunch;
+    set_counter_kernel<<<1, 1, 0, st>>>(counter, value);
+    return cudaGetLastError();
+}
+cudaError_t launch_advance_coef(cudaStream_t st, const StepCoef *all, StepCoef *cur, int *counter, int ndom, int *nlaunch) {
+    ++*nlaunch;
+    advance_coef_kernel<<<1, 64, 0, st>>>(all, cur, counter, ndom);
+    return cudaGetLastError();
+}
+
 }  // namespace mlmd

@@ -23,7 +23,7 @@ struct StepCoef {
 static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
-    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, flag, total;
+    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag, total;
 };
 
 constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
@@ -61,6 +61,15 @@ struct mlmd_domain {
     struct ProfRec { int kind; int e0, e1; };
     std::vector<ProfRec> prof_recs;
     mlmd::StepCoef *coef_host;  // pinned, kCoefCapacity * ndom
+    cudaEvent_t coef_uploaded;  // the pinned staging buffer may be refilled once this has happened
+    // CUDA graph of one time step (small, launch-bound problems; see api.cu)
+    bool graph_allowed;
+    cudaGraphExec_t gexec;
+    cudaStream_t gstream;
+    cudaEvent_t gfork, gjoin;
+    int g_launches;             // kernels per graph launch
+    double g_dt;                // the step size the graph was captured with
+    bool g_yz;
     int *flag_host;             // pinned
     // typed views
     float2 *psi() const { return (float2 *)(ws + off.psi); }
@@ -78,6 +87,8 @@ struct mlmd_domain {
     float *what_lo() const { return (float *)(ws + off.what_lo); }
     float *zpart() const { return (float *)(ws + off.zpart); }
     mlmd::StepCoef *coef() const { return (mlmd::StepCoef *)(ws + off.coef); }
+    mlmd::StepCoef *coef_cur() const { return (mlmd::StepCoef *)(ws + off.coef_cur); }
+    int *step_counter() const { return (int *)(ws + off.flag + 64); }
     int *flag() const { return (int *)(ws + off.flag); }
 };
 
@@ -151,5 +162,8 @@ cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld,
 cudaError_t launch_split_tf32(cudaStream_t st, float *x, float *lo, size_t n, int *nlaunch);
 cudaError_t launch_max_abs(cudaStream_t st, const float *x, size_t n, int *flag_bits, int *nlaunch);
 cudaError_t launch_check_finite(cudaStream_t st, const float *x, size_t n, int *flag, int *nlaunch);
+// graph support: *counter = value;  and  cur[d] = all[*counter * ndom + d], ++*counter
+cudaError_t launch_set_counter(cudaStream_t st, int *counter, int value, int *nlaunch);
+cudaError_t launch_advance_coef(cudaStream_t st, const StepCoef *all, StepCoef *cur, int *counter, int ndom, int *nlaunch);
 
 }  // namespace mlmd
