@@ -315,3 +315,24 @@ def test_perovskite_domain_two_steps():
     d = W.generate(c)
     A = W.laser_samples(c, nsteps=2, t0=0.9)      # near the pulse maximum so that A matters
     check(run_both(c, d, 2, A=A, check_first=False))
+
+
+def test_cuda_graph_step_equals_eager_launches(monkeypatch):
+    """Small batches replay a CUDA graph of the step (device-side coefficient slot): same bits as the
+    eager launches, with a field that changes every step and differs per domain."""
+    c = W.get_config(0, ndom=2, nsteps=9)
+    d = W.generate(c)
+    rng = np.random.default_rng(11)
+    A = 0.05 * rng.standard_normal((9, 2, 3))
+    A[:, :, 1:] = 0.0
+    outs, launches = [], []
+    for flag in ("1", "0"):
+        monkeypatch.setenv("MLMD_GRAPH", flag)
+        dom = make_domain(c, d)
+        dom.propagate(9, c.dt, A)
+        dom.propagate(5, c.dt, A[:5])          # second call reuses the captured graph
+        outs.append((dom.get_orbitals(), dom.density()))
+        launches.append(dom.launch_count())
+        dom.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert launches[0] > launches[1]            # + the coefficient-slot kernels of the graph
