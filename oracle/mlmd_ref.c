@@ -32,9 +32,13 @@
  * eigen-polynomial and expm on 16^3, Hermiticity, exact Taylor-4 norm identity, rank-1
  * projector closed form, Eq. (5) special case, density sum rule, batch independence,
  * Horner == term sum, brute force on an anisotropic 6x5x7 grid, 4th-order convergence.
+ * mlmd_ref_propagate_split (the literal Eq. (2) step, end of this file) is pinned by
+ * tests/test_oracle_split_pins.py: rank-1 kick closed form, reduction to the Taylor step, kick phase on
+ * eigenvectors, dense Kronecker matrices, leading error term against expm.
  * Absolute values printed by the paper: none exist (the paper prints no psi/rho numbers).
  */
 #include <complex.h>
+#include <math.h>
 #include <stdlib.h>
 #include <string.h>
 #ifdef _OPENMP
@@ -45,6 +49,7 @@ typedef double complex zc;
 
 #define MLMD_REF_NO_KINETIC 1 /* oracle-internal switch for pin P6: drop -1/2 D2 - iA.D1 + 1/2|A|^2 */
 #define MLMD_REF_HORNER 2     /* pin P10: evaluate the same polynomial in Horner form */
+#define MLMD_REF_NO_LOCAL 4   /* split step (Eq. 2): drop the whole local part, out = V_NL u */
 
 static const double C2[5] = {-1.0 / 12.0, 4.0 / 3.0, -5.0 / 2.0, 4.0 / 3.0, -1.0 / 12.0};
 static const double C1[5] = {1.0 / 12.0, -2.0 / 3.0, 0.0, 2.0 / 3.0, -1.0 / 12.0};
@@ -73,6 +78,9 @@ int mlmd_ref_apply_h(int nx, int ny, int nz, double hx, double hy, double hz, in
     const double A2 = A[0] * A[0] + A[1] * A[1] + A[2] * A[2];
     const int kinetic = !(flags & MLMD_REF_NO_KINETIC);
 
+    if (flags & MLMD_REF_NO_LOCAL) {
+        for (size_t e = 0; e < (size_t)ngrid * norb; ++e) out[e] = 0.0;
+    } else {
     /* local part: -1/2 D2 u - i A.D1 u + (V_loc + 1/2|A|^2) u */
 #pragma omp parallel for collapse(2) schedule(static)
     for (int ix = 0; ix < nx; ++ix)
@@ -92,6 +100,7 @@ int mlmd_ref_apply_h(int nx, int ny, int nz, double hx, double hy, double hz, in
                         for (int n = 0; n < norb; ++n) out[r * norb + n] += coef * u[rr * norb + n];
                     }
             }
+    }
     if (nproj <= 0) return 0;
 
     /* nonlocal part: C[p][n] = sum_r conj(beta[r][p]) u[r][n]; out[r][n] += sum_p beta[r][p] D_p dv C[p][n] */
@@ -211,6 +220,95 @@ int mlmd_ref_propagate(int ndom, int nx, int ny, int nz, double hx, double hy, d
                 }
                 memcpy(p, acc, ne * sizeof(zc));
             }
+            if (rho) mlmd_ref_density(1, ngrid, norb, p, occ + (size_t)dom * norb, rho + (size_t)dom * ngrid);
+        }
+        if (rho && nsteps == 0)
+            mlmd_ref_density(1, ngrid, norb, p, occ + (size_t)dom * norb, rho + (size_t)dom * ngrid);
+    }
+    free(phi);
+    free(hphi);
+    free(acc);
+    return rc;
+}
+
+
+/* ---- the paper's literal Eq. (2) step (readings D27, D28) ----
+ *
+ *   psi <- K  exp(-i dt h_loc(t_n + dt/2))  K  psi ,     K = (1 - i dt/2 v_nl) / || 1 - i dt/2 v_nl ||
+ *                                                                   PAPER.md Eq. (2), Eq. (3)
+ *   h_loc = 1/2 (-i grad + A)^2 + V_loc  (same finite differences as above),  v_nl = dv B diag(D) B^H;
+ *   with B = Psi(0) and D_p = const this v_nl is the nonlocal correction of Eq. (5)
+ *   (delta = -i dt/2 * D * dv).
+ *   D27: the norm in K's denominator is taken on the state K acts on, orbital by orbital, so that
+ *        each half-kick returns every orbital with the norm it came in with:
+ *        K psi_n = (psi_n - i dt/2 v_nl psi_n) * ||psi_n|| / ||psi_n - i dt/2 v_nl psi_n||.
+ *   D28: exp(-i dt h_loc) is the same 4th-order Taylor sum as the full-H step, applied to h_loc
+ *        alone (the paper's own local solver is only named, L147; NEXT-3).
+ * kick_only != 0 skips the local propagator (pin S3).
+ */
+static double col_norm2(const zc *u, long ngrid, int norb, int n) {
+    double s = 0.0;
+    for (long r = 0; r < ngrid; ++r) {
+        const zc v = u[r * norb + n];
+        s += creal(v) * creal(v) + cimag(v) * cimag(v);
+    }
+    return s;
+}
+
+static int half_kick(int nx, int ny, int nz, double hx, double hy, double hz, int norb, int nproj, zc *p,
+                     zc *vp, const double *vloc, const zc *beta, const double *D, const double *Av, double dt) {
+    const long ngrid = (long)nx * ny * nz;
+    int rc = mlmd_ref_apply_h(nx, ny, nz, hx, hy, hz, norb, nproj, p, vp, vloc, beta, D, Av, MLMD_REF_NO_LOCAL);
+    if (rc) return rc;
+    for (int n = 0; n < norb; ++n) {
+        const double before = col_norm2(p, ngrid, norb, n);
+        for (long r = 0; r < ngrid; ++r) p[r * norb + n] -= I * (0.5 * dt) * vp[r * norb + n];
+        const double after = col_norm2(p, ngrid, norb, n);
+        const double s = after > 0.0 ? sqrt(before / after) : 1.0;
+        for (long r = 0; r < ngrid; ++r) p[r * norb + n] *= s;
+    }
+    return 0;
+}
+
+int mlmd_ref_propagate_split(int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int norb,
+                             int nproj, zc *psi, const double *occ, const double *vloc, const zc *beta,
+                             const double *D, int nsteps, double dt, const double *A, int a_ndom,
+                             double *rho, int kick_only) {
+    const long ngrid = (long)nx * ny * nz;
+    const size_t ne = (size_t)ngrid * norb;
+    zc *phi = (zc *)malloc(ne * sizeof(zc));
+    zc *hphi = (zc *)malloc(ne * sizeof(zc));
+    zc *acc = (zc *)malloc(ne * sizeof(zc));
+    if (!phi || !hphi || !acc) {
+        free(phi);
+        free(hphi);
+        free(acc);
+        return 5;
+    }
+    int rc = 0;
+    for (int dom = 0; dom < ndom && !rc; ++dom) {
+        zc *p = psi + (size_t)dom * ne;
+        const double *v = vloc + (size_t)dom * ngrid;
+        const zc *b = beta ? beta + (size_t)dom * ngrid * nproj : NULL;
+        const double *d = D ? D + (size_t)dom * nproj : NULL;
+        for (int step = 0; step < nsteps && !rc; ++step) {
+            const double *Av = A + ((size_t)step * a_ndom + (a_ndom == 1 ? 0 : dom)) * 3;
+            if (nproj > 0) rc = half_kick(nx, ny, nz, hx, hy, hz, norb, nproj, p, hphi, v, b, d, Av, dt);
+            if (!kick_only && !rc) {
+                /* phi_0 = psi; phi_m = (-i dt/m) h_loc phi_{m-1}; psi_new = sum_{m=0..4} phi_m */
+                memcpy(phi, p, ne * sizeof(zc));
+                memcpy(acc, p, ne * sizeof(zc));
+                for (int m = 1; m <= 4 && !rc; ++m) {
+                    rc = mlmd_ref_apply_h(nx, ny, nz, hx, hy, hz, norb, 0, phi, hphi, v, NULL, NULL, Av, 0);
+                    const zc f = -I * dt / (double)m;
+                    for (size_t e = 0; e < ne; ++e) {
+                        phi[e] = f * hphi[e];
+                        acc[e] += phi[e];
+                    }
+                }
+                memcpy(p, acc, ne * sizeof(zc));
+            }
+            if (nproj > 0 && !rc) rc = half_kick(nx, ny, nz, hx, hy, hz, norb, nproj, p, hphi, v, b, d, Av, dt);
             if (rho) mlmd_ref_density(1, ngrid, norb, p, occ + (size_t)dom * norb, rho + (size_t)dom * ngrid);
         }
         if (rho && nsteps == 0)

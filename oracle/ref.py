@@ -16,6 +16,7 @@ from . import build as _build
 
 NO_KINETIC = 1
 HORNER = 2
+NO_LOCAL = 4
 
 _lib = None
 
@@ -34,6 +35,8 @@ def lib() -> ctypes.CDLL:
         _lib.mlmd_ref_overlap.restype = i
         _lib.mlmd_ref_propagate.argtypes = [i, i, i, i, d, d, d, i, i, p, p, p, p, p, i, d, p, i, p, i]
         _lib.mlmd_ref_propagate.restype = i
+        _lib.mlmd_ref_propagate_split.argtypes = [i, i, i, i, d, d, d, i, i, p, p, p, p, p, i, d, p, i, p, i]
+        _lib.mlmd_ref_propagate_split.restype = i
     return _lib
 
 
@@ -90,6 +93,30 @@ def propagate(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], nsteps:
                                   _ptr(vloc), _ptr(b), _ptr(dd), nsteps, dt, _ptr(A), A.shape[1], _ptr(rho), flags)
     if rc:
         raise RuntimeError("mlmd_ref_propagate failed: %d" % rc)
+    return p, rho
+
+
+def propagate_split(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], nsteps: Optional[int] = None,
+                    kick_only: bool = False) -> Tuple[np.ndarray, np.ndarray]:
+    """nsteps steps of the paper's literal Eq. (2): half-kick, Taylor-4 of h_loc, half-kick.
+    Same arguments and return values as ``propagate``."""
+    p = _c128(psi).copy()
+    ndom, nx, ny, nz, norb = p.shape
+    vloc = _f64(vloc)
+    occ = _f64(occ)
+    nproj = 0 if beta is None else beta.shape[-1]
+    b = _c128(beta.reshape(ndom, -1, nproj)) if nproj else None
+    dd = _f64(D) if nproj else None
+    A = _f64(A)
+    if nsteps is None:
+        nsteps = A.shape[0]
+    assert A.ndim == 3 and A.shape[0] >= nsteps and A.shape[1] in (1, ndom) and A.shape[2] == 3
+    rho = np.empty((ndom, nx, ny, nz), dtype=np.float64)
+    rc = lib().mlmd_ref_propagate_split(ndom, nx, ny, nz, h[0], h[1], h[2], norb, nproj, _ptr(p), _ptr(occ),
+                                        _ptr(vloc), _ptr(b), _ptr(dd), nsteps, dt, _ptr(A), A.shape[1], _ptr(rho),
+                                        1 if kick_only else 0)
+    if rc:
+        raise RuntimeError("mlmd_ref_propagate_split failed: %d" % rc)
     return p, rho
 
 
