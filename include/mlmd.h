@@ -107,6 +107,16 @@ int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode);
  * dt * [ (8/3) sum_d 1/h_d^2 + 1.3722 sum_d |A_d|/h_d + |A|^2/2 + max|V_loc| + max|D| ] > 2 sqrt(2). */
 int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
 
+/* nsteps steps of the paper's literal Eq. (2):
+ *     psi <- K exp(-i dt h_loc(t_n + dt/2)) K psi,   K psi_n = (psi_n - i dt/2 V_NL psi_n) ||psi_n|| / ||psi_n - i dt/2 V_NL psi_n||
+ * i.e. a normalised first-order nonlocal half-kick (the norm is taken per orbital on the state the kick
+ * acts on, reading D27), the 4th-order Taylor sum of h_loc = 1/2(-i grad + A)^2 + V_loc alone (D28), and
+ * a second half-kick.  With beta = Psi(0) (MLMD_BETA_COMPLEX64) and D_p = const this V_NL is the nonlocal
+ * correction of Eq. (5) L199 with delta = -i dt/2 D dv.  Two V_NL applications per step instead of four.
+ * Arguments, density and return values as mlmd_propagate; the stability bound leaves out max|D| (the
+ * normalised kick is stable for any dt |D|).  With nproj = 0 it is the same map as mlmd_propagate. */
+int mlmd_propagate_split(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
+
 /* rho(r) = sum_n f_n |psi_n(r)|^2 of the current state, float [ndom][nx][ny][nz] at `where`. */
 int mlmd_density(mlmd_domain_t *h, float *rho, int where);
 
@@ -120,7 +130,8 @@ int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
  * mlmd_profile(h, 0) stops.  mlmd_profile_read synchronises the stream and returns the summed
  * device time in milliseconds and the number of launches of class `kind` recorded so far. */
 enum { MLMD_K_STENCIL = 0, MLMD_K_PROJ = 1, MLMD_K_BACK = 2, MLMD_K_GLUE = 3, MLMD_K_DENSITY = 4,
-       MLMD_K_NLP = 5 /* fused back-application + projection */, MLMD_K_COUNT = 6 };
+       MLMD_K_NLP = 5 /* fused back-application + projection */,
+       MLMD_K_NORM = 6 /* per-orbital norms of the split step */, MLMD_K_COUNT = 7 };
 int mlmd_profile(mlmd_domain_t *h, int enable);
 int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *launches);
 

@@ -18,6 +18,7 @@ from .api import (  # noqa: F401
     mlmd_set_projectors,
     mlmd_set_gemm_mode,
     mlmd_propagate,
+    mlmd_propagate_split,
     mlmd_density,
     mlmd_overlap,
     mlmd_launch_count,

@@ -24,10 +24,11 @@ KEEP_PSI0, CHECK_FINITE = 1, 2
 EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",
     "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_propagate",
+    "mlmd_propagate_split",
     "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
 ]
-K_STENCIL, K_PROJ, K_BACK, K_GLUE, K_DENSITY, K_NLP = range(6)
-KERNEL_CLASSES = ["stencil", "proj", "back", "glue", "density", "nlp"]
+K_STENCIL, K_PROJ, K_BACK, K_GLUE, K_DENSITY, K_NLP, K_NORM = range(7)
+KERNEL_CLASSES = ["stencil", "proj", "back", "glue", "density", "nlp", "norm"]
 
 
 class MlmdError(RuntimeError):
@@ -58,6 +59,7 @@ def lib() -> ctypes.CDLL:
         L.mlmd_set_projectors.argtypes = [p, i, p, i, p, i]
         L.mlmd_set_gemm_mode.argtypes = [p, i]
         L.mlmd_propagate.argtypes = [p, i, d, p, i]
+        L.mlmd_propagate_split.argtypes = [p, i, d, p, i]
         L.mlmd_density.argtypes = [p, p, i]
         L.mlmd_overlap.argtypes = [p, i, p, i]
         L.mlmd_profile.argtypes = [p, i]
@@ -168,6 +170,15 @@ def mlmd_propagate(h, nsteps, dt, A) -> int:
     return _check(lib().mlmd_propagate(h, nsteps, dt, None if a is None else a.ctypes.data_as(ctypes.c_void_p), a_ndom))
 
 
+def mlmd_propagate_split(h, nsteps, dt, A) -> int:
+    """The paper's literal Eq. (2) step (half-kick, Taylor-4 of h_loc, half-kick); arguments as mlmd_propagate."""
+    a = _host_f64(A)
+    if nsteps > 0 and (a.ndim != 3 or a.shape[0] < nsteps or a.shape[2] != 3):
+        raise ValueError("A must have shape [nsteps, a_ndom, 3]")
+    a_ndom = a.shape[1] if a is not None and a.ndim == 3 else 1
+    return _check(lib().mlmd_propagate_split(h, nsteps, dt, None if a is None else a.ctypes.data_as(ctypes.c_void_p), a_ndom))
+
+
 def mlmd_density(h, out):
     p, where = _ptr_where(out, np.dtype(np.float32))
     _check(lib().mlmd_density(h, p, where))
@@ -248,6 +259,9 @@ class Domain:
 
     def propagate(self, nsteps, dt, A):
         return mlmd_propagate(self.handle, nsteps, dt, A)
+
+    def propagate_split(self, nsteps, dt, A):
+        return mlmd_propagate_split(self.handle, nsteps, dt, A)
 
     def density(self, out=None):
         if out is None:

@@ -84,6 +84,9 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.coef = take((size_t)kCoefCapacity * ndom * sizeof(StepCoef));
     w.coef_cur = take((size_t)ndom * sizeof(StepCoef));
     w.flag = take(256);
+    w.nrm = take((size_t)4 * ndom * pl->ld * sizeof(double));
+    w.nrm_part = take((size_t)ndom * kNormSlabs * pl->ld * sizeof(double));
+    w.scl = take((size_t)ndom * pl->ld * sizeof(float));
     w.total = o;
     return true;
 }
@@ -470,6 +473,105 @@ static int capture_step(mlmd_domain *h, double dt, bool yz) {
     h->g_launches = nl;
     h->g_dt = dt;
     h->g_yz = yz;
+    return MLMD_OK;
+}
+
+// One step of the paper's literal Eq. (2) (readings D27, D28): normalised first-order
+// nonlocal half-kick, Taylor-4 of h_loc alone, half-kick.  The chain runs un-normalised (a per-orbital scale
+// commutes with every operator in it); the four squared norms give the two kick scales, which are applied in
+// the pass that also computes the density.
+static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, int *nl) {
+    const bool kicks = h->nproj > 0;
+    auto norm2 = [&](int which) -> int {
+        ProfScope ps(h, MLMD_K_NORM);
+        CU(launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->nrm_part(), h->nrm(which), nl));
+        return MLMD_OK;
+    };
+    auto half_kick = [&](int which) -> int {     // psi += (-i dt/2) V_NL psi, then its squared norms -> nrm(which)
+        int rc = nonlocal_project(h, h->psi(), (float)(0.5 * dt), nl);
+        if (!rc) rc = nonlocal_back(h, h->psi(), nl);
+        return rc ? rc : norm2(which);
+    };
+    if (kicks) {
+        int rc = half_kick(1);
+        if (rc) return rc;
+    }
+    const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
+    float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
+    for (int i = 0; i < 4; ++i) {
+        ProfScope ps(h, MLMD_K_STENCIL);
+        CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, coef_host, (float)(dt / (4 - i)), nl));
+    }
+    if (!kicks) {
+        ProfScope ps(h, MLMD_K_DENSITY);
+        CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), nl));
+        return MLMD_OK;
+    }
+    int rc = norm2(2);
+    if (!rc) rc = half_kick(3);
+    if (rc) return rc;
+    {
+        ProfScope ps(h, MLMD_K_GLUE);
+        CU(launch_kick_scale(h->stream, h->ndom * h->ld, h->nrm(0), h->nrm(1), h->nrm(2), h->nrm(3), h->scl(), nl));
+    }
+    ProfScope ps(h, MLMD_K_DENSITY);
+    CU(launch_scale_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->scl(), h->occ(), h->rho(), nl));
+    return MLMD_OK;
+}
+
+int mlmd_propagate_split(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom) {
+    if (!h) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: NULL handle");
+    if (nsteps < 0 || !(dt == dt) || std::isinf(dt)) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: nsteps=%d dt=%g", nsteps, dt);
+    if (nsteps > 0 && !A) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: A is NULL");
+    if (a_ndom != 1 && a_ndom != h->ndom) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: a_ndom=%d must be 1 or ndom=%d", a_ndom, h->ndom);
+    if (!h->have_psi || !h->have_vloc) return fail(MLMD_ERR_STATE, "mlmd_propagate_split: call mlmd_set_orbitals and mlmd_set_vloc first");
+    // Taylor-4 acts on h_loc only; the normalised kick is stable for any dt |D|
+    bool yz = false;
+    double bound = 0.0;
+    for (size_t i = 0; i < (size_t)nsteps * a_ndom; ++i) {
+        const double *a = A + 3 * i;
+        if (!std::isfinite(a[0]) || !std::isfinite(a[1]) || !std::isfinite(a[2]))
+            return fail(MLMD_ERR_NONFINITE, "mlmd_propagate_split: A[%zu] is not finite", i);
+        yz = yz || a[1] != 0.0 || a[2] != 0.0;
+        const double b = (8.0 / 3.0) * (1 / (h->hx * h->hx) + 1 / (h->hy * h->hy) + 1 / (h->hz * h->hz)) +
+                         1.3722 * (fabs(a[0]) / h->hx + fabs(a[1]) / h->hy + fabs(a[2]) / h->hz) +
+                         0.5 * (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) + h->vmax;
+        bound = std::max(bound, b);
+    }
+    h->field_yz = yz;
+    int nl = 0;
+    if (nsteps > 0 && h->nproj > 0) {
+        ProfScope ps(h, MLMD_K_NORM);
+        CU(launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->nrm_part(), h->nrm(0), &nl));
+    }
+    CU(cudaEventSynchronize(h->coef_uploaded));
+    for (int s0 = 0; s0 < nsteps; s0 += kCoefCapacity) {
+        const int ns = std::min(kCoefCapacity, nsteps - s0);
+        if (s0 > 0) CU(cudaStreamSynchronize(h->stream));
+        for (int s = 0; s < ns; ++s)
+            for (int d = 0; d < h->ndom; ++d)
+                fill_coef(h, A + ((size_t)(s0 + s) * a_ndom + (a_ndom == 1 ? 0 : d)) * 3, &h->coef_host[(size_t)s * h->ndom + d]);
+        CU(cudaMemcpyAsync(h->coef(), h->coef_host, (size_t)ns * h->ndom * sizeof(StepCoef), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaEventRecord(h->coef_uploaded, h->stream));
+        for (int s = 0; s < ns; ++s) {
+            int rc = enqueue_split_step(h, h->coef() + (size_t)s * h->ndom, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr, dt, &nl);
+            if (rc) return rc;
+        }
+    }
+    h->launches += nl;
+    if (nsteps > 0) h->rho_valid = true;
+    if (h->flags & MLMD_CHECK_FINITE) {
+        int n2 = 0;
+        CU(launch_check_finite(h->stream, (const float *)h->psi(), (size_t)h->ndom * h->ngrid * h->ld * 2, h->flag(), &n2));
+        h->launches += n2;
+        CU(cudaMemcpyAsync(h->flag_host, h->flag(), sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        if (*h->flag_host) return fail(MLMD_ERR_NONFINITE, "mlmd_propagate_split: psi contains NaN/Inf after %d steps", nsteps);
+    }
+    if (dt * bound > 2.0 * sqrt(2.0)) {
+        fail(MLMD_WARN_UNSTABLE, "mlmd_propagate_split: dt*|h_loc|max bound = %.3f > 2 sqrt(2): Taylor-4 may be unstable", dt * bound);
+        return MLMD_WARN_UNSTABLE;
+    }
     return MLMD_OK;
 }
 

@@ -244,4 +244,117 @@ cudaError_t launch_advance_coef(cudaStream_t st, const StepCoef *all, StepCoef *
     return cudaGetLastError();
 }
 
+// ---- the literal Eq. (2) step (mlmd_propagate_split; D27): per-orbital norms and rescaling ----
+// part[dom][slab][c] = sum_{r in slab} |psi[dom][r][c]|^2: FP32 squares summed in FP64, one owner per
+// partial sum, slabs added in a fixed order by colnorm_final_kernel, so the norms are reproducible.
+__global__ void __launch_bounds__(256)
+colnorm_part_kernel(long ngrid, int ld, const float2 *__restrict__ psi, double *__restrict__ part) {
+    const int c = blockIdx.z * 64 + threadIdx.x;
+    const int dom = blockIdx.y, slab = blockIdx.x;
+    const long per = (ngrid + kNormSlabs - 1) / kNormSlabs;
+    const long r0 = slab * per, r1 = r0 + per < ngrid ? r0 + per : ngrid;
+    double s = 0.0;
+    if (c < ld) {
+        const float2 *col = psi + (size_t)dom * ngrid * ld + c;
+#pragma unroll 4
+        for (long r = r0 + threadIdx.y; r < r1; r += 4) {
+            const float2 v = __ldcs(col + r * ld);
+            s += (double)fmaf(v.x, v.x, v.y * v.y);
+        }
+    }
+    __shared__ double sm[4][64];
+    sm[threadIdx.y][threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.y == 0 && c < ld)
+        part[((size_t)dom * kNormSlabs + slab) * ld + c] = (sm[0][threadIdx.x] + sm[1][threadIdx.x]) + (sm[2][threadIdx.x] + sm[3][threadIdx.x]);
+}
+__global__ void colnorm_final_kernel(int n, int ld, const double *__restrict__ part, double *__restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;     // i = dom * ld + c
+    if (i >= n) return;
+    const int dom = i / ld, c = i % ld;
+    double s = 0.0;
+    for (int k = 0; k < kNormSlabs; ++k) s += part[((size_t)dom * kNormSlabs + k) * ld + c];
+    out[i] = s;
+}
+cudaError_t launch_colnorm2(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, double *part, double *out,
+                            int *nlaunch) {
+    *nlaunch += 2;
+    colnorm_part_kernel<<<dim3(kNormSlabs, ndom, (ld + 63) / 64), dim3(64, 4), 0, st>>>(ngrid, ld, psi, part);
+    colnorm_final_kernel<<<(ndom * ld + 127) / 128, 128, 0, st>>>(ndom * ld, ld, part, out);
+    return cudaGetLastError();
+}
+
+// One step's pending scale from the four squared norms (un-normalised chain, D27):
+//   kick 1: ||psi|| / ||psi_a||, kick 2: ||psi_c|| / ||psi_d||;  the true squared norm after the step is
+//   n0 * nc / na (the kicks keep it, the Taylor step changes it by nc / na).
+__global__ void kick_scale_kernel(int n, double *__restrict__ n0, const double *__restrict__ na, const double *__restrict__ nc,
+                                  const double *__restrict__ nd, float *__restrict__ scl) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double a = na[i], d = nd[i];
+    if (a > 0.0 && d > 0.0) {
+        scl[i] = (float)sqrt((n0[i] / a) * (nc[i] / d));
+        n0[i] = n0[i] * (nc[i] / a);
+    } else {
+        scl[i] = 1.f;       // zero (padded) orbitals stay zero
+    }
+}
+cudaError_t launch_kick_scale(cudaStream_t st, int n, double *n0, const double *na, const double *nc, const double *nd,
+                              float *scl, int *nlaunch) {
+    ++*nlaunch;
+    kick_scale_kernel<<<(n + 127) / 128, 128, 0, st>>>(n, n0, na, nc, nd, scl);
+    return cudaGetLastError();
+}
+
+// psi[r][n] *= scl[n] and rho[r] = sum_n occ[n] |psi[r][n]|^2 of the scaled values, in one pass
+// (NP consecutive points of one domain per warp, as density_kernel).
+template <int NP>
+__global__ void __launch_bounds__(256)
+scale_density_kernel(long npoints, long ngrid, int lanes, float4 *__restrict__ psi, const float *__restrict__ scl,
+                     const float *__restrict__ occ, float *__restrict__ rho) {
+    const long p0 = ((long)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32) * NP;
+    if (p0 >= npoints) return;
+    const int lane = threadIdx.x % 32;
+    float s[NP];
+#pragma unroll
+    for (int k = 0; k < NP; ++k) s[k] = 0.f;
+    const size_t dom = (size_t)(p0 / ngrid);
+    const float2 *f = (const float2 *)(occ + dom * lanes * 2);
+    const float2 *sc = (const float2 *)(scl + dom * lanes * 2);
+    for (int l = lane; l < lanes; l += 32) {
+        float4 v[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) v[k] = psi[(p0 + k) * lanes + l];
+        const float2 ff = __ldg(f + l), ss = __ldg(sc + l);
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+            v[k].x *= ss.x; v[k].y *= ss.x; v[k].z *= ss.y; v[k].w *= ss.y;
+            psi[(p0 + k) * lanes + l] = v[k];
+            s[k] = fmaf(ff.x, fmaf(v[k].x, v[k].x, v[k].y * v[k].y), s[k]);
+            s[k] = fmaf(ff.y, fmaf(v[k].z, v[k].z, v[k].w * v[k].w), s[k]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NP; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s[k] += __shfl_xor_sync(0xffffffffu, s[k], o);
+    }
+    if (lane < NP) {
+        float out = s[0];
+#pragma unroll
+        for (int k = 1; k < NP; ++k) out = lane == k ? s[k] : out;
+        rho[p0 + lane] = out;
+    }
+}
+cudaError_t launch_scale_density(cudaStream_t st, int ndom, long ngrid, int ld, float2 *psi, const float *scl,
+                                 const float *occ, float *rho, int *nlaunch) {
+    const long npoints = (long)ndom * ngrid;
+    ++*nlaunch;
+    if (ngrid % 4 == 0)
+        scale_density_kernel<4><<<(unsigned)((npoints / 4 + 7) / 8), 256, 0, st>>>(npoints, ngrid, ld / 2, (float4 *)psi, scl, occ, rho);
+    else
+        scale_density_kernel<1><<<(unsigned)((npoints + 7) / 8), 256, 0, st>>>(npoints, ngrid, ld / 2, (float4 *)psi, scl, occ, rho);
+    return cudaGetLastError();
+}
+
 }  // namespace mlmd

@@ -23,11 +23,13 @@ struct StepCoef {
 static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
-    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag, total;
+    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
+        nrm, nrm_part, scl, total;
 };
 
 constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
 constexpr int kMaxSplit = 64;        // split-K slices of the projection GEMM
+constexpr int kNormSlabs = 64;       // row slabs per domain of the per-orbital norm reduction (split step)
 
 }  // namespace mlmd
 
@@ -90,6 +92,10 @@ struct mlmd_domain {
     mlmd::StepCoef *coef_cur() const { return (mlmd::StepCoef *)(ws + off.coef_cur); }
     int *step_counter() const { return (int *)(ws + off.flag + 64); }
     int *flag() const { return (int *)(ws + off.flag); }
+    // split step (Eq. 2): squared orbital norms [4][ndom][ld] (input, after kick 1, after Taylor, after kick 2)
+    double *nrm(int which) const { return (double *)(ws + off.nrm) + (size_t)which * ndom * ld; }
+    double *nrm_part() const { return (double *)(ws + off.nrm_part); }
+    float *scl() const { return (float *)(ws + off.scl); }
 };
 
 namespace mlmd {
@@ -165,5 +171,13 @@ cudaError_t launch_check_finite(cudaStream_t st, const float *x, size_t n, int *
 // graph support: *counter = value;  and  cur[d] = all[*counter * ndom + d], ++*counter
 cudaError_t launch_set_counter(cudaStream_t st, int *counter, int value, int *nlaunch);
 cudaError_t launch_advance_coef(cudaStream_t st, const StepCoef *all, StepCoef *cur, int *counter, int ndom, int *nlaunch);
+// split step (Eq. (2), reading D27): out[dom][c] = sum_r |psi[dom][r][c]|^2 (FP64, fixed order);
+// scl = sqrt(n0/na * nc/nd), n0 <- n0 nc/na;  psi *= scl fused with the density pass
+cudaError_t launch_colnorm2(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, double *part, double *out,
+                            int *nlaunch);
+cudaError_t launch_kick_scale(cudaStream_t st, int n, double *n0, const double *na, const double *nc, const double *nd,
+                              float *scl, int *nlaunch);
+cudaError_t launch_scale_density(cudaStream_t st, int ndom, long ngrid, int ld, float2 *psi, const float *scl,
+                                 const float *occ, float *rho, int *nlaunch);
 
 }  // namespace mlmd

@@ -1,0 +1,130 @@
+"""GPU parity of mlmd_propagate_split (the paper's literal Eq. (2) step) against
+the FP64 oracle's mlmd_ref_propagate_split on the same seeded inputs, through the C ABI.
+Tolerances are the hot path's (BASELINE.json north_star): per-orbital rel L2 <= 1e-5 after one step,
+<= 1e-4 after the last, density <= 1e-4, Gram <= 1e-5; low-precision GEMM mode 1e-3.
+"""
+import numpy as np
+import pytest
+
+import workloads as W
+from test_gpu_parity import TOL_1STEP, TOL_LAST, TOL_RHO, TOL_GRAM, TOL_LOWP, make_domain, orb_err, rho_err
+
+pytestmark = pytest.mark.gpu
+
+
+def run_split(c, d, nsteps, A=None, mode=None, first=True):
+    from oracle import ref
+    A = d["A"] if A is None else A
+    dom = make_domain(c, d, mode=mode)
+    out = {}
+    if first:
+        dom.propagate_split(1, c.dt, A[:1])
+        r1, _ = ref.propagate_split(d["psi"], d["occ"], d["vloc"], d.get("beta"), d.get("D"), A[:1], c.dt, c.h)
+        out["err1"] = orb_err(dom.get_orbitals(), r1)
+        dom.set_orbitals(d["psi"], d["occ"])
+    dom.propagate_split(nsteps, c.dt, A[:nsteps])
+    g, rho, G = dom.get_orbitals(), dom.density(), dom.overlap(0)
+    r, rho_ref = ref.propagate_split(d["psi"], d["occ"], d["vloc"], d.get("beta"), d.get("D"), A[:nsteps], c.dt, c.h)
+    out.update(err=orb_err(g, r), rho=rho_err(rho, rho_ref), gram=float(np.abs(G - ref.overlap(r, r, c.dv)).max()),
+               launches=dom.launch_count())
+    dom.close()
+    print(out)
+    return out
+
+
+def check(res, lowp=False):
+    if lowp:
+        assert res["err"] <= TOL_LOWP and res["rho"] <= TOL_LOWP and res["gram"] <= TOL_LOWP
+        return
+    if "err1" in res:
+        assert res["err1"] <= TOL_1STEP
+    assert res["err"] <= TOL_LAST and res["rho"] <= TOL_RHO and res["gram"] <= TOL_GRAM
+
+
+def test_split_config0_10_steps():
+    c = W.get_config(0)
+    check(run_split(c, W.generate(c), c.nsteps))
+
+
+def test_split_config1_laser_100_steps():
+    c = W.get_config(1)
+    check(run_split(c, W.generate(c), c.nsteps))
+
+
+def test_split_one_perovskite_domain():
+    """One configs[2]-shaped domain (48^3 x 224 orbitals x 240 projectors): the tensor-core GEMM path."""
+    import paper_2509_00966_b200 as M
+    c = W.get_config(2, ndom=1, nsteps=2)
+    d = W.generate(c)
+    dom = make_domain(c, d)
+    assert M.lib().mlmd_gemm_path(dom.handle) == 1
+    dom.close()
+    check(run_split(c, d, 2, A=W.laser_samples(c, nsteps=2, t0=0.9), first=False))
+
+
+@pytest.mark.parametrize("grid,norb,cplx", [((6, 5, 7), 3, True), ((8, 16, 8), 5, False), ((16, 16, 32), 12, True)])
+def test_split_ragged_shapes_complex_projectors_per_domain_field(grid, norb, cplx):
+    """Anisotropic spacings, grids off the tile sizes, complex projectors (the Eq. (5) form), one field per domain."""
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    rng = np.random.default_rng(7 + norb)
+    ndom, nproj, h, dt, nsteps = 3, 4, (0.5, 0.45, 0.4), 0.02, 3
+    ngrid = int(np.prod(grid))
+    psi = (rng.standard_normal((ndom, *grid, norb)) + 1j * rng.standard_normal((ndom, *grid, norb))).astype(np.complex64)
+    psi /= np.sqrt((np.abs(psi) ** 2).sum(axis=(1, 2, 3), keepdims=True) * np.prod(h))
+    occ = rng.uniform(0, 2, (ndom, norb))
+    vloc = rng.uniform(-1, 0.5, (ndom, *grid)).astype(np.float32)
+    beta = rng.standard_normal((ndom, ngrid, nproj)) + (1j * rng.standard_normal((ndom, ngrid, nproj)) if cplx else 0)
+    beta = (beta * 0.5).astype(np.complex64 if cplx else np.float32)
+    D = rng.uniform(-2, 2, (ndom, nproj))
+    A = rng.uniform(-0.2, 0.2, (nsteps, ndom, 3))
+    dom = M.Domain(ndom, grid, h, norb, nproj * (2 if cplx else 1))
+    dom.set_vloc(vloc)
+    dom.set_orbitals(psi, occ)
+    dom.set_projectors(beta, D)
+    dom.propagate_split(nsteps, dt, A)
+    r, rho_ref = ref.propagate_split(psi, occ, vloc, beta, D, A, dt, h)
+    assert orb_err(dom.get_orbitals(), r) <= TOL_LAST
+    assert rho_err(dom.density(), rho_ref) <= TOL_RHO
+    dom.close()
+
+
+def test_split_kick_keeps_every_orbital_norm():
+    """D27 on the GPU itself: with h_loc's Taylor damping negligible (smooth orbitals) the diagonal of the Gram
+    matrix stays at its initial value through 20 steps of strong kicks."""
+    c = W.get_config(1, smooth_kcut=2.5)
+    d = W.generate(c)
+    d["D"] = d["D"] * 20.0
+    dom = make_domain(c, d)
+    g0 = np.real(np.diagonal(dom.overlap(0), axis1=1, axis2=2)).copy()
+    dom.propagate_split(20, c.dt, d["A"][:20])
+    g1 = np.real(np.diagonal(dom.overlap(0), axis1=1, axis2=2))
+    assert np.abs(g1 - g0).max() <= 1e-5
+    dom.close()
+
+
+def test_split_without_projectors_is_the_taylor_step():
+    c = W.get_config(0)
+    d = W.generate(c)
+    d2 = dict(d, beta=None, D=None)
+    a = make_domain(c, d2)
+    b = make_domain(c, d2)
+    a.propagate_split(3, c.dt, d["A"][:3])
+    b.propagate(3, c.dt, d["A"][:3])
+    assert np.array_equal(a.get_orbitals(), b.get_orbitals())
+    assert np.array_equal(a.density(), b.density())
+    a.close()
+    b.close()
+
+
+def test_split_low_precision_mode_and_errors():
+    import paper_2509_00966_b200 as M
+    c = W.get_config(2, ndom=1, nsteps=2)
+    d = W.generate(c)
+    check(run_split(c, d, 2, mode=M.GEMM_LOWP_BF16, first=False), lowp=True)
+    dom = make_domain(W.get_config(0), W.generate(W.get_config(0)))
+    with pytest.raises(M.MlmdError):
+        dom.propagate_split(1, 0.02, np.full((1, 1, 3), np.nan))
+    with pytest.raises(M.MlmdError):
+        dom.propagate_split(1, 0.02, np.zeros((1, 2, 3)))      # a_ndom must be 1 or ndom
+    dom.close()
