@@ -31,6 +31,7 @@ PAPER_CONTEXT = {
     "note": "PAPER.md L38-39, L298, L302: Aurora, 1,024-orbital domains of unstated mesh size; context only",
 }
 MODE_NAMES = {"fp32grade": 0, "fp64": 1, "bf16": 2, "tf32x1": 3, "simt": 4}
+STEP_NAMES = {"taylor": "Taylor-4 (full H, north_star)", "split": "Eq. (2) split (half-kick, Taylor-4 of h_loc, half-kick)"}
 # tensor peak as a multiple of the measured dense BF16 peak (B200_PROFILING.md nominal ratios:
 # tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
 # the opt-in BF16-operand mode issues its single product on the TF32 pipe (BF16 values are TF32 values)
@@ -83,14 +84,19 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(float(r[2]) for r in self.rows), "reasons": reasons}
 
 
-def algorithmic(c, gemm_real=True):
-    """Algorithmic bytes and flops per step of the whole batch."""
+def algorithmic(c, gemm_real=True, step="taylor"):
+    """Algorithmic bytes and flops per step of the whole batch.  step="split" (the literal
+    Eq. (2) step, mlmd_propagate_split): two V_NL applications instead of four, three per-orbital norm passes
+    (8 B per element each) and the density pass also rescales psi (16 B per element)."""
     elems = c.ndom * c.ngrid * c.norb
     stage_bytes = [16, 24, 24, 24]
-    bytes_step = elems * (sum(stage_bytes) + 8) + c.ndom * c.ngrid * (4 * 4 + 4)
+    split = step == "split"
+    density_b, norm_b, ngemm = (16, 3 * 8, 4) if split else (8, 0, 8)
+    bytes_step = elems * (sum(stage_bytes) + density_b + norm_b) + c.ndom * c.ngrid * (4 * 4 + 4)
     gemm_flops_each = (2 if gemm_real else 4) * 2.0 * c.ndom * c.ngrid * c.nproj * c.norb   # one GEMM batch
     return {"elems": elems, "bytes_step": bytes_step, "stencil_bytes": [elems * b for b in stage_bytes],
-            "density_bytes": elems * 8, "gemm_flops_each": gemm_flops_each, "gemm_flops_step": 8 * gemm_flops_each}
+            "density_bytes": elems * density_b, "norm_bytes": elems * 8, "gemm_flops_each": gemm_flops_each,
+            "gemm_flops_step": ngemm * gemm_flops_each}
 
 
 def ncu_traffic(c, kernel_class):
@@ -116,14 +122,15 @@ def sample_for_oracle(c, d, norb_sample):
             "vloc": d["vloc"][:1], "beta": d["beta"][:1], "D": d["D"][:1]}
 
 
-def time_oracle(c, s, A, steps, warmup):
+def time_oracle(c, s, A, steps, warmup, step="taylor"):
     from oracle import ref
+    prop = ref.propagate_split if step == "split" else ref.propagate
     for _ in range(warmup):
-        ref.propagate(s["psi"], s["occ"], s["vloc"], s["beta"], s["D"], A[:1], c.dt, c.h)
+        prop(s["psi"], s["occ"], s["vloc"], s["beta"], s["D"], A[:1], c.dt, c.h)
     t0 = time.perf_counter()
     psi = s["psi"]
     for k in range(steps):
-        psi, _ = ref.propagate(psi, s["occ"], s["vloc"], s["beta"], s["D"], A[k:k + 1], c.dt, c.h)
+        psi, _ = prop(psi, s["occ"], s["vloc"], s["beta"], s["D"], A[k:k + 1], c.dt, c.h)
     dt = time.perf_counter() - t0
     electrons = float(s["occ"].sum())
     return electrons * steps / dt, dt / steps, ref.num_threads(), electrons
@@ -139,9 +146,9 @@ def run_reference(args):
     d = {k: d1[k][None] for k in ("psi", "occ", "vloc", "beta", "D")}
     A = W.laser_samples(c, nsteps=max(args.steps, 1))
     s = sample_for_oracle(c, d, args.oracle_orbitals)
-    value, sec_step, cores, electrons = time_oracle(c, s, A, args.steps, args.warmup)
-    sample = "domain 0 of configs[%d], first %d of %d orbitals (%g electrons), all %d projectors, 1 Taylor-4 step per bench step" % (
-        c.cfg, s["psi"].shape[-1], c.norb, electrons, c.nproj)
+    value, sec_step, cores, electrons = time_oracle(c, s, A, args.steps, args.warmup, args.step)
+    sample = "domain 0 of configs[%d], first %d of %d orbitals (%g electrons), all %d projectors, 1 %s step per bench step" % (
+        c.cfg, s["psi"].shape[-1], c.norb, electrons, c.nproj, STEP_NAMES[args.step])
     line = {
         "impl": "reference", "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec_step * 1e3,
@@ -157,7 +164,7 @@ def run_reference(args):
 def workload_config(c, args):
     return {"workload": "configs[%d] %s: %d domains x %dx%dx%d grid x %d orbitals x %d projectors, dt=%g" % (
         c.cfg, c.name, c.ndom, *c.grid, c.norb, c.nproj, c.dt),
-        "ndom_per_gpu": c.ndom, "gemm_mode": args.gemm_mode, "gemm_path": getattr(args, "gemm_path", None), "parallelism": "domains sharded, no collective",
+        "ndom_per_gpu": c.ndom, "step": STEP_NAMES[args.step], "gemm_mode": args.gemm_mode, "gemm_path": getattr(args, "gemm_path", None), "parallelism": "domains sharded, no collective",
         "l2": "working set (3 x %.1f GB psi buffers + beta) exceeds the 126 MB L2; no flush needed" % (
             c.ndom * c.ngrid * c.norb * 8 / 1e9) if c.ndom * c.ngrid * c.norb * 8 > 4e8 else
         "working set may fit L2: a 256 MB buffer is written between timed repetitions"}
@@ -172,6 +179,8 @@ def main():
     ap.add_argument("--ndom", type=int, default=0, help="override the number of domains (debug)")
     ap.add_argument("--gemm-mode", default="fp32grade", choices=sorted(MODE_NAMES))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--step", default="taylor", choices=sorted(STEP_NAMES),
+                    help="taylor: mlmd_propagate (north_star hot path, the default bench line); split: mlmd_propagate_split (NEXT-1)")
     ap.add_argument("--oracle-orbitals", type=int, default=32)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -197,7 +206,7 @@ def main():
     if args.ndom:
         c = W.get_config(args.config, ndom=args.ndom)
     K, Wm = args.steps, args.warmup
-    alg = algorithmic(c)
+    alg = algorithmic(c, step=args.step)
     peaks = load_peaks()
 
     # ---- inputs: seeded per (config, global domain index); generated in a thread pool, staged per domain
@@ -230,6 +239,7 @@ def main():
     dom.set_orbitals(psi_dev, occ)
     del beta_dev
     stream = dom.stream
+    propagate = dom.propagate_split if args.step == "split" else dom.propagate
     flush = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device=dev) if alg["elems"] * 8 < 4e8 else None
 
     def barrier():
@@ -239,7 +249,7 @@ def main():
 
     # ---- warm-up (W steps), then EXACTLY K timed steps in one mlmd_propagate call
     if Wm > 0:
-        dom.propagate(Wm, c.dt, A)
+        propagate(Wm, c.dt, A)
     dom.set_orbitals(psi_dev, occ)         # state reset: timed steps start from Psi(0)
     if flush is not None:
         flush.fill_(1.0)
@@ -251,7 +261,7 @@ def main():
     dom.profile(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    dom.propagate(K, c.dt, A)
+    propagate(K, c.dt, A)
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
@@ -280,7 +290,7 @@ def main():
         t0 = time.perf_counter()
         for k in range(K):
             dom.set_vloc(vnp)
-            dom.propagate(1, c.dt, A[k:k + 1])
+            propagate(1, c.dt, A[k:k + 1])
             dom.density(rnp)
         torch.cuda.synchronize()
         sec = time.perf_counter() - t0
@@ -290,7 +300,8 @@ def main():
         sec = float(tt.item())
         e2e = {"value": electrons * K / sec, "unit": "electron-steps/s", "h2d_bytes_per_step": int(vnp.nbytes + 24),
                "d2h_bytes_per_step": int(rnp.nbytes), "ms_per_step": sec / K * 1e3,
-               "what": "per step: mlmd_set_vloc(host pinned) + mlmd_propagate(1, A host) + mlmd_density(host pinned); "
+               "what": "per step: mlmd_set_vloc(host pinned) + %s(1, A host) + mlmd_density(host pinned); " % (
+                   "mlmd_propagate_split" if args.step == "split" else "mlmd_propagate") +
                        "Psi stays device-resident as in the paper's shadow dynamics (L130-132, L145)"}
 
     if rank != 0:
@@ -312,6 +323,8 @@ def main():
             entry.update(bound="hbm", achieved=b / (avg * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
         elif name == "density":
             entry.update(bound="hbm", achieved=alg["density_bytes"] / (avg * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
+        elif name == "norm":
+            entry.update(bound="hbm", achieved=alg["norm_bytes"] / (avg * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
         elif name in ("proj", "back", "nlp"):
             fl = alg["gemm_flops_each"] * (2 if name == "nlp" else 1)
             if gemm_path == "simt":
@@ -324,7 +337,7 @@ def main():
         per_class[name] = entry
     top = max((n for n in per_class if "achieved" in per_class[n]), key=lambda n: per_class[n]["ms_total"])
     roof = {k: per_class[top][k] for k in ("bound", "achieved", "peak", "unit", "frac")}
-    roof.update(kernel=top, traffic=ncu_traffic(c, top), peak_source="%s (%s)" % (
+    roof.update(kernel=top, traffic=ncu_traffic(c, top) if args.step == "taylor" or top != "density" else None, peak_source="%s (%s)" % (
         "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
         "hbm copy" if roof["bound"] == "hbm" else
         "sustained bf16 x nominal ratio for the mode" if roof["bound"] == "tensor" else "derived FP32/FP64 ALU peak, DESIGN.md"))
@@ -334,15 +347,16 @@ def main():
     step_roof = {"t_hbm_ms": t_hbm, "t_tensor_ms": t_tc, "t_roof_ms": t_roof, "bound": "tensor" if t_tc > t_hbm else "hbm",
                  "frac": t_roof / (ms / K), "tensor_peak_tflops": tensor_peak_sus, "tensor_peak_burst_tflops": tensor_peak_burst,
                  "hbm_peak_gbs": peaks["hbm_gbs"], "bytes_step": alg["bytes_step"], "gemm_flops_step": alg["gemm_flops_step"],
-                 "definition": "max(stencil+density bytes / HBM peak, real-beta GEMM flops / tensor peak of the GEMM mode)"}
+                 "definition": "max(stencil+density%s bytes / HBM peak, real-beta GEMM flops / tensor peak of the GEMM mode)" % (
+                     "+norm" if args.step == "split" else "")}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         s = sample_for_oracle(c, first, args.oracle_orbitals)
-        v, sec_step, cores, el = time_oracle(c, s, A, steps=2, warmup=1)
+        v, sec_step, cores, el = time_oracle(c, s, A, steps=2, warmup=1, step=args.step)
         cpu = {"value": v, "unit": "electron-steps/s", "cores": cores, "kind": "oracle", "s_per_step": sec_step,
-               "sample": "domain 0, first %d of %d orbitals (%g electrons), all %d projectors, 2 timed Taylor-4 steps" % (
-                   s["psi"].shape[-1], c.norb, el, c.nproj)}
+               "sample": "domain 0, first %d of %d orbitals (%g electrons), all %d projectors, 2 timed %s steps" % (
+                   s["psi"].shape[-1], c.norb, el, c.nproj, "Eq. (2) split" if args.step == "split" else "Taylor-4")}
 
     line = {
         "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,

@@ -125,6 +125,14 @@ int mlmd_density(mlmd_domain_t *h, float *rho, int where);
  * Always evaluated in the FP32-grade (or FP64) GEMM mode: it is a measurement. */
 int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
 
+/* Occupations of the t = 0 orbitals and number of excited electrons per domain (LFD hands the
+ * occupation numbers f_s back to QXMD; L159: n_exc "is computed from f_s"; L283: overlap matrix between the
+ * orbitals at time t and 0).  The paper gives no formula; reading D29:
+ *     f_s(t) = sum_n f_n |S_sn|^2,  S = dv Psi(0)^H Psi(t) (mlmd_overlap which = 1; needs MLMD_KEEP_PSI0),
+ *     n_exc  = sum_s max(f_s(0) - f_s(t), 0).
+ * f: double [ndom][norb], n_exc: double [ndom], both at `where`. */
+int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int where);
+
 /* Per-kernel-class timing of mlmd_propagate with CUDA events on the handle's stream (bench.py's
  * roofline numbers).  mlmd_profile(h, 1) starts recording (and clears earlier records),
  * mlmd_profile(h, 0) stops.  mlmd_profile_read synchronises the stream and returns the summed

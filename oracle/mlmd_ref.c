@@ -319,3 +319,27 @@ int mlmd_ref_propagate_split(int ndom, int nx, int ny, int nz, double hx, double
     free(acc);
     return rc;
 }
+
+/* Occupations of the reference orbitals and number of excited electrons (LFD returns the
+ * occupation numbers f_s to QXMD; L159: n_exc per domain "is computed from f_s"; L283: from the overlap
+ * matrix between the orbitals at time t and 0).  The paper gives no formula; reading D29:
+ *   f_s(t)  = sum_n f_n |S_sn|^2 ,  S_sn = <psi_s(0)|psi_n(t)>   (orbital n carries f_n electrons)
+ *   n_exc   = sum_s max(f_s(0) - f_s(t), 0)                      (electrons that left their t=0 orbitals)
+ * S: [ndom][norb][norb] as mlmd_ref_overlap(phi = Psi(0), psi = Psi(t)) writes it; occ: [ndom][norb]. */
+int mlmd_ref_occupations(int ndom, int norb, const zc *S, const double *occ, double *f, double *nexc) {
+    for (int dom = 0; dom < ndom; ++dom) {
+        double holes = 0.0;
+        for (int s = 0; s < norb; ++s) {
+            double acc = 0.0;
+            for (int n = 0; n < norb; ++n) {
+                const zc v = S[((size_t)dom * norb + s) * norb + n];
+                acc += occ[(size_t)dom * norb + n] * (creal(v) * creal(v) + cimag(v) * cimag(v));
+            }
+            f[(size_t)dom * norb + s] = acc;
+            const double lost = occ[(size_t)dom * norb + s] - acc;
+            if (lost > 0.0) holes += lost;
+        }
+        nexc[dom] = holes;
+    }
+    return 0;
+}

@@ -37,6 +37,8 @@ def lib() -> ctypes.CDLL:
         _lib.mlmd_ref_propagate.restype = i
         _lib.mlmd_ref_propagate_split.argtypes = [i, i, i, i, d, d, d, i, i, p, p, p, p, p, i, d, p, i, p, i]
         _lib.mlmd_ref_propagate_split.restype = i
+        _lib.mlmd_ref_occupations.argtypes = [i, i, p, p, p, p]
+        _lib.mlmd_ref_occupations.restype = i
     return _lib
 
 
@@ -136,3 +138,14 @@ def overlap(phi, psi, dv: float) -> np.ndarray:
     S = np.empty((ndom, norb, norb), dtype=np.complex128)
     lib().mlmd_ref_overlap(ndom, nx * ny * nz, norb, dv, _ptr(a), _ptr(b), _ptr(S))
     return S
+
+
+def occupations(S, occ) -> Tuple[np.ndarray, np.ndarray]:
+    """(f_s(t) [ndom, norb], n_exc [ndom]) from S = overlap(Psi(0), Psi(t)) and the occupations (reading D29)."""
+    S = _c128(S)
+    occ = _f64(occ)
+    ndom, norb, _ = S.shape
+    f = np.empty((ndom, norb), dtype=np.float64)
+    nexc = np.empty((ndom,), dtype=np.float64)
+    lib().mlmd_ref_occupations(ndom, norb, _ptr(S), _ptr(occ), _ptr(f), _ptr(nexc))
+    return f, nexc

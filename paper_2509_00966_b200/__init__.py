@@ -21,6 +21,7 @@ from .api import (  # noqa: F401
     mlmd_propagate_split,
     mlmd_density,
     mlmd_overlap,
+    mlmd_occupations,
     mlmd_launch_count,
     mlmd_profile,
     mlmd_profile_read,

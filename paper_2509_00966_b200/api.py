@@ -24,7 +24,7 @@ KEEP_PSI0, CHECK_FINITE = 1, 2
 EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",
     "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_propagate",
-    "mlmd_propagate_split",
+    "mlmd_propagate_split", "mlmd_occupations",
     "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
 ]
 K_STENCIL, K_PROJ, K_BACK, K_GLUE, K_DENSITY, K_NLP, K_NORM = range(7)
@@ -62,6 +62,7 @@ def lib() -> ctypes.CDLL:
         L.mlmd_propagate_split.argtypes = [p, i, d, p, i]
         L.mlmd_density.argtypes = [p, p, i]
         L.mlmd_overlap.argtypes = [p, i, p, i]
+        L.mlmd_occupations.argtypes = [p, p, p, i]
         L.mlmd_profile.argtypes = [p, i]
         L.mlmd_profile_read.argtypes = [p, i, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)]
         L.mlmd_launch_count.argtypes = [p]
@@ -191,6 +192,16 @@ def mlmd_overlap(h, which, out):
     return out
 
 
+def mlmd_occupations(h, f, n_exc):
+    """f: [ndom, norb] float64, n_exc: [ndom] float64 (numpy host arrays or CUDA tensors, both of one kind)."""
+    pf, wf = _ptr_where(f, np.dtype(np.float64))
+    pn, wn = _ptr_where(n_exc, np.dtype(np.float64))
+    if wf != wn:
+        raise ValueError("f and n_exc must both be host arrays or both be device tensors")
+    _check(lib().mlmd_occupations(h, pf, pn, wf))
+    return f, n_exc
+
+
 def mlmd_profile(h, enable: bool):
     _check(lib().mlmd_profile(h, 1 if enable else 0))
 
@@ -272,6 +283,12 @@ class Domain:
         if out is None:
             out = np.empty((self.ndom, self.norb, self.norb), dtype=np.complex64)
         return mlmd_overlap(self.handle, which, out)
+
+    def occupations(self):
+        """(f_s(t) [ndom, norb], n_exc [ndom]) as float64 host arrays (needs flags=KEEP_PSI0)."""
+        f = np.empty((self.ndom, self.norb), dtype=np.float64)
+        n_exc = np.empty((self.ndom,), dtype=np.float64)
+        return mlmd_occupations(self.handle, f, n_exc)
 
     def profile(self, enable=True):
         mlmd_profile(self.handle, enable)

@@ -342,6 +342,25 @@ int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
     return MLMD_OK;
 }
 
+int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int where) {
+    if (!h || !f || !n_exc) return fail(MLMD_ERR_ARG, "mlmd_occupations: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_occupations: bad where=%d", where);
+    // S = dv Psi(0)^H Psi(t) into the Z scratch (argument checks as mlmd_overlap(which = 1))
+    int rc = mlmd_overlap(h, 1, h->z(), MLMD_DEVICE);
+    if (rc) return rc;
+    int nl = 0;
+    double *fd = where == MLMD_DEVICE ? f : h->nrm(1);
+    double *nd = where == MLMD_DEVICE ? n_exc : h->nrm(2);
+    CU(launch_occupations(h->stream, h->ndom, h->norb, h->ld, (const float2 *)h->z(), h->occ(), fd, nd, &nl));
+    h->launches += nl;
+    if (where == MLMD_HOST) {
+        CU(cudaMemcpyAsync(f, fd, (size_t)h->ndom * h->norb * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(n_exc, nd, (size_t)h->ndom * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    return MLMD_OK;
+}
+
 // ---- the step --------------------------------------------------------------------------------
 // RAII pair of events around one kernel launch when mlmd_profile is on.
 struct ProfScope {

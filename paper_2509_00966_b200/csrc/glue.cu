@@ -357,4 +357,39 @@ cudaError_t launch_scale_density(cudaStream_t st, int ndom, long ngrid, int ld, 
     return cudaGetLastError();
 }
 
+// Occupations of the reference orbitals (reading D29): f[dom][s] = sum_n occ[dom][n] |S[dom][s][n]|^2 and
+// nexc[dom] = sum_s max(occ[dom][s] - f[dom][s], 0); S from the overlap epilogue.  One block per domain.
+__global__ void __launch_bounds__(256)
+occupations_kernel(int norb, int ld, const float2 *__restrict__ S, const float *__restrict__ occ, double *__restrict__ f,
+                   double *__restrict__ nexc) {
+    const int dom = blockIdx.x;
+    const float *oc = occ + (size_t)dom * ld;
+    double holes = 0.0;
+    for (int s = threadIdx.x; s < norb; s += blockDim.x) {
+        const float2 *row = S + ((size_t)dom * norb + s) * norb;
+        double acc = 0.0;
+        for (int n = 0; n < norb; ++n) {
+            const float2 v = row[n];
+            acc += (double)oc[n] * ((double)v.x * v.x + (double)v.y * v.y);
+        }
+        f[(size_t)dom * norb + s] = acc;
+        const double lost = (double)oc[s] - acc;
+        if (lost > 0.0) holes += lost;
+    }
+    __shared__ double red[256];
+    red[threadIdx.x] = holes;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) nexc[dom] = red[0];
+}
+cudaError_t launch_occupations(cudaStream_t st, int ndom, int norb, int ld, const float2 *S, const float *occ, double *f,
+                               double *nexc, int *nlaunch) {
+    ++*nlaunch;
+    occupations_kernel<<<ndom, 256, 0, st>>>(norb, ld, S, occ, f, nexc);
+    return cudaGetLastError();
+}
+
 }  // namespace mlmd

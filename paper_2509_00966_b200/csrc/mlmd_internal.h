@@ -177,6 +177,8 @@ cudaError_t launch_colnorm2(cudaStream_t st, int ndom, long ngrid, int ld, const
                             int *nlaunch);
 cudaError_t launch_kick_scale(cudaStream_t st, int n, double *n0, const double *na, const double *nc, const double *nd,
                               float *scl, int *nlaunch);
+cudaError_t launch_occupations(cudaStream_t st, int ndom, int norb, int ld, const float2 *S, const float *occ, double *f,
+                               double *nexc, int *nlaunch);
 cudaError_t launch_scale_density(cudaStream_t st, int ndom, long ngrid, int ld, float2 *psi, const float *scl,
                                  const float *occ, float *rho, int *nlaunch);
 

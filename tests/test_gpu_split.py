@@ -128,3 +128,33 @@ def test_split_low_precision_mode_and_errors():
     with pytest.raises(M.MlmdError):
         dom.propagate_split(1, 0.02, np.zeros((1, 2, 3)))      # a_ndom must be 1 or ndom
     dom.close()
+
+
+def test_occupations_and_excited_electrons_after_the_pulse():
+    """mlmd_occupations (reading D29) against the oracle's overlap + occupations on the oracle's own state:
+    config 1 with band-limited orbitals through 20 steps (about 12% of the electrons leave their orbitals), both steppers.
+    Tolerances follow from the Gram tolerance 1e-5 on S: |df_s| <= 2 f_max |S| dS ~ 4e-5 -> 1e-4; n_exc sums
+    the one-sided part of df over the orbitals (the truncating tensor-core accumulation of reading R2 biases
+    diag S low by ~3e-6, i.e. f by ~7e-6 each), so it is held to 1e-5 of the electron count."""
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    c = W.get_config(1, smooth_kcut=2.5)
+    d = W.generate(c)
+    A = d["A"][:20]
+    for split in (False, True):
+        dom = make_domain(c, d, flags=M.KEEP_PSI0)
+        f0, n0 = dom.occupations()
+        ne = float(d["occ"].sum())
+        assert np.abs(f0 - d["occ"]).max() <= 2e-5 and n0.max() <= 1e-5 * ne            # S = 1 at t = 0
+        (dom.propagate_split if split else dom.propagate)(20, c.dt, A)
+        f, nexc = dom.occupations()
+        r, _ = (ref.propagate_split if split else ref.propagate)(d["psi"], d["occ"], d["vloc"], d["beta"], d["D"], A, c.dt, c.h)
+        f_ref, n_ref = ref.occupations(ref.overlap(d["psi"], r, c.dv), d["occ"])
+        print("split" if split else "taylor", "n_exc", nexc, n_ref, "max |df|", np.abs(f - f_ref).max())
+        assert 0.02 * ne < n_ref[0] < 0.5 * ne                                    # a partial excitation
+        assert np.abs(f - f_ref).max() <= 1e-4 and np.abs(nexc - n_ref).max() <= 1e-5 * ne
+        dom.close()
+    dom = make_domain(c, d)
+    with pytest.raises(M.MlmdError):
+        dom.occupations()                                                         # no Psi(0) snapshot
+    dom.close()

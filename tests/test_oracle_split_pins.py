@@ -137,3 +137,47 @@ def test_s5_leading_error_term_of_the_first_order_kick():
         mism.append(rel(out[0].reshape(ngrid, 2) - exact, pred))
     assert mism[1] < 0.04, mism
     assert 1.7 < mism[0] / mism[1] < 2.3, mism
+
+
+def test_o1_two_level_rotation_closed_form():
+    """O1 (reading D29): Psi(t) = Psi(0) U with a rotation by theta between a filled (f=2) and an empty orbital
+    and a pure phase on a third, half-filled one: f(t) = (2 cos^2, 2 sin^2, 1), n_exc = 2 sin^2 theta."""
+    th = 0.37
+    U = np.array([[np.cos(th), -np.sin(th), 0], [np.sin(th), np.cos(th), 0], [0, 0, np.exp(0.9j)]], dtype=np.complex128)
+    f, nexc = ref.occupations(U[None], np.array([[2.0, 0.0, 1.0]]))
+    assert np.allclose(f[0], [2 * np.cos(th) ** 2, 2 * np.sin(th) ** 2, 1.0], atol=1e-15)
+    assert abs(nexc[0] - 2 * np.sin(th) ** 2) < 1e-15
+
+
+def test_o2_sum_rule_phases_and_t0():
+    """O2: for unitary S the electrons are conserved (sum_s f_s(t) = sum_n f_n) and n_exc = (sum_s |f_s(t) - f_s(0)|)/2;
+    column phases of S do not matter; S = 1 gives f(t) = f(0), n_exc = 0; the s and n indices are not interchangeable
+    (a non-normal S distinguishes them)."""
+    n = 6
+    q, _ = np.linalg.qr(RNG.standard_normal((n, n)) + 1j * RNG.standard_normal((n, n)))
+    occ = np.array([[2.0, 2.0, 1.5, 0.5, 0.0, 0.0]])
+    f, nexc = ref.occupations(q[None], occ)
+    assert abs(f.sum() - occ.sum()) < 1e-13
+    assert abs(nexc[0] - 0.5 * np.abs(f - occ).sum()) < 1e-13
+    f2, nexc2 = ref.occupations((q * np.exp(1j * RNG.uniform(0, 6, n))[None, :])[None], occ)
+    assert np.allclose(f, f2, atol=1e-14) and abs(nexc[0] - nexc2[0]) < 1e-14
+    f0, n0 = ref.occupations(np.eye(n, dtype=np.complex128)[None], occ)
+    assert np.array_equal(f0, occ) and n0[0] == 0.0
+    S = np.zeros((1, 2, 2), dtype=np.complex128)
+    S[0, 0, 1] = 1.0                                   # <psi_0(0)|psi_1(t)> = 1: orbital 1's electrons sit on reference 0
+    f3, n3 = ref.occupations(S, np.array([[0.0, 2.0]]))
+    assert np.array_equal(f3, [[2.0, 0.0]]) and n3[0] == 2.0
+
+
+def test_o3_occupations_from_the_oracles_own_overlap():
+    """O3: end to end through mlmd_ref_overlap: orbitals mixed by a known unitary give the O1 numbers on a grid."""
+    grid, h = (5, 6, 5), (0.5, 0.4, 0.45)
+    ngrid, dv = int(np.prod(grid)), float(np.prod(h))
+    B = orthonormal_projectors(ngrid, 2, dv)
+    th = 1.1
+    U = np.array([[np.cos(th), -np.sin(th)], [np.sin(th), np.cos(th)]])
+    psi0 = B.reshape(1, *grid, 2)
+    psit = (B @ U).reshape(1, *grid, 2)
+    f, nexc = ref.occupations(ref.overlap(psi0, psit, dv), np.array([[2.0, 0.0]]))
+    assert np.allclose(f[0], [2 * np.cos(th) ** 2, 2 * np.sin(th) ** 2], atol=1e-13)
+    assert abs(nexc[0] - 2 * np.sin(th) ** 2) < 1e-13
