@@ -511,23 +511,33 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         if (!rc) rc = nonlocal_back(h, h->psi(), nl);
         return rc ? rc : norm2(which);
     };
+    auto kick_only = [&]() -> int {              // psi += (-i dt/2) V_NL psi
+        int rc = nonlocal_project(h, h->psi(), (float)(0.5 * dt), nl);
+        return rc ? rc : nonlocal_back(h, h->psi(), nl);
+    };
     if (kicks) {
-        int rc = half_kick(1);
+        int rc = kick_only();
         if (rc) return rc;
     }
+    // Taylor-4 of h_loc (Horner form).  With kicks, the first stage also sums |psi_a|^2 (its input) and the last
+    // |psi_c|^2 (its output) per orbital: the norms ride on passes that read or write those arrays anyway.
     const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
     float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
     for (int i = 0; i < 4; ++i) {
         ProfScope ps(h, MLMD_K_STENCIL);
-        CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, coef_host, (float)(dt / (4 - i)), nl));
+        const float tau = (float)(dt / (4 - i));
+        if (kicks && (i == 0 || i == 3))
+            CU(launch_stencil_stage_norm(h, src[i], h->psi(), dst[i], coef, coef_host, tau, i == 0 ? 1 : 2, h->nrm_part(),
+                                         h->nrm(i == 0 ? 1 : 2), nl));
+        else
+            CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, coef_host, tau, nl));
     }
     if (!kicks) {
         ProfScope ps(h, MLMD_K_DENSITY);
         CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), nl));
         return MLMD_OK;
     }
-    int rc = norm2(2);
-    if (!rc) rc = half_kick(3);
+    int rc = half_kick(3);
     if (rc) return rc;
     {
         ProfScope ps(h, MLMD_K_GLUE);

@@ -268,20 +268,25 @@ colnorm_part_kernel(long ngrid, int ld, const float2 *__restrict__ psi, double *
     if (threadIdx.y == 0 && c < ld)
         part[((size_t)dom * kNormSlabs + slab) * ld + c] = (sm[0][threadIdx.x] + sm[1][threadIdx.x]) + (sm[2][threadIdx.x] + sm[3][threadIdx.x]);
 }
-__global__ void colnorm_final_kernel(int n, int ld, const double *__restrict__ part, double *__restrict__ out) {
+__global__ void colnorm_final_kernel(int n, int ld, int nslabs, const double *__restrict__ part, double *__restrict__ out) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;     // i = dom * ld + c
     if (i >= n) return;
     const int dom = i / ld, c = i % ld;
     double s = 0.0;
-    for (int k = 0; k < kNormSlabs; ++k) s += part[((size_t)dom * kNormSlabs + k) * ld + c];
+    for (int k = 0; k < nslabs; ++k) s += part[((size_t)dom * nslabs + k) * ld + c];
     out[i] = s;
+}
+cudaError_t launch_colnorm_final(cudaStream_t st, int ndom, int ld, int nslabs, const double *part, double *out, int *nlaunch) {
+    ++*nlaunch;
+    colnorm_final_kernel<<<(ndom * ld + 127) / 128, 128, 0, st>>>(ndom * ld, ld, nslabs, part, out);
+    return cudaGetLastError();
 }
 cudaError_t launch_colnorm2(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, double *part, double *out,
                             int *nlaunch) {
-    *nlaunch += 2;
+    ++*nlaunch;
     colnorm_part_kernel<<<dim3(kNormSlabs, ndom, (ld + 63) / 64), dim3(64, 4), 0, st>>>(ngrid, ld, psi, part);
-    colnorm_final_kernel<<<(ndom * ld + 127) / 128, 128, 0, st>>>(ndom * ld, ld, part, out);
-    return cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
+    return e != cudaSuccess ? e : launch_colnorm_final(st, ndom, ld, kNormSlabs, part, out, nlaunch);
 }
 
 // One step's pending scale from the four squared norms (un-normalised chain, D27):

@@ -118,6 +118,11 @@ struct DeviceOnce {
 // w, psi, out: [ndom][ngrid][ld] complex64; coef: [ndom] for this step; out may alias psi.
 cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
                                  const StepCoef *coef, const StepCoef *coef_host, float tau, int *nlaunch);
+// The same stage that also delivers squared per-orbital norms (split step): norm_mode 1 = of w, 2 = of out,
+// into nrm_out[dom][ld]; fused into the TMA pass when that runs, otherwise a separate reduction pass.
+cudaError_t launch_stencil_stage_norm(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
+                                      const StepCoef *coef, const StepCoef *coef_host, float tau, int norm_mode,
+                                      double *npart, double *nrm_out, int *nlaunch);
 
 // ---- stencil_tma.cu ---------------------------------------------------------------------------
 // The same stage with TMA-staged x-planes (needs ny % 16 == 0, nz % 16 == 0).
@@ -125,7 +130,10 @@ bool stencil_tma_supported(const mlmd_domain *h);
 // coef_host: the one coefficient set of this step when every domain sees the same field (passed by
 // value through the constant bank), NULL when coef[dom] differs per domain.
 cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
-                               const StepCoef *coef_host, float tau, int *nlaunch);
+                               const StepCoef *coef_host, float tau, int *nlaunch, int norm_mode = 0, double *npart = nullptr);
+// norm_mode 1 / 2: the pass also writes per-CTA partial sums of |w|^2 / |out|^2 per orbital into
+// npart[dom][slot][ld], slot < stencil_tma_norm_slots(h) (split step, reading D27)
+int stencil_tma_norm_slots(const mlmd_domain *h);
 
 // ---- gemm_simt.cu ----------------------------------------------------------------------------
 // Projection (S2a): zpart[dom][s][p][c] = sum_{r in slice s} B[dom][r][p] * Y[dom][r][c]
@@ -175,6 +183,8 @@ cudaError_t launch_advance_coef(cudaStream_t st, const StepCoef *all, StepCoef *
 // scl = sqrt(n0/na * nc/nd), n0 <- n0 nc/na;  psi *= scl fused with the density pass
 cudaError_t launch_colnorm2(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, double *part, double *out,
                             int *nlaunch);
+// out[dom][c] = sum_{k < nslabs} part[dom][k][c] in index order
+cudaError_t launch_colnorm_final(cudaStream_t st, int ndom, int ld, int nslabs, const double *part, double *out, int *nlaunch);
 cudaError_t launch_kick_scale(cudaStream_t st, int n, double *n0, const double *na, const double *nc, const double *nd,
                               float *scl, int *nlaunch);
 cudaError_t launch_occupations(cudaStream_t st, int ndom, int norb, int ld, const float2 *S, const float *occ, double *f,

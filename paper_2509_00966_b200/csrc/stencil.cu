@@ -214,4 +214,20 @@ cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const fl
     return launch_march<4, 8, 8>(P, h->ndom, ayz, h->stream);
 }
 
+cudaError_t launch_stencil_stage_norm(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
+                                      const StepCoef *coef, const StepCoef *coef_host, float tau, int norm_mode,
+                                      double *npart, double *nrm_out, int *nlaunch) {
+    if (env_int("MLMD_STENCIL", 2) == 2 && env_int("MLMD_NORM_FUSED", 1) && stencil_tma_supported(h)) {
+        const int slots = stencil_tma_norm_slots(h);
+        if (slots <= kNormSlabs) {     // npart holds kNormSlabs partial rows per domain
+            cudaError_t e = launch_stencil_tma(h, w, psi, out, coef, coef_host, tau, nlaunch, norm_mode, npart);
+            return e != cudaSuccess ? e : launch_colnorm_final(h->stream, h->ndom, h->ld, slots, npart, nrm_out, nlaunch);
+        }
+    }
+    // w may alias out only through psi (Horner buffers), never directly, so w is intact after the stage
+    cudaError_t e = launch_stencil_stage(h, w, psi, out, coef, coef_host, tau, nlaunch);
+    if (e != cudaSuccess) return e;
+    return launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, norm_mode == 1 ? w : out, npart, nrm_out, nlaunch);
+}
+
 }  // namespace mlmd

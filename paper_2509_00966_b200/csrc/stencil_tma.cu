@@ -38,6 +38,8 @@ struct TmaStencilParams {
     int nx, ny, nz, lanes;   // lanes = float4 per grid point
     int xs, nxseg;           // planes per CTA, segments per domain
     int nchunk;              // 64-byte chunks per grid point
+    double *npart;           // NORM variants: [dom][slot][ld] partial squared norms, slot = (yt, zt, seg)
+    int ld;
 };
 
 __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, uint64_t *bar, int c0, int c1, int c2, int c3) {
@@ -79,7 +81,9 @@ __device__ __forceinline__ void pair_acc_real(float4 &acc, const float4 a, const
     acc.w = fmaf(p, a.w + b.w, acc.w);
 }
 
-template <bool AYZ, bool PERDOM>
+// NORM (split step, reading D27): 1 = also sum |w|^2 of the CTA's own points per orbital, 2 = |out|^2;
+// one partial sum per (CTA, orbital), reduced in a fixed order, so the norms are reproducible.
+template <bool AYZ, bool PERDOM, int NORM>
 __global__ void __launch_bounds__(S_THREADS, 1)
 stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_z,
                    const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_p,
@@ -179,10 +183,15 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // critical path of the first FMA
     float vAn = __ldg(vp), vBn = __ldg(vp + 8);
 
+    float nrm0 = 0.f, nrm1 = 0.f;   // NORM: this thread's two orbitals, summed over its points
     auto point = [&](const uint32_t buf, const uint32_t o, const uint32_t ozm1, const uint32_t ozm2, const uint32_t ozp1,
-                     const uint32_t ozp2, const uint32_t dy, const float cen, float4 &A0, float4 &A1, float4 &A2,
-                     float4 &A3, float4 &A4) {
+                     const uint32_t ozp2, const uint32_t dy, const float cen, const bool own_plane, float4 &A0, float4 &A1,
+                     float4 &A2, float4 &A3, float4 &A4) {
         const float4 u = lds4(buf + o);
+        if (NORM == 1 && own_plane) {
+            nrm0 = fmaf(u.x, u.x, fmaf(u.y, u.y, nrm0));
+            nrm1 = fmaf(u.z, u.z, fmaf(u.w, u.w, nrm1));
+        }
         A2.x = fmaf(cen, u.x, A2.x);
         A2.y = fmaf(cen, u.y, A2.y);
         A2.z = fmaf(cen, u.z, A2.z);
@@ -226,16 +235,25 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         vBn = __ldg(vp + 8);
         mbar_wait(&full[k], it & 1);
         const uint32_t buf = sbase + k * S_PLANE;
-        point(buf, own, oAzm1, oAzm2, own + 64, own + 128, 0u, c.centre + vA, A0, A1, A2, A3, A4);
-        point(buf, own + 512, own + 512 - 64, own + 512 - 128, oBzp1, oBzp2, 512u, c.centre + vB, B0, B1, B2, B3, B4);
+        const bool own_plane = n >= 2 && n < nplanes - 2;
+        point(buf, own, oAzm1, oAzm2, own + 64, own + 128, 0u, c.centre + vA, own_plane, A0, A1, A2, A3, A4);
+        point(buf, own + 512, own + 512 - 64, own + 512 - 128, oBzp1, oBzp2, 512u, c.centre + vB, own_plane, B0, B1, B2, B3, B4);
         // plane q-2 (output n - 4) is complete: out = psi + (-i tau) acc
         if (n >= 4) {
             const float4 psA = lds4(buf + S_PLANE_W + own), psB = lds4(buf + S_PLANE_W + own + 512);
-            out_p[0] = make_float4(fmaf(P.tau, A0.y, psA.x), fmaf(-P.tau, A0.x, psA.y), fmaf(P.tau, A0.w, psA.z),
-                                   fmaf(-P.tau, A0.z, psA.w));
-            out_p[dB] = make_float4(fmaf(P.tau, B0.y, psB.x), fmaf(-P.tau, B0.x, psB.y), fmaf(P.tau, B0.w, psB.z),
-                                    fmaf(-P.tau, B0.z, psB.w));
+            const float4 oA = make_float4(fmaf(P.tau, A0.y, psA.x), fmaf(-P.tau, A0.x, psA.y), fmaf(P.tau, A0.w, psA.z),
+                                          fmaf(-P.tau, A0.z, psA.w));
+            const float4 oB = make_float4(fmaf(P.tau, B0.y, psB.x), fmaf(-P.tau, B0.x, psB.y), fmaf(P.tau, B0.w, psB.z),
+                                          fmaf(-P.tau, B0.z, psB.w));
+            out_p[0] = oA;
+            out_p[dB] = oB;
             out_p += sx;
+            if (NORM == 2) {
+                nrm0 = fmaf(oA.x, oA.x, fmaf(oA.y, oA.y, nrm0));
+                nrm1 = fmaf(oA.z, oA.z, fmaf(oA.w, oA.w, nrm1));
+                nrm0 = fmaf(oB.x, oB.x, fmaf(oB.y, oB.y, nrm0));
+                nrm1 = fmaf(oB.z, oB.z, fmaf(oB.w, oB.w, nrm1));
+            }
         }
         __syncwarp();
         if (tid % 32 == 0) mbar_arrive(&empty[k]);
@@ -248,6 +266,27 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         if (n + 2 < nplanes) step(n + 2, 2, it, a2, a3, a4, a0, a1, b2, b3, b4, b0, b1);
         if (n + 3 < nplanes) step(n + 3, 3, it, a3, a4, a0, a1, a2, b3, b4, b0, b1, b2);
         if (n + 4 < nplanes) step(n + 4, 4, it, a4, a0, a1, a2, a3, b4, b0, b1, b2, b3);
+    }
+    if (NORM != 0) {
+        // threads with the same l hold the same two orbitals: lanes l, l+4, .. of a warp, then the 16 warps
+        __shared__ float red[S_THREADS / 32][SL][2];
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            nrm0 += __shfl_xor_sync(0xffffffffu, nrm0, o);
+            nrm1 += __shfl_xor_sync(0xffffffffu, nrm1, o);
+        }
+        if (tid % 32 < SL) {
+            red[tid / 32][l][0] = nrm0;
+            red[tid / 32][l][1] = nrm1;
+        }
+        __syncthreads();
+        if (tid < 2 * SL) {
+            double sum = 0.0;
+            for (int wq = 0; wq < S_THREADS / 32; ++wq) sum += (double)red[wq][tid / 2][tid % 2];
+            const int nslots = nyt * nzt * P.nxseg;
+            const int slot = (yt * nzt + zt) * P.nxseg + seg;
+            P.npart[((size_t)dom * nslots + slot) * P.ld + chunk * 2 * SL + tid] = sum;
+        }
     }
 }
 
@@ -284,14 +323,51 @@ bool stencil_tma_supported(const mlmd_domain *h) {
     return encode_fn2() != nullptr && h->ny % SY == 0 && h->nz % SZ == 0 && h->nx >= 5 && h->ld % 8 == 0;
 }
 
+namespace {
+template <int NORM>
+cudaError_t set_attrs() {
+    cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    return e;
+}
+template <int NORM>
+void launch_variant(bool yz, bool perdom, unsigned g, cudaStream_t st, const CUtensorMap &mc, const CUtensorMap &mz,
+                    const CUtensorMap &my, const CUtensorMap &mp, const TmaStencilParams &P) {
+    if (!perdom) {
+        if (yz) stencil_tma_kernel<true, false, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, false, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+    } else {
+        if (yz) stencil_tma_kernel<true, true, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, true, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+    }
+}
+}  // namespace
+
+// x-march segments per (domain, chunk, patch): enough CTAs to fill the GPU twice on small batches
+static void x_segments(const mlmd_domain *h, int *xs, int *nxseg) {
+    const long base = (long)h->ndom * (h->ld / 8) * (h->ny / SY) * (h->nz / SZ);
+    int n = 1;
+    while (base * n < 2 * 148 && h->nx / (n * 2) >= 8) n *= 2;
+    const char *env = getenv("MLMD_XSEG");
+    if (env && atoi(env) > 0) n = (h->nx + atoi(env) - 1) / atoi(env);
+    *xs = (h->nx + n - 1) / n;
+    *nxseg = (h->nx + *xs - 1) / *xs;
+}
+int stencil_tma_norm_slots(const mlmd_domain *h) {
+    int xs, nxseg;
+    x_segments(h, &xs, &nxseg);
+    return (h->ny / SY) * (h->nz / SZ) * nxseg;
+}
+
 cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
-                               const StepCoef *coef_host, float tau, int *nlaunch) {
+                               const StepCoef *coef_host, float tau, int *nlaunch, int norm_mode, double *npart) {
     static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
     if (!attr_set.done()) {
-        cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+        cudaError_t e = set_attrs<0>();
+        if (e == cudaSuccess) e = set_attrs<1>();
+        if (e == cudaSuccess) e = set_attrs<2>();
         if (e != cudaSuccess) return e;
         attr_set.mark();
     }
@@ -312,25 +388,17 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
     P.nz = h->nz;
     P.lanes = h->ld / 2;
     P.nchunk = h->ld / 8;
+    P.npart = npart;
+    P.ld = h->ld;
     const long base = (long)h->ndom * P.nchunk * (h->ny / SY) * (h->nz / SZ);
-    int nxseg = 1;
-    while (base * nxseg < 2 * 148 && h->nx / (nxseg * 2) >= 8) nxseg *= 2;
-    const char *env = getenv("MLMD_XSEG");
-    if (env && atoi(env) > 0) nxseg = (h->nx + atoi(env) - 1) / atoi(env);
-    P.xs = (h->nx + nxseg - 1) / nxseg;
-    P.nxseg = (h->nx + P.xs - 1) / P.xs;
+    x_segments(h, &P.xs, &P.nxseg);
     const long grid = base * P.nxseg;
     ++*nlaunch;
     const unsigned g = (unsigned)grid;
-    if (coef_host) {
-        P.cval = *coef_host;
-        if (h->field_yz) stencil_tma_kernel<true, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
-        else stencil_tma_kernel<false, false><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
-    } else {
-        P.cval = StepCoef();
-        if (h->field_yz) stencil_tma_kernel<true, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
-        else stencil_tma_kernel<false, true><<<g, S_THREADS, S_SMEM, h->stream>>>(mc, mz, my, mp, P);
-    }
+    P.cval = coef_host ? *coef_host : StepCoef();
+    if (norm_mode == 1) launch_variant<1>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    else if (norm_mode == 2) launch_variant<2>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    else launch_variant<0>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
     return cudaGetLastError();
 }
 
