@@ -343,3 +343,63 @@ int mlmd_ref_occupations(int ndom, int norb, const zc *S, const double *occ, dou
     }
     return 0;
 }
+
+/* ---- observables of SURVEY.md 8(f) NEXT-2 ("GEMMification is applied to nonlocal correction in
+ * energy and electric current ... with the latter used in Maxwell's equations") ----
+ *
+ * Nonlocal energy of one domain:  E_nl = sum_n f_n <psi_n|V_NL|psi_n>,  V_NL = dv B diag(D) B^H, <a|b> = dv sum conj(a) b
+ *                                      = dv^2 sum_n f_n sum_p D_p |sum_r conj(beta[r][p]) psi[r][n]|^2 .            */
+int mlmd_ref_energy_nl(int ndom, long ngrid, int norb, int nproj, double dv, const zc *psi, const double *occ,
+                       const zc *beta, const double *D, double *E) {
+    for (int dom = 0; dom < ndom; ++dom) {
+        const zc *p = psi + (size_t)dom * ngrid * norb;
+        const zc *b = beta + (size_t)dom * ngrid * nproj;
+        double e = 0.0;
+        for (int n = 0; n < norb; ++n)
+            for (int q = 0; q < nproj; ++q) {
+                zc c = 0.0;
+                for (long r = 0; r < ngrid; ++r) c += conj(b[r * nproj + q]) * p[r * norb + n];
+                e += occ[(size_t)dom * norb + n] * D[(size_t)dom * nproj + q] * dv * dv * (creal(c) * creal(c) + cimag(c) * cimag(c));
+            }
+        E[dom] = e;
+    }
+    return 0;
+}
+
+/* Local current of one domain (the velocity operator of h_loc in Eq. (3) L142 is -i grad + A; reading D30: the
+ * nonlocal-pseudopotential term -i[r, V_NL] of the TDCDFT current is named at L201 but not given and is left out):
+ *   J_d = sum_n f_n Re <psi_n| -i D1_d + A_d |psi_n>,   D1_d = the 4th-order central first difference of H.
+ * A: [a_ndom][3]; J: [ndom][3]. */
+int mlmd_ref_current(int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int norb, const zc *psi,
+                     const double *occ, const double *A, int a_ndom, double *J) {
+    const int n3[3] = {nx, ny, nz};
+    const double h[3] = {hx, hy, hz};
+    const long ngrid = (long)nx * ny * nz;
+    const double dv = hx * hy * hz;
+    for (int dom = 0; dom < ndom; ++dom) {
+        const zc *p = psi + (size_t)dom * ngrid * norb;
+        const double *Av = A + (size_t)(a_ndom == 1 ? 0 : dom) * 3;
+        for (int d = 0; d < 3; ++d) {
+            double acc = 0.0;
+            for (int ix = 0; ix < nx; ++ix)
+                for (int iy = 0; iy < ny; ++iy)
+                    for (int iz = 0; iz < nz; ++iz) {
+                        const int i3[3] = {ix, iy, iz};
+                        const long r = ((long)ix * ny + iy) * nz + iz;
+                        for (int n = 0; n < norb; ++n) {
+                            zc g = 0.0;
+                            for (int j = -2; j <= 2; ++j) {
+                                int q3[3] = {i3[0], i3[1], i3[2]};
+                                q3[d] = wrap(i3[d] + j, n3[d]);
+                                const long rr = ((long)q3[0] * ny + q3[1]) * nz + q3[2];
+                                g += C1[j + 2] / h[d] * p[rr * norb + n];
+                            }
+                            const zc u = p[r * norb + n];
+                            acc += occ[(size_t)dom * norb + n] * dv * creal(conj(u) * (-I * g + Av[d] * u));
+                        }
+                    }
+            J[(size_t)dom * 3 + d] = acc;
+        }
+    }
+    return 0;
+}

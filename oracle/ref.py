@@ -39,6 +39,10 @@ def lib() -> ctypes.CDLL:
         _lib.mlmd_ref_propagate_split.restype = i
         _lib.mlmd_ref_occupations.argtypes = [i, i, p, p, p, p]
         _lib.mlmd_ref_occupations.restype = i
+        _lib.mlmd_ref_energy_nl.argtypes = [i, l, i, i, d, p, p, p, p, p]
+        _lib.mlmd_ref_energy_nl.restype = i
+        _lib.mlmd_ref_current.argtypes = [i, i, i, i, d, d, d, i, p, p, p, i, p]
+        _lib.mlmd_ref_current.restype = i
     return _lib
 
 
@@ -149,3 +153,25 @@ def occupations(S, occ) -> Tuple[np.ndarray, np.ndarray]:
     nexc = np.empty((ndom,), dtype=np.float64)
     lib().mlmd_ref_occupations(ndom, norb, _ptr(S), _ptr(occ), _ptr(f), _ptr(nexc))
     return f, nexc
+
+
+def energy_nl(psi, occ, beta, D, dv: float) -> np.ndarray:
+    """E_nl[dom] = sum_n f_n <psi_n|V_NL|psi_n>."""
+    p = _c128(psi)
+    ndom, nx, ny, nz, norb = p.shape
+    nproj = beta.shape[-1]
+    b = _c128(beta.reshape(ndom, -1, nproj))
+    E = np.empty((ndom,), dtype=np.float64)
+    lib().mlmd_ref_energy_nl(ndom, nx * ny * nz, norb, nproj, dv, _ptr(p), _ptr(_f64(occ)), _ptr(b), _ptr(_f64(D)), _ptr(E))
+    return E
+
+
+def current(psi, occ, A, h: Sequence[float]) -> np.ndarray:
+    """J[dom][d] = sum_n f_n Re<psi_n| -i D1_d + A_d |psi_n>; A: [a_ndom, 3]."""
+    p = _c128(psi)
+    ndom, nx, ny, nz, norb = p.shape
+    A = _f64(A).reshape(-1, 3)
+    assert A.shape[0] in (1, ndom)
+    J = np.empty((ndom, 3), dtype=np.float64)
+    lib().mlmd_ref_current(ndom, nx, ny, nz, h[0], h[1], h[2], norb, _ptr(p), _ptr(_f64(occ)), _ptr(A), A.shape[0], _ptr(J))
+    return J
