@@ -133,6 +133,17 @@ int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
  * f: double [ndom][norb], n_exc: double [ndom], both at `where`. */
 int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int where);
 
+/* Observables of the current state that feed the light-matter loop ("GEMMification is applied to
+ * nonlocal correction in energy and electric current ... used in Maxwell's equations"; SURVEY.md 8(f) NEXT-2;
+ * the paper gives no formulas: reading D30).
+ * mlmd_energy_nl: E[dom] = sum_n f_n <psi_n|V_NL|psi_n> = dv^2 sum_n f_n sum_p D_p |sum_r conj(beta_rp) psi_rn|^2
+ *   in Hartree (the projection GEMM of the step + a reduction); double [ndom] at `where`; 0 when nproj = 0.
+ * mlmd_current: J[dom][d] = sum_n f_n Re<psi_n| -i D1_d + A_d |psi_n>, D1 the 4th-order first difference of H,
+ *   A: double [a_ndom][3] HOST (a_ndom = 1 or ndom), J: double [ndom][3] at `where`.  This is the current of
+ *   h_loc's velocity operator; the nonlocal-pseudopotential term -i[r, V_NL] is not included (D30). */
+int mlmd_energy_nl(mlmd_domain_t *h, double *E, int where);
+int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int where);
+
 /* Per-kernel-class timing of mlmd_propagate with CUDA events on the handle's stream (bench.py's
  * roofline numbers).  mlmd_profile(h, 1) starts recording (and clears earlier records),
  * mlmd_profile(h, 0) stops.  mlmd_profile_read synchronises the stream and returns the summed

@@ -354,13 +354,18 @@ int mlmd_ref_energy_nl(int ndom, long ngrid, int norb, int nproj, double dv, con
     for (int dom = 0; dom < ndom; ++dom) {
         const zc *p = psi + (size_t)dom * ngrid * norb;
         const zc *b = beta + (size_t)dom * ngrid * nproj;
-        double e = 0.0;
+        double *en = (double *)calloc((size_t)norb, sizeof(double));   /* one orbital per thread, summed in order below */
+        if (!en) return 5;
+#pragma omp parallel for schedule(dynamic)
         for (int n = 0; n < norb; ++n)
             for (int q = 0; q < nproj; ++q) {
                 zc c = 0.0;
                 for (long r = 0; r < ngrid; ++r) c += conj(b[r * nproj + q]) * p[r * norb + n];
-                e += occ[(size_t)dom * norb + n] * D[(size_t)dom * nproj + q] * dv * dv * (creal(c) * creal(c) + cimag(c) * cimag(c));
+                en[n] += occ[(size_t)dom * norb + n] * D[(size_t)dom * nproj + q] * dv * dv * (creal(c) * creal(c) + cimag(c) * cimag(c));
             }
+        double e = 0.0;
+        for (int n = 0; n < norb; ++n) e += en[n];
+        free(en);
         E[dom] = e;
     }
     return 0;
@@ -380,8 +385,11 @@ int mlmd_ref_current(int ndom, int nx, int ny, int nz, double hx, double hy, dou
         const zc *p = psi + (size_t)dom * ngrid * norb;
         const double *Av = A + (size_t)(a_ndom == 1 ? 0 : dom) * 3;
         for (int d = 0; d < 3; ++d) {
-            double acc = 0.0;
-            for (int ix = 0; ix < nx; ++ix)
+            double *plane = (double *)calloc((size_t)nx, sizeof(double));   /* one x-plane per thread, summed in order below */
+            if (!plane) return 5;
+#pragma omp parallel for schedule(static)
+            for (int ix = 0; ix < nx; ++ix) {
+                double acc = 0.0;
                 for (int iy = 0; iy < ny; ++iy)
                     for (int iz = 0; iz < nz; ++iz) {
                         const int i3[3] = {ix, iy, iz};
@@ -398,6 +406,11 @@ int mlmd_ref_current(int ndom, int nx, int ny, int nz, double hx, double hy, dou
                             acc += occ[(size_t)dom * norb + n] * dv * creal(conj(u) * (-I * g + Av[d] * u));
                         }
                     }
+                plane[ix] = acc;
+            }
+            double acc = 0.0;
+            for (int ix = 0; ix < nx; ++ix) acc += plane[ix];
+            free(plane);
             J[(size_t)dom * 3 + d] = acc;
         }
     }

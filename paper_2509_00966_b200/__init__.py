@@ -22,6 +22,8 @@ from .api import (  # noqa: F401
     mlmd_density,
     mlmd_overlap,
     mlmd_occupations,
+    mlmd_energy_nl,
+    mlmd_current,
     mlmd_launch_count,
     mlmd_profile,
     mlmd_profile_read,

@@ -24,7 +24,7 @@ KEEP_PSI0, CHECK_FINITE = 1, 2
 EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",
     "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_propagate",
-    "mlmd_propagate_split", "mlmd_occupations",
+    "mlmd_propagate_split", "mlmd_occupations", "mlmd_energy_nl", "mlmd_current",
     "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
 ]
 K_STENCIL, K_PROJ, K_BACK, K_GLUE, K_DENSITY, K_NLP, K_NORM = range(7)
@@ -63,6 +63,8 @@ def lib() -> ctypes.CDLL:
         L.mlmd_density.argtypes = [p, p, i]
         L.mlmd_overlap.argtypes = [p, i, p, i]
         L.mlmd_occupations.argtypes = [p, p, p, i]
+        L.mlmd_energy_nl.argtypes = [p, p, i]
+        L.mlmd_current.argtypes = [p, p, i, p, i]
         L.mlmd_profile.argtypes = [p, i]
         L.mlmd_profile_read.argtypes = [p, i, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)]
         L.mlmd_launch_count.argtypes = [p]
@@ -202,6 +204,21 @@ def mlmd_occupations(h, f, n_exc):
     return f, n_exc
 
 
+def mlmd_energy_nl(h, E):
+    """E: [ndom] float64 (numpy host array or CUDA tensor)."""
+    p, where = _ptr_where(E, np.dtype(np.float64))
+    _check(lib().mlmd_energy_nl(h, p, where))
+    return E
+
+
+def mlmd_current(h, A, J):
+    """A: [a_ndom, 3] host float64; J: [ndom, 3] float64 (numpy host array or CUDA tensor)."""
+    a = _host_f64(A).reshape(-1, 3)
+    p, where = _ptr_where(J, np.dtype(np.float64))
+    _check(lib().mlmd_current(h, a.ctypes.data_as(ctypes.c_void_p), a.shape[0], p, where))
+    return J
+
+
 def mlmd_profile(h, enable: bool):
     _check(lib().mlmd_profile(h, 1 if enable else 0))
 
@@ -289,6 +306,12 @@ class Domain:
         f = np.empty((self.ndom, self.norb), dtype=np.float64)
         n_exc = np.empty((self.ndom,), dtype=np.float64)
         return mlmd_occupations(self.handle, f, n_exc)
+
+    def energy_nl(self):
+        return mlmd_energy_nl(self.handle, np.empty((self.ndom,), dtype=np.float64))
+
+    def current(self, A):
+        return mlmd_current(self.handle, A, np.empty((self.ndom, 3), dtype=np.float64))
 
     def profile(self, enable=True):
         mlmd_profile(self.handle, enable)

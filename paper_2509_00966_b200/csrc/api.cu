@@ -361,6 +361,63 @@ int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int where) {
     return MLMD_OK;
 }
 
+int mlmd_energy_nl(mlmd_domain_t *h, double *E, int where) {
+    if (!h || !E) return fail(MLMD_ERR_ARG, "mlmd_energy_nl: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_energy_nl: bad where=%d", where);
+    if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_energy_nl: no orbitals set");
+    double *ed = where == MLMD_DEVICE ? E : h->nrm(3);
+    int nl = 0;
+    if (h->nproj == 0) {
+        CU(cudaMemsetAsync(ed, 0, (size_t)h->ndom * sizeof(double), h->stream));
+    } else {
+        // the projection GEMM of the hot path (S2a), then a reduction instead of the scaling step
+        const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
+        const bool tc = use_tensor_cores(h);
+        const int nsplit = tc ? h->nsplit_tc : h->nsplit;
+        if (tc)
+            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)h->psi(),
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, tc_nprod(h), kProjChain, &nl));
+        else
+            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)h->psi(),
+                                2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, &nl));
+        CU(launch_energy_nl(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, nsplit, h->zpart(), h->dprime(),
+                            h->occ(), h->dv, ed, &nl));
+    }
+    h->launches += nl;
+    if (where == MLMD_HOST) {
+        CU(cudaMemcpyAsync(E, ed, (size_t)h->ndom * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    return MLMD_OK;
+}
+
+int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int where) {
+    if (!h || !A || !J) return fail(MLMD_ERR_ARG, "mlmd_current: NULL argument");
+    if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_current: bad where=%d", where);
+    if (a_ndom != 1 && a_ndom != h->ndom) return fail(MLMD_ERR_ARG, "mlmd_current: a_ndom=%d must be 1 or ndom=%d", a_ndom, h->ndom);
+    if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_current: no orbitals set");
+    for (int i = 0; i < 3 * a_ndom; ++i)
+        if (!std::isfinite(A[i])) return fail(MLMD_ERR_NONFINITE, "mlmd_current: A[%d] is not finite", i);
+    // A goes through the pinned coefficient staging buffer into the (graph-only) current-coefficient slot
+    static_assert(sizeof(StepCoef) >= 3 * sizeof(double), "staging slot holds one field vector");
+    CU(cudaEventSynchronize(h->coef_uploaded));
+    double *a_host = (double *)h->coef_host;
+    memcpy(a_host, A, (size_t)3 * a_ndom * sizeof(double));
+    double *a_dev = (double *)h->coef_cur();
+    CU(cudaMemcpyAsync(a_dev, a_host, (size_t)3 * a_ndom * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaEventRecord(h->coef_uploaded, h->stream));
+    double *jd = where == MLMD_DEVICE ? J : h->nrm(3);
+    int nl = 0;
+    CU(launch_current(h->stream, h->ndom, h->nx, h->ny, h->nz, h->hx, h->hy, h->hz, h->ld, h->psi(), h->occ(), a_dev, a_ndom,
+                      h->nrm_part(), (size_t)h->ndom * kNormSlabs * h->ld, jd, &nl));
+    h->launches += nl;
+    if (where == MLMD_HOST) {
+        CU(cudaMemcpyAsync(J, jd, (size_t)h->ndom * 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    return MLMD_OK;
+}
+
 // ---- the step --------------------------------------------------------------------------------
 // RAII pair of events around one kernel launch when mlmd_profile is on.
 struct ProfScope {

@@ -397,4 +397,145 @@ cudaError_t launch_occupations(cudaStream_t st, int ndom, int norb, int ld, cons
     return cudaGetLastError();
 }
 
+// ---- observables (reading D30) ----
+// E_nl[dom] = dv sum_n f_n sum_p D'_p |C[p][n]|^2, C = split-K sum of the projection (as reduce_scale_kernel),
+// D' = D dv.  One block per domain, orbitals across threads, fixed summation order.
+__global__ void __launch_bounds__(256)
+energy_nl_kernel(int nproj, int beta_complex, int ld, int prows, int nsplit, const float *__restrict__ zpart,
+                 const float *__restrict__ dprime, const float *__restrict__ occ, double dv, double *__restrict__ E) {
+    const int dom = blockIdx.x;
+    const int N = 2 * ld;
+    const float *zp = zpart + (size_t)dom * nsplit * prows * N;
+    const size_t slice = (size_t)prows * N;
+    double e = 0.0;
+    for (int n = threadIdx.x; n < ld; n += blockDim.x) {
+        double en = 0.0;
+        for (int p = 0; p < nproj; ++p) {
+            float cre = 0.f, cim = 0.f;
+            if (!beta_complex) {
+                for (int s = 0; s < nsplit; ++s) {
+                    const float2 v = *(const float2 *)(zp + s * slice + (size_t)p * N + 2 * n);
+                    cre += v.x;
+                    cim += v.y;
+                }
+            } else {
+                for (int s = 0; s < nsplit; ++s) {
+                    const float2 a = *(const float2 *)(zp + s * slice + (size_t)(2 * p) * N + 2 * n);
+                    const float2 b = *(const float2 *)(zp + s * slice + (size_t)(2 * p + 1) * N + 2 * n);
+                    cre += a.x + b.y;
+                    cim += a.y - b.x;
+                }
+            }
+            en += (double)dprime[(size_t)dom * nproj + p] * ((double)cre * cre + (double)cim * cim);
+        }
+        e += (double)occ[(size_t)dom * ld + n] * en;
+    }
+    __shared__ double red[256];
+    red[threadIdx.x] = e;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) E[dom] = dv * red[0];
+}
+cudaError_t launch_energy_nl(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows, int nsplit,
+                             const float *zpart, const float *dprime, const float *occ, double dv, double *E, int *nlaunch) {
+    ++*nlaunch;
+    energy_nl_kernel<<<ndom, 256, 0, st>>>(nproj, beta_complex, ld, prows, nsplit, zpart, dprime, occ, dv, E);
+    return cudaGetLastError();
+}
+
+// Local current: part[dom][blk][0..2] = sum over the block's points and all orbitals of
+//   f_n * 2 * sum_{j=1,2} c1_j / h_d * Im( conj(psi(r)) psi(r + j e_d) )      (= f_n Im<psi|D1_d psi> restricted to r;
+//   the -j taps are the +j taps of the shifted sum, so only forward neighbours are read)
+// and part[..][3] = sum f_n |psi(r)|^2.  One warp per point, lanes stride over the float4 (two orbitals) of the row.
+__global__ void __launch_bounds__(256)
+current_part_kernel(int nx, int ny, int nz, int lanes, int pts, int nblk, const float4 *__restrict__ psi,
+                    const float *__restrict__ occ, float wx1, float wx2, float wy1, float wy2, float wz1, float wz2,
+                    double *__restrict__ part) {
+    const int dom = blockIdx.x / nblk, blk = blockIdx.x % nblk;
+    const long ngrid = (long)nx * ny * nz;
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const float4 *base = psi + (size_t)dom * ngrid * lanes;
+    const float2 *f = (const float2 *)(occ + (size_t)dom * lanes * 2);
+    double jx = 0.0, jy = 0.0, jz = 0.0, ne = 0.0;
+    const long r0 = (long)blk * pts, r1 = r0 + pts < ngrid ? r0 + pts : ngrid;
+    for (long r = r0 + warp; r < r1; r += 8) {
+        const int iz = (int)(r % nz), iy = (int)((r / nz) % ny), ix = (int)(r / ((long)nz * ny));
+        const long rz1 = r + (iz + 1 < nz ? 1 : 1 - nz), rz2 = r + (iz + 2 < nz ? 2 : 2 - nz);
+        const long ry1 = r + (long)nz * (iy + 1 < ny ? 1 : 1 - ny), ry2 = r + (long)nz * (iy + 2 < ny ? 2 : 2 - ny);
+        const long sx = (long)nz * ny;
+        const long rx1 = r + sx * (ix + 1 < nx ? 1 : 1 - nx), rx2 = r + sx * (ix + 2 < nx ? 2 : 2 - nx);
+        float ax = 0.f, ay = 0.f, az = 0.f, an = 0.f;
+        for (int l = lane; l < lanes; l += 32) {
+            const float4 u = __ldg(base + r * lanes + l);
+            const float2 ff = __ldg(f + l);
+            auto im = [&](const float4 v) {     // f_n Im(conj(u) v) summed over the two orbitals of the float4
+                return ff.x * (u.x * v.y - u.y * v.x) + ff.y * (u.z * v.w - u.w * v.z);
+            };
+            ax += wx1 * im(__ldg(base + rx1 * lanes + l)) + wx2 * im(__ldg(base + rx2 * lanes + l));
+            ay += wy1 * im(__ldg(base + ry1 * lanes + l)) + wy2 * im(__ldg(base + ry2 * lanes + l));
+            az += wz1 * im(__ldg(base + rz1 * lanes + l)) + wz2 * im(__ldg(base + rz2 * lanes + l));
+            an += ff.x * (u.x * u.x + u.y * u.y) + ff.y * (u.z * u.z + u.w * u.w);
+        }
+        jx += (double)ax;
+        jy += (double)ay;
+        jz += (double)az;
+        ne += (double)an;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        jx += __shfl_xor_sync(0xffffffffu, jx, o);
+        jy += __shfl_xor_sync(0xffffffffu, jy, o);
+        jz += __shfl_xor_sync(0xffffffffu, jz, o);
+        ne += __shfl_xor_sync(0xffffffffu, ne, o);
+    }
+    __shared__ double red[8][4];
+    if (lane == 0) {
+        red[warp][0] = jx;
+        red[warp][1] = jy;
+        red[warp][2] = jz;
+        red[warp][3] = ne;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
+        part[((size_t)dom * nblk + blk) * 4 + threadIdx.x] = s;
+    }
+}
+// J[dom][d] = dv (sum_blk part[d] + A[dom or 0][d] * sum_blk part[3]); one thread per (dom, d)
+__global__ void current_final_kernel(int ndom, int nblk, int a_ndom, double dv, const double *__restrict__ part,
+                                     const double *__restrict__ A, double *__restrict__ J) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ndom * 3) return;
+    const int dom = i / 3, d = i % 3;
+    double s = 0.0, ne = 0.0;
+    for (int b = 0; b < nblk; ++b) {
+        s += part[((size_t)dom * nblk + b) * 4 + d];
+        ne += part[((size_t)dom * nblk + b) * 4 + 3];
+    }
+    J[i] = dv * (s + A[(size_t)(a_ndom == 1 ? 0 : dom) * 3 + d] * ne);
+}
+cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int ld,
+                           const float2 *psi, const float *occ, const double *A_dev, int a_ndom, double *part,
+                           size_t part_doubles, double *J, int *nlaunch) {
+    const long ngrid = (long)nx * ny * nz;
+    // points per block: at least 64, and few enough blocks for the partial-sum scratch
+    long pts = 64;
+    const long max_blk = (long)(part_doubles / 4 / ndom);
+    if (max_blk < 1) return cudaErrorInvalidValue;
+    if ((ngrid + pts - 1) / pts > max_blk) pts = ((ngrid + max_blk - 1) / max_blk + 7) / 8 * 8;
+    const int nblk = (int)((ngrid + pts - 1) / pts);
+    // 2 c1_j / h_d with c1 = (2/3, -1/12): weights of the 4th-order first difference (north_star)
+    const float w1 = (float)(2.0 * 2.0 / 3.0), w2 = (float)(2.0 * -1.0 / 12.0);
+    *nlaunch += 2;
+    current_part_kernel<<<ndom * nblk, 256, 0, st>>>(nx, ny, nz, ld / 2, (int)pts, nblk, (const float4 *)psi, occ,
+                                                     (float)(w1 / hx), (float)(w2 / hx), (float)(w1 / hy), (float)(w2 / hy),
+                                                     (float)(w1 / hz), (float)(w2 / hz), part);
+    current_final_kernel<<<(ndom * 3 + 127) / 128, 128, 0, st>>>(ndom, nblk, a_ndom, hx * hy * hz, part, A_dev, J);
+    return cudaGetLastError();
+}
+
 }  // namespace mlmd

@@ -187,6 +187,12 @@ cudaError_t launch_colnorm2(cudaStream_t st, int ndom, long ngrid, int ld, const
 cudaError_t launch_colnorm_final(cudaStream_t st, int ndom, int ld, int nslabs, const double *part, double *out, int *nlaunch);
 cudaError_t launch_kick_scale(cudaStream_t st, int n, double *n0, const double *na, const double *nc, const double *nd,
                               float *scl, int *nlaunch);
+// NEXT-2 observables (reading D30): E_nl from the projection partials; local current by a forward-neighbour pass
+cudaError_t launch_energy_nl(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows, int nsplit,
+                             const float *zpart, const float *dprime, const float *occ, double dv, double *E, int *nlaunch);
+cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int ld,
+                           const float2 *psi, const float *occ, const double *A_dev, int a_ndom, double *part,
+                           size_t part_doubles, double *J, int *nlaunch);
 cudaError_t launch_occupations(cudaStream_t st, int ndom, int norb, int ld, const float2 *S, const float *occ, double *f,
                                double *nexc, int *nlaunch);
 cudaError_t launch_scale_density(cudaStream_t st, int ndom, long ngrid, int ld, float2 *psi, const float *scl,
