@@ -185,6 +185,7 @@ def main():
     ap.add_argument("--oracle-orbitals", type=int, default=32)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-observables", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -305,6 +306,31 @@ def main():
                    "mlmd_propagate_split" if args.step == "split" else "mlmd_propagate") +
                        "Psi stays device-resident as in the paper's shadow dynamics (L130-132, L145)"}
 
+    # ---- on-request observables (NEXT rows of SURVEY.md 8(f)): device time of one call each, CUDA events
+    def time_call(fn, reps=3):
+        fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    observables = None
+    if rank == 0 and not args.no_observables:
+        e_dev = torch.empty(c.ndom, dtype=torch.float64, device=dev)
+        j_dev = torch.empty((c.ndom, 3), dtype=torch.float64, device=dev)
+        elems = alg["elems"]
+        t_e = time_call(lambda: M.mlmd_energy_nl(dom.handle, e_dev))
+        t_j = time_call(lambda: M.mlmd_current(dom.handle, A[0], j_dev))
+        observables = {
+            "energy_nl": {"ms": t_e, "tflops": alg["gemm_flops_each"] / (t_e * 1e-3) / 1e12,
+                          "what": "projection GEMM + reduction (mlmd_energy_nl), device buffers"},
+            "current": {"ms": t_j, "gbs": elems * 8 / (t_j * 1e-3) / 1e9, "frac_hbm": elems * 8 / (t_j * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        "what": "forward-neighbour pass over psi (mlmd_current), algorithmic bytes = one read of psi"},
+        }
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -363,7 +389,7 @@ def main():
         "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "complex64",
         "data": "synthetic", "config": workload_config(c, args), "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-        "roofline": roof, "cpu_baseline": cpu, "step_roofline": step_roof, "kernels": per_class,
+        "roofline": roof, "cpu_baseline": cpu, "step_roofline": step_roof, "kernels": per_class, "observables": observables,
         "orbital_steps_per_s": c.ndom * c.norb * world * K / (ms * 1e-3), "input_generation_s": t_gen,
         "paper_context": PAPER_CONTEXT,
     }

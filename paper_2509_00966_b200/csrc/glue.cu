@@ -505,6 +505,73 @@ current_part_kernel(int nx, int ny, int nz, int lanes, int pts, int nblk, const 
         part[((size_t)dom * nblk + blk) * 4 + threadIdx.x] = s;
     }
 }
+// The same sums with each x-plane read once: a block owns an 8(y) x 8(z) patch for one 64-byte orbital chunk
+// (thread = point x float4 lane) and marches along x; the x taps come from a three-plane register history,
+// the y/z taps are the patch neighbours' own centre loads (L1 hits), only the +2 halo rows add L2 traffic.
+__global__ void __launch_bounds__(256)
+current_march_kernel(int nx, int ny, int nz, int lanes, int xs, int nxseg, const float4 *__restrict__ psi,
+                     const float *__restrict__ occ, float wx1, float wx2, float wy1, float wy2, float wz1, float wz2,
+                     double *__restrict__ part) {
+    const int l = threadIdx.x % 4, tz = (threadIdx.x / 4) % 8, ty = threadIdx.x / 32;
+    int item = blockIdx.x;
+    const int seg = item % nxseg;
+    item /= nxseg;
+    const int nzt = nz / 8, nyt = ny / 8, nchunk = lanes / 4;
+    const int zt = item % nzt;
+    item /= nzt;
+    const int yt = item % nyt;
+    item /= nyt;
+    const int chunk = item % nchunk;
+    const int dom = item / nchunk;
+    const int y = yt * 8 + ty, z = zt * 8 + tz;
+    const int y1 = y + 1 < ny ? y + 1 : y + 1 - ny, y2 = y + 2 < ny ? y + 2 : y + 2 - ny;
+    const int z1 = z + 1 < nz ? z + 1 : z + 1 - nz, z2 = z + 2 < nz ? z + 2 : z + 2 - nz;
+    const long sy = (long)nz * lanes, sx = (long)ny * sy;
+    const float4 *base = psi + (size_t)dom * nx * sx + chunk * 4 + l;
+    const long oc = (long)y * sy + (long)z * lanes;
+    const long oy1 = (long)y1 * sy + (long)z * lanes, oy2 = (long)y2 * sy + (long)z * lanes;
+    const long oz1 = (long)y * sy + (long)z1 * lanes, oz2 = (long)y * sy + (long)z2 * lanes;
+    const float2 ff = __ldg((const float2 *)(occ + (size_t)dom * lanes * 2) + chunk * 4 + l);
+    const int x0 = seg * xs, x1 = min(x0 + xs, nx);
+    auto xw = [&](int x) { return x < nx ? x : x - nx; };
+    float4 u0 = __ldg(base + (long)x0 * sx + oc), u1 = __ldg(base + (long)xw(x0 + 1) * sx + oc);
+    float ax = 0.f, ay = 0.f, az = 0.f, an = 0.f;
+    // unrolled so that the loads of several planes are in flight per thread (only one load in five is new HBM data)
+#pragma unroll 4
+    for (int x = x0; x < x1; ++x) {
+        const float4 *pl = base + (long)x * sx;
+        const float4 u2 = __ldg(base + (long)xw(x + 2) * sx + oc);
+        const float4 vy1 = __ldg(pl + oy1), vy2 = __ldg(pl + oy2), vz1 = __ldg(pl + oz1), vz2 = __ldg(pl + oz2);
+        auto im = [&](const float4 v) { return ff.x * (u0.x * v.y - u0.y * v.x) + ff.y * (u0.z * v.w - u0.w * v.z); };
+        ax += wx1 * im(u1) + wx2 * im(u2);
+        ay += wy1 * im(vy1) + wy2 * im(vy2);
+        az += wz1 * im(vz1) + wz2 * im(vz2);
+        an += ff.x * (u0.x * u0.x + u0.y * u0.y) + ff.y * (u0.z * u0.z + u0.w * u0.w);
+        u0 = u1;
+        u1 = u2;
+    }
+    double jx = (double)ax, jy = (double)ay, jz = (double)az, ne = (double)an;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        jx += __shfl_xor_sync(0xffffffffu, jx, o);
+        jy += __shfl_xor_sync(0xffffffffu, jy, o);
+        jz += __shfl_xor_sync(0xffffffffu, jz, o);
+        ne += __shfl_xor_sync(0xffffffffu, ne, o);
+    }
+    __shared__ double red[8][4];
+    if (threadIdx.x % 32 == 0) {
+        red[ty][0] = jx;
+        red[ty][1] = jy;
+        red[ty][2] = jz;
+        red[ty][3] = ne;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double sum = 0.0;
+        for (int w = 0; w < 8; ++w) sum += red[w][threadIdx.x];
+        part[(size_t)blockIdx.x * 4 + threadIdx.x] = sum;      // blocks of one domain are contiguous
+    }
+}
 // J[dom][d] = dv (sum_blk part[d] + A[dom or 0][d] * sum_blk part[3]); one thread per (dom, d)
 __global__ void current_final_kernel(int ndom, int nblk, int a_ndom, double dv, const double *__restrict__ part,
                                      const double *__restrict__ A, double *__restrict__ J) {
@@ -522,14 +589,30 @@ cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, do
                            const float2 *psi, const float *occ, const double *A_dev, int a_ndom, double *part,
                            size_t part_doubles, double *J, int *nlaunch) {
     const long ngrid = (long)nx * ny * nz;
-    // points per block: at least 64, and few enough blocks for the partial-sum scratch
-    long pts = 64;
     const long max_blk = (long)(part_doubles / 4 / ndom);
     if (max_blk < 1) return cudaErrorInvalidValue;
-    if ((ngrid + pts - 1) / pts > max_blk) pts = ((ngrid + max_blk - 1) / max_blk + 7) / 8 * 8;
-    const int nblk = (int)((ngrid + pts - 1) / pts);
     // 2 c1_j / h_d with c1 = (2/3, -1/12): weights of the 4th-order first difference (north_star)
     const float w1 = (float)(2.0 * 2.0 / 3.0), w2 = (float)(2.0 * -1.0 / 12.0);
+    if (ny % 8 == 0 && nz % 8 == 0 && !getenv("MLMD_CURRENT_SIMPLE")) {
+        const long tiles = (long)(ld / 8) * (ny / 8) * (nz / 8);
+        int nxseg = 1;
+        while (tiles * ndom * nxseg < 4 * 148 && nx / (nxseg * 2) >= 8) nxseg *= 2;
+        const int xs = (nx + nxseg - 1) / nxseg;
+        nxseg = (nx + xs - 1) / xs;
+        if (tiles * nxseg <= max_blk) {
+            const int nblk = (int)(tiles * nxseg);
+            *nlaunch += 2;
+            current_march_kernel<<<(unsigned)(ndom * nblk), 256, 0, st>>>(nx, ny, nz, ld / 2, xs, nxseg, (const float4 *)psi, occ,
+                                                                          (float)(w1 / hx), (float)(w2 / hx), (float)(w1 / hy),
+                                                                          (float)(w2 / hy), (float)(w1 / hz), (float)(w2 / hz), part);
+            current_final_kernel<<<(ndom * 3 + 127) / 128, 128, 0, st>>>(ndom, nblk, a_ndom, hx * hy * hz, part, A_dev, J);
+            return cudaGetLastError();
+        }
+    }
+    // any shape: one warp per point; points per block at least 64, and few enough blocks for the scratch
+    long pts = 64;
+    if ((ngrid + pts - 1) / pts > max_blk) pts = ((ngrid + max_blk - 1) / max_blk + 7) / 8 * 8;
+    const int nblk = (int)((ngrid + pts - 1) / pts);
     *nlaunch += 2;
     current_part_kernel<<<ndom * nblk, 256, 0, st>>>(nx, ny, nz, ld / 2, (int)pts, nblk, (const float4 *)psi, occ,
                                                      (float)(w1 / hx), (float)(w2 / hx), (float)(w1 / hy), (float)(w2 / hy),
