@@ -1,0 +1,112 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (whole batch in one
+handle, device-resident inputs, the tcgen05 path with the split-K / cluster configuration that batch size selects).
+
+The oracle cannot run a whole batch in test time, but the map is linear and couples neither domains nor orbitals
+(H acts on each orbital separately, D22), so a SAMPLE of (domain, orbital) pairs is computed exactly by running
+the oracle on those orbitals alone with the domain's V_loc, projectors and field.  The density, which mixes all
+orbitals of a point, is checked against an FP64 sum over the GPU's own orbitals of a sampled domain (the
+orbitals themselves being covered by the sample), plus the electron-count sum rule on every domain.
+Tolerances are north_star's (1e-5 after one step, 1e-4 after the last, density 1e-4).
+"""
+import os
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+import workloads as W
+from test_gpu_parity import TOL_1STEP, TOL_LAST, TOL_RHO
+
+pytestmark = pytest.mark.gpu
+
+
+def load_batch(c, keep):
+    """The whole batch on the device, generated domain by domain as bench.py does; host copies of `keep` only."""
+    import torch
+    dev = torch.device("cuda", 0)
+    psi_dev = torch.empty((c.ndom, *c.grid, c.norb), dtype=torch.complex64, device=dev)
+    beta_dev = torch.empty((c.ndom, c.ngrid, c.nproj), dtype=torch.float32, device=dev)
+    vloc = np.empty((c.ndom, *c.grid), dtype=np.float32)
+    occ = np.empty((c.ndom, c.norb))
+    D = np.empty((c.ndom, c.nproj))
+    kept = {}
+    with ThreadPoolExecutor(max_workers=max(1, min(8, (os.cpu_count() or 2) // 2))) as ex:
+        for k, dd in enumerate(ex.map(lambda k: W.generate_domain(c, k), range(c.ndom))):
+            psi_dev[k].copy_(torch.from_numpy(dd["psi"]))
+            beta_dev[k].copy_(torch.from_numpy(dd["beta"]))
+            vloc[k], occ[k], D[k] = dd["vloc"], dd["occ"], dd["D"]
+            if k in keep:
+                kept[k] = dd
+    return psi_dev, beta_dev, vloc, occ, D, kept
+
+
+def run_full(cfg, sample, nsteps, split=False):
+    """sample: {domain: [orbital indices]}"""
+    import torch
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    c = W.get_config(cfg)
+    psi_dev, beta_dev, vloc, occ, D, kept = load_batch(c, set(sample))
+    A = W.laser_samples(c, nsteps=nsteps, t0=0.9)
+    dom = M.Domain(c.ndom, c.grid, c.h, c.norb, c.nproj)
+    dom.set_vloc(vloc)
+    dom.set_projectors(beta_dev, D)
+    dom.set_orbitals(psi_dev, occ)
+    del beta_dev
+    assert dom.gemm_path() == "tcgen05"
+    prop = dom.propagate_split if split else dom.propagate
+    oracle_prop = ref.propagate_split if split else ref.propagate
+    errs = {}
+    for label, n in (("first", 1), ("last", nsteps)):
+        if label == "last" and nsteps == 1:
+            break
+        dom.set_orbitals(psi_dev, occ)
+        prop(n, c.dt, A[:n])
+        out = torch.empty_like(psi_dev)
+        M.mlmd_get_orbitals(dom.handle, out)
+        worst = 0.0
+        for k, orbs in sample.items():
+            dd = kept[k]
+            sub = np.ascontiguousarray(dd["psi"][None, ..., orbs])
+            r, _ = oracle_prop(sub, np.full((1, len(orbs)), 2.0), dd["vloc"][None], dd["beta"][None], dd["D"][None], A[:n], c.dt, c.h)
+            g = out[k][..., orbs].cpu().numpy().astype(np.complex128)
+            num = np.sqrt((np.abs(g - r[0]) ** 2).sum(axis=(0, 1, 2)))
+            den = np.sqrt((np.abs(r[0]) ** 2).sum(axis=(0, 1, 2)))
+            worst = max(worst, float((num / den).max()))
+        errs[label] = worst
+    # density of the final state: FP64 sum over the GPU's own orbitals of one sampled domain, sum rule on all
+    rho = torch.empty((c.ndom, *c.grid), dtype=torch.float32, device=psi_dev.device)
+    M.mlmd_density(dom.handle, rho)
+    k0 = next(iter(sample))
+    pk = out[k0].to(torch.complex128)
+    rho_ref = (pk.real ** 2 + pk.imag ** 2) @ torch.from_numpy(occ[k0]).to(pk.device)
+    errs["rho"] = float(((rho[k0].double() - rho_ref).abs().max() / rho_ref.max()).item())
+    ne_gpu = rho.double().sum(dim=(1, 2, 3)) * c.dv
+    occ_t = torch.from_numpy(occ).to(out.device)
+    ne_ref = torch.stack([(((out[k].real.double() ** 2 + out[k].imag.double() ** 2).sum(dim=(0, 1, 2))) * occ_t[k]).sum() * c.dv
+                          for k in range(c.ndom)])
+    errs["electrons"] = float(((ne_gpu - ne_ref).abs() / ne_ref).max().item())
+    dom.close()
+    print(cfg, "split" if split else "taylor", errs)
+    assert errs["first"] <= TOL_1STEP
+    assert errs.get("last", 0.0) <= TOL_LAST
+    assert errs["rho"] <= TOL_RHO and errs["electrons"] <= 1e-5
+    return errs
+
+
+def test_config2_full_batch():
+    run_full(2, {5: [0, 1, 100, 111, 112, 223], 0: [7]}, nsteps=3)
+
+
+def test_config3_full_batch_as_benchmarked():
+    """The default bench.py workload: 64 domains x 48^3 x 224 orbitals x 240 projectors."""
+    run_full(3, {41: [0, 1, 111, 112, 223], 0: [5], 63: [222]}, nsteps=2)
+
+
+def test_config3_full_batch_split_step():
+    run_full(3, {17: [0, 113, 223], 63: [3]}, nsteps=1, split=True)
+
+
+def test_config4_full_batch_large_domains():
+    """4 domains x 64^3 x 696 orbitals x 810 projectors (ld = 704 columns, 4 N-tiles; the GEMM-heavy shape)."""
+    run_full(4, {2: [0, 347, 348, 695], 3: [1]}, nsteps=1)
