@@ -87,6 +87,7 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.nrm = take((size_t)4 * ndom * pl->ld * sizeof(double));
     w.nrm_part = take((size_t)ndom * kNormSlabs * pl->ld * sizeof(double));
     w.scl = take((size_t)ndom * pl->ld * sizeof(float));
+    w.avec = take((size_t)ndom * 3 * sizeof(double));
     w.total = o;
     return true;
 }
@@ -398,12 +399,12 @@ int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int w
     if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_current: no orbitals set");
     for (int i = 0; i < 3 * a_ndom; ++i)
         if (!std::isfinite(A[i])) return fail(MLMD_ERR_NONFINITE, "mlmd_current: A[%d] is not finite", i);
-    // A goes through the pinned coefficient staging buffer into the (graph-only) current-coefficient slot
+    // A goes through the pinned coefficient staging buffer (one StepCoef slot per domain is large enough)
     static_assert(sizeof(StepCoef) >= 3 * sizeof(double), "staging slot holds one field vector");
     CU(cudaEventSynchronize(h->coef_uploaded));
     double *a_host = (double *)h->coef_host;
     memcpy(a_host, A, (size_t)3 * a_ndom * sizeof(double));
-    double *a_dev = (double *)h->coef_cur();
+    double *a_dev = h->avec();
     CU(cudaMemcpyAsync(a_dev, a_host, (size_t)3 * a_ndom * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     CU(cudaEventRecord(h->coef_uploaded, h->stream));
     double *jd = where == MLMD_DEVICE ? J : h->nrm(3);

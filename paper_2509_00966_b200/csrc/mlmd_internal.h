@@ -24,7 +24,7 @@ static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
     size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
-        nrm, nrm_part, scl, total;
+        nrm, nrm_part, scl, avec, total;
 };
 
 constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
@@ -96,6 +96,7 @@ struct mlmd_domain {
     double *nrm(int which) const { return (double *)(ws + off.nrm) + (size_t)which * ndom * ld; }
     double *nrm_part() const { return (double *)(ws + off.nrm_part); }
     float *scl() const { return (float *)(ws + off.scl); }
+    double *avec() const { return (double *)(ws + off.avec); }   // mlmd_current: A[a_ndom][3]
 };
 
 namespace mlmd {
