@@ -26,7 +26,7 @@ constexpr int S_STRIP = 2 * 16 * 64;
 constexpr int S_PLANE_W = S_CENTER + 4 * S_STRIP;  // w: centre, z-lo, z-hi, y-lo, y-hi
 constexpr int S_PLANE = S_PLANE_W + S_CENTER;      // + the Horner base psi of the plane completed by this step
 constexpr int S_NBUF = 5, S_PF = 3;                // NBUF = unroll factor of the march: buffer index is static
-constexpr int S_THREADS = SY * (SZ / 2) * SL;      // 512: every thread owns the points (y, z) and (y, z + 8)
+constexpr int S_THREADS = (SY / 2) * SZ * SL;      // 512: every thread owns the points (y, z) and (y + 1, z), y even
 constexpr int S_SMEM = S_NBUF * S_PLANE + 256;
 
 struct TmaStencilParams {
@@ -91,7 +91,7 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t *full = (uint64_t *)(smem + S_NBUF * S_PLANE), *empty = full + S_NBUF;
     const int tid = threadIdx.x;
-    const int l = tid % SL, tz = (tid / SL) % (SZ / 2), ty = tid / (SL * SZ / 2);   // tz in 0..7
+    const int l = tid % SL, tz = (tid / SL) % SZ, ty = 2 * (tid / (SL * SZ));   // a warp = 8 z x 4 lanes: 512 contiguous bytes
 
     // work item
     int item = blockIdx.x;
@@ -144,9 +144,9 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     if (tid == 0)
         for (int n = 0; n < S_PF && n < nplanes; ++n) issue(n);
 
-    // Byte offsets inside a plane buffer.  Point A = (ty, tz), point B = (ty, tz + 8): B's centre and
-    // y-neighbour offsets are A's + 512; z-neighbours that stay inside the centre box are +-64/128 from
-    // the own offset, only A's z-1, z-2 and B's z+1, z+2 can fall into a halo strip.
+    // Byte offsets inside a plane buffer.  Point A = (ty, tz), point B = (ty + 1, tz), ty even: the six rows
+    // ty-2 .. ty+3 at the own z serve as centre and y-neighbours of BOTH points (6 loads instead of 10); the
+    // z-neighbours of B are those of A one row up (+1024 in the centre box, +128 in a z halo strip).
     const uint32_t own = (uint32_t)((ty * SZ + tz) * 64 + l * 16);
     auto zoff = [&](int t) -> uint32_t {
         if (t < 0) return (uint32_t)(S_CENTER + (ty * 2 + (t + 2)) * 64 + l * 16);
@@ -158,13 +158,15 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         if (t >= SY) return (uint32_t)(S_CENTER + 3 * S_STRIP + ((t - SY) * SZ + tz) * 64 + l * 16);
         return (uint32_t)((t * SZ + tz) * 64 + l * 16);
     };
-    const uint32_t oAzm1 = zoff(tz - 1), oAzm2 = zoff(tz - 2), oBzp1 = zoff(tz + 9), oBzp2 = zoff(tz + 10);
-    const uint32_t oyp1 = yoff(ty + 1), oym1 = yoff(ty - 1), oyp2 = yoff(ty + 2), oym2 = yoff(ty - 2);
+    const uint32_t ozm1 = zoff(tz - 1), ozm2 = zoff(tz - 2), ozp1 = zoff(tz + 1), ozp2 = zoff(tz + 2);
+    const uint32_t dzm = tz < 2 ? 128u : 1024u, dzp = tz >= SZ - 2 ? 128u : 1024u;   // B's z offsets = A's + these
+    const uint32_t dzm1 = tz < 1 ? 128u : 1024u, dzp1 = tz >= SZ - 1 ? 128u : 1024u;
+    const uint32_t oym2 = yoff(ty - 2), oym1 = yoff(ty - 1), oyp2 = yoff(ty + 2), oyp3 = yoff(ty + 3);
 
     const StepCoef c = PERDOM ? P.coef[dom] : P.cval;   // by-value copy lives in the constant bank: no registers
     const long sz = P.lanes, sy = sz * P.nz, sx = sy * P.ny;
     const long pbase = (long)dom * sx * P.nx + (long)(y0 + ty) * sy + (long)(z0 + tz) * sz + chunk * SL + l;
-    const float *vd = P.vloc + ((long)dom * P.nx * P.ny + (y0 + ty)) * P.nz + (z0 + tz);
+    const float *vd = P.vloc + ((long)dom * P.nx * P.ny + (y0 + ty)) * P.nz + (z0 + tz);   // B: + nz
     const long vsx = (long)P.ny * P.nz;
     const uint32_t sbase = smem_u32(smem);
 
@@ -172,8 +174,8 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     float4 a0 = zero4, a1 = zero4, a2 = zero4, a3 = zero4, a4 = zero4;   // point A, planes q-2 .. q+2
     float4 b0 = zero4, b1 = zero4, b2 = zero4, b3 = zero4, b4 = zero4;   // point B
     // running element offsets (no per-step 64-bit index arithmetic): Horner base / output of the plane
-    // being completed, V_loc of the plane being consumed.  B = A + 8 grid points along z.
-    const long dB = 8 * sz;
+    // being completed, V_loc of the plane being consumed.  B = A + one grid row along y.
+    const long dB = sy;
     float4 *out_p = P.out + pbase + (long)x0 * sx;
     int xq = x0 - 2;
     xq = xq < 0 ? xq + P.nx : xq;
@@ -181,13 +183,13 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const long vwrap = (long)P.nx * vsx;
     // V_loc of the plane consumed by the NEXT step, loaded one step ahead so that its latency is off the
     // critical path of the first FMA
-    float vAn = __ldg(vp), vBn = __ldg(vp + 8);
+    float vAn = __ldg(vp), vBn = __ldg(vp + P.nz);
 
     float nrm0 = 0.f, nrm1 = 0.f;   // NORM: this thread's two orbitals, summed over its points
-    auto point = [&](const uint32_t buf, const uint32_t o, const uint32_t ozm1, const uint32_t ozm2, const uint32_t ozp1,
-                     const uint32_t ozp2, const uint32_t dy, const float cen, const bool own_plane, float4 &A0, float4 &A1,
-                     float4 &A2, float4 &A3, float4 &A4) {
-        const float4 u = lds4(buf + o);
+    // centre, y and z taps of one point: u = centre value, (yp1, ym1), (yp2, ym2) its y-neighbours (already loaded)
+    auto point = [&](const uint32_t buf, const float4 u, const float4 yp1, const float4 ym1, const float4 yp2, const float4 ym2,
+                     const uint32_t zm1, const uint32_t zm2, const uint32_t zp1, const uint32_t zp2, const float cen,
+                     const bool own_plane, float4 &A0, float4 &A1, float4 &A2, float4 &A3, float4 &A4) {
         if (NORM == 1 && own_plane) {
             nrm0 = fmaf(u.x, u.x, fmaf(u.y, u.y, nrm0));
             nrm1 = fmaf(u.z, u.z, fmaf(u.w, u.w, nrm1));
@@ -196,16 +198,12 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         A2.y = fmaf(cen, u.y, A2.y);
         A2.z = fmaf(cen, u.z, A2.z);
         A2.w = fmaf(cen, u.w, A2.w);
+        if (AYZ) pair_acc(A2, yp1, ym1, c.p[1][0], c.q[1][0]); else pair_acc_real(A2, yp1, ym1, c.p[1][0]);
+        if (AYZ) pair_acc(A2, yp2, ym2, c.p[1][1], c.q[1][1]); else pair_acc_real(A2, yp2, ym2, c.p[1][1]);
         {
-            const float4 p1 = lds4(buf + oyp1 + dy), m1 = lds4(buf + oym1 + dy);
-            if (AYZ) pair_acc(A2, p1, m1, c.p[1][0], c.q[1][0]); else pair_acc_real(A2, p1, m1, c.p[1][0]);
-            const float4 p2 = lds4(buf + oyp2 + dy), m2 = lds4(buf + oym2 + dy);
-            if (AYZ) pair_acc(A2, p2, m2, c.p[1][1], c.q[1][1]); else pair_acc_real(A2, p2, m2, c.p[1][1]);
-        }
-        {
-            const float4 p1 = lds4(buf + ozp1), m1 = lds4(buf + ozm1);
+            const float4 p1 = lds4(buf + zp1), m1 = lds4(buf + zm1);
             if (AYZ) pair_acc(A2, p1, m1, c.p[2][0], c.q[2][0]); else pair_acc_real(A2, p1, m1, c.p[2][0]);
-            const float4 p2 = lds4(buf + ozp2), m2 = lds4(buf + ozm2);
+            const float4 p2 = lds4(buf + zp2), m2 = lds4(buf + zm2);
             if (AYZ) pair_acc(A2, p2, m2, c.p[2][1], c.q[2][1]); else pair_acc_real(A2, p2, m2, c.p[2][1]);
         }
         // x taps: u = w(plane q) is the +j neighbour of plane q-j (coefficient p_j - i q_j) and the -j
@@ -232,15 +230,20 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             vp -= vwrap;
         }
         vAn = __ldg(vp);
-        vBn = __ldg(vp + 8);
+        vBn = __ldg(vp + P.nz);
         mbar_wait(&full[k], it & 1);
         const uint32_t buf = sbase + k * S_PLANE;
         const bool own_plane = n >= 2 && n < nplanes - 2;
-        point(buf, own, oAzm1, oAzm2, own + 64, own + 128, 0u, c.centre + vA, own_plane, A0, A1, A2, A3, A4);
-        point(buf, own + 512, own + 512 - 64, own + 512 - 128, oBzp1, oBzp2, 512u, c.centre + vB, own_plane, B0, B1, B2, B3, B4);
+        {
+            const float4 rm2 = lds4(buf + oym2), rm1 = lds4(buf + oym1), r0 = lds4(buf + own), r1 = lds4(buf + own + 1024),
+                         r2 = lds4(buf + oyp2), r3 = lds4(buf + oyp3);
+            point(buf, r0, r1, rm1, r2, rm2, ozm1, ozm2, ozp1, ozp2, c.centre + vA, own_plane, A0, A1, A2, A3, A4);
+            point(buf, r1, r2, r0, r3, rm1, ozm1 + dzm1, ozm2 + dzm, ozp1 + dzp1, ozp2 + dzp, c.centre + vB, own_plane, B0, B1, B2,
+                  B3, B4);
+        }
         // plane q-2 (output n - 4) is complete: out = psi + (-i tau) acc
         if (n >= 4) {
-            const float4 psA = lds4(buf + S_PLANE_W + own), psB = lds4(buf + S_PLANE_W + own + 512);
+            const float4 psA = lds4(buf + S_PLANE_W + own), psB = lds4(buf + S_PLANE_W + own + 1024);
             const float4 oA = make_float4(fmaf(P.tau, A0.y, psA.x), fmaf(-P.tau, A0.x, psA.y), fmaf(P.tau, A0.w, psA.z),
                                           fmaf(-P.tau, A0.z, psA.w));
             const float4 oB = make_float4(fmaf(P.tau, B0.y, psB.x), fmaf(-P.tau, B0.x, psB.y), fmaf(P.tau, B0.w, psB.z),
