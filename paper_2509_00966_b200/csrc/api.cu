@@ -143,7 +143,7 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->vmax = h->dmax = 0.0; h->launches = 0;
     h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
     h->coef_uploaded = nullptr; h->gexec = nullptr; h->gstream = nullptr; h->gfork = h->gjoin = nullptr;
-    h->g_launches = 0; h->g_dt = 0.0; h->g_yz = false;
+    h->g_launches = 0; h->g_dt = 0.0; h->g_yz = false; h->g_split = false;
     {
         const char *g = getenv("MLMD_GRAPH");   // "0": never capture the step into a CUDA graph
         h->graph_allowed = !(g && g[0] == '0');
@@ -517,8 +517,10 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
     return MLMD_OK;
 }
 
+static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, int *nl);
+
 // Capture one step (coefficients taken from the device slot that advance_coef refills) into h->gexec.
-static int capture_step(mlmd_domain *h, double dt, bool yz) {
+static int capture_step(mlmd_domain *h, double dt, bool yz, bool split) {
     if (!h->gstream) {
         CU(cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking));
         CU(cudaEventCreateWithFlags(&h->gfork, cudaEventDisableTiming));
@@ -530,7 +532,8 @@ static int capture_step(mlmd_domain *h, double dt, bool yz) {
     CU(cudaStreamBeginCapture(h->gstream, cudaStreamCaptureModeThreadLocal));
     h->stream = h->gstream;
     cudaError_t e = launch_advance_coef(h->gstream, h->coef(), h->coef_cur(), h->step_counter(), h->ndom, &nl);
-    int rc = e == cudaSuccess ? enqueue_step(h, h->coef_cur(), nullptr, dt, &nl) : MLMD_ERR_CUDA;
+    int rc = e != cudaSuccess ? MLMD_ERR_CUDA
+             : split ? enqueue_split_step(h, h->coef_cur(), nullptr, dt, &nl) : enqueue_step(h, h->coef_cur(), nullptr, dt, &nl);
     h->stream = user;
     cudaError_t e2 = cudaStreamEndCapture(h->gstream, &graph);
     if (rc || e != cudaSuccess || e2 != cudaSuccess || !graph) {
@@ -550,6 +553,7 @@ static int capture_step(mlmd_domain *h, double dt, bool yz) {
     h->g_launches = nl;
     h->g_dt = dt;
     h->g_yz = yz;
+    h->g_split = split;
     return MLMD_OK;
 }
 
@@ -606,79 +610,26 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
     return MLMD_OK;
 }
 
-int mlmd_propagate_split(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom) {
-    if (!h) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: NULL handle");
-    if (nsteps < 0 || !(dt == dt) || std::isinf(dt)) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: nsteps=%d dt=%g", nsteps, dt);
-    if (nsteps > 0 && !A) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: A is NULL");
-    if (a_ndom != 1 && a_ndom != h->ndom) return fail(MLMD_ERR_ARG, "mlmd_propagate_split: a_ndom=%d must be 1 or ndom=%d", a_ndom, h->ndom);
-    if (!h->have_psi || !h->have_vloc) return fail(MLMD_ERR_STATE, "mlmd_propagate_split: call mlmd_set_orbitals and mlmd_set_vloc first");
-    // Taylor-4 acts on h_loc only; the normalised kick is stable for any dt |D|
+// Shared driver of mlmd_propagate (split = false) and mlmd_propagate_split (split = true).
+static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom, bool split) {
+    const char *fn = split ? "mlmd_propagate_split" : "mlmd_propagate";
+    if (!h) return fail(MLMD_ERR_ARG, "%s: NULL handle", fn);
+    if (nsteps < 0 || !(dt == dt) || std::isinf(dt)) return fail(MLMD_ERR_ARG, "%s: nsteps=%d dt=%g", fn, nsteps, dt);
+    if (nsteps > 0 && !A) return fail(MLMD_ERR_ARG, "%s: A is NULL", fn);
+    if (a_ndom != 1 && a_ndom != h->ndom) return fail(MLMD_ERR_ARG, "%s: a_ndom=%d must be 1 or ndom=%d", fn, a_ndom, h->ndom);
+    if (!h->have_psi || !h->have_vloc) return fail(MLMD_ERR_STATE, "%s: call mlmd_set_orbitals and mlmd_set_vloc first", fn);
+    // a-priori stability bound of Taylor-4 (reading D14): dt * |lambda|max(H) <= 2 sqrt(2); in the split step the
+    // Taylor sum acts on h_loc only and the normalised kick is stable for any dt |D|
     bool yz = false;
     double bound = 0.0;
     for (size_t i = 0; i < (size_t)nsteps * a_ndom; ++i) {
         const double *a = A + 3 * i;
         if (!std::isfinite(a[0]) || !std::isfinite(a[1]) || !std::isfinite(a[2]))
-            return fail(MLMD_ERR_NONFINITE, "mlmd_propagate_split: A[%zu] is not finite", i);
+            return fail(MLMD_ERR_NONFINITE, "%s: A[%zu] is not finite", fn, i);
         yz = yz || a[1] != 0.0 || a[2] != 0.0;
         const double b = (8.0 / 3.0) * (1 / (h->hx * h->hx) + 1 / (h->hy * h->hy) + 1 / (h->hz * h->hz)) +
                          1.3722 * (fabs(a[0]) / h->hx + fabs(a[1]) / h->hy + fabs(a[2]) / h->hz) +
-                         0.5 * (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) + h->vmax;
-        bound = std::max(bound, b);
-    }
-    h->field_yz = yz;
-    int nl = 0;
-    if (nsteps > 0 && h->nproj > 0) {
-        ProfScope ps(h, MLMD_K_NORM);
-        CU(launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->nrm_part(), h->nrm(0), &nl));
-    }
-    CU(cudaEventSynchronize(h->coef_uploaded));
-    for (int s0 = 0; s0 < nsteps; s0 += kCoefCapacity) {
-        const int ns = std::min(kCoefCapacity, nsteps - s0);
-        if (s0 > 0) CU(cudaStreamSynchronize(h->stream));
-        for (int s = 0; s < ns; ++s)
-            for (int d = 0; d < h->ndom; ++d)
-                fill_coef(h, A + ((size_t)(s0 + s) * a_ndom + (a_ndom == 1 ? 0 : d)) * 3, &h->coef_host[(size_t)s * h->ndom + d]);
-        CU(cudaMemcpyAsync(h->coef(), h->coef_host, (size_t)ns * h->ndom * sizeof(StepCoef), cudaMemcpyHostToDevice, h->stream));
-        CU(cudaEventRecord(h->coef_uploaded, h->stream));
-        for (int s = 0; s < ns; ++s) {
-            int rc = enqueue_split_step(h, h->coef() + (size_t)s * h->ndom, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr, dt, &nl);
-            if (rc) return rc;
-        }
-    }
-    h->launches += nl;
-    if (nsteps > 0) h->rho_valid = true;
-    if (h->flags & MLMD_CHECK_FINITE) {
-        int n2 = 0;
-        CU(launch_check_finite(h->stream, (const float *)h->psi(), (size_t)h->ndom * h->ngrid * h->ld * 2, h->flag(), &n2));
-        h->launches += n2;
-        CU(cudaMemcpyAsync(h->flag_host, h->flag(), sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-        CU(cudaStreamSynchronize(h->stream));
-        if (*h->flag_host) return fail(MLMD_ERR_NONFINITE, "mlmd_propagate_split: psi contains NaN/Inf after %d steps", nsteps);
-    }
-    if (dt * bound > 2.0 * sqrt(2.0)) {
-        fail(MLMD_WARN_UNSTABLE, "mlmd_propagate_split: dt*|h_loc|max bound = %.3f > 2 sqrt(2): Taylor-4 may be unstable", dt * bound);
-        return MLMD_WARN_UNSTABLE;
-    }
-    return MLMD_OK;
-}
-
-int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom) {
-    if (!h) return fail(MLMD_ERR_ARG, "mlmd_propagate: NULL handle");
-    if (nsteps < 0 || !(dt == dt) || std::isinf(dt)) return fail(MLMD_ERR_ARG, "mlmd_propagate: nsteps=%d dt=%g", nsteps, dt);
-    if (nsteps > 0 && !A) return fail(MLMD_ERR_ARG, "mlmd_propagate: A is NULL");
-    if (a_ndom != 1 && a_ndom != h->ndom) return fail(MLMD_ERR_ARG, "mlmd_propagate: a_ndom=%d must be 1 or ndom=%d", a_ndom, h->ndom);
-    if (!h->have_psi || !h->have_vloc) return fail(MLMD_ERR_STATE, "mlmd_propagate: call mlmd_set_orbitals and mlmd_set_vloc first");
-    // a-priori stability bound of Taylor-4 (reading D14): dt * |lambda|max(H) <= 2 sqrt(2)
-    bool yz = false;
-    double bound = 0.0;
-    for (size_t i = 0; i < (size_t)nsteps * a_ndom; ++i) {
-        const double *a = A + 3 * i;
-        if (!std::isfinite(a[0]) || !std::isfinite(a[1]) || !std::isfinite(a[2]))
-            return fail(MLMD_ERR_NONFINITE, "mlmd_propagate: A[%zu] is not finite", i);
-        yz = yz || a[1] != 0.0 || a[2] != 0.0;
-        const double b = (8.0 / 3.0) * (1 / (h->hx * h->hx) + 1 / (h->hy * h->hy) + 1 / (h->hz * h->hz)) +
-                         1.3722 * (fabs(a[0]) / h->hx + fabs(a[1]) / h->hy + fabs(a[2]) / h->hz) +
-                         0.5 * (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) + h->vmax + (h->nproj ? h->dmax : 0.0);
+                         0.5 * (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) + h->vmax + (h->nproj && !split ? h->dmax : 0.0);
         bound = std::max(bound, b);
     }
     h->field_yz = yz;
@@ -687,7 +638,14 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
     // into a CUDA graph that reads its stencil coefficients from a device slot.
     const bool want_graph = h->graph_allowed && !h->prof_on && nsteps >= 4 &&
                             (double)h->ndom * (double)h->ngrid * h->ld <= (double)(1 << 23);
-    if (h->gexec && (h->g_dt != dt || h->g_yz != yz)) drop_graph(h);
+    if (h->gexec && (h->g_dt != dt || h->g_yz != yz || h->g_split != split)) drop_graph(h);
+    auto one_step = [&](const StepCoef *coef, const StepCoef *coef_host) {
+        return split ? enqueue_split_step(h, coef, coef_host, dt, &nl) : enqueue_step(h, coef, coef_host, dt, &nl);
+    };
+    if (split && nsteps > 0 && h->nproj > 0) {      // squared norms of the incoming orbitals (reading D27)
+        ProfScope ps(h, MLMD_K_NORM);
+        CU(launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->nrm_part(), h->nrm(0), &nl));
+    }
     CU(cudaEventSynchronize(h->coef_uploaded));   // an earlier call's upload has left the pinned staging buffer
     for (int s0 = 0; s0 < nsteps; s0 += kCoefCapacity) {
         const int ns = std::min(kCoefCapacity, nsteps - s0);
@@ -701,10 +659,10 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
         if (want_graph) {
             if (!h->gexec) {
                 // one eager step first: it also sets the per-function attributes, which must not happen in a capture
-                int rc = enqueue_step(h, h->coef(), a_ndom == 1 ? &h->coef_host[0] : nullptr, dt, &nl);
+                int rc = one_step(h->coef(), a_ndom == 1 ? &h->coef_host[0] : nullptr);
                 if (rc) return rc;
                 s = 1;
-                rc = capture_step(h, dt, yz);
+                rc = capture_step(h, dt, yz, split);
                 if (rc) return rc;
             }
             if (h->gexec && s < ns) {
@@ -720,7 +678,7 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
             }
         }
         for (; s < ns; ++s) {
-            int rc = enqueue_step(h, h->coef() + (size_t)s * h->ndom, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr, dt, &nl);
+            int rc = one_step(h->coef() + (size_t)s * h->ndom, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr);
             if (rc) return rc;
         }
     }
@@ -732,13 +690,21 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
         h->launches += n2;
         CU(cudaMemcpyAsync(h->flag_host, h->flag(), sizeof(int), cudaMemcpyDeviceToHost, h->stream));
         CU(cudaStreamSynchronize(h->stream));
-        if (*h->flag_host) return fail(MLMD_ERR_NONFINITE, "mlmd_propagate: psi contains NaN/Inf after %d steps", nsteps);
+        if (*h->flag_host) return fail(MLMD_ERR_NONFINITE, "%s: psi contains NaN/Inf after %d steps", fn, nsteps);
     }
     if (dt * bound > 2.0 * sqrt(2.0)) {
-        fail(MLMD_WARN_UNSTABLE, "mlmd_propagate: dt*|H|max bound = %.3f > 2 sqrt(2): Taylor-4 may be unstable", dt * bound);
+        fail(MLMD_WARN_UNSTABLE, "%s: dt*|%s|max bound = %.3f > 2 sqrt(2): Taylor-4 may be unstable", fn, split ? "h_loc" : "H", dt * bound);
         return MLMD_WARN_UNSTABLE;
     }
     return MLMD_OK;
+}
+
+int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom) {
+    return propagate_impl(h, nsteps, dt, A, a_ndom, false);
+}
+
+int mlmd_propagate_split(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom) {
+    return propagate_impl(h, nsteps, dt, A, a_ndom, true);
 }
 
 int mlmd_density(mlmd_domain_t *h, float *rho, int where) {

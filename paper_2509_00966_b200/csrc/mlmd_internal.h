@@ -72,6 +72,7 @@ struct mlmd_domain {
     int g_launches;             // kernels per graph launch
     double g_dt;                // the step size the graph was captured with
     bool g_yz;
+    bool g_split;               // the graph holds the Eq. (2) split step, not the Taylor-4 step
     int *flag_host;             // pinned
     // typed views
     float2 *psi() const { return (float2 *)(ws + off.psi); }

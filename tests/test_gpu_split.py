@@ -158,3 +158,22 @@ def test_occupations_and_excited_electrons_after_the_pulse():
     with pytest.raises(M.MlmdError):
         dom.occupations()                                                         # no Psi(0) snapshot
     dom.close()
+
+
+def test_split_cuda_graph_equals_eager_launches(monkeypatch):
+    """Small batches replay a CUDA graph of the split step too; switching between the two steppers on one handle
+    re-captures.  Same bits as the eager launches."""
+    c = W.get_config(0, ndom=2, nsteps=9)
+    d = W.generate(c)
+    rng = np.random.default_rng(12)
+    A = 0.05 * rng.standard_normal((9, 2, 3))
+    outs = []
+    for flag in ("1", "0"):
+        monkeypatch.setenv("MLMD_GRAPH", flag)
+        dom = make_domain(c, d)
+        dom.propagate_split(9, c.dt, A)
+        dom.propagate(6, c.dt, A[:6])
+        dom.propagate_split(5, c.dt, A[:5])
+        outs.append((dom.get_orbitals(), dom.density()))
+        dom.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
