@@ -108,7 +108,7 @@ def ncu_traffic(c, kernel_class):
         return None
     with open(path) as f:
         t = json.load(f)["dram_bytes_per_launch"]
-    pick = {"stencil": ["stencil_tma_kernel<0, 0>"], "proj": ["proj_tc_kernel"], "back": ["back2_tc_kernel", "back_tc_kernel"],
+    pick = {"stencil": ["stencil_tma_kernel<0, 0, 0>"], "proj": ["proj_tc_kernel"], "back": ["back2_tc_kernel", "back_tc_kernel"],
             "density": ["density_kernel"]}.get(kernel_class, [])
     for name in pick:
         if name in t:
