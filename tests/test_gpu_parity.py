@@ -336,3 +336,27 @@ def test_cuda_graph_step_equals_eager_launches(monkeypatch):
         dom.close()
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
     assert launches[0] > launches[1]            # + the coefficient-slot kernels of the graph
+
+
+def test_long_call_crosses_coefficient_upload_chunks(monkeypatch):
+    """One mlmd_propagate call of 600 steps (N_QD ~ 10^3 per MD step): the per-step coefficients are
+    uploaded in chunks of 256 steps, so the call crosses two chunk boundaries, with and without the CUDA graph; the
+    field changes every step and differs per domain.  Against the oracle, and graph == eager bit for bit."""
+    from oracle import ref
+    c = W.get_config(0, ndom=2, nsteps=600)
+    d = W.generate(c)
+    rng = np.random.default_rng(13)
+    t = np.arange(600)[:, None, None] * c.dt
+    A = 0.05 * np.sin(0.7 * t + rng.uniform(0, 6, (1, 2, 3)))
+    outs = []
+    for flag in ("1", "0"):
+        monkeypatch.setenv("MLMD_GRAPH", flag)
+        dom = make_domain(c, d)
+        dom.propagate(600, c.dt, A)
+        outs.append((dom.get_orbitals(), dom.density()))
+        dom.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    r, rho_ref = ref.propagate(d["psi"], d["occ"], d["vloc"], d["beta"], d["D"], A, c.dt, c.h)
+    e, er = orb_err(outs[0][0], r), rho_err(outs[0][1], rho_ref)
+    print("600 steps:", e, er)
+    assert e <= TOL_LAST and er <= TOL_RHO
