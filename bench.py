@@ -31,6 +31,7 @@ PAPER_CONTEXT = {
     "note": "PAPER.md L38-39, L298, L302: Aurora, 1,024-orbital domains of unstated mesh size; context only",
 }
 MODE_NAMES = {"fp32grade": 0, "fp64": 1, "bf16": 2, "tf32x1": 3, "simt": 4}
+CPU_STEPS = 8            # timed oracle steps of the cpu_baseline leg
 STEP_NAMES = {"taylor": "Taylor-4 (full H, north_star)", "split": "Eq. (2) split (half-kick, Taylor-4 of h_loc, half-kick)"}
 # tensor peak as a multiple of the measured dense BF16 peak (B200_PROFILING.md nominal ratios:
 # tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
@@ -379,11 +380,12 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
-        s = sample_for_oracle(c, first, args.oracle_orbitals)
-        v, sec_step, cores, el = time_oracle(c, s, A, steps=2, warmup=1, step=args.step)
+        # a bounded sample sized for roughly 10 s of host work at configs[3] (1 warm-up + CPU_STEPS timed steps)
+        s = sample_for_oracle(c, first, 2 * args.oracle_orbitals)
+        v, sec_step, cores, el = time_oracle(c, s, W.laser_samples(c, nsteps=CPU_STEPS, t0=0.9), steps=CPU_STEPS, warmup=1, step=args.step)
         cpu = {"value": v, "unit": "electron-steps/s", "cores": cores, "kind": "oracle", "s_per_step": sec_step,
-               "sample": "domain 0, first %d of %d orbitals (%g electrons), all %d projectors, 2 timed %s steps" % (
-                   s["psi"].shape[-1], c.norb, el, c.nproj, "Eq. (2) split" if args.step == "split" else "Taylor-4")}
+               "sample": "domain 0, first %d of %d orbitals (%g electrons), all %d projectors, %d timed %s steps" % (
+                   s["psi"].shape[-1], c.norb, el, c.nproj, CPU_STEPS, "Eq. (2) split" if args.step == "split" else "Taylor-4")}
 
     line = {
         "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,
