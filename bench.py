@@ -373,9 +373,12 @@ def main():
     t_tc = alg["gemm_flops_step"] / (tensor_peak_sus * 1e12) * 1e3
     t_roof = max(t_hbm, t_tc)
     step_roof = {"t_hbm_ms": t_hbm, "t_tensor_ms": t_tc, "t_roof_ms": t_roof, "bound": "tensor" if t_tc > t_hbm else "hbm",
-                 "frac": t_roof / (ms / K), "tensor_peak_tflops": tensor_peak_sus, "tensor_peak_burst_tflops": tensor_peak_burst,
+                 "frac": t_roof / (ms / K), "t_sum_ms": t_hbm + t_tc, "frac_of_sum": (t_hbm + t_tc) / (ms / K),
+                 "tensor_peak_tflops": tensor_peak_sus, "tensor_peak_burst_tflops": tensor_peak_burst,
                  "hbm_peak_gbs": peaks["hbm_gbs"], "bytes_step": alg["bytes_step"], "gemm_flops_step": alg["gemm_flops_step"],
-                 "definition": "max(stencil+density%s bytes / HBM peak, real-beta GEMM flops / tensor peak of the GEMM mode)" % (
+                 "definition": "max(stencil+density%s bytes / HBM peak, real-beta GEMM flops / tensor peak of the GEMM mode); "
+                               "t_sum / frac_of_sum: the same two terms added, the bound for kernels that do not overlap "
+                               "(at the power cap overlap buys little: DESIGN.md section 8)" % (
                      "+norm" if args.step == "split" else "")}
 
     cpu = None
