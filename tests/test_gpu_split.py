@@ -177,3 +177,36 @@ def test_split_cuda_graph_equals_eager_launches(monkeypatch):
         outs.append((dom.get_orbitals(), dom.density()))
         dom.close()
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+def test_split_scissor_form_of_eq5():
+    """PAPER.md Eq. (5): the nonlocal correction delta Psi(0) Psi^H(0) Psi(t).  With beta = Psi(0) (complex,
+    one projector per orbital) and D_p = the scissor shift, the half-kick is exactly that with delta = -i dt/2 D dv;
+    config 1 (64 orbitals -> 128 real projector rows on the tensor-core path), 5 steps, plus the occupations."""
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    c = W.get_config(1)
+    d = W.generate(c)
+    beta = np.ascontiguousarray(d["psi"].reshape(c.ndom, c.ngrid, c.norb))          # Psi(0), complex64
+    D = np.full((c.ndom, c.norb), 0.35)                                              # scissor shift (Hartree)
+    dom = M.Domain(c.ndom, c.grid, c.h, c.norb, 2 * c.norb, flags=M.KEEP_PSI0)
+    dom.set_vloc(d["vloc"])
+    dom.set_orbitals(d["psi"], d["occ"])
+    dom.set_projectors(beta, D)
+    assert M.lib().mlmd_gemm_path(dom.handle) == 1
+    dom.propagate_split(5, c.dt, d["A"][:5])
+    r, rho_ref = ref.propagate_split(d["psi"], d["occ"], d["vloc"], beta, D, d["A"][:5], c.dt, c.h)
+    assert orb_err(dom.get_orbitals(), r) <= TOL_LAST and rho_err(dom.density(), rho_ref) <= TOL_RHO
+    f, nexc = dom.occupations()
+    f_ref, n_ref = ref.occupations(ref.overlap(d["psi"], r, c.dv), d["occ"])
+    assert np.abs(f - f_ref).max() <= 1e-4 and np.abs(nexc - n_ref).max() <= 1e-5 * d["occ"].sum()
+    # one kick alone against the literal formula: psi + delta Psi(0) (Psi^H(0) psi), then per-orbital renormalisation
+    x = d["psi"].reshape(c.ngrid, c.norb).astype(np.complex128)
+    delta = -0.5j * c.dt * 0.35 * c.dv
+    y = x + delta * (x @ (x.conj().T @ x))
+    y *= (np.linalg.norm(x, axis=0) / np.linalg.norm(y, axis=0))[None, :]
+    k, _ = ref.propagate_split(d["psi"], d["occ"], d["vloc"], beta, D, d["A"][:1], c.dt, c.h, nsteps=1, kick_only=True)
+    y2 = y + delta * (x @ (x.conj().T @ y))
+    y2 *= (np.linalg.norm(y, axis=0) / np.linalg.norm(y2, axis=0))[None, :]
+    assert np.linalg.norm(k[0].reshape(c.ngrid, c.norb) - y2) <= 1e-12 * np.linalg.norm(y2)
+    dom.close()

@@ -181,3 +181,19 @@ def test_o3_occupations_from_the_oracles_own_overlap():
     f, nexc = ref.occupations(ref.overlap(psi0, psit, dv), np.array([[2.0, 0.0]]))
     assert np.allclose(f[0], [2 * np.cos(th) ** 2, 2 * np.sin(th) ** 2], atol=1e-13)
     assert abs(nexc[0] - 2 * np.sin(th) ** 2) < 1e-13
+
+
+def test_s6_scissor_kick_is_eq5():
+    """S6: with beta = Psi(0) and D_p = D the half-kick is PAPER.md Eq. (5), psi + delta Psi(0) Psi^H(0) psi with
+    delta = -i dt/2 D dv, followed by the per-orbital renormalisation of reading D27 (plain numpy matrices)."""
+    grid, h, dt, D = (5, 6, 5), (0.5, 0.4, 0.45), 0.05, 0.35
+    ngrid, dv = int(np.prod(grid)), float(np.prod(h))
+    x = rand_c(ngrid, 4)
+    delta = -0.5j * dt * D * dv
+    y = x
+    for _ in range(2):                                        # kick_only: the two half-kicks of one step
+        z = y + delta * (x @ (x.conj().T @ y))
+        y = z * (np.linalg.norm(y, axis=0) / np.linalg.norm(z, axis=0))[None, :]
+    out, _ = ref.propagate_split(x.reshape(1, *grid, 4), np.full((1, 4), 2.0), np.zeros((1, *grid)), x.reshape(1, ngrid, 4),
+                                 np.full((1, 4), D), np.zeros((1, 1, 3)), dt, h, kick_only=True)
+    assert rel(out[0].reshape(ngrid, 4), y) < 1e-13
