@@ -65,6 +65,11 @@ def test_argument_errors_without_gpu(M):
     assert L.mlmd_domain_create(ctypes.byref(h), 1, 16, 16, 3, 0.5, 0.5, 0.5, 8, 8, ctypes.c_void_p(256), 1 << 30, None, 0) == M.api.ERR_SHAPE
     assert L.mlmd_domain_destroy(None) == M.api.OK
     assert M.mlmd_launch_count(None) == 0
+    # the NEXT-row calls check their arguments before touching the device too
+    assert L.mlmd_propagate_split(None, 1, 0.02, None, 1) == M.api.ERR_ARG and b"mlmd_propagate_split" in L.mlmd_last_error()
+    assert L.mlmd_occupations(None, None, None, 0) == M.api.ERR_ARG
+    assert L.mlmd_energy_nl(None, None, 0) == M.api.ERR_ARG
+    assert L.mlmd_current(None, None, 1, None, 0) == M.api.ERR_ARG
 
 
 def test_product_does_not_import_oracle():
