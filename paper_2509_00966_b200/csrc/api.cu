@@ -88,6 +88,7 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.nrm_part = take((size_t)ndom * kNormSlabs * pl->ld * sizeof(double));
     w.scl = take((size_t)ndom * pl->ld * sizeof(float));
     w.avec = take((size_t)ndom * 3 * sizeof(double));
+    w.gram = take((size_t)ndom * pl->ldp_max * pl->ldp_max * sizeof(float));
     w.total = o;
     return true;
 }
@@ -144,6 +145,7 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
     h->coef_uploaded = nullptr; h->gexec = nullptr; h->gstream = nullptr; h->gfork = h->gjoin = nullptr;
     h->g_launches = 0; h->g_dt = 0.0; h->g_yz = false; h->g_split = false;
+    h->gram_valid = false; h->ldg = pl.ldp_max;
     {
         const char *g = getenv("MLMD_GRAPH");   // "0": never capture the step into a CUDA graph
         h->graph_allowed = !(g && g[0] == '0');
@@ -300,6 +302,7 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: NULL handle");
     if (nproj < 0) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: nproj=%d", nproj);
     drop_graph(h);
+    h->gram_valid = false;
     if (nproj == 0) {
         h->nproj = h->P = 0;
         h->dmax = 0.0;
@@ -599,7 +602,19 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), nl));
         return MLMD_OK;
     }
-    int rc = half_kick(3);
+    int rc;
+    if (h->gram_valid) {
+        // ||psi_c + beta W||^2 = ||psi_c||^2 + W^T (beta^T beta) W: no pass over psi for the norm after the second kick
+        rc = nonlocal_project(h, h->psi(), (float)(0.5 * dt), nl);
+        if (!rc) {
+            ProfScope ps(h, MLMD_K_GLUE);
+            CU(launch_kick_quad(h->stream, h->ndom, h->P, h->ldg, h->ld, h->prows, h->gram(), h->what(), h->what_lo(), h->nrm(2),
+                                h->nrm(3), nl));
+        }
+        if (!rc) rc = nonlocal_back(h, h->psi(), nl);
+    } else {
+        rc = half_kick(3);
+    }
     if (rc) return rc;
     {
         ProfScope ps(h, MLMD_K_GLUE);
@@ -642,6 +657,18 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
     auto one_step = [&](const StepCoef *coef, const StepCoef *coef_host) {
         return split ? enqueue_split_step(h, coef, coef_host, dt, &nl) : enqueue_step(h, coef, coef_host, dt, &nl);
     };
+    if (split && nsteps > 0 && h->nproj > 0 && !h->gram_valid && h->ldp <= 2 * h->ld && h->P <= 1024 &&
+        !(getenv("MLMD_KICK_IDENTITY") && atoi(getenv("MLMD_KICK_IDENTITY")) == 0)) {
+        // one-time per projector set: G = beta^T beta from two CUDA-core projections of beta (stored as hi + lo) onto
+        // its hi and its lo part (the zpart scratch holds [prows][ldp] partials per slice, ldp <= 2 ld)
+        ProfScope ps(h, MLMD_K_GLUE);
+        for (int part = 0; part < 2; ++part) {
+            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, part ? h->beta_lo() : h->beta(),
+                                h->ldp, h->ldp, h->zpart(), h->prows, h->nsplit, false, &nl));
+            CU(launch_gram_reduce(h->stream, h->ndom, h->P, h->ldg, h->prows, h->ldp, h->nsplit, h->zpart(), h->gram(), part, &nl));
+        }
+        h->gram_valid = true;
+    }
     if (split && nsteps > 0 && h->nproj > 0) {      // squared norms of the incoming orbitals (reading D27)
         ProfScope ps(h, MLMD_K_NORM);
         CU(launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->nrm_part(), h->nrm(0), &nl));

@@ -621,4 +621,78 @@ cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, do
     return cudaGetLastError();
 }
 
+// ---- split step: ||psi + beta W||^2 without a pass over psi ----
+// Static Gram matrix of the (real-embedded) projector rows, G[dom][p][q] = sum_r beta[r][p] beta[r][q], from the
+// split-K partials of a projection of beta onto itself: G (+)= sum_s zpart[dom][s][p][q].
+__global__ void gram_reduce_kernel(int P, int ldg, int prows, int N, int nsplit, const float *__restrict__ zpart,
+                                   float *__restrict__ G, int accumulate) {
+    const int qq = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.y, dom = blockIdx.z;
+    if (qq >= P) return;
+    const float *zp = zpart + ((size_t)dom * nsplit * prows + p) * N + qq;
+    float s = 0.f;
+    for (int k = 0; k < nsplit; ++k) s += zp[(size_t)k * prows * N];
+    float *g = G + ((size_t)dom * ldg + p) * ldg + qq;
+    *g = accumulate ? *g + s : s;
+}
+cudaError_t launch_gram_reduce(cudaStream_t st, int ndom, int P, int ldg, int prows, int N, int nsplit, const float *zpart,
+                               float *G, int accumulate, int *nlaunch) {
+    ++*nlaunch;
+    gram_reduce_kernel<<<dim3((P + 127) / 128, P, ndom), 128, 0, st>>>(P, ldg, prows, N, nsplit, zpart, G, accumulate);
+    return cudaGetLastError();
+}
+// nd[dom][n] = nc[dom][n] + sum_{c in {2n, 2n+1}} W[:, c]^T G W[:, c], W = what + what_lo ([prows][2 ld], rows < P).
+// The cross term 2 Re<psi|beta W> vanishes because W = -i tau D' beta^H psi with a Hermitian V_NL.
+// Block = (domain, 32 columns): the W tile [P x 32] sits in shared memory; thread = (column, one of 8 slices of p),
+// five rows of G per trip so that one shared-memory read of W feeds five FMAs; FP32 products, FP64 sums.
+constexpr int KQ_MAXP = 1024;   // rows of W a block can stage (dynamic shared memory: P * 128 B)
+__global__ void __launch_bounds__(256)
+kick_quad_kernel(int P, int ldg, int ld, int prows, const float *__restrict__ G, const float *__restrict__ what,
+                 const float *__restrict__ wlo, const double *__restrict__ nc, double *__restrict__ nd) {
+    extern __shared__ float Ws[];    // [P][32]
+    const int dom = blockIdx.y, lane = threadIdx.x % 32, c = blockIdx.x * 32 + lane, slice = threadIdx.x / 32;
+    const int N = 2 * ld;
+    const float *g = G + (size_t)dom * ldg * ldg;
+    const float *wh = what + (size_t)dom * prows * N + c, *wl = wlo + (size_t)dom * prows * N + c;
+    for (int p = slice; p < P; p += 8) Ws[p * 32 + lane] = wh[(size_t)p * N] + wl[(size_t)p * N];
+    __syncthreads();
+    double acc = 0.0;
+    for (int p0 = slice * 5; p0 < P; p0 += 40) {
+        float t[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+        const float *gr[5];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) gr[k] = g + (size_t)min(p0 + k, P - 1) * ldg;
+        for (int qq = 0; qq < P; ++qq) {
+            const float w = Ws[qq * 32 + lane];
+#pragma unroll
+            for (int k = 0; k < 5; ++k) t[k] = fmaf(__ldg(gr[k] + qq), w, t[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < 5; ++k)
+            if (p0 + k < P) acc += (double)Ws[(p0 + k) * 32 + lane] * (double)t[k];
+    }
+    __shared__ double red[8][32];
+    red[slice][lane] = acc;
+    __syncthreads();
+    if (threadIdx.x < 16) {             // orbital n = columns 2n, 2n+1
+        double s = 0.0;
+        for (int k = 0; k < 8; ++k) s += red[k][2 * threadIdx.x] + red[k][2 * threadIdx.x + 1];
+        const int n = blockIdx.x * 16 + threadIdx.x;
+        if (n < ld) nd[(size_t)dom * ld + n] = nc[(size_t)dom * ld + n] + s;
+    }
+}
+cudaError_t launch_kick_quad(cudaStream_t st, int ndom, int P, int ldg, int ld, int prows, const float *G, const float *what,
+                             const float *wlo, const double *nc, double *nd, int *nlaunch) {
+    ++*nlaunch;
+    if (P > KQ_MAXP) return cudaErrorInvalidValue;
+    static DeviceOnce attr_set;
+    if (!attr_set.done()) {
+        cudaError_t e = cudaFuncSetAttribute(kick_quad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, KQ_MAXP * 128);
+        if (e != cudaSuccess) return e;
+        attr_set.mark();
+    }
+    kick_quad_kernel<<<dim3(2 * ld / 32, ndom), 256, (size_t)P * 128, st>>>(P, ldg, ld, prows, G, what, wlo, nc, nd);
+    return cudaGetLastError();
+}
+
 }  // namespace mlmd

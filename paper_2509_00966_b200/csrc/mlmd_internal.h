@@ -24,7 +24,7 @@ static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
     size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
-        nrm, nrm_part, scl, avec, total;
+        nrm, nrm_part, scl, avec, gram, total;
 };
 
 constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
@@ -72,6 +72,8 @@ struct mlmd_domain {
     int g_launches;             // kernels per graph launch
     double g_dt;                // the step size the graph was captured with
     bool g_yz;
+    bool gram_valid;            // gram() matches the current projectors
+    int ldg;                    // pitch of gram() = ldp_max
     bool g_split;               // the graph holds the Eq. (2) split step, not the Taylor-4 step
     int *flag_host;             // pinned
     // typed views
@@ -98,6 +100,7 @@ struct mlmd_domain {
     double *nrm_part() const { return (double *)(ws + off.nrm_part); }
     float *scl() const { return (float *)(ws + off.scl); }
     double *avec() const { return (double *)(ws + off.avec); }   // mlmd_current: A[a_ndom][3]
+    float *gram() const { return (float *)(ws + off.gram); }      // split step: beta^T beta, [ndom][ldp_max][ldp_max]
 };
 
 namespace mlmd {
@@ -195,6 +198,10 @@ cudaError_t launch_energy_nl(cudaStream_t st, int ndom, int nproj, int beta_comp
 cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int ld,
                            const float2 *psi, const float *occ, const double *A_dev, int a_ndom, double *part,
                            size_t part_doubles, double *J, int *nlaunch);
+cudaError_t launch_gram_reduce(cudaStream_t st, int ndom, int P, int ldg, int prows, int N, int nsplit, const float *zpart,
+                               float *G, int accumulate, int *nlaunch);
+cudaError_t launch_kick_quad(cudaStream_t st, int ndom, int P, int ldg, int ld, int prows, const float *G, const float *what,
+                             const float *wlo, const double *nc, double *nd, int *nlaunch);
 cudaError_t launch_occupations(cudaStream_t st, int ndom, int norb, int ld, const float2 *S, const float *occ, double *f,
                                double *nexc, int *nlaunch);
 cudaError_t launch_scale_density(cudaStream_t st, int ndom, long ngrid, int ld, float2 *psi, const float *scl,
