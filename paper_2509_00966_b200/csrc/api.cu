@@ -87,6 +87,7 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.nrm = take((size_t)4 * ndom * pl->ld * sizeof(double));
     w.nrm_part = take((size_t)ndom * kNormSlabs * pl->ld * sizeof(double));
     w.scl = take((size_t)ndom * pl->ld * sizeof(float));
+    w.occ_eff = take((size_t)ndom * pl->ld * sizeof(float));
     w.avec = take((size_t)ndom * 3 * sizeof(double));
     w.gram = take((size_t)ndom * pl->ldp_max * pl->ldp_max * sizeof(float));
     w.total = o;
@@ -145,7 +146,7 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
     h->coef_uploaded = nullptr; h->gexec = nullptr; h->gstream = nullptr; h->gfork = h->gjoin = nullptr;
     h->g_launches = 0; h->g_dt = 0.0; h->g_yz = false; h->g_split = false;
-    h->gram_valid = false; h->ldg = pl.ldp_max;
+    h->gram_valid = false; h->ldg = pl.ldp_max; h->split_pending = false;
     {
         const char *g = getenv("MLMD_GRAPH");   // "0": never capture the step into a CUDA graph
         h->graph_allowed = !(g && g[0] == '0');
@@ -520,7 +521,7 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
     return MLMD_OK;
 }
 
-static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, int *nl);
+static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, bool last, int *nl);
 
 // Capture one step (coefficients taken from the device slot that advance_coef refills) into h->gexec.
 static int capture_step(mlmd_domain *h, double dt, bool yz, bool split) {
@@ -536,7 +537,7 @@ static int capture_step(mlmd_domain *h, double dt, bool yz, bool split) {
     h->stream = h->gstream;
     cudaError_t e = launch_advance_coef(h->gstream, h->coef(), h->coef_cur(), h->step_counter(), h->ndom, &nl);
     int rc = e != cudaSuccess ? MLMD_ERR_CUDA
-             : split ? enqueue_split_step(h, h->coef_cur(), nullptr, dt, &nl) : enqueue_step(h, h->coef_cur(), nullptr, dt, &nl);
+             : split ? enqueue_split_step(h, h->coef_cur(), nullptr, dt, false, &nl) : enqueue_step(h, h->coef_cur(), nullptr, dt, &nl);
     h->stream = user;
     cudaError_t e2 = cudaStreamEndCapture(h->gstream, &graph);
     if (rc || e != cudaSuccess || e2 != cudaSuccess || !graph) {
@@ -564,7 +565,7 @@ static int capture_step(mlmd_domain *h, double dt, bool yz, bool split) {
 // nonlocal half-kick, Taylor-4 of h_loc alone, half-kick.  The chain runs un-normalised (a per-orbital scale
 // commutes with every operator in it); the four squared norms give the two kick scales, which are applied in
 // the pass that also computes the density.
-static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, int *nl) {
+static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, bool last, int *nl) {
     const bool kicks = h->nproj > 0;
     auto norm2 = [&](int which) -> int {
         ProfScope ps(h, MLMD_K_NORM);
@@ -620,8 +621,30 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         ProfScope ps(h, MLMD_K_GLUE);
         CU(launch_kick_scale(h->stream, h->ndom * h->ld, h->nrm(0), h->nrm(1), h->nrm(2), h->nrm(3), h->scl(), nl));
     }
+    if (last) {
+        ProfScope ps(h, MLMD_K_DENSITY);
+        CU(launch_scale_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->scl(), h->occ(), h->rho(), nl));
+        h->split_pending = false;
+        return MLMD_OK;
+    }
+    // Not the last step of the call: psi stays un-normalised in memory (the next step's scale is expressed through the
+    // carried true norms nrm(0), so nothing accumulates) and the density takes the scale through the occupations.
+    {
+        ProfScope ps(h, MLMD_K_GLUE);
+        CU(launch_occ_eff(h->stream, h->ndom * h->ld, h->occ(), h->scl(), h->occ_eff(), nl));
+    }
+    ProfScope ps(h, MLMD_K_DENSITY);
+    CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ_eff(), h->rho(), nl));
+    h->split_pending = true;
+    return MLMD_OK;
+}
+
+// psi <- scl * psi (and rho from the scaled values) when a call ended on a deferred scale
+static int flush_split_scale(mlmd_domain *h, int *nl) {
+    if (!h->split_pending) return MLMD_OK;
     ProfScope ps(h, MLMD_K_DENSITY);
     CU(launch_scale_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->scl(), h->occ(), h->rho(), nl));
+    h->split_pending = false;
     return MLMD_OK;
 }
 
@@ -654,9 +677,13 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
     const bool want_graph = h->graph_allowed && !h->prof_on && nsteps >= 4 &&
                             (double)h->ndom * (double)h->ngrid * h->ld <= (double)(1 << 23);
     if (h->gexec && (h->g_dt != dt || h->g_yz != yz || h->g_split != split)) drop_graph(h);
-    auto one_step = [&](const StepCoef *coef, const StepCoef *coef_host) {
-        return split ? enqueue_split_step(h, coef, coef_host, dt, &nl) : enqueue_step(h, coef, coef_host, dt, &nl);
+    auto one_step = [&](const StepCoef *coef, const StepCoef *coef_host, bool last) {
+        return split ? enqueue_split_step(h, coef, coef_host, dt, last, &nl) : enqueue_step(h, coef, coef_host, dt, &nl);
     };
+    {
+        int rc = flush_split_scale(h, &nl);      // only after a split call that failed half-way
+        if (rc) return rc;
+    }
     if (split && nsteps > 0 && h->nproj > 0 && !h->gram_valid && h->ldp <= 2 * h->ld && h->P <= 1024 &&
         !(getenv("MLMD_KICK_IDENTITY") && atoi(getenv("MLMD_KICK_IDENTITY")) == 0)) {
         // one-time per projector set: G = beta^T beta from two CUDA-core projections of beta (stored as hi + lo) onto
@@ -686,7 +713,7 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
         if (want_graph) {
             if (!h->gexec) {
                 // one eager step first: it also sets the per-function attributes, which must not happen in a capture
-                int rc = one_step(h->coef(), a_ndom == 1 ? &h->coef_host[0] : nullptr);
+                int rc = one_step(h->coef(), a_ndom == 1 ? &h->coef_host[0] : nullptr, false);
                 if (rc) return rc;
                 s = 1;
                 rc = capture_step(h, dt, yz, split);
@@ -702,12 +729,18 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
                 }
                 CU(cudaEventRecord(h->gjoin, h->gstream));
                 CU(cudaStreamWaitEvent(h->stream, h->gjoin, 0));
+                if (split && h->nproj > 0) h->split_pending = true;   // every replayed split step defers its scale
             }
         }
         for (; s < ns; ++s) {
-            int rc = one_step(h->coef() + (size_t)s * h->ndom, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr);
+            int rc = one_step(h->coef() + (size_t)s * h->ndom, a_ndom == 1 ? &h->coef_host[(size_t)s * h->ndom] : nullptr,
+                              s0 + s == nsteps - 1);
             if (rc) return rc;
         }
+    }
+    {
+        int rc = flush_split_scale(h, &nl);      // graph replays end on a deferred scale
+        if (rc) return rc;
     }
     h->launches += nl;
     if (nsteps > 0) h->rho_valid = true;

@@ -695,4 +695,15 @@ cudaError_t launch_kick_quad(cudaStream_t st, int ndom, int P, int ldg, int ld, 
     return cudaGetLastError();
 }
 
+// occ_eff[i] = occ[i] * scl[i]^2: the density of the true (normalised) orbitals from the un-normalised ones in memory
+__global__ void occ_eff_kernel(int n, const float *__restrict__ occ, const float *__restrict__ scl, float *__restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = occ[i] * scl[i] * scl[i];
+}
+cudaError_t launch_occ_eff(cudaStream_t st, int n, const float *occ, const float *scl, float *out, int *nlaunch) {
+    ++*nlaunch;
+    occ_eff_kernel<<<(n + 127) / 128, 128, 0, st>>>(n, occ, scl, out);
+    return cudaGetLastError();
+}
+
 }  // namespace mlmd

@@ -24,7 +24,7 @@ static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
     size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
-        nrm, nrm_part, scl, avec, gram, total;
+        nrm, nrm_part, scl, occ_eff, avec, gram, total;
 };
 
 constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
@@ -73,6 +73,7 @@ struct mlmd_domain {
     double g_dt;                // the step size the graph was captured with
     bool g_yz;
     bool gram_valid;            // gram() matches the current projectors
+    bool split_pending;         // psi in memory is the un-normalised chain of the split step; true psi = scl() * psi
     int ldg;                    // pitch of gram() = ldp_max
     bool g_split;               // the graph holds the Eq. (2) split step, not the Taylor-4 step
     int *flag_host;             // pinned
@@ -99,6 +100,7 @@ struct mlmd_domain {
     double *nrm(int which) const { return (double *)(ws + off.nrm) + (size_t)which * ndom * ld; }
     double *nrm_part() const { return (double *)(ws + off.nrm_part); }
     float *scl() const { return (float *)(ws + off.scl); }
+    float *occ_eff() const { return (float *)(ws + off.occ_eff); }
     double *avec() const { return (double *)(ws + off.avec); }   // mlmd_current: A[a_ndom][3]
     float *gram() const { return (float *)(ws + off.gram); }      // split step: beta^T beta, [ndom][ldp_max][ldp_max]
 };
@@ -202,6 +204,7 @@ cudaError_t launch_gram_reduce(cudaStream_t st, int ndom, int P, int ldg, int pr
                                float *G, int accumulate, int *nlaunch);
 cudaError_t launch_kick_quad(cudaStream_t st, int ndom, int P, int ldg, int ld, int prows, const float *G, const float *what,
                              const float *wlo, const double *nc, double *nd, int *nlaunch);
+cudaError_t launch_occ_eff(cudaStream_t st, int n, const float *occ, const float *scl, float *out, int *nlaunch);
 cudaError_t launch_occupations(cudaStream_t st, int ndom, int norb, int ld, const float2 *S, const float *occ, double *f,
                                double *nexc, int *nlaunch);
 cudaError_t launch_scale_density(cudaStream_t st, int ndom, long ngrid, int ld, float2 *psi, const float *scl,
