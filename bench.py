@@ -89,11 +89,12 @@ def algorithmic(c, gemm_real=True, step="taylor"):
     """Algorithmic bytes and flops per step of the whole batch.  step="split" (the literal
     Eq. (2) step, mlmd_propagate_split): two V_NL applications instead of four, no per-step norm pass (two
     norms ride on stencil passes, the third comes from the projector Gram matrix; one 8 B/element pass per
-    CALL for the incoming norms is not counted) and the density pass also rescales psi (16 B per element)."""
+    CALL for the incoming norms and one 16 B/element rescaling pass per CALL are not counted: inside a call psi stays
+    un-normalised and the density takes the scale through the occupations)."""
     elems = c.ndom * c.ngrid * c.norb
     stage_bytes = [16, 24, 24, 24]
     split = step == "split"
-    density_b, norm_b, ngemm = (16, 0, 4) if split else (8, 0, 8)
+    density_b, norm_b, ngemm = (8, 0, 4) if split else (8, 0, 8)
     bytes_step = elems * (sum(stage_bytes) + density_b + norm_b) + c.ndom * c.ngrid * (4 * 4 + 4)
     gemm_flops_each = (2 if gemm_real else 4) * 2.0 * c.ndom * c.ngrid * c.nproj * c.norb   # one GEMM batch
     return {"elems": elems, "bytes_step": bytes_step, "stencil_bytes": [elems * b for b in stage_bytes],
