@@ -210,3 +210,30 @@ def test_split_scissor_form_of_eq5():
     y2 *= (np.linalg.norm(y, axis=0) / np.linalg.norm(y2, axis=0))[None, :]
     assert np.linalg.norm(k[0].reshape(c.ngrid, c.norb) - y2) <= 1e-12 * np.linalg.norm(y2)
     dom.close()
+
+
+def test_split_more_projector_rows_than_orbital_columns(monkeypatch):
+    """ldp > 2 ld: the Gram-matrix identity for the norm after the second kick does not apply (its scratch is sized by
+    the psi columns), so the per-step norm pass runs; also forced on a normal shape with MLMD_KICK_IDENTITY=0."""
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    rng = np.random.default_rng(5)
+    for grid, norb, nproj, env in (((8, 8, 8), 2, 40, None), ((16, 16, 16), 6, 5, "0")):
+        if env is not None:
+            monkeypatch.setenv("MLMD_KICK_IDENTITY", env)
+        ndom, h, dt, nsteps = 2, (0.5, 0.45, 0.4), 0.02, 4
+        ngrid = int(np.prod(grid))
+        psi = (rng.standard_normal((ndom, *grid, norb)) + 1j * rng.standard_normal((ndom, *grid, norb))).astype(np.complex64)
+        occ = rng.uniform(0, 2, (ndom, norb))
+        vloc = rng.uniform(-1, 0.5, (ndom, *grid)).astype(np.float32)
+        beta = (0.3 * rng.standard_normal((ndom, ngrid, nproj))).astype(np.float32)
+        D = rng.uniform(-2, 2, (ndom, nproj))
+        A = rng.uniform(-0.2, 0.2, (nsteps, 1, 3))
+        dom = M.Domain(ndom, grid, h, norb, nproj)
+        dom.set_vloc(vloc)
+        dom.set_orbitals(psi, occ)
+        dom.set_projectors(beta, D)
+        dom.propagate_split(nsteps, dt, A)
+        r, rho_ref = ref.propagate_split(psi, occ, vloc, beta, D, A, dt, h)
+        assert orb_err(dom.get_orbitals(), r) <= TOL_LAST and rho_err(dom.density(), rho_ref) <= TOL_RHO
+        dom.close()
