@@ -360,3 +360,44 @@ def test_long_call_crosses_coefficient_upload_chunks(monkeypatch):
     e, er = orb_err(outs[0][0], r), rho_err(outs[0][1], rho_ref)
     print("600 steps:", e, er)
     assert e <= TOL_LAST and er <= TOL_RHO
+
+
+def test_degenerate_cases_zero_steps_zero_dt_single_orbital_minimal_grid():
+    """Empty and degenerate inputs: nsteps = 0 is a no-op that still serves the density; dt = 0 returns psi bit for bit
+    (both steppers); one orbital (15 of the 16 padded columns empty) on the smallest legal grid (5 points per axis)
+    with one projector; zero occupations give zero density."""
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    c = W.get_config(0)
+    d = W.generate(c)
+    dom = make_domain(c, d)
+    assert dom.propagate(0, c.dt, None) == M.OK and dom.propagate_split(0, c.dt, None) == M.OK
+    assert np.array_equal(dom.get_orbitals(), d["psi"])
+    assert rho_err(dom.density(), ref.density(d["psi"], d["occ"])) <= 1e-6
+    dom.propagate(2, 0.0, d["A"][:2])
+    assert np.array_equal(dom.get_orbitals(), d["psi"])
+    dom.propagate_split(2, 0.0, d["A"][:2])
+    assert orb_err(dom.get_orbitals(), d["psi"].astype(np.complex128)) <= 2e-7      # the kick renormalises: one rounding
+    dom.close()
+    rng = np.random.default_rng(3)
+    grid, h, dt = (5, 5, 5), (0.6, 0.5, 0.55), 0.02
+    psi = (rng.standard_normal((2, *grid, 1)) + 1j * rng.standard_normal((2, *grid, 1))).astype(np.complex64)
+    vloc = rng.uniform(-1, 0.5, (2, *grid)).astype(np.float32)
+    beta = rng.standard_normal((2, 125, 1)).astype(np.float32)
+    D = np.array([[0.7], [-1.2]])
+    A = rng.uniform(-0.2, 0.2, (3, 2, 3))
+    for occ in (np.array([[2.0], [1.0]]), np.zeros((2, 1))):
+        for split in (False, True):
+            dom = M.Domain(2, grid, h, 1, 1)
+            dom.set_vloc(vloc)
+            dom.set_orbitals(psi, occ)
+            dom.set_projectors(beta, D)
+            (dom.propagate_split if split else dom.propagate)(3, dt, A)
+            r, rho_ref = (ref.propagate_split if split else ref.propagate)(psi, occ, vloc, beta, D, A, dt, h)
+            assert orb_err(dom.get_orbitals(), r) <= TOL_LAST
+            rho = dom.density()
+            if occ.any():
+                assert rho_err(rho, rho_ref) <= TOL_RHO
+            else:
+                assert not rho.any()
+            dom.close()
