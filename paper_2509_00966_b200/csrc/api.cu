@@ -258,6 +258,7 @@ int mlmd_set_orbitals(mlmd_domain_t *h, const void *psi, const double *occ, int 
     if (where == MLMD_HOST) CU(cudaStreamSynchronize(h->stream));
     h->have_psi = true;
     h->rho_valid = false;
+    h->split_pending = false;   // a scale left over from a failed split call belongs to the old orbitals
     return MLMD_OK;
 }
 
