@@ -30,14 +30,17 @@ PAPER_CONTEXT = {
     "t2s_s_per_electron_step": 1.11e-7, "sustained_eflops": 1.87, "gpus": 60000,
     "note": "PAPER.md L38-39, L298, L302: Aurora, 1,024-orbital domains of unstated mesh size; context only",
 }
-MODE_NAMES = {"fp32grade": 0, "fp64": 1, "bf16": 2, "tf32x1": 3, "simt": 4}
+MODE_NAMES = {"fp32grade": 0, "fp64": 1, "bf16": 2, "tf32x1": 3, "simt": 4, "staged": 5}
 CPU_STEPS = 8            # timed oracle steps of the cpu_baseline leg
 STEP_NAMES = {"taylor": "Taylor-4 (full H, north_star)", "split": "Eq. (2) split (half-kick, Taylor-4 of h_loc, half-kick)"}
 # tensor peak as a multiple of the measured dense BF16 peak (B200_PROFILING.md nominal ratios:
 # tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
 # the opt-in BF16-operand mode issues its single product on the TF32 pipe (BF16 values are TF32 values)
 TF32_OVER_BF16 = 1.1 / 2.25     # nominal dense peaks (B200_PROFILING.md): tf32 1.1 PF, bf16 2.25 PF
-TENSOR_RATIO = {"fp32grade": TF32_OVER_BF16 / 3.0, "tf32x1": TF32_OVER_BF16, "bf16": TF32_OVER_BF16}
+# "staged" (MLMD_GEMM_FP32GRADE_STAGED, Taylor step): of the 8 GEMMs of a step the outer 4 issue 3 products per MAC, the
+# inner projections 1 and the inner back-applications 2: (4 x 3 + 2 x 1 + 2 x 2) / 8 = 2.25 products on average
+TENSOR_RATIO = {"fp32grade": TF32_OVER_BF16 / 3.0, "tf32x1": TF32_OVER_BF16, "bf16": TF32_OVER_BF16,
+                "staged": TF32_OVER_BF16 / 2.25}
 FP32_ALU_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FMA lanes x 2 flop x max SM clock
 FP64_ALU_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12    # nominal 64 DFMA lanes per SM (guide: ~40 TF)
 
@@ -340,6 +343,8 @@ def main():
 
     # ---- roofline of the dominant kernel class and of the whole step
     mode = args.gemm_mode
+    if mode == "staged" and args.step == "split":
+        mode = "fp32grade"      # the staged mode only changes mlmd_propagate's inner Horner stages
     tensor_peak_sus = peaks["bf16_sustained"] * TENSOR_RATIO.get(mode, TENSOR_RATIO["fp32grade"])
     tensor_peak_burst = peaks["bf16_burst"] * TENSOR_RATIO.get(mode, TENSOR_RATIO["fp32grade"])
     per_class = {}

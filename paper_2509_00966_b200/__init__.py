@@ -31,7 +31,7 @@ from .api import (  # noqa: F401
     mlmd_last_error,
     EXPORTED_SYMBOLS,
     HOST, DEVICE, BETA_REAL32, BETA_COMPLEX64,
-    GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT,
+    GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT, GEMM_FP32GRADE_STAGED,
     KEEP_PSI0, CHECK_FINITE,
     OK, WARN_UNSTABLE,
 )

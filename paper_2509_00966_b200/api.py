@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libmlmd.so")
 OK, ERR_ARG, ERR_SHAPE, ERR_STATE, ERR_CUDA, ERR_NOMEM, ERR_NONFINITE, WARN_UNSTABLE = range(8)
 HOST, DEVICE = 0, 1
 BETA_REAL32, BETA_COMPLEX64 = 0, 1
-GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT = range(5)
+GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT, GEMM_FP32GRADE_STAGED = range(6)
 KEEP_PSI0, CHECK_FINITE = 1, 2
 
 EXPORTED_SYMBOLS = [

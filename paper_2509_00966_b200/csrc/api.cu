@@ -141,6 +141,8 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
         h->tc_ok = tc_available() && pl.ngrid % 128 == 0 && !(force && strcmp(force, "simt") == 0);
     }
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
+    h->staged_mask = 0x3;                                // stages 0, 1 (tau = dt/4, dt/3) of the staged mode
+    if (const char *m = getenv("MLMD_STAGED_MASK")) h->staged_mask = atoi(m) & 0xf;   // A/B checks
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
     h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
@@ -214,7 +216,7 @@ long long mlmd_launch_count(const mlmd_domain_t *h) { return h ? h->launches : 0
 
 static bool use_tensor_cores(const mlmd_domain *h) {
     return h->tc_ok && (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_TF32X1 ||
-                        h->gemm_mode == MLMD_GEMM_LOWP_BF16);
+                        h->gemm_mode == MLMD_GEMM_LOWP_BF16 || h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED);
 }
 // products per MAC on the tensor-core path: 3 = 3xTF32, 1 = TF32x1, 0 = BF16-rounded operands x1
 static int tc_nprod(const mlmd_domain *h) {
@@ -343,7 +345,7 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
 int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: NULL handle");
     drop_graph(h);
-    if (mode < MLMD_GEMM_FP32GRADE || mode > MLMD_GEMM_FP32_SIMT) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: bad mode %d", mode);
+    if (mode < MLMD_GEMM_FP32GRADE || mode > MLMD_GEMM_FP32GRADE_STAGED) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: bad mode %d", mode);
     h->gemm_mode = mode;
     return MLMD_OK;
 }
@@ -463,8 +465,9 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
     c->pad = 0.f;
 }
 
-static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl) {
-    // S2a + S2b: What = (-i tau) D' (beta^H w)
+static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl, int nprod = -1) {
+    // S2a + S2b: What = (-i tau) D' (beta^H w); nprod >= 0 overrides the mode's products per MAC (staged mode)
+    if (nprod < 0) nprod = tc_nprod(h);
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     const bool tc = use_tensor_cores(h);
     const int nsplit = tc ? h->nsplit_tc : h->nsplit;
@@ -472,7 +475,7 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl)
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, tc_nprod(h), kProjChain, nl));
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, kProjChain, nl));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
@@ -483,12 +486,13 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl)
     return MLMD_OK;
 }
 
-static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl) {
+static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl, int nprod = -1) {
+    if (nprod < 0) nprod = tc_nprod(h);
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     ProfScope ps(h, MLMD_K_BACK);
     if (use_tensor_cores(h))
         CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
-                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, tc_nprod(h), nl));
+                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, nprod, nl));
     else
         CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
                             (float *)out, 2 * h->ld, 2 * h->ld, h->prows, fp64, nl));
@@ -502,10 +506,15 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
     // Horner form of sum_{m<=4} (-i dt H)^m/m!: w4 = psi, w_{k-1} = psi + (-i dt/k) H w_k
     const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
     float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
+    // MLMD_GEMM_FP32GRADE_STAGED: the V_NL term of Horner stage i reaches the result through
+    // 3 - i further applications of (dt/k) H, so the two innermost stages take a single TF32 product in the
+    // projection and beta_hi + beta_lo times a single-TF32 W in the back-application; the outer two stay 3xTF32.
+    const bool staged = h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED && use_tensor_cores(h);
     for (int i = 0; i < 4; ++i) {
         const float tau = (float)(dt / (4 - i));
+        const bool reduced = staged && ((h->staged_mask >> i) & 1);
         if (h->nproj > 0) {
-            int rc = nonlocal_project(h, src[i], tau, nl);
+            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? 1 : -1);
             if (rc) return rc;
         }
         {
@@ -513,7 +522,7 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
             CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, coef_host, tau, nl));
         }
         if (h->nproj > 0) {
-            int rc = nonlocal_back(h, dst[i], nl);
+            int rc = nonlocal_back(h, dst[i], nl, reduced ? 2 : -1);
             if (rc) return rc;
         }
     }

@@ -419,10 +419,11 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     const int total = q.ndom * nrp * q.ntile_n;    // cluster units
     const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
     const int nk = (q.P + 7) / 8;
-    const bool need_lo = q.nprod == 3;
+    // nprod 3: beta_hi W_hi + beta_lo W_hi + beta_hi W_lo; nprod 2 (staged mode): the first two (W taken as one TF32)
+    const bool need_lo = q.nprod >= 2, need_wlo = q.nprod == 3;
     const int nchunk = q.BN / 32, chalf = (nchunk + 1) / 2;   // W chunks: this CTA fetches `chalf` of them
     const uint32_t w_bytes = (uint32_t)(2 * chalf) * 1024;
-    const uint32_t tx_bytes = (need_lo ? 2u : 1u) * (BK_A_BYTES + w_bytes);
+    const uint32_t tx_bytes = (need_lo ? 2u : 1u) * BK_A_BYTES + (need_wlo ? 2u : 1u) * w_bytes;
     const int ninstr = q.BN > 256 ? 2 : 1;
     const int NI = q.BN / ninstr;                   // columns per UMMA instruction (multiple of 32)
 
@@ -440,11 +441,10 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                     tma_load_2d(st, &map_ahi, &full[s], k * 8, row);
                     tma_load_3d_mc(st + 2 * BK_A_BYTES + crank * chalf * 1024, &map_whi, &full[s], 0, dom * q.prows + k * 8,
                                    nt * nchunk + crank * chalf, (uint16_t)3);
-                    if (need_lo) {
-                        tma_load_2d(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
+                    if (need_lo) tma_load_2d(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
+                    if (need_wlo)
                         tma_load_3d_mc(st + 2 * BK_A_BYTES + BK_W_BYTES + crank * chalf * 1024, &map_wlo, &full[s], 0,
                                        dom * q.prows + k * 8, nt * nchunk + crank * chalf, (uint16_t)3);
-                    }
                 }
             }
         }
@@ -468,9 +468,9 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         const uint64_t dw = smem_desc(st + 2 * BK_A_BYTES + woff, 1024, 512, LAYOUT_SW128_32B);
                         const uint32_t d = tmem + h * NI;
                         umma_tf32(d, da, dw, idesc, k > 0 ? 1u : 0u);
-                        if (need_lo) {
+                        if (need_lo) umma_tf32(d, dal, dw, idesc, 1u);
+                        if (need_wlo) {
                             const uint64_t dwl = smem_desc(st + 2 * BK_A_BYTES + BK_W_BYTES + woff, 1024, 512, LAYOUT_SW128_32B);
-                            umma_tf32(d, dal, dw, idesc, 1u);
                             umma_tf32(d, da, dwl, idesc, 1u);
                         }
                     }
@@ -577,10 +577,10 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
     const int total = q.ndom * nrp * q.ntile_n;    // cluster units: a pair of row tiles x one column tile
     const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
     const int nk = (q.P + 7) / 8;
-    const bool need_lo = q.nprod == 3;
+    const bool need_lo = q.nprod >= 2, need_wlo = q.nprod == 3;   // as in back_tc_kernel
     const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;   // UMMA pieces (columns); per CTA n/2 of each
     const int h0 = n0 / 64, h1 = n1 / 64;                      // this CTA's 32-column chunks of each piece
-    const uint32_t cta_bytes = (need_lo ? 2u : 1u) * (BK_A_BYTES + (uint32_t)(h0 + h1) * 1024);
+    const uint32_t cta_bytes = (need_lo ? 2u : 1u) * BK_A_BYTES + (need_wlo ? 2u : 1u) * (uint32_t)(h0 + h1) * 1024;
 
     if (warp == 0) {
         if (lane == 0) {
@@ -598,8 +598,8 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
                     tma_load_2d_2cta(st, &map_ahi, &full[s], k * 8, row);
                     tma_load_3d_2cta(st + 2 * BK_A_BYTES, &map_w0h, &full[s], 0, wrow, ch0);
                     if (h1) tma_load_3d_2cta(st + 2 * BK_A_BYTES + h0 * 1024, &map_w1h, &full[s], 0, wrow, ch1);
-                    if (need_lo) {
-                        tma_load_2d_2cta(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
+                    if (need_lo) tma_load_2d_2cta(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
+                    if (need_wlo) {
                         tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES, &map_w0l, &full[s], 0, wrow, ch0);
                         if (h1)
                             tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES + h0 * 1024, &map_w1l, &full[s], 0, wrow, ch1);
@@ -627,18 +627,15 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
                     {
                         const uint64_t dw = smem_desc(wh, 1024, 512, LAYOUT_SW128_32B);
                         umma_tf32_2cta(tmem, da, dw, id0, acc);
-                        if (need_lo) {
-                            umma_tf32_2cta(tmem, dal, dw, id0, 1u);
-                            umma_tf32_2cta(tmem, da, smem_desc(wl, 1024, 512, LAYOUT_SW128_32B), id0, 1u);
-                        }
+                        if (need_lo) umma_tf32_2cta(tmem, dal, dw, id0, 1u);
+                        if (need_wlo) umma_tf32_2cta(tmem, da, smem_desc(wl, 1024, 512, LAYOUT_SW128_32B), id0, 1u);
                     }
                     if (h1) {
                         const uint64_t dw = smem_desc(wh + h0 * 1024, 1024, 512, LAYOUT_SW128_32B);
                         umma_tf32_2cta(tmem + n0, da, dw, id1, acc);
-                        if (need_lo) {
-                            umma_tf32_2cta(tmem + n0, dal, dw, id1, 1u);
+                        if (need_lo) umma_tf32_2cta(tmem + n0, dal, dw, id1, 1u);
+                        if (need_wlo)
                             umma_tf32_2cta(tmem + n0, da, smem_desc(wl + h0 * 1024, 1024, 512, LAYOUT_SW128_32B), id1, 1u);
-                        }
                     }
                     umma_commit_2cta_mc(&empty[s], (uint16_t)3);
                 }
