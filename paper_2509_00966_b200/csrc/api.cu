@@ -143,6 +143,8 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
     h->staged_mask = 0x3;                                // stages 0, 1 (tau = dt/4, dt/3) of the staged mode
     if (const char *m = getenv("MLMD_STAGED_MASK")) h->staged_mask = atoi(m) & 0xf;   // A/B checks
+    h->staged_proj_nprod = 4;                            // one product, psi rounded to nearest (1: truncated by the MMA)
+    if (const char *m = getenv("MLMD_STAGED_PROJ")) h->staged_proj_nprod = atoi(m) == 1 ? 1 : 4;
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
     h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
@@ -470,11 +472,12 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl,
     if (nprod < 0) nprod = tc_nprod(h);
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     const bool tc = use_tensor_cores(h);
+    static const bool conva = getenv("MLMD_PROJ_CONVA") && atoi(getenv("MLMD_PROJ_CONVA")) == 1;
     const int nsplit = tc ? h->nsplit_tc : h->nsplit;
     {
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
-            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
+            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), conva ? nullptr : h->beta_lo(), h->ldp, h->P, (const float *)w,
                               2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, kProjChain, nl));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
@@ -514,7 +517,7 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
         const float tau = (float)(dt / (4 - i));
         const bool reduced = staged && ((h->staged_mask >> i) & 1);
         if (h->nproj > 0) {
-            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? 1 : -1);
+            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? h->staged_proj_nprod : -1);
             if (rc) return rc;
         }
         {

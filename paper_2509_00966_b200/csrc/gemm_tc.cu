@@ -123,6 +123,14 @@ __device__ __forceinline__ float4 split4(float4 &v) {
     return l;
 }
 
+// round-to-nearest-even to TF32 precision (13 low mantissa bits cleared afterwards)
+__device__ __forceinline__ float tf32_rn(float x) {
+    uint32_t u = __float_as_uint(x);
+    u += 0xfffu + ((u >> 13) & 1u);
+    return __uint_as_float(u & 0xffffe000u);
+}
+__device__ __forceinline__ float4 tf32_rn4(const float4 v) { return make_float4(tf32_rn(v.x), tf32_rn(v.y), tf32_rn(v.z), tf32_rn(v.w)); }
+
 // round-to-nearest-even to BF16 precision, kept in an FP32 container (every BF16 value is a TF32 value)
 __device__ __forceinline__ float bf16_round(float x) {
     uint32_t u = __float_as_uint(x);
@@ -149,7 +157,7 @@ constexpr int PJ_SMEM = PJ_STAGES * PJ_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 /
 constexpr int PJ_THREADS = 192;          // warp 0 TMA, warp 1 MMA, warps 2-5 convert + epilogue
 
 struct ProjParams {
-    int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, chain, lowp;
+    int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, chain, lowp, rn;
     float *zpart;
 };
 
@@ -191,7 +199,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     const int nntp = (q.ntile_n + 1) / 2;          // pairs of column tiles: one per cluster unit
     const int total = q.ndom * q.ntile_m * nntp * q.nsplit;   // cluster units
     const bool need_lo = q.nprod == 3;
-    const bool need_conv = need_lo || q.lowp;   // converter warps touch every stage
+    const bool need_conv = need_lo || q.lowp || q.rn;   // converter warps touch every stage
     const bool load_alo = need_lo && !q.conv_a;
     const uint32_t y_bytes = (uint32_t)(q.BN / 32) * PJ_BK * 128;
     const uint32_t tx_bytes = PJ_A_BYTES * (load_alo ? 2u : 1u) + y_bytes;
@@ -298,6 +306,17 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         for (int i = t; i < ny4; i += 128) y4[i] = bf16_round4(y4[i]);
                         float4 *a4 = (float4 *)st;
                         for (int i = t; i < PJ_A_BYTES / 16; i += 128) a4[i] = bf16_round4(a4[i]);
+                        fence_proxy_async_smem();
+                        mbar_arrive(&conv[s]);
+                    }
+                } else if (q.rn) {
+                    // one product, unbiased: psi rounded to the nearest TF32 in place (the MMA alone would truncate;
+                    // beta_hi was rounded to nearest when the projectors were set)
+                    for (int kb = c0k; kb < c1k; ++kb, ++it) {
+                        const int s = it % PJ_STAGES;
+                        mbar_wait(&full[s], (it / PJ_STAGES) & 1);
+                        float4 *y4 = (float4 *)(smem + s * PJ_STAGE_BYTES + 2 * PJ_A_BYTES);
+                        for (int i = t; i < ny4; i += 128) y4[i] = tf32_rn4(y4[i]);
                         fence_proxy_async_smem();
                         mbar_arrive(&conv[s]);
                     }
@@ -737,7 +756,8 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.zpart = zpart;
     q.chain = chain > 0 ? chain : (1 << 30);
     q.lowp = nprod == 0 ? 1 : 0;     // nprod 0 = one product of BF16-rounded operands
-    if (q.lowp) q.nprod = 1;
+    q.rn = nprod == 4 ? 1 : 0;       // nprod 4 = one product, psi rounded to the nearest TF32 in shared memory
+    if (q.lowp || q.rn) q.nprod = 1;
     const uint64_t rows = (uint64_t)ndom * ngrid;
     CUtensorMap ma, mal, my;
     // 4-chunk boxes: each CTA of a cluster fetches (and multicasts) half of the 8 beta chunks of a stage

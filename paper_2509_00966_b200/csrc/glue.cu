@@ -4,8 +4,14 @@
 
 namespace mlmd {
 
-// x with the 13 low mantissa bits cleared: the part of x a kind::tf32 tensor-core operand keeps
-__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+// x rounded to the nearest TF32 value (ties to even; 13 low mantissa bits cleared afterwards, so a kind::tf32
+// tensor-core operand, which drops those bits, keeps it exactly).  Nearest rather than truncated: the hi part
+// alone is then an UNBIASED single-product operand (staged mode), and x - hi is still exact in FP32.
+__device__ __forceinline__ float tf32_hi(float x) {
+    unsigned u = __float_as_uint(x);
+    u += 0xfffu + ((u >> 13) & 1u);
+    return __uint_as_float(u & 0xffffe000u);
+}
 
 __device__ __forceinline__ float bf16_rne(float x) {
     unsigned u = __float_as_uint(x);
@@ -45,7 +51,7 @@ __global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int pro
     }
     const float f = tau * dprime[(size_t)dom * nproj + p];
     const float wre = f * cim, wim = -f * cre;   // (-i f)(cre + i cim)
-    // stored as TF32-representable hi part + exact FP32 remainder lo (hi + lo == W exactly)
+    // stored as TF32-representable hi part (nearest) + exact FP32 remainder lo (hi + lo == W exactly)
     // low-precision mode: W rounded to BF16 (round-to-nearest-even), no remainder
     const float wre_h = lowp ? bf16_rne(wre) : tf32_hi(wre), wim_h = lowp ? bf16_rne(wim) : tf32_hi(wim);
     const float wre_l = lowp ? 0.f : wre - wre_h, wim_l = lowp ? 0.f : wim - wim_h;
@@ -172,8 +178,8 @@ cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld,
     return cudaGetLastError();
 }
 
-// In place: x -> hi = x with the low 13 mantissa bits cleared (what a TF32 operand keeps), lo = x - hi
-// (exact in FP32, so hi + lo restores x bit for bit).
+// In place: x -> hi = x rounded to the nearest TF32 value, lo = x - hi (exact in FP32, so hi + lo restores
+// x bit for bit).
 __global__ void split_tf32_kernel(float *__restrict__ x, float *__restrict__ lo, size_t n) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const float v = x[i];

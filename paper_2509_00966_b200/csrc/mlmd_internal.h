@@ -53,6 +53,7 @@ struct mlmd_domain {
     int nsplit_tc, nsplit_tc_ovl;   // split-K factors of the tcgen05 projection (beta rows / overlap)
     bool tc_ok;                 // shape and device allow the tcgen05 GEMM kernels
     int gemm_mode;
+    int staged_proj_nprod; // its projection: 4 = one product of nearest-rounded operands, 1 = truncated
     int staged_mask;      // MLMD_GEMM_FP32GRADE_STAGED: bit i = Horner stage i runs with reduced products
     bool have_psi, have_vloc, have_occ, rho_valid;
     bool field_yz;              // any A_y or A_z non-zero in the current propagate call
@@ -157,7 +158,7 @@ cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float 
 
 // ---- gemm_tc.cu ------------------------------------------------------------------------------
 // The same two contractions on tcgen05 tensor cores, operands staged by TMA.  nprod = 3: 3xTF32
-// (FP32-grade), nprod = 2 (back-application only): beta_hi + beta_lo times W_hi, nprod = 1: single TF32 product, nprod = 0: single product of operands rounded to BF16
+// (FP32-grade), nprod = 2 (back-application only): beta_hi + beta_lo times W_hi, nprod = 1: single TF32 product (psi truncated by the MMA), nprod = 4 (projection only): single product with psi rounded to nearest in shared memory, nprod = 0: single product of operands rounded to BF16
 // in shared memory (opt-in low precision).  A_lo == NULL with nprod == 3: the kernel splits A
 // itself (overlap, where A is a psi buffer).  Requires ngrid % 128 == 0, N % 32 == 0, lda % 8 == 0.
 bool tc_available();

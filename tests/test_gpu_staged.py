@@ -34,7 +34,7 @@ def test_staged_perovskite_domain_on_tensor_cores():
     d = W.generate(c)
     A = W.laser_samples(c, nsteps=3, t0=0.9)
     dom = make_domain(c, d, mode=M.GEMM_FP32GRADE_STAGED)
-    assert M.mlmd_gemm_path(dom.handle) == 1
+    assert dom.gemm_path() == "tcgen05"
     dom.close()
     res = run_both(c, d, 3, A=A, mode=M.GEMM_FP32GRADE_STAGED)
     check(res)
