@@ -37,10 +37,10 @@ STEP_NAMES = {"taylor": "Taylor-4 (full H, north_star)", "split": "Eq. (2) split
 # tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
 # the opt-in BF16-operand mode issues its single product on the TF32 pipe (BF16 values are TF32 values)
 TF32_OVER_BF16 = 1.1 / 2.25     # nominal dense peaks (B200_PROFILING.md): tf32 1.1 PF, bf16 2.25 PF
-# "staged" (MLMD_GEMM_FP32GRADE_STAGED, Taylor step): of the 8 GEMMs of a step the outer 4 issue 3 products per MAC, the
-# inner projections 1 and the inner back-applications 2: (4 x 3 + 2 x 1 + 2 x 2) / 8 = 2.25 products on average
+# "staged" (MLMD_GEMM_FP32GRADE_STAGED, Taylor step): of the 8 GEMMs of a step the outermost 2 issue 3 products per MAC, the
+# inner projections 1 and the inner back-applications 2: (2 x 3 + 3 x 1 + 3 x 2) / 8 = 1.875 products on average
 TENSOR_RATIO = {"fp32grade": TF32_OVER_BF16 / 3.0, "tf32x1": TF32_OVER_BF16, "bf16": TF32_OVER_BF16,
-                "staged": TF32_OVER_BF16 / 2.25}
+                "staged": TF32_OVER_BF16 / 1.875}
 FP32_ALU_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FMA lanes x 2 flop x max SM clock
 FP64_ALU_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12    # nominal 64 DFMA lanes per SM (guide: ~40 TF)
 
@@ -191,6 +191,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-observables", action="store_true")
+    ap.add_argument("--no-staged", action="store_true", help="skip the extra timing of the same steps in the staged GEMM mode")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -336,6 +337,28 @@ def main():
                         "what": "forward-neighbour pass over psi (mlmd_current), algorithmic bytes = one read of psi"},
         }
 
+    # ---- the same K steps in the opt-in stage-adaptive GEMM mode, reported beside the default line
+    also_staged = None
+    if rank == 0 and args.step == "taylor" and args.gemm_mode == "fp32grade" and gemm_path == "tcgen05" and not args.no_staged:
+        dom.set_gemm_mode(MODE_NAMES["staged"])
+        propagate(min(Wm, 3) or 1, c.dt, A)
+        dom.set_orbitals(psi_dev, occ)
+        if flush is not None:
+            flush.fill_(1.0)
+        torch.cuda.synchronize()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(stream)
+        propagate(K, c.dt, A)
+        s1.record(stream)
+        torch.cuda.synchronize()
+        ms_s = s0.elapsed_time(s1)
+        also_staged = {"gemm_mode": "staged", "value": c.ndom * c.electrons_per_domain * K / (ms_s * 1e-3), "unit": "electron-steps/s",
+                       "ms_per_step": ms_s / K, "n_gpus": 1,
+                       "what": "mlmd_set_gemm_mode(MLMD_GEMM_FP32GRADE_STAGED): 3xTF32 in the outermost Horner stage, 1 (projection) / 2 "
+                               "(back-application) TF32 products in the three inner ones; same FP32-grade tolerances, "
+                               "tests/test_gpu_staged.py; this rank only"}
+        dom.set_gemm_mode(MODE_NAMES[args.gemm_mode])
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -402,7 +425,7 @@ def main():
         "data": "synthetic", "config": workload_config(c, args), "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "roofline": roof, "cpu_baseline": cpu, "step_roofline": step_roof, "kernels": per_class, "observables": observables,
         "orbital_steps_per_s": c.ndom * c.norb * world * K / (ms * 1e-3), "input_generation_s": t_gen,
-        "paper_context": PAPER_CONTEXT,
+        "paper_context": PAPER_CONTEXT, "also_staged": also_staged,
     }
     print(json.dumps(line))
     dom.close()

@@ -61,10 +61,11 @@ enum {
     MLMD_GEMM_LOWP_BF16 = 2, /* opt-in: BF16 operands, FP32 accumulate      */
     MLMD_GEMM_TF32X1 = 3,    /* optional rung: single TF32 product, FP32 accumulate               */
     MLMD_GEMM_FP32_SIMT = 4, /* plain FP32 FMA on CUDA cores (portable fallback, any shape)       */
-    MLMD_GEMM_FP32GRADE_STAGED = 5 /* opt-in: mlmd_propagate's two innermost Horner stages (weights dt^4/24,
-                                * dt^3/6) use 1 TF32 product in the projection and 2 in the back-application,
-                                * the outer two stay 3xTF32; same tolerances as mode 0.
-                                * Every other call behaves as mode 0. */
+    MLMD_GEMM_FP32GRADE_STAGED = 5 /* opt-in: mlmd_propagate's three inner Horner stages (whose V_NL terms reach
+                                * the result with weights dt^4/24, dt^3/6, dt^2/2) use 1 product of
+                                * nearest-rounded TF32 operands in the projection and 2 in the back-application
+                                * (beta hi + lo, W hi); the outermost stage stays 3xTF32.  Same tolerances as
+                                * mode 0.  Every other call behaves as mode 0. */
 };
 enum {
     MLMD_KEEP_PSI0 = 1u,    /* snapshot Psi(0) at mlmd_set_orbitals for mlmd_overlap(which=1)     */

@@ -141,7 +141,7 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
         h->tc_ok = tc_available() && pl.ngrid % 128 == 0 && !(force && strcmp(force, "simt") == 0);
     }
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
-    h->staged_mask = 0x3;                                // stages 0, 1 (tau = dt/4, dt/3) of the staged mode
+    h->staged_mask = 0x7;                                // stages 0-2 (tau = dt/4, dt/3, dt/2) of the staged mode
     if (const char *m = getenv("MLMD_STAGED_MASK")) h->staged_mask = atoi(m) & 0xf;   // A/B checks
     h->staged_proj_nprod = 4;                            // one product, psi rounded to nearest (1: truncated by the MMA)
     if (const char *m = getenv("MLMD_STAGED_PROJ")) h->staged_proj_nprod = atoi(m) == 1 ? 1 : 4;
@@ -510,8 +510,9 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
     const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
     float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
     // MLMD_GEMM_FP32GRADE_STAGED: the V_NL term of Horner stage i reaches the result through
-    // 3 - i further applications of (dt/k) H, so the two innermost stages take a single TF32 product in the
-    // projection and beta_hi + beta_lo times a single-TF32 W in the back-application; the outer two stay 3xTF32.
+    // 3 - i further applications of (dt/k) H, so the three inner stages take a single product of nearest-rounded
+    // TF32 operands in the projection and beta_hi + beta_lo times a single-TF32 W in the back-application; the
+    // outermost stage (weight dt) stays 3xTF32.
     const bool staged = h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED && use_tensor_cores(h);
     for (int i = 0; i < 4; ++i) {
         const float tau = (float)(dt / (4 - i));

@@ -12,8 +12,9 @@
 // 1 = MMA issuer (+ TMEM allocation), the rest convert (hi/lo split) and run the epilogue.
 //
 // FP32-grade accuracy = 3xTF32 (PAPER.md L239 describes the same idea as BF16x3):
-//   a*b ~= a_hi*b_hi + a_lo*b_hi + a_hi*b_lo,  x_hi = x with the 13 low mantissa bits cleared (what
-// a kind::tf32 operand keeps), x_lo = x - x_hi (exact in FP32); FP32 accumulation in TMEM.
+//   a*b ~= a_hi*b_hi + a_lo*b_hi + a_hi*b_lo,  x_hi = a TF32-representable value within one TF32 ulp of x
+// (beta, W: nearest, rounded when they are written; psi: the 13 low mantissa bits cleared, which is what a
+// kind::tf32 operand keeps of the tile as loaded), x_lo = x - x_hi (exact in FP32); FP32 accumulation in TMEM.
 // beta_hi / beta_lo are split once at mlmd_set_projectors; psi-side lo tiles are produced in shared
 // memory by the converter warps; W hi/lo are written by the glue kernel.
 #include <stdio.h>
@@ -161,20 +162,26 @@ struct ProjParams {
     float *zpart;
 };
 
+// LO = true: stages hold hi and lo tiles of both operands (3xTF32), 3 stages; LO = false (one product per MAC):
+// one tile per operand, so the same shared memory gives a 6-stage pipeline for the then HBM-latency-bound kernel.
+template <bool LO>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PJ_THREADS, 1)
 proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
                const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_z, const ProjParams q) {
+    constexpr int NST = LO ? PJ_STAGES : 2 * PJ_STAGES;
+    constexpr int YOFF = (LO ? 2 : 1) * PJ_A_BYTES;            // Y tile(s) follow the beta tile(s)
+    constexpr int SB = LO ? PJ_STAGE_BYTES : PJ_STAGE_BYTES / 2;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    uint8_t *stage = smem + PJ_STAGES * PJ_STAGE_BYTES;
+    uint8_t *stage = smem + NST * SB;
     uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
-    uint64_t *full = bars, *empty = bars + PJ_STAGES, *conv = bars + 2 * PJ_STAGES;
-    uint64_t *acc_full = bars + 3 * PJ_STAGES, *acc_empty = acc_full + 1;
+    uint64_t *full = bars, *empty = bars + NST, *conv = bars + 2 * NST;
+    uint64_t *acc_full = bars + 3 * NST, *acc_empty = acc_full + 1;
     uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < PJ_STAGES; ++s) {
+        for (int s = 0; s < NST; ++s) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], 2);    // this CTA's MMAs and the peer's (its multicast half lands here too)
             mbar_init(&conv[s], 128);
@@ -222,16 +229,16 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 int dom, mt, nt, kb0, kb1;
                 decode(u, dom, mt, nt, kb0, kb1);
                 for (int kb = kb0; kb < kb1; ++kb, ++it) {
-                    const int s = it % PJ_STAGES;
-                    mbar_wait(&empty[s], ((it / PJ_STAGES) & 1) ^ 1);
-                    uint8_t *st = smem + s * PJ_STAGE_BYTES;
+                    const int s = it % NST;
+                    mbar_wait(&empty[s], ((it / NST) & 1) ^ 1);
+                    uint8_t *st = smem + s * SB;
                     mbar_expect_tx(&full[s], tx_bytes);
                     const int row = dom * q.ngrid + kb * PJ_BK;
                     const int ahalf = crank * 4 * (PJ_BK * 128);   // this CTA fetches 4 of the 8 beta chunks for both
                     tma_load_3d_mc(st + ahalf, &map_ahi, &full[s], 0, row, mt * 8 + crank * 4, (uint16_t)3);
                     if (load_alo)
                         tma_load_3d_mc(st + PJ_A_BYTES + ahalf, &map_alo, &full[s], 0, row, mt * 8 + crank * 4, (uint16_t)3);
-                    tma_load_3d(st + 2 * PJ_A_BYTES, &map_y, &full[s], 0, row, nt * (q.BN / 32));
+                    tma_load_3d(st + YOFF, &map_y, &full[s], 0, row, nt * (q.BN / 32));
                 }
             }
         }
@@ -251,14 +258,14 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         mbar_wait(acc_empty, (nd & 1) ^ 1);
                         tc_fence_after();
                     }
-                    const int s = it % PJ_STAGES;
-                    const uint32_t ph = (it / PJ_STAGES) & 1;
+                    const int s = it % NST;
+                    const uint32_t ph = (it / NST) & 1;
                     mbar_wait(&full[s], ph);
                     if (need_conv) mbar_wait(&conv[s], ph);
                     tc_fence_after();
-                    const uint32_t st = smem_u32(smem + s * PJ_STAGE_BYTES);
-                    const uint32_t a_hi = st, a_lo = st + PJ_A_BYTES, y_hi = st + 2 * PJ_A_BYTES,
-                                   y_lo = st + 2 * PJ_A_BYTES + PJ_Y_BYTES;
+                    const uint32_t st = smem_u32(smem + s * SB);
+                    const uint32_t a_hi = st, a_lo = st + PJ_A_BYTES, y_hi = st + YOFF,
+                                   y_lo = st + YOFF + PJ_Y_BYTES;
 #pragma unroll
                     for (int k8 = 0; k8 < PJ_BK / 8; ++k8) {
                         const uint64_t dy = smem_desc(y_hi + k8 * 1024, PJ_BK * 128, 512, LAYOUT_SW128_32B);
@@ -299,10 +306,10 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 if (q.lowp) {
                     // opt-in low precision (PAPER.md L207, L239 float_to_BF16): both operands rounded to BF16
                     for (int kb = c0k; kb < c1k; ++kb, ++it) {
-                        const int s = it % PJ_STAGES;
-                        mbar_wait(&full[s], (it / PJ_STAGES) & 1);
-                        uint8_t *st = smem + s * PJ_STAGE_BYTES;
-                        float4 *y4 = (float4 *)(st + 2 * PJ_A_BYTES);
+                        const int s = it % NST;
+                        mbar_wait(&full[s], (it / NST) & 1);
+                        uint8_t *st = smem + s * SB;
+                        float4 *y4 = (float4 *)(st + YOFF);
                         for (int i = t; i < ny4; i += 128) y4[i] = bf16_round4(y4[i]);
                         float4 *a4 = (float4 *)st;
                         for (int i = t; i < PJ_A_BYTES / 16; i += 128) a4[i] = bf16_round4(a4[i]);
@@ -313,21 +320,21 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                     // one product, unbiased: psi rounded to the nearest TF32 in place (the MMA alone would truncate;
                     // beta_hi was rounded to nearest when the projectors were set)
                     for (int kb = c0k; kb < c1k; ++kb, ++it) {
-                        const int s = it % PJ_STAGES;
-                        mbar_wait(&full[s], (it / PJ_STAGES) & 1);
-                        float4 *y4 = (float4 *)(smem + s * PJ_STAGE_BYTES + 2 * PJ_A_BYTES);
+                        const int s = it % NST;
+                        mbar_wait(&full[s], (it / NST) & 1);
+                        float4 *y4 = (float4 *)(smem + s * SB + YOFF);
                         for (int i = t; i < ny4; i += 128) y4[i] = tf32_rn4(y4[i]);
                         fence_proxy_async_smem();
                         mbar_arrive(&conv[s]);
                     }
                 } else if (need_lo) {
                     for (int kb = c0k; kb < c1k; ++kb, ++it) {
-                        const int s = it % PJ_STAGES;
-                        mbar_wait(&full[s], (it / PJ_STAGES) & 1);
-                        uint8_t *st = smem + s * PJ_STAGE_BYTES;
+                        const int s = it % NST;
+                        mbar_wait(&full[s], (it / NST) & 1);
+                        uint8_t *st = smem + s * SB;
                         // elementwise on the swizzled image: the lo tile has the same layout as the hi tile
-                        float4 *ysrc = (float4 *)(st + 2 * PJ_A_BYTES);
-                        float4 *ydst = (float4 *)(st + 2 * PJ_A_BYTES + PJ_Y_BYTES);
+                        float4 *ysrc = (float4 *)(st + YOFF);
+                        float4 *ydst = (float4 *)(st + YOFF + PJ_Y_BYTES);
                         for (int i = t; i < ny4; i += 128) {
                             float4 v = ysrc[i];
                             ydst[i] = split4(v);   // the hi tile stays as loaded: kind::tf32 ignores the 13 low bits
@@ -737,7 +744,8 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
                            int chain, int *nlaunch) {
     static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
     if (!attr_set.done()) {
-        cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
+        cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(proj_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
         if (e != cudaSuccess) return e;
         attr_set.mark();
     }
@@ -769,7 +777,8 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     const int total = ndom * q.ntile_m * ((q.ntile_n + 1) / 2) * nsplit;   // cluster units
     const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
-    proj_tc_kernel<<<grid, PJ_THREADS, PJ_SMEM, st>>>(ma, mal, my, mz, q);
+    if (q.nprod == 3) proj_tc_kernel<true><<<grid, PJ_THREADS, PJ_SMEM, st>>>(ma, mal, my, mz, q);
+    else proj_tc_kernel<false><<<grid, PJ_THREADS, PJ_SMEM, st>>>(ma, mal, my, mz, q);
     return cudaGetLastError();
 }
 

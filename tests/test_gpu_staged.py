@@ -1,8 +1,8 @@
 """GPU parity of the opt-in stage-adaptive GEMM mode (MLMD_GEMM_FP32GRADE_STAGED) against the
 FP64 oracle, at the FP32-grade tolerances of BASELINE.json north_star (not the low-precision 1e-3):
   per-orbital relative L2 error <= 1e-5 after 1 step, <= 1e-4 after 100 steps; density <= 1e-4; Gram <= 1e-5.
-The mode keeps 3xTF32 in the two outer Horner stages of mlmd_propagate and takes one TF32 product in the
-projection / two in the back-application of the two inner stages (weights dt^4/24, dt^3/6 of the result).
+The mode keeps 3xTF32 in the outermost Horner stage of mlmd_propagate and takes one product of nearest-rounded TF32
+operands in the projection / two in the back-application of the three inner stages (weights dt^4/24, dt^3/6, dt^2/2).
 """
 import numpy as np
 import pytest
