@@ -472,12 +472,11 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl,
     if (nprod < 0) nprod = tc_nprod(h);
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     const bool tc = use_tensor_cores(h);
-    static const bool conva = getenv("MLMD_PROJ_CONVA") && atoi(getenv("MLMD_PROJ_CONVA")) == 1;
     const int nsplit = tc ? h->nsplit_tc : h->nsplit;
     {
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
-            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), conva ? nullptr : h->beta_lo(), h->ldp, h->P, (const float *)w,
+            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
                               2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, kProjChain, nl));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
