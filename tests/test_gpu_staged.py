@@ -109,3 +109,43 @@ def test_staged_stage_sweep_errors_against_the_oracle(monkeypatch):
     assert res["staged_0-2"]["err10"] <= res["default"]["err10"] + 2e-8
     # ... and reducing the outermost stage too is what would show
     assert res["staged_0-3"]["err10"] >= 1.5 * res["default"]["err10"]
+
+
+@pytest.mark.parametrize("grid,norb,cplx", [((6, 5, 7), 3, True), ((16, 8, 16), 12, True), ((16, 8, 16), 40, False)])
+def test_staged_ragged_and_complex_projectors(grid, norb, cplx):
+    """Shapes off the tensor-core tiling run the CUDA-core FP32 GEMMs in every stage (bit-equal to mode 0); a
+    tileable grid with padded orbital counts and complex projectors (2 nproj real rows) runs the staged tcgen05
+    stages and meets the FP32-grade bars against the oracle; per-domain field with y / z components."""
+    from oracle import ref
+    import paper_2509_00966_b200 as M
+    from test_gpu_parity import rho_err
+    rng = np.random.default_rng(11)
+    ndom, nproj, h, dt, nsteps = 2, 5, (0.41, 0.37, 0.45), 0.02, 4
+    ngrid = grid[0] * grid[1] * grid[2]
+    dv = h[0] * h[1] * h[2]
+    psi = (rng.standard_normal((ndom, *grid, norb)) + 1j * rng.standard_normal((ndom, *grid, norb))).astype(np.complex64)
+    psi /= np.sqrt(dv * ngrid)
+    beta = rng.standard_normal((ndom, ngrid, nproj)) + (1j * rng.standard_normal((ndom, ngrid, nproj)) if cplx else 0)
+    beta /= np.sqrt(dv * (np.abs(beta) ** 2).sum(axis=1, keepdims=True))
+    beta = beta.astype(np.complex64 if cplx else np.float32)
+    D = rng.uniform(-1, 1, (ndom, nproj))
+    vloc = (0.3 * rng.standard_normal((ndom, *grid))).astype(np.float32)
+    occ = rng.uniform(0, 2, (ndom, norb))
+    A = 0.1 * rng.standard_normal((nsteps, ndom, 3))
+    out = {}
+    for mode in (M.GEMM_FP32GRADE, M.GEMM_FP32GRADE_STAGED):
+        dom = M.Domain(ndom, grid, h, norb, nproj * (2 if cplx else 1))
+        dom.set_gemm_mode(mode)
+        dom.set_vloc(vloc)
+        dom.set_orbitals(psi, occ)
+        dom.set_projectors(beta, D)
+        dom.propagate(nsteps, dt, A)
+        out[mode] = (dom.get_orbitals(), dom.density(), dom.gemm_path())
+        dom.close()
+    g, rho, path = out[M.GEMM_FP32GRADE_STAGED]
+    assert path == ("tcgen05" if ngrid % 128 == 0 else "simt")
+    if path == "simt":
+        assert np.array_equal(g, out[M.GEMM_FP32GRADE][0]) and np.array_equal(rho, out[M.GEMM_FP32GRADE][1])
+    r, rho_ref = ref.propagate(psi, occ, vloc, beta, D, A, dt, h)
+    assert orb_err(g, r) <= 1e-5
+    assert rho_err(rho, rho_ref) <= 1e-4
