@@ -33,3 +33,19 @@ def test_algorithmic_counts_match_design():
     assert a["bytes_step"] == elems * 96 + 64 * 48 ** 3 * 20           # 88 B stage passes + 8 B density
     assert abs(a["gemm_flops_step"] - 8 * 4.0 * 64 * 48 ** 3 * 240 * 224) < 1.0   # real beta: 32 N_grid N_proj N_orb per domain
     assert abs(bench.TENSOR_RATIO["fp32grade"] - (1.1 / 2.25) / 3) < 1e-12
+    # staged mode: (2 x 3 + 3 x 1 + 3 x 2) / 8 products per MAC on average over the 8 GEMMs of a step
+    assert abs(bench.TENSOR_RATIO["staged"] - (1.1 / 2.25) / 1.875) < 1e-12
+    assert bench.MODE_NAMES["staged"] == 5
+
+
+def test_gemm_mode_enum_matches_header():
+    """The binding's mode constants are the header's enum values (include/mlmd.h)."""
+    import re
+    sys.path.insert(0, ROOT)
+    from paper_2509_00966_b200 import api
+    text = open(os.path.join(ROOT, "include", "mlmd.h")).read()
+    enum = dict((m.group(1), int(m.group(2))) for m in re.finditer(r"MLMD_(GEMM_\w+)\s*=\s*(\d+)", text))
+    assert enum == {"GEMM_FP32GRADE": 0, "GEMM_FP64": 1, "GEMM_LOWP_BF16": 2, "GEMM_TF32X1": 3, "GEMM_FP32_SIMT": 4,
+                    "GEMM_FP32GRADE_STAGED": 5}
+    for name, value in enum.items():
+        assert getattr(api, name) == value
