@@ -15,7 +15,14 @@ using namespace mlmd;
 
 // TMEM accumulation chain lengths (16-row stages) of the tcgen05 projection: tensor-core FP32
 // accumulation truncates, so long chains drift by ~1 ulp per MMA.
-static const int kProjChain = 64, kOverlapChain = 4;
+static const int kProjChain = 128, kOverlapChain = 4;
+// The drift counts MMAs, not stages: a one-product projection issues a third of the MMAs per stage, so three times
+// the stages give the same accumulation error with a third of the chain drains (each drain idles the tensor pipe).
+static int proj_chain(int nprod) {
+    static const int c3 = getenv("MLMD_PROJ_CHAIN") ? atoi(getenv("MLMD_PROJ_CHAIN")) : 0;   // A/B checks
+    const int base = c3 > 0 ? c3 : kProjChain;
+    return nprod == 3 ? base : 3 * base;
+}
 
 static thread_local char g_err[512] = "";
 
@@ -143,6 +150,8 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
     h->staged_mask = 0x7;                                // stages 0-2 (tau = dt/4, dt/3, dt/2) of the staged mode
     if (const char *m = getenv("MLMD_STAGED_MASK")) h->staged_mask = atoi(m) & 0xf;   // A/B checks
+    h->staged_chain = 8 * kProjChain;
+    if (const char *m = getenv("MLMD_STAGED_CHAIN")) h->staged_chain = atoi(m) > 0 ? atoi(m) : h->staged_chain;   // A/B checks
     h->staged_proj_nprod = 4;                            // one product, psi rounded to nearest (1: truncated by the MMA)
     if (const char *m = getenv("MLMD_STAGED_PROJ")) h->staged_proj_nprod = atoi(m) == 1 ? 1 : 4;
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
@@ -386,7 +395,7 @@ int mlmd_energy_nl(mlmd_domain_t *h, double *E, int where) {
         const int nsplit = tc ? h->nsplit_tc : h->nsplit;
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)h->psi(),
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, tc_nprod(h), kProjChain, &nl));
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, tc_nprod(h), proj_chain(tc_nprod(h)), &nl));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)h->psi(),
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, &nl));
@@ -467,7 +476,7 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
     c->pad = 0.f;
 }
 
-static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl, int nprod = -1) {
+static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl, int nprod = -1, int chain = -1) {
     // S2a + S2b: What = (-i tau) D' (beta^H w); nprod >= 0 overrides the mode's products per MAC (staged mode)
     if (nprod < 0) nprod = tc_nprod(h);
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
@@ -477,7 +486,7 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl,
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, kProjChain, nl));
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, chain > 0 ? chain : proj_chain(nprod), nl));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
@@ -517,7 +526,9 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
         const float tau = (float)(dt / (4 - i));
         const bool reduced = staged && ((h->staged_mask >> i) & 1);
         if (h->nproj > 0) {
-            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? h->staged_proj_nprod : -1);
+            // inner stages: their accumulation drift is damped like every other projection error (weights <= dt/2 E
+            // ~ 0.05 of the outer stage's), so the chains are 1024 stages: one or two drains per K slice instead of one per 128 stages
+            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? h->staged_proj_nprod : -1, reduced ? h->staged_chain : -1);
             if (rc) return rc;
         }
         {
