@@ -149,3 +149,30 @@ def test_staged_ragged_and_complex_projectors(grid, norb, cplx):
     r, rho_ref = ref.propagate(psi, occ, vloc, beta, D, A, dt, h)
     assert orb_err(g, r) <= 1e-5
     assert rho_err(rho, rho_ref) <= 1e-4
+
+
+def test_staged_cuda_graph_equals_eager_and_mode_switch_drops_the_graph(monkeypatch):
+    """Small batches replay a captured step: in the staged mode the graph holds the staged launches (same bits as the
+    eager launches), and switching the mode on a live handle re-captures (results equal a fresh handle's)."""
+    import paper_2509_00966_b200 as M
+    c = W.get_config(1, nsteps=9)
+    d = W.generate(c)
+    A = d["A"][:9]
+    outs = {}
+    for flag in ("1", "0"):
+        monkeypatch.setenv("MLMD_GRAPH", flag)
+        dom = make_domain(c, d, mode=M.GEMM_FP32GRADE_STAGED)
+        dom.propagate(9, c.dt, A)
+        outs[flag] = (dom.get_orbitals(), dom.density())
+        dom.close()
+    assert np.array_equal(outs["1"][0], outs["0"][0]) and np.array_equal(outs["1"][1], outs["0"][1])
+    monkeypatch.setenv("MLMD_GRAPH", "1")
+    dom = make_domain(c, d, mode=M.GEMM_FP32GRADE)
+    dom.propagate(9, c.dt, A)                       # captures the default-mode step
+    pure = dom.get_orbitals()
+    dom.set_gemm_mode(M.GEMM_FP32GRADE_STAGED)
+    dom.set_orbitals(d["psi"], d["occ"])
+    dom.propagate(9, c.dt, A)                       # must not replay the default-mode graph
+    assert np.array_equal(dom.get_orbitals(), outs["1"][0])
+    assert not np.array_equal(pure, outs["1"][0])
+    dom.close()
