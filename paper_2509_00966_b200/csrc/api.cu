@@ -150,6 +150,8 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
     h->staged_mask = 0x7;                                // stages 0-2 (tau = dt/4, dt/3, dt/2) of the staged mode
     if (const char *m = getenv("MLMD_STAGED_MASK")) h->staged_mask = atoi(m) & 0xf;   // A/B checks
+    h->inner_chain = 8 * kProjChain;
+    if (const char *m = getenv("MLMD_INNER_CHAIN")) h->inner_chain = atoi(m);   // A/B checks; <= 0: the mode's own length
     h->staged_chain = 8 * kProjChain;
     if (const char *m = getenv("MLMD_STAGED_CHAIN")) h->staged_chain = atoi(m) > 0 ? atoi(m) : h->staged_chain;   // A/B checks
     h->staged_proj_nprod = 4;                            // one product, psi rounded to nearest (1: truncated by the MMA)
@@ -528,7 +530,9 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
         if (h->nproj > 0) {
             // inner stages: their accumulation drift is damped like every other projection error (weights <= dt/2 E
             // ~ 0.05 of the outer stage's), so the chains are 1024 stages: one or two drains per K slice instead of one per 128 stages
-            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? h->staged_proj_nprod : -1, reduced ? h->staged_chain : -1);
+            // the three inner stages of every tensor-core mode take the long chains (the products stay as the mode says)
+            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? h->staged_proj_nprod : -1,
+                                      reduced ? h->staged_chain : (i < 3 ? h->inner_chain : -1));
             if (rc) return rc;
         }
         {

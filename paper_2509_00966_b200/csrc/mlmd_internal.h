@@ -54,6 +54,7 @@ struct mlmd_domain {
     bool tc_ok;                 // shape and device allow the tcgen05 GEMM kernels
     int gemm_mode;
     int staged_proj_nprod; // its projection: 4 = one product of nearest-rounded operands, 1 = truncated
+    int inner_chain;       // chain length of the three inner Horner stages' projections (any tensor-core mode)
     int staged_chain;      // its projection: TMEM accumulation chain length in 16-row stages
     int staged_mask;      // MLMD_GEMM_FP32GRADE_STAGED: bit i = Horner stage i runs with reduced products
     bool have_psi, have_vloc, have_occ, rho_valid;
