@@ -106,19 +106,23 @@ def algorithmic(c, gemm_real=True, step="taylor"):
 
 
 def ncu_traffic(c, kernel_class):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the class's kernel from the committed
-    `ncu --set full` capture of the same workload (profiles/r1_traffic_cfg3.json), else None."""
-    path = os.path.join(ROOT, "profiles", "r1_traffic_cfg3.json")
-    if c.cfg != 3 or c.ndom != 64 or not os.path.exists(path):
-        return None
-    with open(path) as f:
-        t = json.load(f)["dram_bytes_per_launch"]
-    pick = {"stencil": ["stencil_tma_kernel<0, 0, 0>"], "proj": ["proj_tc_kernel"], "back": ["back2_tc_kernel", "back_tc_kernel"],
-            "density": ["density_kernel"]}.get(kernel_class, [])
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of the class's kernel, where it comes from): read from
+    the newest committed `ncu --set full` capture of the same workload (profiles/r*_traffic_cfg3.json, which names the
+    commit it was taken at); (None, None) when there is none.  It is NOT measured by this run: ncu replays kernels."""
+    import glob
+    paths = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic_cfg3.json")))
+    if c.cfg != 3 or c.ndom != 64 or not paths:
+        return None, None
+    with open(paths[-1]) as f:
+        j = json.load(f)
+    t = j["dram_bytes_per_launch"]
+    pick = {"stencil": ["stencil_tma_kernel<0, 0, 0>", "stencil_tma_kernel"], "proj": ["proj2_tc_kernel", "proj_tc_kernel"],
+            "back": ["back2_tc_kernel", "back_tc_kernel"], "density": ["density_kernel"]}.get(kernel_class, [])
+    src = "%s (ncu --set full at commit %s)" % (os.path.relpath(paths[-1], ROOT), j.get("commit", "?"))
     for name in pick:
         if name in t:
-            return t[name]
-    return None
+            return t[name], src
+    return None, None
 
 
 def sample_for_oracle(c, d, norb_sample):
@@ -170,7 +174,7 @@ def run_reference(args):
 def workload_config(c, args):
     return {"workload": "configs[%d] %s: %d domains x %dx%dx%d grid x %d orbitals x %d projectors, dt=%g" % (
         c.cfg, c.name, c.ndom, *c.grid, c.norb, c.nproj, c.dt),
-        "ndom_per_gpu": c.ndom, "step": STEP_NAMES[args.step], "gemm_mode": args.gemm_mode, "gemm_path": getattr(args, "gemm_path", None), "parallelism": "domains sharded, no collective",
+        "ndom_per_gpu": c.ndom, "step": STEP_NAMES[args.step], "gemm_mode": args.gemm_mode, "parallelism": "domains sharded, no collective",
         "l2": "working set (3 x %.1f GB psi buffers + beta) exceeds the 126 MB L2; no flush needed" % (
             c.ndom * c.ngrid * c.norb * 8 / 1e9) if c.ndom * c.ngrid * c.norb * 8 > 4e8 else
         "working set may fit L2: a 256 MB buffer is written between timed repetitions"}
@@ -266,19 +270,30 @@ def main():
     if sampler:
         sampler.start()
     launches0 = dom.launch_count()
-    dom.profile(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    propagate(K, c.dt, A)
+    propagate(K, c.dt, A)            # the timed region: un-instrumented (the library's own launch path, CUDA graph included)
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
-    dom.profile(False)
     launches = dom.launch_count() - launches0
-    gemm_path = dom.gemm_path()
-    args.gemm_path = gemm_path
-    kern = dom.profile_read()
     clocks = sampler.summary() if sampler else None
+    gemm_path = dom.gemm_path()
+    # second pass over the same K steps with mlmd_profile on: CUDA events around every launch on the library's
+    # stream give the per-kernel-class table (this pass forces eager launches and is not what `value` is taken from)
+    dom.set_orbitals(psi_dev, occ)
+    if flush is not None:
+        flush.fill_(1.0)
+    torch.cuda.synchronize()
+    dom.profile(True)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(stream)
+    propagate(K, c.dt, A)
+    p1.record(stream)
+    torch.cuda.synchronize()
+    ms_profiled = p0.elapsed_time(p1)
+    dom.profile(False)
+    kern = dom.profile_read()
     t = torch.tensor([ms], dtype=torch.float64, device=dev)
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -339,7 +354,7 @@ def main():
 
     # ---- the same K steps in the opt-in stage-adaptive GEMM mode, reported beside the default line
     also_staged = None
-    if rank == 0 and args.step == "taylor" and args.gemm_mode == "fp32grade" and gemm_path == "tcgen05" and not args.no_staged:
+    if rank == 0 and world == 1 and args.step == "taylor" and args.gemm_mode == "fp32grade" and gemm_path == "tcgen05" and not args.no_staged:
         dom.set_gemm_mode(MODE_NAMES["staged"])
         propagate(min(Wm, 3) or 1, c.dt, A)
         dom.set_orbitals(psi_dev, occ)
@@ -394,7 +409,8 @@ def main():
         per_class[name] = entry
     top = max((n for n in per_class if "achieved" in per_class[n]), key=lambda n: per_class[n]["ms_total"])
     roof = {k: per_class[top][k] for k in ("bound", "achieved", "peak", "unit", "frac")}
-    roof.update(kernel=top, traffic=ncu_traffic(c, top) if args.step == "taylor" or top != "density" else None, peak_source="%s (%s)" % (
+    traffic, traffic_src = ncu_traffic(c, top) if args.step == "taylor" or top != "density" else (None, None)
+    roof.update(kernel=top, traffic=traffic, traffic_source=traffic_src, peak_source="%s (%s)" % (
         "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
         "hbm copy" if roof["bound"] == "hbm" else
         "sustained bf16 x nominal ratio for the mode" if roof["bound"] == "tensor" else "derived FP32/FP64 ALU peak, DESIGN.md"))
@@ -411,7 +427,10 @@ def main():
                      "+norm" if args.step == "split" else "")}
 
     cpu = None
-    if not args.no_cpu_baseline and world == 1:
+    if world > 1:
+        cpu = {"value": None, "unit": "electron-steps/s", "cores": None, "kind": "oracle",
+               "sample": "not timed at N > 1: the oracle is timed on rank 0 at N = 1 only"}
+    elif not args.no_cpu_baseline:
         # a bounded sample sized for roughly 10 s of host work at configs[3] (1 warm-up + CPU_STEPS timed steps)
         s = sample_for_oracle(c, first, 2 * args.oracle_orbitals)
         v, sec_step, cores, el = time_oracle(c, s, W.laser_samples(c, nsteps=CPU_STEPS, t0=0.9), steps=CPU_STEPS, warmup=1, step=args.step)
@@ -423,7 +442,8 @@ def main():
         "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "complex64",
         "data": "synthetic", "config": workload_config(c, args), "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-        "roofline": roof, "cpu_baseline": cpu, "step_roofline": step_roof, "kernels": per_class, "observables": observables,
+        "roofline": roof, "cpu_baseline": cpu, "step_roofline": step_roof, "gemm_path": gemm_path,
+        "kernels": per_class, "kernels_pass_ms_per_step": ms_profiled / K, "observables": observables,
         "orbital_steps_per_s": c.ndom * c.norb * world * K / (ms * 1e-3), "input_generation_s": t_gen,
         "paper_context": PAPER_CONTEXT, "also_staged": also_staged,
     }

@@ -41,6 +41,13 @@
 extern "C" {
 #endif
 
+/* The library is built with hidden visibility: these are its only exported symbols. */
+#if defined(__GNUC__)
+#define MLMD_API __attribute__((visibility("default")))
+#else
+#define MLMD_API
+#endif
+
 typedef struct mlmd_domain mlmd_domain_t;
 
 enum {
@@ -69,48 +76,67 @@ enum {
 };
 enum {
     MLMD_KEEP_PSI0 = 1u,    /* snapshot Psi(0) at mlmd_set_orbitals for mlmd_overlap(which=1)     */
-    MLMD_CHECK_FINITE = 2u  /* scan psi for NaN/Inf at the end of every mlmd_propagate            */
+    MLMD_CHECK_FINITE = 2u, /* scan psi for NaN/Inf at the end of every mlmd_propagate            */
+    MLMD_BORROW_PSI = 4u    /* Psi lives in the CALLER's device buffer: mlmd_set_orbitals(where = MLMD_DEVICE)
+                             * adopts the pointer instead of copying, every step updates that buffer in place and the
+                             * workspace holds no Psi copy.  The buffer is complex64
+                             * [ndom][nx][ny][nz][norb], 256-byte aligned, norb a multiple of 16 (rows need no padding),
+                             * and must stay alive and untouched by the caller while a call is in flight.            */
+};
+/* Run-time options (mlmd_set_option); each is read when it is set, never from the environment. */
+enum {
+    MLMD_OPT_GRAPH = 0,     /* 1 (default): small, launch-bound batches replay a CUDA graph of the step; 0: eager launches */
+    MLMD_OPT_STENCIL = 1,   /* 0 (default): TMA-staged kernel when ny, nz are multiples of 16, else the fallbacks;
+                             * 1: register-marching kernel; 2: one-thread-per-output kernel (cross-checks)            */
+    MLMD_OPT_GEMM_PATH = 2, /* 0 (default): tcgen05 kernels when ngrid is a multiple of 128; 1: CUDA-core kernels        */
+    MLMD_OPT_KICK_NORM = 3, /* mlmd_propagate_split, norm after the second kick: 0 (default) from the projector Gram
+                             * matrix when it applies; 1: always by a pass over psi                                   */
+    MLMD_OPT_COUNT = 4
 };
 
 /* Bytes of device workspace mlmd_domain_create needs for this shape (0 on invalid arguments).
  * Holds Psi, two Psi-sized stage buffers (Horner form of the Taylor sum), optional Psi(0),
  * V_loc, beta (and its split copies), D, occupations, rho, projection scratch. */
-size_t mlmd_workspace_bytes(int ndom, int nx, int ny, int nz, int norb, int nproj_max, unsigned flags);
+MLMD_API size_t mlmd_workspace_bytes(int ndom, int nx, int ny, int nz, int norb, int nproj_max, unsigned flags);
 
 /* Create a batch of ndom periodic domains of nx*ny*nz points (each axis >= 5: the five radius-2
  * periodic neighbours must be distinct), spacings hx,hy,hz (bohr), norb orbitals, at most
- * nproj_max projectors (complex projectors count once).  workspace_dev: device memory, 256-byte
+ * nproj_max REAL projector rows (a complex64 projector counts twice: mlmd_set_projectors needs
+ * nproj <= nproj_max for MLMD_BETA_REAL32 and 2*nproj <= nproj_max for MLMD_BETA_COMPLEX64).  workspace_dev: device memory, 256-byte
  * aligned, >= mlmd_workspace_bytes(...).  cuda_stream: a cudaStream_t passed as void*
  * (NULL = legacy default stream). */
-int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, double hx, double hy,
+MLMD_API int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, double hx, double hy,
                        double hz, int norb, int nproj_max, void *workspace_dev, size_t workspace_bytes,
                        void *cuda_stream, unsigned flags);
-int mlmd_domain_destroy(mlmd_domain_t *h);
+MLMD_API int mlmd_domain_destroy(mlmd_domain_t *h);
 
 /* Psi(t=0) and occupations f_n >= 0 (occ may be NULL = keep previous / all 2.0).
  * psi: complex64 [ndom][nx][ny][nz][norb] at `where`; occ: double [ndom][norb], HOST. */
-int mlmd_set_orbitals(mlmd_domain_t *h, const void *psi_c64, const double *occ, int where);
-int mlmd_get_orbitals(mlmd_domain_t *h, void *psi_c64, int where);
+MLMD_API int mlmd_set_orbitals(mlmd_domain_t *h, const void *psi_c64, const double *occ, int where);
+MLMD_API int mlmd_get_orbitals(mlmd_domain_t *h, void *psi_c64, int where);
 
 /* Local potential v_loc(r) of Eq. (3) in Hartree, float [ndom][nx][ny][nz]; frozen during a
  * propagate call (only Delta v_loc is passed once per MD step; reading D25). */
-int mlmd_set_vloc(mlmd_domain_t *h, const float *vloc, int where);
+MLMD_API int mlmd_set_vloc(mlmd_domain_t *h, const float *vloc, int where);
 
 /* Nonlocal operator V_NL = dv * B diag(D) B^H (north_star; Eq. (5) L199 is the case
  * B = Psi(0)).  beta: [ndom][ngrid][nproj], float (MLMD_BETA_REAL32) or complex64
  * (MLMD_BETA_COMPLEX64) at `where`; D: double [ndom][nproj] in Hartree, HOST.
  * nproj = 0 switches V_NL off (beta, D may be NULL). */
-int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_dtype, const double *D,
+MLMD_API int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_dtype, const double *D,
                         int where);
 
-int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode);
+MLMD_API int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode);
+
+/* Set one MLMD_OPT_* option (unknown key or value -> MLMD_ERR_ARG).  Takes effect from the next call on. */
+MLMD_API int mlmd_set_option(mlmd_domain_t *h, int key, int value);
 
 /* nsteps Taylor-4 steps of size dt.  A: double [nsteps][a_ndom][3], HOST; A[n] is the vector
  * potential at the step midpoint t_n + dt/2 (Eq. (2)), uniform inside a domain;
  * a_ndom = 1 (same field for every domain) or ndom.  The density of the final state is kept
  * for mlmd_density.  Returns MLMD_WARN_UNSTABLE (work still done) if
  * dt * [ (8/3) sum_d 1/h_d^2 + 1.3722 sum_d |A_d|/h_d + |A|^2/2 + max|V_loc| + max|D| ] > 2 sqrt(2). */
-int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
+MLMD_API int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
 
 /* nsteps steps of the paper's literal Eq. (2):
  *     psi <- K exp(-i dt h_loc(t_n + dt/2)) K psi,   K psi_n = (psi_n - i dt/2 V_NL psi_n) ||psi_n|| / ||psi_n - i dt/2 V_NL psi_n||
@@ -120,15 +146,15 @@ int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const double *A, int
  * correction of Eq. (5) L199 with delta = -i dt/2 D dv.  Two V_NL applications per step instead of four.
  * Arguments, density and return values as mlmd_propagate; the stability bound leaves out max|D| (the
  * normalised kick is stable for any dt |D|).  With nproj = 0 it is the same map as mlmd_propagate. */
-int mlmd_propagate_split(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
+MLMD_API int mlmd_propagate_split(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
 
 /* rho(r) = sum_n f_n |psi_n(r)|^2 of the current state, float [ndom][nx][ny][nz] at `where`. */
-int mlmd_density(mlmd_domain_t *h, float *rho, int where);
+MLMD_API int mlmd_density(mlmd_domain_t *h, float *rho, int where);
 
 /* S[dom] = dv * Phi^H Psi(t), complex64 [ndom][norb][norb] at `where` (CGEMM(1)):
  * which = 0: Phi = Psi(t) (Gram matrix); which = 1: Phi = Psi(0) (needs MLMD_KEEP_PSI0).
  * Always evaluated in the FP32-grade (or FP64) GEMM mode: it is a measurement. */
-int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
+MLMD_API int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
 
 /* Occupations of the t = 0 orbitals and number of excited electrons per domain (LFD hands the
  * occupation numbers f_s back to QXMD; L159: n_exc "is computed from f_s"; L283: overlap matrix between the
@@ -136,7 +162,7 @@ int mlmd_overlap(mlmd_domain_t *h, int which, void *S_c64, int where);
  *     f_s(t) = sum_n f_n |S_sn|^2,  S = dv Psi(0)^H Psi(t) (mlmd_overlap which = 1; needs MLMD_KEEP_PSI0),
  *     n_exc  = sum_s max(f_s(0) - f_s(t), 0).
  * f: double [ndom][norb], n_exc: double [ndom], both at `where`. */
-int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int where);
+MLMD_API int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int where);
 
 /* Observables of the current state that feed the light-matter loop ("GEMMification is applied to
  * nonlocal correction in energy and electric current ... used in Maxwell's equations"; SURVEY.md 8(f) NEXT-2;
@@ -146,8 +172,8 @@ int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int where);
  * mlmd_current: J[dom][d] = sum_n f_n Re<psi_n| -i D1_d + A_d |psi_n>, D1 the 4th-order first difference of H,
  *   A: double [a_ndom][3] HOST (a_ndom = 1 or ndom), J: double [ndom][3] at `where`.  This is the current of
  *   h_loc's velocity operator; the nonlocal-pseudopotential term -i[r, V_NL] is not included (D30). */
-int mlmd_energy_nl(mlmd_domain_t *h, double *E, int where);
-int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int where);
+MLMD_API int mlmd_energy_nl(mlmd_domain_t *h, double *E, int where);
+MLMD_API int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int where);
 
 /* Per-kernel-class timing of mlmd_propagate with CUDA events on the handle's stream (bench.py's
  * roofline numbers).  mlmd_profile(h, 1) starts recording (and clears earlier records),
@@ -156,18 +182,18 @@ int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int w
 enum { MLMD_K_STENCIL = 0, MLMD_K_PROJ = 1, MLMD_K_BACK = 2, MLMD_K_GLUE = 3, MLMD_K_DENSITY = 4,
        MLMD_K_NLP = 5 /* fused back-application + projection */,
        MLMD_K_NORM = 6 /* per-orbital norms of the split step */, MLMD_K_COUNT = 7 };
-int mlmd_profile(mlmd_domain_t *h, int enable);
-int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *launches);
+MLMD_API int mlmd_profile(mlmd_domain_t *h, int enable);
+MLMD_API int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *launches);
 
 /* Which kernels run the nonlocal GEMMs for the current mode and shape: 0 = CUDA cores (SIMT),
  * 1 = tcgen05 tensor cores. */
-int mlmd_gemm_path(const mlmd_domain_t *h);
+MLMD_API int mlmd_gemm_path(const mlmd_domain_t *h);
 
 /* Number of kernels the library launched on this handle since create (bench.py's gpu_launches). */
-long long mlmd_launch_count(const mlmd_domain_t *h);
+MLMD_API long long mlmd_launch_count(const mlmd_domain_t *h);
 
 /* Thread-local description of the last failure in this thread; never NULL. */
-const char *mlmd_last_error(void);
+MLMD_API const char *mlmd_last_error(void);
 
 #ifdef __cplusplus
 }

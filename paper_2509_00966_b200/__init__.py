@@ -17,6 +17,7 @@ from .api import (  # noqa: F401
     mlmd_set_vloc,
     mlmd_set_projectors,
     mlmd_set_gemm_mode,
+    mlmd_set_option,
     mlmd_propagate,
     mlmd_propagate_split,
     mlmd_density,
@@ -32,6 +33,7 @@ from .api import (  # noqa: F401
     EXPORTED_SYMBOLS,
     HOST, DEVICE, BETA_REAL32, BETA_COMPLEX64,
     GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT, GEMM_FP32GRADE_STAGED,
-    KEEP_PSI0, CHECK_FINITE,
+    KEEP_PSI0, CHECK_FINITE, BORROW_PSI,
+    OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM,
     OK, WARN_UNSTABLE,
 )

@@ -14,16 +14,18 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmlmd.so")
+TEST_LIB_PATH = os.path.join(HERE, "libmlmd_test.so")   # product objects + kernel-level test hooks; tests/ only
 
 OK, ERR_ARG, ERR_SHAPE, ERR_STATE, ERR_CUDA, ERR_NOMEM, ERR_NONFINITE, WARN_UNSTABLE = range(8)
 HOST, DEVICE = 0, 1
 BETA_REAL32, BETA_COMPLEX64 = 0, 1
 GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT, GEMM_FP32GRADE_STAGED = range(6)
-KEEP_PSI0, CHECK_FINITE = 1, 2
+KEEP_PSI0, CHECK_FINITE, BORROW_PSI = 1, 2, 4
+OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM = range(4)
 
 EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",
-    "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_propagate",
+    "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_set_option", "mlmd_propagate",
     "mlmd_propagate_split", "mlmd_occupations", "mlmd_energy_nl", "mlmd_current",
     "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
 ]
@@ -58,6 +60,7 @@ def lib() -> ctypes.CDLL:
         L.mlmd_set_vloc.argtypes = [p, p, i]
         L.mlmd_set_projectors.argtypes = [p, i, p, i, p, i]
         L.mlmd_set_gemm_mode.argtypes = [p, i]
+        L.mlmd_set_option.argtypes = [p, i, i]
         L.mlmd_propagate.argtypes = [p, i, d, p, i]
         L.mlmd_propagate_split.argtypes = [p, i, d, p, i]
         L.mlmd_density.argtypes = [p, p, i]
@@ -162,6 +165,10 @@ def mlmd_set_projectors(h, nproj, beta, D):
 
 def mlmd_set_gemm_mode(h, mode):
     _check(lib().mlmd_set_gemm_mode(h, mode))
+
+
+def mlmd_set_option(h, key, value):
+    _check(lib().mlmd_set_option(h, key, value))
 
 
 def mlmd_propagate(h, nsteps, dt, A) -> int:
@@ -284,6 +291,9 @@ class Domain:
 
     def set_gemm_mode(self, mode):
         mlmd_set_gemm_mode(self.handle, mode)
+
+    def set_option(self, key, value):
+        mlmd_set_option(self.handle, key, value)
 
     def propagate(self, nsteps, dt, A):
         return mlmd_propagate(self.handle, nsteps, dt, A)

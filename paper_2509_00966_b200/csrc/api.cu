@@ -18,11 +18,13 @@ using namespace mlmd;
 static const int kProjChain = 128, kOverlapChain = 4;
 // The drift counts MMAs, not stages: a one-product projection issues a third of the MMAs per stage, so three times
 // the stages give the same accumulation error with a third of the chain drains (each drain idles the tensor pipe).
-static int proj_chain(int nprod) {
-    static const int c3 = getenv("MLMD_PROJ_CHAIN") ? atoi(getenv("MLMD_PROJ_CHAIN")) : 0;   // A/B checks
-    const int base = c3 > 0 ? c3 : kProjChain;
-    return nprod == 3 ? base : 3 * base;
-}
+static int proj_chain(int nprod) { return nprod == 3 ? kProjChain : 3 * kProjChain; }
+// The three inner Horner stages: whatever error their projections make reaches psi damped by the later stages
+// (DESIGN.md 5.6), so their chains are 1024 stages: one or two drains per K slice.
+static const int kInnerChain = 8 * kProjChain;
+// MLMD_GEMM_FP32GRADE_STAGED: Horner stages 0-2 (tau = dt/4, dt/3, dt/2) run with reduced products; their projection
+// is one product with psi rounded to the nearest TF32 in shared memory (nprod code 4)
+static const int kStagedMask = 0x7, kStagedProjNprod = 4;
 
 static thread_local char g_err[512] = "";
 
@@ -72,14 +74,13 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
         return at;
     };
     Workspace &w = pl->off;
-    w.psi = take(psi_b);
+    w.psi = take((flags & MLMD_BORROW_PSI) ? 0 : psi_b);
     w.ua = take(psi_b);
     w.ub = take(psi_b);
     w.psi0 = take((flags & MLMD_KEEP_PSI0) ? psi_b : 0);
     w.vloc = take(npts * sizeof(float));
     // + slack: the last 32-column TMA chunk of a row may read up to 128 B past the row
-    w.beta = take(npts * pl->ldp_max * sizeof(float) + 256);
-    w.beta_lo = take(npts * pl->ldp_max * sizeof(float) + 256);
+    w.beta = take(npts * pl->ldp_max * sizeof(float) + 256);   // ONE FP32 copy: the kernels form hi / lo in shared memory
     w.dprime = take((size_t)ndom * pl->ldp_max * sizeof(float));
     w.occ = take((size_t)ndom * pl->ld * sizeof(float));
     w.rho = take(npts * sizeof(float));
@@ -118,11 +119,15 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     *out = nullptr;
     if (!workspace_dev) return fail(MLMD_ERR_ARG, "mlmd_domain_create: workspace is NULL");
     if (!(hx > 0) || !(hy > 0) || !(hz > 0)) return fail(MLMD_ERR_ARG, "mlmd_domain_create: grid spacings must be > 0");
-    if (flags & ~(MLMD_KEEP_PSI0 | MLMD_CHECK_FINITE)) return fail(MLMD_ERR_ARG, "mlmd_domain_create: unknown flags 0x%x", flags);
+    if (flags & ~(MLMD_KEEP_PSI0 | MLMD_CHECK_FINITE | MLMD_BORROW_PSI))
+        return fail(MLMD_ERR_ARG, "mlmd_domain_create: unknown flags 0x%x", flags);
     Plan pl;
     if (!make_plan(ndom, nx, ny, nz, norb, nproj_max, flags, &pl))
         return fail(MLMD_ERR_SHAPE, "mlmd_domain_create: bad shape ndom=%d grid=%dx%dx%d norb=%d nproj_max=%d "
                     "(every grid axis must be >= 5)", ndom, nx, ny, nz, norb, nproj_max);
+    if ((flags & MLMD_BORROW_PSI) && norb % 16)
+        return fail(MLMD_ERR_SHAPE, "mlmd_domain_create: MLMD_BORROW_PSI needs norb %% 16 == 0 (rows of the caller's buffer are "
+                    "used unpadded), got norb=%d", norb);
     if (workspace_bytes < pl.off.total)
         return fail(MLMD_ERR_SHAPE, "mlmd_domain_create: workspace has %zu bytes, needs %zu", workspace_bytes, pl.off.total);
     if (((uintptr_t)workspace_dev) % 256) return fail(MLMD_ERR_ARG, "mlmd_domain_create: workspace must be 256-byte aligned");
@@ -143,29 +148,18 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->ws = (char *)workspace_dev; h->ws_bytes = workspace_bytes; h->off = pl.off;
     h->nproj = 0; h->beta_complex = 0; h->P = 0; h->ldp = pl.ldp_max; h->prows = pl.prows; h->nsplit = pl.nsplit;
     h->nsplit_tc = pl.nsplit_tc; h->nsplit_tc_ovl = pl.nsplit_tc_ovl;
-    {
-        const char *force = getenv("MLMD_GEMM_PATH");   // "simt": keep the GEMMs on CUDA cores (A/B checks)
-        h->tc_ok = tc_available() && pl.ngrid % 128 == 0 && !(force && strcmp(force, "simt") == 0);
-    }
+    h->tc_ok = tc_available() && pl.ngrid % 128 == 0;
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
-    h->staged_mask = 0x7;                                // stages 0-2 (tau = dt/4, dt/3, dt/2) of the staged mode
-    if (const char *m = getenv("MLMD_STAGED_MASK")) h->staged_mask = atoi(m) & 0xf;   // A/B checks
-    h->inner_chain = 8 * kProjChain;
-    if (const char *m = getenv("MLMD_INNER_CHAIN")) h->inner_chain = atoi(m);   // A/B checks; <= 0: the mode's own length
-    h->staged_chain = 8 * kProjChain;
-    if (const char *m = getenv("MLMD_STAGED_CHAIN")) h->staged_chain = atoi(m) > 0 ? atoi(m) : h->staged_chain;   // A/B checks
-    h->staged_proj_nprod = 4;                            // one product, psi rounded to nearest (1: truncated by the MMA)
-    if (const char *m = getenv("MLMD_STAGED_PROJ")) h->staged_proj_nprod = atoi(m) == 1 ? 1 : 4;
+    for (int k = 0; k < MLMD_OPT_COUNT; ++k) h->opt[k] = 0;
+    h->opt[MLMD_OPT_GRAPH] = 1;
+    h->psi_ptr = (flags & MLMD_BORROW_PSI) ? nullptr : (float2 *)(h->ws + pl.off.psi);
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
     h->coef_host = nullptr; h->flag_host = nullptr; h->prof_on = false;
     h->coef_uploaded = nullptr; h->gexec = nullptr; h->gstream = nullptr; h->gfork = h->gjoin = nullptr;
     h->g_launches = 0; h->g_dt = 0.0; h->g_yz = false; h->g_split = false;
     h->gram_valid = false; h->ldg = pl.ldp_max; h->split_pending = false;
-    {
-        const char *g = getenv("MLMD_GRAPH");   // "0": never capture the step into a CUDA graph
-        h->graph_allowed = !(g && g[0] == '0');
-    }
+    h->graph_allowed = true;
     cudaError_t e = cudaMallocHost((void **)&h->coef_host, (size_t)kCoefCapacity * ndom * sizeof(StepCoef));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&h->flag_host, 256);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->coef_uploaded, cudaEventDisableTiming);
@@ -228,7 +222,7 @@ int mlmd_profile_read(mlmd_domain_t *h, int kind, double *ms_total, long long *l
 long long mlmd_launch_count(const mlmd_domain_t *h) { return h ? h->launches : 0; }
 
 static bool use_tensor_cores(const mlmd_domain *h) {
-    return h->tc_ok && (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_TF32X1 ||
+    return h->tc_ok && h->opt[MLMD_OPT_GEMM_PATH] == 0 && (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_TF32X1 ||
                         h->gemm_mode == MLMD_GEMM_LOWP_BF16 || h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED);
 }
 // products per MAC on the tensor-core path: 3 = 3xTF32, 1 = TF32x1, 0 = BF16-rounded operands x1
@@ -265,9 +259,16 @@ int mlmd_set_orbitals(mlmd_domain_t *h, const void *psi, const double *occ, int 
         CU(cudaStreamSynchronize(h->stream));
         h->have_occ = true;
     }
-    if (h->ld != h->norb) CU(cudaMemsetAsync(h->psi(), 0, rows * h->ld * sizeof(float2), h->stream));
-    CU(cudaMemcpy2DAsync(h->psi(), (size_t)h->ld * sizeof(float2), psi, (size_t)h->norb * sizeof(float2),
-                         (size_t)h->norb * sizeof(float2), rows, kind_in(where), h->stream));
+    if (h->flags & MLMD_BORROW_PSI) {
+        // adopt the caller's device buffer: every step updates it in place
+        if (where != MLMD_DEVICE) return fail(MLMD_ERR_ARG, "mlmd_set_orbitals: MLMD_BORROW_PSI needs a device pointer");
+        if (((uintptr_t)psi) % 256) return fail(MLMD_ERR_ARG, "mlmd_set_orbitals: a borrowed Psi buffer must be 256-byte aligned");
+        h->psi_ptr = (float2 *)psi;
+    } else {
+        if (h->ld != h->norb) CU(cudaMemsetAsync(h->psi(), 0, rows * h->ld * sizeof(float2), h->stream));
+        CU(cudaMemcpy2DAsync(h->psi(), (size_t)h->ld * sizeof(float2), psi, (size_t)h->norb * sizeof(float2),
+                             (size_t)h->norb * sizeof(float2), rows, kind_in(where), h->stream));
+    }
     if (h->flags & MLMD_KEEP_PSI0)
         CU(cudaMemcpyAsync(h->psi0(), h->psi(), rows * h->ld * sizeof(float2), cudaMemcpyDeviceToDevice, h->stream));
     if (where == MLMD_HOST) CU(cudaStreamSynchronize(h->stream));
@@ -282,8 +283,9 @@ int mlmd_get_orbitals(mlmd_domain_t *h, void *psi, int where) {
     if (bad_where(where)) return fail(MLMD_ERR_ARG, "mlmd_get_orbitals: bad where=%d", where);
     if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_get_orbitals: no orbitals set");
     const size_t rows = (size_t)h->ndom * h->ngrid;
-    CU(cudaMemcpy2DAsync(psi, (size_t)h->norb * sizeof(float2), h->psi(), (size_t)h->ld * sizeof(float2),
-                         (size_t)h->norb * sizeof(float2), rows, kind_out(where), h->stream));
+    if (psi != (void *)h->psi())    // a borrowed buffer read back into itself is already there
+        CU(cudaMemcpy2DAsync(psi, (size_t)h->norb * sizeof(float2), h->psi(), (size_t)h->ld * sizeof(float2),
+                             (size_t)h->norb * sizeof(float2), rows, kind_out(where), h->stream));
     if (where == MLMD_HOST) CU(cudaStreamSynchronize(h->stream));
     return MLMD_OK;
 }
@@ -347,9 +349,9 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
     if (ldp != P) CU(cudaMemsetAsync(h->beta(), 0, rows * ldp * sizeof(float), h->stream));
     CU(cudaMemcpy2DAsync(h->beta(), (size_t)ldp * sizeof(float), beta, (size_t)P * sizeof(float), (size_t)P * sizeof(float),
                          rows, kind_in(where), h->stream));
-    int nl = 0;
-    CU(launch_split_tf32(h->stream, h->beta(), h->beta_lo(), rows * ldp, &nl));
-    h->launches += nl;
+    // rows [P, ldp) of W are read (times zero columns of beta) by the K = 8 slabs of the back-application: a stale NaN
+    // left there by an earlier projector set or a diverged run would poison psi
+    CU(cudaMemsetAsync(h->what(), 0, 2 * (h->off.what_lo - h->off.what), h->stream));
     CU(cudaStreamSynchronize(h->stream));   // dp is a temporary; host beta may be reused by the caller
     h->nproj = nproj; h->beta_complex = cplx; h->P = P; h->ldp = ldp; h->dmax = dmax;
     return MLMD_OK;
@@ -360,6 +362,16 @@ int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
     drop_graph(h);
     if (mode < MLMD_GEMM_FP32GRADE || mode > MLMD_GEMM_FP32GRADE_STAGED) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: bad mode %d", mode);
     h->gemm_mode = mode;
+    return MLMD_OK;
+}
+
+int mlmd_set_option(mlmd_domain_t *h, int key, int value) {
+    if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_option: NULL handle");
+    static const int nvalues[MLMD_OPT_COUNT] = {2, 3, 2, 2};
+    if (key < 0 || key >= MLMD_OPT_COUNT) return fail(MLMD_ERR_ARG, "mlmd_set_option: unknown key %d", key);
+    if (value < 0 || value >= nvalues[key]) return fail(MLMD_ERR_ARG, "mlmd_set_option: key %d takes 0..%d, got %d", key, nvalues[key] - 1, value);
+    drop_graph(h);      // a captured step bakes the kernel choice in
+    h->opt[key] = value;
     return MLMD_OK;
 }
 
@@ -396,10 +408,10 @@ int mlmd_energy_nl(mlmd_domain_t *h, double *E, int where) {
         const bool tc = use_tensor_cores(h);
         const int nsplit = tc ? h->nsplit_tc : h->nsplit;
         if (tc)
-            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)h->psi(),
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, tc_nprod(h), proj_chain(tc_nprod(h)), &nl));
+            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)h->psi(),
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, tc_nprod(h), proj_chain(tc_nprod(h)), &nl, &h->tmaps));
         else
-            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)h->psi(),
+            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)h->psi(),
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, &nl));
         CU(launch_energy_nl(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, nsplit, h->zpart(), h->dprime(),
                             h->occ(), h->dv, ed, &nl));
@@ -487,10 +499,10 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl,
     {
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
-            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, chain > 0 ? chain : proj_chain(nprod), nl));
+            CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, chain > 0 ? chain : proj_chain(nprod), nl, &h->tmaps));
         else
-            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, (const float *)w,
+            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
     }
     ProfScope ps(h, MLMD_K_GLUE);
@@ -504,10 +516,10 @@ static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl, int nprod = -1) {
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     ProfScope ps(h, MLMD_K_BACK);
     if (use_tensor_cores(h))
-        CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
-                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, nprod, nl));
+        CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, h->what(), h->what_lo(),
+                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, nprod, nl, &h->tmaps));
     else
-        CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
+        CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, h->what(), h->what_lo(),
                             (float *)out, 2 * h->ld, 2 * h->ld, h->prows, fp64, nl));
     return MLMD_OK;
 }
@@ -526,13 +538,12 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
     const bool staged = h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED && use_tensor_cores(h);
     for (int i = 0; i < 4; ++i) {
         const float tau = (float)(dt / (4 - i));
-        const bool reduced = staged && ((h->staged_mask >> i) & 1);
+        const bool reduced = staged && ((kStagedMask >> i) & 1);
         if (h->nproj > 0) {
             // inner stages: their accumulation drift is damped like every other projection error (weights <= dt/2 E
             // ~ 0.05 of the outer stage's), so the chains are 1024 stages: one or two drains per K slice instead of one per 128 stages
             // the three inner stages of every tensor-core mode take the long chains (the products stay as the mode says)
-            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? h->staged_proj_nprod : -1,
-                                      reduced ? h->staged_chain : (i < 3 ? h->inner_chain : -1));
+            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? kStagedProjNprod : -1, i < 3 ? kInnerChain : -1);
             if (rc) return rc;
         }
         {
@@ -702,7 +713,7 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
     int nl = 0;
     // Small problems are launch-bound (17 launches per step): after one eager step the step is captured
     // into a CUDA graph that reads its stencil coefficients from a device slot.
-    const bool want_graph = h->graph_allowed && !h->prof_on && nsteps >= 4 &&
+    const bool want_graph = h->graph_allowed && h->opt[MLMD_OPT_GRAPH] && !h->prof_on && nsteps >= 4 &&
                             (double)h->ndom * (double)h->ngrid * h->ld <= (double)(1 << 23);
     if (h->gexec && (h->g_dt != dt || h->g_yz != yz || h->g_split != split)) drop_graph(h);
     auto one_step = [&](const StepCoef *coef, const StepCoef *coef_host, bool last) {
@@ -712,16 +723,15 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
         int rc = flush_split_scale(h, &nl);      // only after a split call that failed half-way
         if (rc) return rc;
     }
+    if (h->opt[MLMD_OPT_KICK_NORM]) h->gram_valid = false;
     if (split && nsteps > 0 && h->nproj > 0 && !h->gram_valid && h->ldp <= 2 * h->ld && h->P <= 1024 &&
-        !(getenv("MLMD_KICK_IDENTITY") && atoi(getenv("MLMD_KICK_IDENTITY")) == 0)) {
-        // one-time per projector set: G = beta^T beta from two CUDA-core projections of beta (stored as hi + lo) onto
-        // its hi and its lo part (the zpart scratch holds [prows][ldp] partials per slice, ldp <= 2 ld)
+        !h->opt[MLMD_OPT_KICK_NORM]) {
+        // one-time per projector set: G = beta^T beta by a CUDA-core projection of beta onto itself (exact FP32 products;
+        // the zpart scratch holds [prows][ldp] partials per slice, ldp <= 2 ld)
         ProfScope ps(h, MLMD_K_GLUE);
-        for (int part = 0; part < 2; ++part) {
-            CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, part ? h->beta_lo() : h->beta(),
-                                h->ldp, h->ldp, h->zpart(), h->prows, h->nsplit, false, &nl));
-            CU(launch_gram_reduce(h->stream, h->ndom, h->P, h->ldg, h->prows, h->ldp, h->nsplit, h->zpart(), h->gram(), part, &nl));
-        }
+        CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, h->beta(), h->ldp, h->ldp, h->zpart(),
+                            h->prows, h->nsplit, false, &nl));
+        CU(launch_gram_reduce(h->stream, h->ndom, h->P, h->ldg, h->prows, h->ldp, h->nsplit, h->zpart(), h->gram(), 0, &nl));
         h->gram_valid = true;
     }
     if (split && nsteps > 0 && h->nproj > 0) {      // squared norms of the incoming orbitals (reading D27)
@@ -821,11 +831,12 @@ int mlmd_overlap(mlmd_domain_t *h, int which, void *S, int where) {
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     // projection GEMM with B := float view of Phi (2*ld real rows), S4 of SURVEY.md 8(a); always
     // FP32-grade (3xTF32 on tensor cores, or the CUDA-core path): it is a measurement
-    const bool tc = h->tc_ok && h->gemm_mode != MLMD_GEMM_FP64 && h->gemm_mode != MLMD_GEMM_FP32_SIMT;
+    const bool tc = h->tc_ok && h->opt[MLMD_OPT_GEMM_PATH] == 0 && h->gemm_mode != MLMD_GEMM_FP64 &&
+                    h->gemm_mode != MLMD_GEMM_FP32_SIMT;
     const int nsplit = tc ? h->nsplit_tc_ovl : h->nsplit;
     if (tc)
         CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, (const float *)phi, nullptr, 2 * h->ld, 2 * h->ld,
-                          (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, 3, kOverlapChain, &nl));
+                          (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, 3, kOverlapChain, &nl, &h->tmaps));
     else
         CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, (const float *)phi, nullptr, 2 * h->ld, 2 * h->ld,
                             (const float *)h->psi(), 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, &nl));

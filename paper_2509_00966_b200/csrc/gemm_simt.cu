@@ -20,8 +20,12 @@ proj_simt_kernel(long ngrid, const float *__restrict__ B, const float *__restric
                  const float *__restrict__ Y, int ldy, int N, float *__restrict__ zpart, int prows, int nsplit) {
     __shared__ float Bs[TK][TM + 4];
     __shared__ float Ys[TK][TN + 4];
-    const int dom = blockIdx.z / nsplit, split = blockIdx.z % nsplit;
-    const int p0 = blockIdx.y * TM, c0 = blockIdx.x * TN;
+    // grid.x = column tile + ntile_n * (split + nsplit * dom): the batch rides on the x dimension (2^31 - 1 blocks),
+    // so neither many domains nor many slices can exceed the 65535 limit of grid.y / grid.z
+    const int ntile_n = (N + TN - 1) / TN;
+    const int bz = blockIdx.x / ntile_n;
+    const int dom = bz / nsplit, split = bz % nsplit;
+    const int p0 = blockIdx.y * TM, c0 = (blockIdx.x % ntile_n) * TN;
     const long rlo = ngrid * split / nsplit, rhi = ngrid * (split + 1) / nsplit;
     const float *Bd = B + (size_t)dom * ngrid * ldb;
     const float *Bl = Blo ? Blo + (size_t)dom * ngrid * ldb : nullptr;   // B = hi + lo (exact)
@@ -78,11 +82,13 @@ back_simt_kernel(long ngrid, const float *__restrict__ B, const float *__restric
                  int prows) {
     __shared__ float As[TK][TM + 4];   // As[k][r]
     __shared__ float Ws[TK][TN + 4];
-    const int dom = blockIdx.z;
-    const long r0 = (long)blockIdx.y * TM;
-    const int c0 = blockIdx.x * TN;
+    // grid.x = row tile + nrt * dom (large grids: up to 2^31 - 1 blocks), grid.y = column tile
+    const long nrt = (ngrid + TM - 1) / TM;
+    const int dom = (int)(blockIdx.x / nrt);
+    const long r0 = (long)(blockIdx.x % nrt) * TM;
+    const int c0 = blockIdx.y * TN;
     const float *Bd = B + (size_t)dom * ngrid * ldb;
-    const float *Bl = Blo + (size_t)dom * ngrid * ldb;     // operands are stored as exact hi + lo pairs
+    const float *Bl = Blo ? Blo + (size_t)dom * ngrid * ldb : nullptr;   // optional exact remainder of B
     const float *Wd = What + (size_t)dom * prows * N;
     const float *Wl = Wlo + (size_t)dom * prows * N;
     float *Yd = Y + (size_t)dom * ngrid * ldy;
@@ -99,7 +105,7 @@ back_simt_kernel(long ngrid, const float *__restrict__ B, const float *__restric
             {   // A tile: 64 rows x 16 k; consecutive threads walk k (contiguous in memory)
                 const int rr = idx / 16, kk = idx % 16;
                 const long r = r0 + rr;
-                As[kk][rr] = (r < ngrid && k0 + kk < P) ? Bd[r * ldb + k0 + kk] + Bl[r * ldb + k0 + kk] : 0.f;
+                As[kk][rr] = (r < ngrid && k0 + kk < P) ? (Bl ? Bd[r * ldb + k0 + kk] + Bl[r * ldb + k0 + kk] : Bd[r * ldb + k0 + kk]) : 0.f;
             }
             {
                 const int kk = idx / 64, cc = idx % 64;
@@ -136,7 +142,9 @@ back_simt_kernel(long ngrid, const float *__restrict__ B, const float *__restric
 cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
                              const float *Y, int ldy, int N, float *zpart, int prows, int nsplit,
                              bool fp64, int *nlaunch) {
-    dim3 grid((N + TN - 1) / TN, (P + TM - 1) / TM, ndom * nsplit);
+    const long gx = (long)((N + TN - 1) / TN) * ndom * nsplit;
+    if (gx > 0x7fffffffL || (P + TM - 1) / TM > 65535) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)gx, (P + TM - 1) / TM, 1);
     ++*nlaunch;
     if (fp64)
         proj_simt_kernel<double><<<grid, 256, 0, st>>>(ngrid, B, Blo, ldb, P, Y, ldy, N, zpart, prows, nsplit);
@@ -148,7 +156,9 @@ cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float 
 cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
                              const float *What, const float *Wlo, float *Y, int ldy, int N, int prows, bool fp64,
                              int *nlaunch) {
-    dim3 grid((N + TN - 1) / TN, (unsigned)((ngrid + TM - 1) / TM), ndom);
+    const long gx = ((ngrid + TM - 1) / TM) * ndom;
+    if (gx > 0x7fffffffL || (N + TN - 1) / TN > 65535) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)gx, (N + TN - 1) / TN, 1);
     ++*nlaunch;
     if (fp64)
         back_simt_kernel<double><<<grid, 256, 0, st>>>(ngrid, B, Blo, ldb, P, What, Wlo, Y, ldy, N, prows);

@@ -52,8 +52,10 @@ EncodeTiledFn encode_fn() {
 // columns); a box (32, box_rows, box_chunks) lands in shared memory as box_chunks consecutive
 // [box_rows x 128 B] regions in the 128B-span / 32B-atom swizzle = UMMA MN-major SWIZZLE_128B_BASE32B
 // atoms (4 K-rows x 32 MN-elements each; the only MN-major layout tcgen05 takes for TF32 operands).
-bool make_chunk_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t pitch, uint64_t nchunk, uint32_t box_rows,
-                    uint32_t box_chunks) {
+bool make_chunk_map(TmapCache *cache, CUtensorMap *m, const float *base, uint64_t rows, uint64_t pitch, uint64_t nchunk,
+                    uint32_t box_rows, uint32_t box_chunks);
+bool make_chunk_map_raw(CUtensorMap *m, const float *base, uint64_t rows, uint64_t pitch, uint64_t nchunk, uint32_t box_rows,
+                        uint32_t box_chunks) {
     EncodeTiledFn f = encode_fn();
     if (!f) return false;
     cuuint64_t dims[3] = {32, rows, nchunk};
@@ -66,7 +68,7 @@ bool make_chunk_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t p
 
 // Plain 2-D view (cols, rows) with a (8 floats = 32 B, box_rows) box and the 32-byte swizzle = UMMA
 // K-major SWIZZLE_32B layout of one K = 8 slab.
-bool make_k8_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch, uint32_t box_rows) {
+bool make_k8_map_raw(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch, uint32_t box_rows) {
     EncodeTiledFn f = encode_fn();
     if (!f) return false;
     cuuint64_t dims[2] = {cols, rows};
@@ -78,7 +80,7 @@ bool make_k8_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols
 }
 
 // (cols, rows) view with a [128 rows x 32 floats] box in the plain 128-byte swizzle: epilogue staging tiles
-bool make_out_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch) {
+bool make_out_map_raw(CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch) {
     EncodeTiledFn f = encode_fn();
     if (!f) return false;
     cuuint64_t dims[2] = {cols, rows};
@@ -87,6 +89,21 @@ bool make_out_map(CUtensorMap *m, const float *base, uint64_t rows, uint64_t col
     cuuint32_t es[2] = {1, 1};
     return f(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// the same three encoders through the handle's cache
+bool make_chunk_map(TmapCache *cache, CUtensorMap *m, const float *base, uint64_t rows, uint64_t pitch, uint64_t nchunk,
+                    uint32_t box_rows, uint32_t box_chunks) {
+    const TmapKey k{1, base, rows, pitch, nchunk, 0, box_rows, box_chunks};
+    return cached_tmap(cache, k, m, [&](CUtensorMap *o) { return make_chunk_map_raw(o, base, rows, pitch, nchunk, box_rows, box_chunks); });
+}
+bool make_k8_map(TmapCache *cache, CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch, uint32_t box_rows) {
+    const TmapKey k{2, base, rows, cols, pitch, 0, box_rows, 0};
+    return cached_tmap(cache, k, m, [&](CUtensorMap *o) { return make_k8_map_raw(o, base, rows, cols, pitch, box_rows); });
+}
+bool make_out_map(TmapCache *cache, CUtensorMap *m, const float *base, uint64_t rows, uint64_t cols, uint64_t pitch) {
+    const TmapKey k{3, base, rows, cols, pitch, 0, 0, 0};
+    return cached_tmap(cache, k, m, [&](CUtensorMap *o) { return make_out_map_raw(o, base, rows, cols, pitch); });
 }
 
 constexpr int EPI_TILE_BYTES = 128 * 128;   // one staging tile: 128 rows x 32 floats
@@ -131,6 +148,14 @@ __device__ __forceinline__ float tf32_rn(float x) {
     return __uint_as_float(u & 0xffffe000u);
 }
 __device__ __forceinline__ float4 tf32_rn4(const float4 v) { return make_float4(tf32_rn(v.x), tf32_rn(v.y), tf32_rn(v.z), tf32_rn(v.w)); }
+
+// in place: v -> nearest TF32 value hi, returns lo = v - hi (exact in FP32; |lo| <= half a TF32 ulp of v)
+__device__ __forceinline__ float4 split4_rn(float4 &v) {
+    const float4 h = tf32_rn4(v);
+    const float4 l = make_float4(v.x - h.x, v.y - h.y, v.z - h.z, v.w - h.w);
+    v = h;
+    return l;
+}
 
 // round-to-nearest-even to BF16 precision, kept in an FP32 container (every BF16 value is a TF32 value)
 __device__ __forceinline__ float bf16_round(float x) {
@@ -206,7 +231,7 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     const int nntp = (q.ntile_n + 1) / 2;          // pairs of column tiles: one per cluster unit
     const int total = q.ndom * q.ntile_m * nntp * q.nsplit;   // cluster units
     const bool need_lo = q.nprod == 3;
-    const bool need_conv = need_lo || q.lowp || q.rn;   // converter warps touch every stage
+    const bool need_conv = true;        // beta arrives as one raw FP32 copy: the converter warps touch every stage
     const bool load_alo = need_lo && !q.conv_a;
     const uint32_t y_bytes = (uint32_t)(q.BN / 32) * PJ_BK * 128;
     const uint32_t tx_bytes = PJ_A_BYTES * (load_alo ? 2u : 1u) + y_bytes;
@@ -316,18 +341,23 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                         fence_proxy_async_smem();
                         mbar_arrive(&conv[s]);
                     }
-                } else if (q.rn) {
-                    // one product, unbiased: psi rounded to the nearest TF32 in place (the MMA alone would truncate;
-                    // beta_hi was rounded to nearest when the projectors were set)
+                } else if (!need_lo) {
+                    // one product: beta rounded to the nearest TF32 in place (an unbiased operand; the MMA alone would
+                    // truncate), and psi too when q.rn (staged inner stages); plain TF32x1 leaves psi to the MMA
                     for (int kb = c0k; kb < c1k; ++kb, ++it) {
                         const int s = it % NST;
                         mbar_wait(&full[s], (it / NST) & 1);
-                        float4 *y4 = (float4 *)(smem + s * SB + YOFF);
-                        for (int i = t; i < ny4; i += 128) y4[i] = tf32_rn4(y4[i]);
+                        uint8_t *st = smem + s * SB;
+                        float4 *a4 = (float4 *)st;
+                        for (int i = t; i < PJ_A_BYTES / 16; i += 128) a4[i] = tf32_rn4(a4[i]);
+                        if (q.rn) {
+                            float4 *y4 = (float4 *)(st + YOFF);
+                            for (int i = t; i < ny4; i += 128) y4[i] = tf32_rn4(y4[i]);
+                        }
                         fence_proxy_async_smem();
                         mbar_arrive(&conv[s]);
                     }
-                } else if (need_lo) {
+                } else {
                     for (int kb = c0k; kb < c1k; ++kb, ++it) {
                         const int s = it % NST;
                         mbar_wait(&full[s], (it / NST) & 1);
@@ -340,11 +370,13 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                             ydst[i] = split4(v);   // the hi tile stays as loaded: kind::tf32 ignores the 13 low bits
                         }
                         if (q.conv_a) {
+                            // beta / Phi: nearest TF32 in place + exact remainder (as round 1's stored hi / lo pair)
                             float4 *asrc = (float4 *)st;
                             float4 *adst = (float4 *)(st + PJ_A_BYTES);
                             for (int i = t; i < PJ_A_BYTES / 16; i += 128) {
                                 float4 v = asrc[i];
-                                adst[i] = split4(v);
+                                adst[i] = split4_rn(v);
+                                asrc[i] = v;
                             }
                         }
                         fence_proxy_async_smem();
@@ -384,6 +416,243 @@ proj_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
 }
 
 // =================================================================================================
+// Projection on CTA PAIRS (tcgen05 cta_group::2): Z[p][c] = sum_r A[r][p] * Y[r][c] over one K slice.
+// One UMMA spans two SMs: M = 256 projector rows (128 per CTA: each CTA stages only its own 4 chunks of the beta
+// tile) x BN <= 448 columns, the psi tile split by columns between the two shared memories.  With single-CTA UMMAs
+// (proj_tc_kernel) every CTA re-reads the psi tile once per 128-row block and the operand reads alone take ~98 of the
+// 128 B/cycle of shared-memory bandwidth (tensor pipe 67 % active, round 1); the pair reads every operand byte once:
+// ~49 B/cycle.  beta and psi both arrive as plain FP32; the four converter / epilogue warps of EACH CTA form the
+// operand pairs of their own tiles in shared memory (beta: nearest TF32 in place + exact remainder; psi: remainder
+// only, the hi product reads the raw tile, whose 13 low bits kind::tf32 ignores), so the leader's single MMA thread
+// needs to know that BOTH CTAs have converted a stage: the leader's converters arrive on its `conv` barrier directly,
+// the peer's arrive on a local barrier that four otherwise idle lanes of the peer's MMA warp (round-robin over the
+// stages, so a slow cluster-scope arrive is off everybody's critical path) forward to the leader.
+// =================================================================================================
+constexpr int P2_A_BYTES = 4 * PJ_BK * 128;             // this CTA's 128 projector rows: 4 chunks of [16 r x 32 p]
+constexpr int P2_Y_BYTES = 7 * PJ_BK * 128;             // this CTA's half of the psi tile: <= 224 columns
+constexpr int P2_STAGE_BYTES = 2 * P2_A_BYTES + 2 * P2_Y_BYTES;   // 44 KB (3xTF32); one-product modes use half
+constexpr int P2_STAGES = 4;
+constexpr int P2_SMEM = P2_STAGES * P2_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 512;
+constexpr int P2_FWD = 4;                               // forwarding lanes of the peer's MMA warp
+
+template <bool LO>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PJ_THREADS, 1)
+proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_y0,
+                const __grid_constant__ CUtensorMap map_y1, const __grid_constant__ CUtensorMap map_z, const ProjParams q) {
+    constexpr int NST = LO ? P2_STAGES : 2 * P2_STAGES;
+    constexpr int SB = LO ? P2_STAGE_BYTES : P2_STAGE_BYTES / 2;
+    constexpr int YOFF = (LO ? 2 : 1) * P2_A_BYTES;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *stage = smem + NST * SB;
+    uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
+    uint64_t *full = bars, *empty = bars + NST, *conv = bars + 2 * NST, *cdone = bars + 3 * NST;
+    uint64_t *acc_full = bars + 4 * NST, *acc_empty = acc_full + 1;
+    uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const int crank = (int)cluster_ctarank();
+    const bool leader = crank == 0;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST; ++s) {
+            mbar_init(&full[s], 1);          // LOCAL: this CTA's tiles have landed
+            mbar_init(&empty[s], 1);         // the leader's tcgen05.commit, multicast to both CTAs
+            mbar_init(&conv[s], 128 + 1);    // used in the leader: its 128 converter threads + the peer's forwarder
+            mbar_init(&cdone[s], 128);       // used in the peer: its 128 converter threads
+        }
+        mbar_init(acc_full, 1);              // commit multicast
+        mbar_init(acc_empty, 2);             // one elected epilogue thread per CTA (remote arrive on the leader)
+        fence_barrier_init();
+        prefetch_tmap(&map_a);
+        prefetch_tmap(&map_y0);
+        prefetch_tmap(&map_y1);
+        prefetch_tmap(&map_z);
+    }
+    if (warp == 1) tmem_alloc_2cta(tmem_slot, 512);
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
+
+    const int nkb = q.ngrid / PJ_BK;
+    const int total = q.ndom * q.ntile_m * q.ntile_n * q.nsplit;   // pair units
+    const bool need_lo = q.nprod == 3;
+    const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;        // UMMA pieces (columns); per CTA n/2 of each
+    const int h0 = n0 / 64, h1 = n1 / 64;                           // this CTA's 32-column chunks of each piece
+    const uint32_t tx_bytes = P2_A_BYTES + (uint32_t)(h0 + h1) * PJ_BK * 128;
+
+    auto decode = [&](int u, int &dom, int &mt, int &nt, int &sp, int &kb0, int &kb1) {
+        nt = u % q.ntile_n;
+        u /= q.ntile_n;
+        sp = u % q.nsplit;
+        u /= q.nsplit;
+        mt = u % q.ntile_m;
+        dom = u / q.ntile_m;
+        kb0 = (int)((long)nkb * sp / q.nsplit);
+        kb1 = (int)((long)nkb * (sp + 1) / q.nsplit);
+    };
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int it = 0;
+            for (int u = cl; u < total; u += ncl) {
+                int dom, mt, nt, sp, kb0, kb1;
+                decode(u, dom, mt, nt, sp, kb0, kb1);
+                const int ch0 = nt * (q.BN / 32) + crank * h0, ch1 = nt * (q.BN / 32) + n0 / 32 + crank * h1;
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    const int s = it % NST;
+                    mbar_wait(&empty[s], ((it / NST) & 1) ^ 1);
+                    uint8_t *st = smem + s * SB;
+                    mbar_expect_tx(&full[s], tx_bytes);
+                    const int row = dom * q.ngrid + kb * PJ_BK;
+                    tma_load_3d(st, &map_a, &full[s], 0, row, mt * 8 + crank * 4);
+                    tma_load_3d(st + YOFF, &map_y0, &full[s], 0, row, ch0);
+                    if (h1) tma_load_3d(st + YOFF + h0 * (PJ_BK * 128), &map_y1, &full[s], 0, row, ch1);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (leader) {
+            if (lane == 0) {
+                const uint32_t id0 = instr_desc(FMT_TF32, 1, 1, 256, (uint32_t)n0);
+                const uint32_t id1 = instr_desc(FMT_TF32, 1, 1, 256, (uint32_t)(n1 ? n1 : 64));
+                int it = 0, nd = 0;   // nd: accumulator hand-overs (drains) so far
+                for (int u = cl; u < total; u += ncl) {
+                    int dom, mt, nt, sp, kb0, kb1;
+                    decode(u, dom, mt, nt, sp, kb0, kb1);
+                    for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                        const bool first = (kb - kb0) % q.chain == 0;
+                        if (first) {
+                            mbar_wait(acc_empty, (nd & 1) ^ 1);
+                            tc_fence_after();
+                        }
+                        const int s = it % NST;
+                        mbar_wait(&conv[s], (it / NST) & 1);   // both CTAs' tiles landed and converted
+                        tc_fence_after();
+                        const uint32_t st = smem_u32(smem + s * SB);
+                        const uint32_t a_hi = st, a_lo = st + P2_A_BYTES, y_hi = st + YOFF, y_lo = st + YOFF + P2_Y_BYTES;
+#pragma unroll
+                        for (int k8 = 0; k8 < PJ_BK / 8; ++k8) {
+                            const uint32_t acc = (!first || k8 > 0) ? 1u : 0u;
+                            const uint64_t da = smem_desc(a_hi + k8 * 1024, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                            const uint64_t dal = smem_desc(a_lo + k8 * 1024, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                            {
+                                const uint64_t dy = smem_desc(y_hi + k8 * 1024, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                                umma_tf32_2cta(tmem, da, dy, id0, acc);
+                                if (need_lo) {
+                                    umma_tf32_2cta(tmem, dal, dy, id0, 1u);
+                                    umma_tf32_2cta(tmem, da, smem_desc(y_lo + k8 * 1024, PJ_BK * 128, 512, LAYOUT_SW128_32B), id0, 1u);
+                                }
+                            }
+                            if (h1) {
+                                const uint32_t yo = (uint32_t)h0 * (PJ_BK * 128) + k8 * 1024;
+                                const uint64_t dy = smem_desc(y_hi + yo, PJ_BK * 128, 512, LAYOUT_SW128_32B);
+                                umma_tf32_2cta(tmem + n0, da, dy, id1, acc);
+                                if (need_lo) {
+                                    umma_tf32_2cta(tmem + n0, dal, dy, id1, 1u);
+                                    umma_tf32_2cta(tmem + n0, da, smem_desc(y_lo + yo, PJ_BK * 128, 512, LAYOUT_SW128_32B), id1, 1u);
+                                }
+                            }
+                        }
+                        umma_commit_2cta_mc(&empty[s], (uint16_t)3);
+                        if ((kb - kb0 + 1) % q.chain == 0 || kb + 1 == kb1) {
+                            umma_commit_2cta_mc(acc_full, (uint16_t)3);
+                            ++nd;
+                        }
+                    }
+                }
+            }
+        } else if (lane < P2_FWD) {
+            // the peer's MMA warp has nothing to issue: its first lanes forward "stage converted" to the leader
+            int it = 0;
+            for (int u = cl; u < total; u += ncl) {
+                int dom, mt, nt, sp, kb0, kb1;
+                decode(u, dom, mt, nt, sp, kb0, kb1);
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    if (it % P2_FWD != lane) continue;
+                    const int s = it % NST;
+                    mbar_wait(&cdone[s], (it / NST) & 1);
+                    mbar_arrive_remote(&conv[s], 0);
+                }
+            }
+        }
+    } else {
+        const int t = threadIdx.x - 64;   // 0..127
+        const int quarter = warp % 4;
+        const int er = quarter * 32 + lane;   // TMEM lane = accumulator row of this thread; er == 0 leads the TMA stores
+        uint64_t *done = leader ? conv : cdone;
+        int it = 0, nd = 0, slot = 0;
+        const int ny4 = (h0 + h1) * PJ_BK * 8;    // float4 count of this CTA's psi tile
+        for (int u = cl; u < total; u += ncl) {
+            int dom, mt, nt, sp, kb0, kb1;
+            decode(u, dom, mt, nt, sp, kb0, kb1);
+            const bool rows_live = q.P - mt * 256 - crank * 128 > 0;
+            for (int c0k = kb0; c0k < kb1; c0k += q.chain) {
+                const int c1k = min(c0k + q.chain, kb1);
+                for (int kb = c0k; kb < c1k; ++kb, ++it) {
+                    const int s = it % NST;
+                    mbar_wait(&full[s], (it / NST) & 1);
+                    uint8_t *st = smem + s * SB;
+                    float4 *a4 = (float4 *)st;
+                    float4 *y4 = (float4 *)(st + YOFF);
+                    if (q.lowp) {
+                        // opt-in low precision (PAPER.md L207, L239 float_to_BF16): both operands rounded to BF16
+                        for (int i = t; i < ny4; i += 128) y4[i] = bf16_round4(y4[i]);
+                        for (int i = t; i < P2_A_BYTES / 16; i += 128) a4[i] = bf16_round4(a4[i]);
+                    } else if (!LO) {
+                        for (int i = t; i < P2_A_BYTES / 16; i += 128) a4[i] = tf32_rn4(a4[i]);
+                        if (q.rn)
+                            for (int i = t; i < ny4; i += 128) y4[i] = tf32_rn4(y4[i]);
+                    } else {
+                        // elementwise on the swizzled image: the lo tile has the same layout as the hi tile
+                        float4 *yl = (float4 *)(st + YOFF + P2_Y_BYTES);
+                        for (int i = t; i < ny4; i += 128) {
+                            float4 v = y4[i];
+                            yl[i] = split4(v);   // the hi tile stays as loaded: kind::tf32 ignores the 13 low bits
+                        }
+                        float4 *al = (float4 *)(st + P2_A_BYTES);
+                        for (int i = t; i < P2_A_BYTES / 16; i += 128) {
+                            float4 v = a4[i];
+                            al[i] = split4_rn(v);
+                            a4[i] = v;
+                        }
+                    }
+                    fence_proxy_async_smem();
+                    mbar_arrive(&done[s]);
+                }
+                // drain this chain: TMEM -> (+)= FP32 partial sums of this K slice (round-to-nearest adds)
+                mbar_wait(acc_full, nd & 1);
+                ++nd;
+                tc_fence_after();
+                const bool add = c0k > kb0;
+                // the store of the slice's first chain must have landed before later chains add to it
+                if (add && c0k == kb0 + q.chain && er == 0) bulk_wait<0>();
+                const int zrow = (dom * q.nsplit + sp) * q.prows + mt * 256 + crank * 128;
+                for (int cb = 0; cb < q.BN / 32; ++cb) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
+                    tmem_ld_wait();
+                    const int c0 = nt * q.BN + cb * 32;
+                    if (c0 < q.N && rows_live) epi_tile_out<2>(stage, slot, &map_z, c0, zrow, v, er, add);
+                }
+                tc_fence_before();
+                named_bar_sync(EPI_BAR, 128);
+                if (er == 0) mbar_arrive_remote(acc_empty, 0);   // this CTA's half of the accumulator is drained
+            }
+        }
+        if (er == 0) bulk_wait<0>();
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc_2cta(tmem, 512);
+    }
+}
+
+// =================================================================================================
 // Back-application: Y[r][c] += sum_p A[r][p] * W[p][c].
 // CTA tile: 128 grid points x BN <= 448 columns (TMEM accumulator), K pipeline of 8 projector rows.
 // CTAs run as clusters of two on neighbouring row tiles: the W slab of a stage is the same for both, so
@@ -396,7 +665,7 @@ constexpr int BK_MAXBN = 448;
 constexpr int BK_A_BYTES = 128 * 32;                    // [128 rows x 8 floats], SWIZZLE_32B
 constexpr int BK_W_BYTES = (BK_MAXBN / 32) * 1024;      // chunks of [8 rows x 128 B], SWIZZLE_128B
 constexpr int BK_STAGE_BYTES = 2 * BK_A_BYTES + 2 * BK_W_BYTES;
-constexpr int BK_SMEM = BK_STAGES * BK_STAGE_BYTES + BK_EPI_NB * EPI_TILE_BYTES + 1024 + 256;
+constexpr int BK_SMEM = BK_STAGES * BK_STAGE_BYTES + BK_EPI_NB * EPI_TILE_BYTES + 1024 + 512;
 constexpr int BK_EPI_WARPS = 4;
 constexpr int BK_THREADS = 64 + 32 * BK_EPI_WARPS;
 
@@ -405,10 +674,28 @@ struct BackParams {
     float *Y;
 };
 
+// beta arrives as ONE FP32 copy (raw); the operand pair of 3xTF32 is formed in shared memory:
+//   hi = beta rounded to the nearest TF32 (in place), lo = beta - hi (exact) into the second slot.
+// mode: 0 = hi/lo pair, 1 = hi only (one-product modes), 2 = BF16 rounding in place (low precision)
+__device__ __forceinline__ void convert_a_slab(uint8_t *st, int t, int nthreads, int mode) {
+    float4 *a4 = (float4 *)st;
+    float4 *l4 = (float4 *)(st + BK_A_BYTES);
+    if (mode == 0) {
+        for (int i = t; i < BK_A_BYTES / 16; i += nthreads) {
+            float4 v = a4[i];
+            l4[i] = split4_rn(v);
+            a4[i] = v;
+        }
+    } else if (mode == 1) {
+        for (int i = t; i < BK_A_BYTES / 16; i += nthreads) a4[i] = tf32_rn4(a4[i]);
+    } else {
+        for (int i = t; i < BK_A_BYTES / 16; i += nthreads) a4[i] = bf16_round4(a4[i]);
+    }
+}
+
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(BK_THREADS, 1)
-back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
-               const __grid_constant__ CUtensorMap map_whi, const __grid_constant__ CUtensorMap map_wlo,
-               const __grid_constant__ CUtensorMap map_out, const BackParams q) {
+back_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_whi,
+               const __grid_constant__ CUtensorMap map_wlo, const __grid_constant__ CUtensorMap map_out, const BackParams q) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *stage = smem + BK_STAGES * BK_STAGE_BYTES;
@@ -427,8 +714,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
         mbar_init(acc_full, 1);
         mbar_init(acc_empty, 32 * BK_EPI_WARPS);
         fence_barrier_init();
-        prefetch_tmap(&map_ahi);
-        prefetch_tmap(&map_alo);
+        prefetch_tmap(&map_a);
         prefetch_tmap(&map_whi);
         prefetch_tmap(&map_wlo);
         prefetch_tmap(&map_out);
@@ -447,9 +733,10 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
     const int nk = (q.P + 7) / 8;
     // nprod 3: beta_hi W_hi + beta_lo W_hi + beta_hi W_lo; nprod 2 (staged mode): the first two (W taken as one TF32)
     const bool need_lo = q.nprod >= 2, need_wlo = q.nprod == 3;
+    const int cmode = q.lowp ? 2 : (need_lo ? 0 : 1);
     const int nchunk = q.BN / 32, chalf = (nchunk + 1) / 2;   // W chunks: this CTA fetches `chalf` of them
     const uint32_t w_bytes = (uint32_t)(2 * chalf) * 1024;
-    const uint32_t tx_bytes = (need_lo ? 2u : 1u) * BK_A_BYTES + (need_wlo ? 2u : 1u) * w_bytes;
+    const uint32_t tx_bytes = BK_A_BYTES + (need_wlo ? 2u : 1u) * w_bytes;
     const int ninstr = q.BN > 256 ? 2 : 1;
     const int NI = q.BN / ninstr;                   // columns per UMMA instruction (multiple of 32)
 
@@ -464,10 +751,9 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                     mbar_wait(&empty[s], ((it / BK_STAGES) & 1) ^ 1);
                     uint8_t *st = smem + s * BK_STAGE_BYTES;
                     mbar_expect_tx(&full[s], tx_bytes);
-                    tma_load_2d(st, &map_ahi, &full[s], k * 8, row);
+                    tma_load_2d(st, &map_a, &full[s], k * 8, row);
                     tma_load_3d_mc(st + 2 * BK_A_BYTES + crank * chalf * 1024, &map_whi, &full[s], 0, dom * q.prows + k * 8,
                                    nt * nchunk + crank * chalf, (uint16_t)3);
-                    if (need_lo) tma_load_2d(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
                     if (need_wlo)
                         tma_load_3d_mc(st + 2 * BK_A_BYTES + BK_W_BYTES + crank * chalf * 1024, &map_wlo, &full[s], 0,
                                        dom * q.prows + k * 8, nt * nchunk + crank * chalf, (uint16_t)3);
@@ -484,7 +770,7 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
                 for (int k = 0; k < nk; ++k, ++it) {
                     const int s = it % BK_STAGES;
                     mbar_wait(&full[s], (it / BK_STAGES) & 1);
-                    if (q.lowp) mbar_wait(&conv[s], (it / BK_STAGES) & 1);
+                    mbar_wait(&conv[s], (it / BK_STAGES) & 1);
                     tc_fence_after();
                     const uint32_t st = smem_u32(smem + s * BK_STAGE_BYTES);
                     const uint64_t da = smem_desc(st, 16, 256, LAYOUT_SW32);
@@ -513,17 +799,13 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
             const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
             const int row0 = dom * q.ngrid + rt * 128;
             const bool live = rt < nrt;           // odd tile count: the last pair's second CTA only keeps the protocol going
-            if (q.lowp) {
-                // low-precision mode: the otherwise idle epilogue warps round the beta slab of every stage
-                // to BF16 in place (W was rounded by the glue kernel)
-                for (int k = 0; k < nk; ++k, ++it) {
-                    const int s = it % BK_STAGES;
-                    mbar_wait(&full[s], (it / BK_STAGES) & 1);
-                    float4 *a4 = (float4 *)(smem + s * BK_STAGE_BYTES);
-                    for (int i = er; i < BK_A_BYTES / 16; i += 32 * BK_EPI_WARPS) a4[i] = bf16_round4(a4[i]);
-                    fence_proxy_async_smem();
-                    mbar_arrive(&conv[s]);
-                }
+            // the epilogue warps (idle during the main loop) form the operand pair of every beta slab in place
+            for (int k = 0; k < nk; ++k, ++it) {
+                const int s = it % BK_STAGES;
+                mbar_wait(&full[s], (it / BK_STAGES) & 1);
+                convert_a_slab(smem + s * BK_STAGE_BYTES, er, 32 * BK_EPI_WARPS, cmode);
+                fence_proxy_async_smem();
+                mbar_arrive(&conv[s]);
             }
             mbar_wait(acc_full, nu & 1);
             tc_fence_after();
@@ -557,14 +839,21 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constan
 // operand reads alone take ~98 of the 128 B/cycle of shared-memory bandwidth and, together with the
 // TMA fills, cap the tensor pipe near 75 % (measured); this is what cta_group::2 exists for.
 // Per CTA: 128 x BN accumulator in TMEM (BN <= 448, BN % 64 == 0), UMMA pieces of N = 256 and BN - 256.
+//
+// beta is read from HBM ONCE as plain FP32: four converter warps per CTA (each takes every fourth stage) round the slab
+// to TF32 in place and write the exact remainder next to it, then tell the LEADER (whose single thread issues the
+// pair's UMMAs) with a cluster-scope arrive on its `conv` barrier: the beta_lo stream of round 1 (6.8 GB per launch at
+// configs[3]) is gone from HBM and from L2.
 // =================================================================================================
 constexpr int B2_STAGES = 7;
 constexpr int B2_WH_BYTES = 7 * 1024;                  // this CTA's half of the W slab: <= 224 columns
 constexpr int B2_STAGE_BYTES = 2 * BK_A_BYTES + 2 * B2_WH_BYTES;
-constexpr int B2_SMEM = B2_STAGES * B2_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 256;
+constexpr int B2_SMEM = B2_STAGES * B2_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 512;
+constexpr int B2_CONV_WARPS = 4;
+constexpr int B2_THREADS = BK_THREADS + 32 * B2_CONV_WARPS;
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(BK_THREADS, 1)
-back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(B2_THREADS, 1)
+back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
                 const __grid_constant__ CUtensorMap map_w0h, const __grid_constant__ CUtensorMap map_w0l,
                 const __grid_constant__ CUtensorMap map_w1h, const __grid_constant__ CUtensorMap map_w1l,
                 const __grid_constant__ CUtensorMap map_out, const BackParams q) {
@@ -572,8 +861,8 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *stage = smem + B2_STAGES * B2_STAGE_BYTES;
     uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
-    uint64_t *full = bars, *empty = bars + B2_STAGES;
-    uint64_t *acc_full = bars + 2 * B2_STAGES, *acc_empty = acc_full + 1;
+    uint64_t *full = bars, *empty = bars + B2_STAGES, *afull = bars + 2 * B2_STAGES, *conv = bars + 3 * B2_STAGES;
+    uint64_t *acc_full = bars + 4 * B2_STAGES, *acc_empty = acc_full + 1;
     uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
     const int crank = (int)cluster_ctarank();
@@ -581,14 +870,15 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < B2_STAGES; ++s) {
-            mbar_init(&full[s], 1);     // used in the leader: its own expect_tx arrive; both CTAs' TMA bytes land on it
+            mbar_init(&full[s], 1);     // used in the leader: its own expect_tx arrive; both CTAs' W bytes land on it
             mbar_init(&empty[s], 1);    // the leader's tcgen05.commit, multicast to both CTAs
+            mbar_init(&afull[s], 1);    // LOCAL: this CTA's beta slab has landed (its converter warp waits here)
+            mbar_init(&conv[s], 2);     // used in the leader: one converter warp per CTA has split the slab
         }
         mbar_init(acc_full, 1);         // commit multicast
         mbar_init(acc_empty, 2);        // one elected epilogue thread per CTA (remote arrive on the leader)
         fence_barrier_init();
-        prefetch_tmap(&map_ahi);
-        prefetch_tmap(&map_alo);
+        prefetch_tmap(&map_a);
         prefetch_tmap(&map_w0h);
         prefetch_tmap(&map_w0l);
         prefetch_tmap(&map_out);
@@ -606,7 +896,7 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
     const bool need_lo = q.nprod >= 2, need_wlo = q.nprod == 3;   // as in back_tc_kernel
     const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;   // UMMA pieces (columns); per CTA n/2 of each
     const int h0 = n0 / 64, h1 = n1 / 64;                      // this CTA's 32-column chunks of each piece
-    const uint32_t cta_bytes = (need_lo ? 2u : 1u) * BK_A_BYTES + (need_wlo ? 2u : 1u) * (uint32_t)(h0 + h1) * 1024;
+    const uint32_t w_bytes = (need_wlo ? 2u : 1u) * (uint32_t)(h0 + h1) * 1024;   // per CTA
 
     if (warp == 0) {
         if (lane == 0) {
@@ -619,12 +909,12 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
                     const int s = it % B2_STAGES;
                     mbar_wait(&empty[s], ((it / B2_STAGES) & 1) ^ 1);
                     uint8_t *st = smem + s * B2_STAGE_BYTES;
-                    if (leader) mbar_expect_tx(&full[s], 2 * cta_bytes);
+                    if (leader) mbar_expect_tx(&full[s], 2 * w_bytes);
+                    mbar_expect_tx(&afull[s], BK_A_BYTES);
                     const int wrow = dom * q.prows + k * 8;
-                    tma_load_2d_2cta(st, &map_ahi, &full[s], k * 8, row);
+                    tma_load_2d(st, &map_a, &afull[s], k * 8, row);          // raw beta slab, this CTA's barrier
                     tma_load_3d_2cta(st + 2 * BK_A_BYTES, &map_w0h, &full[s], 0, wrow, ch0);
                     if (h1) tma_load_3d_2cta(st + 2 * BK_A_BYTES + h0 * 1024, &map_w1h, &full[s], 0, wrow, ch1);
-                    if (need_lo) tma_load_2d_2cta(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
                     if (need_wlo) {
                         tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES, &map_w0l, &full[s], 0, wrow, ch0);
                         if (h1)
@@ -644,6 +934,7 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
                 for (int k = 0; k < nk; ++k, ++it) {
                     const int s = it % B2_STAGES;
                     mbar_wait(&full[s], (it / B2_STAGES) & 1);
+                    mbar_wait(&conv[s], (it / B2_STAGES) & 1);
                     tc_fence_after();
                     const uint32_t st = smem_u32(smem + s * B2_STAGE_BYTES);
                     const uint64_t da = smem_desc(st, 16, 256, LAYOUT_SW32);
@@ -668,7 +959,7 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
                 umma_commit_2cta_mc(acc_full, (uint16_t)3);
             }
         }
-    } else {
+    } else if (warp < 2 + BK_EPI_WARPS) {
         const int quarter = warp % 4;
         const int er = quarter * 32 + lane;         // accumulator row of this thread
         int nu = 0, slot = 0;
@@ -690,6 +981,22 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
             if (er == 0) mbar_arrive_remote(acc_empty, 0);   // this CTA's half of the accumulator is drained
         }
         if (er == 0) bulk_wait<0>();
+    } else {
+        // converter warps: warp j takes the stages it == j (mod B2_CONV_WARPS) of the CTA's stage sequence
+        const int cw = warp - (2 + BK_EPI_WARPS);
+        const int cmode = need_lo ? 0 : 1;
+        int it = 0;
+        for (int u = cl; u < total; u += ncl) {
+            for (int k = 0; k < nk; ++k, ++it) {
+                if (it % B2_CONV_WARPS != cw) continue;
+                const int s = it % B2_STAGES;
+                mbar_wait(&afull[s], (it / B2_STAGES) & 1);
+                convert_a_slab(smem + s * B2_STAGE_BYTES, lane, 32, cmode);
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(&conv[s], 0);
+            }
+        }
     }
     tc_fence_before();
     __syncthreads();
@@ -741,11 +1048,13 @@ int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
 
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
-                           int chain, int *nlaunch) {
+                           int chain, int *nlaunch, TmapCache *cache) {
     static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
     if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(proj_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(proj2_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(proj2_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM);
         if (e != cudaSuccess) return e;
         attr_set.mark();
     }
@@ -755,8 +1064,6 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.P = P;
     q.N = N;
     q.ntile_m = (P + 255) / 256;
-    q.ntile_n = proj_ntile_n(N);
-    q.BN = ((N + q.ntile_n - 1) / q.ntile_n + 31) / 32 * 32;
     q.nsplit = nsplit;
     q.prows = prows;
     q.nprod = nprod;
@@ -767,13 +1074,31 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.rn = nprod == 4 ? 1 : 0;       // nprod 4 = one product, psi rounded to the nearest TF32 in shared memory
     if (q.lowp || q.rn) q.nprod = 1;
     const uint64_t rows = (uint64_t)ndom * ngrid;
+    CUtensorMap mz;
+    if (!make_out_map(cache, &mz, zpart, (uint64_t)ndom * nsplit * prows, N, N)) return cudaErrorInvalidValue;
+    if (N % 64 == 0 && A_lo == nullptr) {
+        // CTA pairs (cta_group::2): one pair per (domain, 256-row tile, column tile of <= 448, K slice)
+        q.ntile_n = (N + BK_MAXBN - 1) / BK_MAXBN;
+        q.BN = ((N + q.ntile_n - 1) / q.ntile_n + 63) / 64 * 64;
+        const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;
+        CUtensorMap ma, my0, my1;
+        if (!make_chunk_map(cache, &ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &my0, Y, rows, ldy, N / 32, PJ_BK, n0 / 64)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &my1, Y, rows, ldy, N / 32, PJ_BK, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
+        const int total = ndom * q.ntile_m * q.ntile_n * nsplit;
+        const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
+        ++*nlaunch;
+        if (q.nprod == 3) proj2_tc_kernel<true><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, mz, q);
+        else proj2_tc_kernel<false><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, mz, q);
+        return cudaGetLastError();
+    }
+    q.ntile_n = proj_ntile_n(N);
+    q.BN = ((N + q.ntile_n - 1) / q.ntile_n + 31) / 32 * 32;
     CUtensorMap ma, mal, my;
     // 4-chunk boxes: each CTA of a cluster fetches (and multicasts) half of the 8 beta chunks of a stage
-    if (!make_chunk_map(&ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
-    if (!make_chunk_map(&mal, A_lo ? A_lo : A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
-    if (!make_chunk_map(&my, Y, rows, ldy, N / 32, PJ_BK, q.BN / 32)) return cudaErrorInvalidValue;
-    CUtensorMap mz;
-    if (!make_out_map(&mz, zpart, (uint64_t)ndom * nsplit * prows, N, N)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(cache, &ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(cache, &mal, A_lo ? A_lo : A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(cache, &my, Y, rows, ldy, N / 32, PJ_BK, q.BN / 32)) return cudaErrorInvalidValue;
     const int total = ndom * q.ntile_m * ((q.ntile_n + 1) / 2) * nsplit;   // cluster units
     const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
@@ -782,9 +1107,9 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     return cudaGetLastError();
 }
 
-cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
+cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
-                           int *nlaunch) {
+                           int *nlaunch, TmapCache *cache) {
     static DeviceOnce attr_set;
     if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(back_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, BK_SMEM);
@@ -805,19 +1130,14 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.ldy = ldy;
     q.Y = Y;
     const uint64_t rows = (uint64_t)ndom * ngrid;
-    CUtensorMap ma, mal, mw, mwl;
-    if (!make_k8_map(&ma, A_hi, rows, lda, lda, 128)) return cudaErrorInvalidValue;
-    if (!make_k8_map(&mal, A_lo, rows, lda, lda, 128)) return cudaErrorInvalidValue;
-    const int chalf = (q.BN / 32 + 1) / 2;   // each CTA of a cluster fetches (and multicasts) half of the W chunks
-    if (!make_chunk_map(&mw, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, chalf)) return cudaErrorInvalidValue;
-    if (!make_chunk_map(&mwl, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, chalf)) return cudaErrorInvalidValue;
+    CUtensorMap ma, mw, mwl;
+    if (!make_k8_map(cache, &ma, A, rows, lda, lda, 128)) return cudaErrorInvalidValue;
     CUtensorMap mo;
-    if (!make_out_map(&mo, Y, rows, N, ldy)) return cudaErrorInvalidValue;
+    if (!make_out_map(cache, &mo, Y, rows, N, ldy)) return cudaErrorInvalidValue;
     const int total = ndom * (int)((ngrid / 128 + 1) / 2) * q.ntile_n;   // cluster units (pairs of row tiles)
     const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
-    const char *pair = getenv("MLMD_BACK_PAIR");   // "0": keep single-CTA UMMAs (A/B checks)
-    if (q.BN % 64 == 0 && !q.lowp && !(pair && pair[0] == '0')) {
+    if (q.BN % 64 == 0 && !q.lowp) {
         static DeviceOnce attr2;
         if (!attr2.done()) {
             cudaError_t e = cudaFuncSetAttribute(back2_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, B2_SMEM);
@@ -826,14 +1146,17 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
         }
         const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;
         CUtensorMap w0h, w0l, w1h, w1l;
-        if (!make_chunk_map(&w0h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(&w0l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(&w1h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(&w1l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
-        back2_tc_kernel<<<grid, BK_THREADS, B2_SMEM, st>>>(ma, mal, w0h, w0l, w1h, w1l, mo, q);
+        if (!make_chunk_map(cache, &w0h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &w0l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &w1h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &w1l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
+        back2_tc_kernel<<<grid, B2_THREADS, B2_SMEM, st>>>(ma, w0h, w0l, w1h, w1l, mo, q);
         return cudaGetLastError();
     }
-    back_tc_kernel<<<grid, BK_THREADS, BK_SMEM, st>>>(ma, mal, mw, mwl, mo, q);
+    const int chalf = (q.BN / 32 + 1) / 2;   // each CTA of a cluster fetches (and multicasts) half of the W chunks
+    if (!make_chunk_map(cache, &mw, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, chalf)) return cudaErrorInvalidValue;
+    if (!make_chunk_map(cache, &mwl, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, chalf)) return cudaErrorInvalidValue;
+    back_tc_kernel<<<grid, BK_THREADS, BK_SMEM, st>>>(ma, mw, mwl, mo, q);
     return cudaGetLastError();
 }
 

@@ -599,7 +599,7 @@ cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, do
     if (max_blk < 1) return cudaErrorInvalidValue;
     // 2 c1_j / h_d with c1 = (2/3, -1/12): weights of the 4th-order first difference (north_star)
     const float w1 = (float)(2.0 * 2.0 / 3.0), w2 = (float)(2.0 * -1.0 / 12.0);
-    if (ny % 8 == 0 && nz % 8 == 0 && !getenv("MLMD_CURRENT_SIMPLE")) {
+    if (ny % 8 == 0 && nz % 8 == 0) {
         const long tiles = (long)(ld / 8) * (ny / 8) * (nz / 8);
         int nxseg = 1;
         while (tiles * ndom * nxseg < 4 * 148 && nx / (nxseg * 2) >= 8) nxseg *= 2;

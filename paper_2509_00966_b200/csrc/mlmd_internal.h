@@ -4,6 +4,8 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include <cuda.h>
+
 #include <vector>
 
 #include "../../include/mlmd.h"
@@ -23,9 +25,46 @@ struct StepCoef {
 static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
-    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
+    size_t psi, ua, ub, psi0, vloc, beta, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
         nrm, nrm_part, scl, occ_eff, avec, gram, total;
 };
+
+// Tensor maps are pure functions of (base pointer, shape, box): encoded once per distinct key and kept in the
+// handle, instead of 70+ cuTensorMapEncodeTiled calls per time step.
+struct TmapKey {
+    int kind;                 // which encoder (tag chosen by the caller)
+    const void *base;
+    unsigned long long a, b, c, d;
+    unsigned e, f;
+};
+struct TmapCache {
+    struct Entry { TmapKey key; CUtensorMap map; };
+    std::vector<Entry> entries;
+    const CUtensorMap *find(const TmapKey &k) const {
+        for (const Entry &e : entries)
+            if (e.key.kind == k.kind && e.key.base == k.base && e.key.a == k.a && e.key.b == k.b && e.key.c == k.c &&
+                e.key.d == k.d && e.key.e == k.e && e.key.f == k.f)
+                return &e.map;
+        return nullptr;
+    }
+    void insert(const TmapKey &k, const CUtensorMap &m) {
+        if (entries.size() >= 256) entries.clear();     // e.g. a caller cycling through many borrowed buffers
+        entries.push_back(Entry{k, m});
+    }
+    void clear() { entries.clear(); }
+};
+// *out = the cached map of key k, or build(out) (and remember it).  cache may be NULL (kernel-level test hooks).
+template <class Build>
+bool cached_tmap(TmapCache *cache, const TmapKey &k, CUtensorMap *out, Build build) {
+    if (cache)
+        if (const CUtensorMap *m = cache->find(k)) {
+            *out = *m;
+            return true;
+        }
+    if (!build(out)) return false;
+    if (cache) cache->insert(k, *out);
+    return true;
+}
 
 constexpr int kCoefCapacity = 256;   // steps per coefficient upload chunk
 constexpr int kMaxSplit = 64;        // split-K slices of the projection GEMM
@@ -53,10 +92,9 @@ struct mlmd_domain {
     int nsplit_tc, nsplit_tc_ovl;   // split-K factors of the tcgen05 projection (beta rows / overlap)
     bool tc_ok;                 // shape and device allow the tcgen05 GEMM kernels
     int gemm_mode;
-    int staged_proj_nprod; // its projection: 4 = one product of nearest-rounded operands, 1 = truncated
-    int inner_chain;       // chain length of the three inner Horner stages' projections (any tensor-core mode)
-    int staged_chain;      // its projection: TMEM accumulation chain length in 16-row stages
-    int staged_mask;      // MLMD_GEMM_FP32GRADE_STAGED: bit i = Horner stage i runs with reduced products
+    int opt[MLMD_OPT_COUNT];    // mlmd_set_option values
+    float2 *psi_ptr;            // Psi: inside the workspace, or the caller's buffer (MLMD_BORROW_PSI)
+    mutable mlmd::TmapCache tmaps;
     bool have_psi, have_vloc, have_occ, rho_valid;
     bool field_yz;              // any A_y or A_z non-zero in the current propagate call
     double vmax, dmax;
@@ -82,13 +120,12 @@ struct mlmd_domain {
     bool g_split;               // the graph holds the Eq. (2) split step, not the Taylor-4 step
     int *flag_host;             // pinned
     // typed views
-    float2 *psi() const { return (float2 *)(ws + off.psi); }
+    float2 *psi() const { return psi_ptr; }
     float2 *ua() const { return (float2 *)(ws + off.ua); }
     float2 *ub() const { return (float2 *)(ws + off.ub); }
     float2 *psi0() const { return (float2 *)(ws + off.psi0); }
     float *vloc() const { return (float *)(ws + off.vloc); }
     float *beta() const { return (float *)(ws + off.beta); }
-    float *beta_lo() const { return (float *)(ws + off.beta_lo); }
     float *dprime() const { return (float *)(ws + off.dprime); }
     float *occ() const { return (float *)(ws + off.occ); }
     float *rho() const { return (float *)(ws + off.rho); }
@@ -149,11 +186,11 @@ int stencil_tma_norm_slots(const mlmd_domain *h);
 // ---- gemm_simt.cu ----------------------------------------------------------------------------
 // Projection (S2a): zpart[dom][s][p][c] = sum_{r in slice s} B[dom][r][p] * Y[dom][r][c]
 //   B: [ndom][ngrid][ldb] float (p fastest), Y: [ndom][ngrid][ldy] float, P rows, N columns used.
-//   Blo (may be NULL): B is stored as an exact hi + lo pair and summed on load.
+//   Blo (may be NULL): B is given as an exact hi + lo pair and summed on load.
 cudaError_t launch_proj_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
                              const float *Y, int ldy, int N, float *zpart, int prows, int nsplit,
                              bool fp64, int *nlaunch);
-// Back-application (S2d): Y[dom][r][c] += sum_p B[dom][r][p] * What[dom][p][c]  (both stored as hi + lo)
+// Back-application (S2d): Y[dom][r][c] += sum_p B[dom][r][p] * What[dom][p][c]  (W stored as hi + lo; Blo may be NULL)
 cudaError_t launch_back_simt(cudaStream_t st, int ndom, long ngrid, const float *B, const float *Blo, int ldb, int P,
                              const float *What, const float *Wlo, float *Y, int ldy, int N, int prows, bool fp64,
                              int *nlaunch);
@@ -167,10 +204,11 @@ bool tc_available();
 int tc_choose_nsplit(int ndom, long ngrid, int P, int N);
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
-                           int chain /* 16-row stages per TMEM accumulation chain, 0 = whole slice */, int *nlaunch);
-cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
+                           int chain /* 16-row stages per TMEM accumulation chain, 0 = whole slice */, int *nlaunch,
+                           TmapCache *cache = nullptr);
+cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A /* raw FP32 */, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
-                           int *nlaunch);
+                           int *nlaunch, TmapCache *cache = nullptr);
 
 // ---- glue.cu ---------------------------------------------------------------------------------
 // S2b: reduce split-K partials in fixed order and build What = (-i tau) D' C in real-GEMM form.

@@ -172,11 +172,6 @@ static cudaError_t launch_march(const StencilParams &P, int ndom, bool ayz, cuda
     return cudaGetLastError();
 }
 
-static int env_int(const char *name, int dflt) {
-    const char *s = getenv(name);
-    return s ? atoi(s) : dflt;
-}
-
 cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
                                  const StepCoef *coef, const StepCoef *coef_host, float tau, int *nlaunch) {
     StencilParams P;
@@ -190,12 +185,11 @@ cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const fl
     P.ny = h->ny;
     P.nz = h->nz;
     P.lanes = h->ld / 2;
-    const int variant = env_int("MLMD_STENCIL", 2);   // 0: simple (cross-check), 1: register marching, 2: TMA planes
-    if (variant == 2 && stencil_tma_supported(h)) return launch_stencil_tma(h, w, psi, out, coef, coef_host, tau, nlaunch);
-    const int xseg_env = env_int("MLMD_XSEG", 0);     // tuning override: planes per CTA
+    const int variant = h->opt[MLMD_OPT_STENCIL];   // 0: TMA planes when the shape allows, 1: register marching, 2: simple
+    if (variant == 0 && stencil_tma_supported(h)) return launch_stencil_tma(h, w, psi, out, coef, coef_host, tau, nlaunch);
     ++*nlaunch;
     const bool tile_ok = (h->ny % 8 == 0) && (h->nz % 8 == 0);
-    if (variant == 0 || !tile_ok) {
+    if (variant == 2 || !tile_ok) {
         const long total = (long)h->ndom * h->ngrid * P.lanes;
         P.xseg = P.nxseg = 1;
         stencil_simple_kernel<<<(unsigned)((total + 255) / 256), 256, 0, h->stream>>>(P, total);
@@ -206,7 +200,6 @@ cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const fl
     const long ctas_per_seg = (long)((P.lanes + 7) / 8) * (h->ny / 8) * (h->nz / 8) * h->ndom;
     int nxseg = 1;
     while (ctas_per_seg * nxseg < 4 * 296 && h->nx / (nxseg * 2) >= 8) nxseg *= 2;
-    if (xseg_env > 0) nxseg = (h->nx + xseg_env - 1) / xseg_env;
     P.xseg = (h->nx + nxseg - 1) / nxseg;
     P.nxseg = (h->nx + P.xseg - 1) / P.xseg;
     if (P.lanes % 8 == 0 || P.lanes > 8)
@@ -217,7 +210,7 @@ cudaError_t launch_stencil_stage(const mlmd_domain *h, const float2 *w, const fl
 cudaError_t launch_stencil_stage_norm(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out,
                                       const StepCoef *coef, const StepCoef *coef_host, float tau, int norm_mode,
                                       double *npart, double *nrm_out, int *nlaunch) {
-    if (env_int("MLMD_STENCIL", 2) == 2 && env_int("MLMD_NORM_FUSED", 1) && stencil_tma_supported(h)) {
+    if (h->opt[MLMD_OPT_STENCIL] == 0 && stencil_tma_supported(h)) {
         const int slots = stencil_tma_norm_slots(h);
         if (slots <= kNormSlabs) {     // npart holds kNormSlabs partial rows per domain
             cudaError_t e = launch_stencil_tma(h, w, psi, out, coef, coef_host, tau, nlaunch, norm_mode, npart);

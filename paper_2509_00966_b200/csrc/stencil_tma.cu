@@ -321,7 +321,7 @@ EncodeTiledFn encode_fn2() {
     }
     return fn;
 }
-bool make_plane_map(CUtensorMap *m, const float *base, int F, int nz, int ny, long nxd, int bz, int by) {
+bool make_plane_map_raw(CUtensorMap *m, const float *base, int F, int nz, int ny, long nxd, int bz, int by) {
     EncodeTiledFn f = encode_fn2();
     if (!f) return false;
     cuuint64_t dims[4] = {(cuuint64_t)F, (cuuint64_t)nz, (cuuint64_t)ny, (cuuint64_t)nxd};
@@ -330,6 +330,12 @@ bool make_plane_map(CUtensorMap *m, const float *base, int F, int nz, int ny, lo
     cuuint32_t es[4] = {1, 1, 1, 1};
     return f(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+bool make_plane_map(TmapCache *cache, CUtensorMap *m, const float *base, int F, int nz, int ny, long nxd, int bz, int by) {
+    const TmapKey k{4, base, (unsigned long long)F, (unsigned long long)nz, (unsigned long long)ny, (unsigned long long)nxd,
+                    (unsigned)bz, (unsigned)by};
+    return cached_tmap(cache, k, m, [&](CUtensorMap *o) { return make_plane_map_raw(o, base, F, nz, ny, nxd, bz, by); });
 }
 
 }  // namespace
@@ -365,8 +371,6 @@ static void x_segments(const mlmd_domain *h, int *xs, int *nxseg) {
     const long base = (long)h->ndom * (h->ld / 8) * (h->ny / SY) * (h->nz / SZ);
     int n = 1;
     while (base * n < 2 * 148 && h->nx / (n * 2) >= 8) n *= 2;
-    const char *env = getenv("MLMD_XSEG");
-    if (env && atoi(env) > 0) n = (h->nx + atoi(env) - 1) / atoi(env);
     *xs = (h->nx + n - 1) / n;
     *nxseg = (h->nx + *xs - 1) / *xs;
 }
@@ -389,10 +393,10 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
     const int F = 2 * h->ld;
     CUtensorMap mc, mz, my, mp;
     const long nxd = (long)h->nx * h->ndom;
-    if (!make_plane_map(&mc, (const float *)w, F, h->nz, h->ny, nxd, SZ, SY)) return cudaErrorInvalidValue;
-    if (!make_plane_map(&mz, (const float *)w, F, h->nz, h->ny, nxd, 2, SY)) return cudaErrorInvalidValue;
-    if (!make_plane_map(&my, (const float *)w, F, h->nz, h->ny, nxd, SZ, 2)) return cudaErrorInvalidValue;
-    if (!make_plane_map(&mp, (const float *)psi, F, h->nz, h->ny, nxd, SZ, SY)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&h->tmaps, &mc, (const float *)w, F, h->nz, h->ny, nxd, SZ, SY)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&h->tmaps, &mz, (const float *)w, F, h->nz, h->ny, nxd, 2, SY)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&h->tmaps, &my, (const float *)w, F, h->nz, h->ny, nxd, SZ, 2)) return cudaErrorInvalidValue;
+    if (!make_plane_map(&h->tmaps, &mp, (const float *)psi, F, h->nz, h->ny, nxd, SZ, SY)) return cudaErrorInvalidValue;
     TmaStencilParams P;
     P.out = (float4 *)out;
     P.vloc = h->vloc();
@@ -409,8 +413,7 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
         // at once then cover only 148 / npatch adjacent 64-byte chunks of a row; when that is under 1 KB (many patches,
         // e.g. 64^2 planes) DRAM page locality wins: chunk-fastest (configs[4]: 4.31 -> 3.58 ms; configs[3] stays, 1 % the other way).
         const int npatch = (h->ny / SY) * (h->nz / SZ);
-        const char *o = getenv("MLMD_STENCIL_ORDER");
-        P.chunk_fast = o ? atoi(o) : (64 * 148 / npatch < 1024 ? 1 : 0);
+        P.chunk_fast = 64 * 148 / npatch < 1024 ? 1 : 0;
     }
     P.ld = h->ld;
     const long base = (long)h->ndom * P.nchunk * (h->ny / SY) * (h->nz / SZ);

@@ -33,11 +33,23 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-// Spin with a watchdog: a protocol bug traps (-> a CUDA error at the next API call) instead of hanging.
+__device__ __forceinline__ uint64_t global_timer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// Spin with a watchdog bounded by TIME (20 s of %globaltimer, looked at once per 65536 failed tries), not by a
+// spin count: a protocol bug traps (-> a CUDA error at the next API call) instead of hanging the GPU, while a
+// legitimate long stall (profiler replay, time-slicing, a throttled clock) never comes near the bound.
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     uint32_t spins = 0;
+    uint64_t t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > (1u << 27)) __trap();
+        if ((++spins & 0xffffu) == 0) {
+            const uint64_t now = global_timer_ns();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 20000000000ull) __trap();
+        }
     }
 }
 

@@ -1,0 +1,41 @@
+// Kernel-level test hooks: run one nonlocal GEMM on caller-owned DEVICE buffers so that tests can check the
+// tensor-core kernels against a dense reference product.  Not part of include/mlmd.h and NOT linked into
+// libmlmd.so: build.py puts this file into libmlmd_test.so only, which tests/ load and the product never does.
+#include "mlmd_internal.h"
+
+using namespace mlmd;
+
+#define HOOK __attribute__((visibility("default")))
+
+extern "C" {
+
+// Z partials [ndom][nsplit][prows][N] = per-K-slice sums of A^T Y.  A_lo may be NULL (kernel splits A).
+// path: 0 = CUDA cores, 1 = tcgen05.  Returns a cudaError_t value.
+HOOK int mlmd_debug_proj(int path, void *stream, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
+                    const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod, int chain) {
+    int nl = 0;
+    cudaError_t e;
+    if (path == 1)
+        e = launch_proj_tc((cudaStream_t)stream, ndom, ngrid, A_hi, A_lo, lda, P, Y, ldy, N, zpart, prows, nsplit, nprod, chain, &nl);
+    else
+        e = launch_proj_simt((cudaStream_t)stream, ndom, ngrid, A_hi, A_lo, lda, P, Y, ldy, N, zpart, prows, nsplit, false, &nl);
+    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+    return (int)e;
+}
+
+// Y[dom][r][c] += sum_p A[dom][r][p] * (W_hi + W_lo)[dom][p][c]   (A: plain FP32, split by the kernel)
+HOOK int mlmd_debug_back(int path, void *stream, int ndom, long ngrid, const float *A, int lda, int P,
+                    const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod) {
+    int nl = 0;
+    cudaError_t e;
+    if (path == 1)
+        e = launch_back_tc((cudaStream_t)stream, ndom, ngrid, A, lda, P, W_hi, W_lo, Y, ldy, N, prows, nprod, &nl);
+    else
+        e = launch_back_simt((cudaStream_t)stream, ndom, ngrid, A, nullptr, lda, P, W_hi, W_lo, Y, ldy, N, prows, false, &nl);
+    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+    return (int)e;
+}
+
+HOOK int mlmd_debug_nsplit(int ndom, long ngrid, int P, int N) { return tc_choose_nsplit(ndom, ngrid, P, N); }
+
+}  // extern "C"

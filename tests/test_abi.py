@@ -33,12 +33,32 @@ def test_library_exports_every_declared_symbol(M):
     assert sorted(M.EXPORTED_SYMBOLS) == names
 
 
+def test_library_exports_nothing_but_the_header(M):
+    """Hidden visibility: the dynamic symbol table holds exactly the declared calls (no kernel-level test hooks, no
+    internal launchers); the hooks live in libmlmd_test.so, which only tests/ load."""
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", M.api.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = sorted(line.split()[-1] for line in out.splitlines() if "mlmd" in line.lower())
+    assert exported == declared_functions()
+    out = subprocess.run(["nm", "-D", "--defined-only", M.api.TEST_LIB_PATH], capture_output=True, text=True, check=True).stdout
+    assert "mlmd_debug_proj" in out and "mlmd_debug_back" in out
+
+
+def test_product_reads_no_environment_variables():
+    """Run-time switches go through mlmd_set_option / create flags, never through getenv."""
+    csrc = os.path.join(ROOT, "paper_2509_00966_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+
+
 def test_workspace_bytes(M):
     wb = M.mlmd_workspace_bytes
     assert wb(1, 4, 16, 16, 8, 8) == 0 and wb(0, 16, 16, 16, 8, 8) == 0 and wb(1, 16, 16, 16, 0, 8) == 0
     small = wb(1, 16, 16, 16, 8, 8)
     assert small >= 3 * 4096 * 8 * 8
     assert wb(2, 16, 16, 16, 8, 8) > small and wb(1, 16, 16, 16, 8, 8, M.KEEP_PSI0) >= small + 4096 * 8 * 8
+    # MLMD_BORROW_PSI: Psi stays in the caller's buffer, the workspace is one Psi-sized buffer smaller
+    assert wb(1, 16, 16, 16, 16, 8) - wb(1, 16, 16, 16, 16, 8, M.BORROW_PSI) == 4096 * 16 * 8
     # configs[3] and configs[4] fit one B200's 180 GB
     assert wb(64, 48, 48, 48, 224, 240) < 100e9 and wb(4, 64, 64, 64, 696, 810) < 100e9
     psi3 = 64 * 48 ** 3 * 224 * 8
@@ -63,6 +83,10 @@ def test_argument_errors_without_gpu(M):
     h = ctypes.c_void_p()
     assert L.mlmd_domain_create(ctypes.byref(h), 1, 16, 16, 16, 0.5, 0.5, 0.5, 8, 8, None, 0, None, 0) == M.api.ERR_ARG
     assert L.mlmd_domain_create(ctypes.byref(h), 1, 16, 16, 3, 0.5, 0.5, 0.5, 8, 8, ctypes.c_void_p(256), 1 << 30, None, 0) == M.api.ERR_SHAPE
+    # unknown create flags; MLMD_BORROW_PSI needs unpadded rows (norb a multiple of 16)
+    assert L.mlmd_domain_create(ctypes.byref(h), 1, 16, 16, 16, 0.5, 0.5, 0.5, 8, 8, ctypes.c_void_p(256), 1 << 30, None, 64) == M.api.ERR_ARG
+    assert L.mlmd_domain_create(ctypes.byref(h), 1, 16, 16, 16, 0.5, 0.5, 0.5, 8, 8, ctypes.c_void_p(256), 1 << 30, None, M.BORROW_PSI) == M.api.ERR_SHAPE
+    assert L.mlmd_set_option(None, 0, 0) == M.api.ERR_ARG
     assert L.mlmd_domain_destroy(None) == M.api.OK
     assert M.mlmd_launch_count(None) == 0
     # the NEXT-row calls check their arguments before touching the device too

@@ -22,6 +22,35 @@ def test_reference_arm_prints_one_json_line():
     assert "workload" in j["config"] and "model" not in j["config"]
 
 
+def test_reference_arm_under_torchrun_two_ranks():
+    """The driver launches both arms the same way; for N > 1 that is torch.distributed.run: rank 0 alone runs the
+    oracle and prints the line, the other rank exits 0 without work."""
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29541", os.path.join(ROOT, "bench.py"),
+                          "--impl", "reference", "--gpus", "2", "--config", "0", "--steps", "1", "--warmup", "0"],
+                         capture_output=True, text=True, timeout=900, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert j["impl"] == "reference" and j["n_gpus"] == 2 and j["value"] > 0
+    for key in ("metric", "unit", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline", "dtype",
+                "data", "config", "cpu_baseline", "e2e", "gpu_launches"):
+        assert key in j, key
+
+
+def test_both_arms_describe_the_workload_identically():
+    """`config` is built by one function from the arguments both arms share (no keys that only one arm can fill)."""
+    sys.path.insert(0, ROOT)
+    import argparse
+    import bench
+    import workloads as W
+    args = argparse.Namespace(step="taylor", gemm_mode="fp32grade")
+    cfg = bench.workload_config(W.get_config(3), args)
+    assert set(cfg) == {"workload", "ndom_per_gpu", "step", "gemm_mode", "parallelism", "l2"}
+    assert "configs[3]" in cfg["workload"] and cfg["ndom_per_gpu"] == 64
+
+
 def test_algorithmic_counts_match_design():
     sys.path.insert(0, ROOT)
     import bench

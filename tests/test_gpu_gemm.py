@@ -1,5 +1,6 @@
 """Kernel-level GPU checks of the tcgen05 GEMMs (csrc/gemm_tc.cu) against a dense FP64 product of the
-same operands (torch on the GPU), through the test hooks of csrc/debug.cu.  Shapes span several M / N
+same operands (torch on the GPU), through the test hooks of csrc/test_hooks.cu
+(libmlmd_test.so: the product objects plus the hooks; the product library does not export them).  Shapes span several M / N
 tiles, a ragged projector count, several split-K slices and accumulation chains.
 
 What they pin: operand layouts (MN-major 32B-atom swizzle, K-major SW32), descriptor strides, the
@@ -16,10 +17,11 @@ pytestmark = pytest.mark.gpu
 @pytest.fixture(scope="module")
 def L():
     import paper_2509_00966_b200 as M
-    lib = M.lib()
+    M.lib()
+    lib = ctypes.CDLL(M.api.TEST_LIB_PATH)
     i, p, l = ctypes.c_int, ctypes.c_void_p, ctypes.c_long
     lib.mlmd_debug_proj.argtypes = [i, p, i, l, p, p, i, i, p, i, i, p, i, i, i, i]
-    lib.mlmd_debug_back.argtypes = [i, p, i, l, p, p, i, i, p, p, p, i, i, i, i]
+    lib.mlmd_debug_back.argtypes = [i, p, i, l, p, i, i, p, p, p, i, i, i, i]
     return lib
 
 
@@ -29,7 +31,9 @@ def hi_lo(x):
     return h, x - h
 
 
-def run_proj(L, path, ndom, ngrid, P, N, nsplit, nprod, chain, positive=False, split_in_kernel=False):
+def run_proj(L, path, ndom, ngrid, P, N, nsplit, nprod, chain, positive=False, split_in_kernel=True):
+    """split_in_kernel (the product path): A is ONE plain FP32 array, the kernel forms hi / lo in shared memory;
+    False: a pre-split (hi, lo) pair is handed over (the kernel's second operand stream, kept for callers that have it)."""
     import torch
     g = torch.Generator(device="cuda").manual_seed(1234)
     lda = (P + 7) // 8 * 8
@@ -62,9 +66,8 @@ def run_back(L, path, ndom, ngrid, P, N, nprod):
     W[:, :P] = torch.randn(ndom, P, N, device="cuda", generator=g)
     Y0 = torch.randn(ndom, ngrid, N, device="cuda", generator=g)
     Y = Y0.clone()
-    Ah, Al = hi_lo(A)
     Wh, Wl = hi_lo(W)
-    rc = L.mlmd_debug_back(path, None, ndom, ngrid, Ah.data_ptr(), Al.data_ptr(), lda, P, Wh.data_ptr(), Wl.data_ptr(),
+    rc = L.mlmd_debug_back(path, None, ndom, ngrid, A.data_ptr(), lda, P, Wh.data_ptr(), Wl.data_ptr(),
                            Y.data_ptr(), N, N, prows, nprod)
     assert rc == 0
     ref = Y0.double() + torch.einsum("drp,dpc->drc", A.double(), W[:, :lda].double())
@@ -89,8 +92,8 @@ def test_projection_chain_bounds_truncation_drift(L):
     assert short_chain < 4e-6 and long_chain > 4 * short_chain
 
 
-def test_projection_splits_A_in_kernel(L):
-    assert run_proj(L, 1, 2, 2048, 448, 448, 2, 3, 4, split_in_kernel=True) < 4e-6
+def test_projection_with_presplit_operand_pair(L):
+    assert run_proj(L, 1, 2, 2048, 448, 448, 2, 3, 4, split_in_kernel=False) < 4e-6
 
 
 @pytest.mark.parametrize("nprod,tol", [(1, 2e-3), (0, 1.5e-2)])

@@ -31,7 +31,7 @@ def rho_err(a, b):
     return float((np.abs(a - b).max(axis=(1, 2, 3)) / b.max(axis=(1, 2, 3))).max())
 
 
-def make_domain(c, d, flags=0, mode=None, nproj_max=None):
+def make_domain(c, d, flags=0, mode=None, nproj_max=None, options=()):
     import paper_2509_00966_b200 as M
     beta = d.get("beta")
     nproj = 0 if beta is None else beta.shape[-1]
@@ -39,6 +39,8 @@ def make_domain(c, d, flags=0, mode=None, nproj_max=None):
     if nproj_max is None:
         nproj_max = nproj * (2 if cplx else 1)
     dom = M.Domain(c.ndom, c.grid, c.h, c.norb, nproj_max, flags=flags)
+    for key, value in options:
+        dom.set_option(key, value)
     dom.set_vloc(d["vloc"])
     dom.set_orbitals(d["psi"], d["occ"])
     dom.set_projectors(beta, d.get("D"))
@@ -108,11 +110,11 @@ def test_config1_smooth_orbitals_gram_identity():
     dom.close()
 
 
-@pytest.mark.parametrize("variant,grid", [("0", (16, 8, 24)), ("1", (16, 8, 24)), ("2", (10, 16, 32)), ("2", (7, 32, 16))])
-def test_plane_wave_closed_form_on_gpu(variant, grid, monkeypatch):
+# variant = MLMD_OPT_STENCIL: 2 one thread per output, 1 register marching, 0 TMA planes (ny, nz multiples of 16)
+@pytest.mark.parametrize("variant,grid", [(2, (16, 8, 24)), (1, (16, 8, 24)), (0, (10, 16, 32)), (0, (7, 32, 16))])
+def test_plane_wave_closed_form_on_gpu(variant, grid):
     """P1 on the GPU itself (FP32 tolerance): V=0, no projectors, amplification P4(-i dt eps)^n."""
     import paper_2509_00966_b200 as M
-    monkeypatch.setenv("MLMD_STENCIL", variant)
     h, dt, nsteps = (0.5, 0.45, 0.4), 0.02, 5
     A = (0.07, -0.04, 0.11)
     box = [n * s for n, s in zip(grid, h)]
@@ -132,6 +134,7 @@ def test_plane_wave_closed_form_on_gpu(variant, grid, monkeypatch):
         eps.append(e)
     psi32 = psi.astype(np.complex64)
     dom = M.Domain(1, grid, h, len(ms), 0)
+    dom.set_option(M.OPT_STENCIL, variant)
     dom.set_vloc(np.zeros((1, *grid), dtype=np.float32))
     dom.set_orbitals(psi32, np.ones((1, len(ms))))
     dom.propagate(nsteps, dt, np.tile(np.array(A), (nsteps, 1, 1)))
@@ -178,16 +181,15 @@ def test_ragged_shapes_complex_projectors_per_domain_field(grid, norb, cplx):
     dom.close()
 
 
-def test_stencil_variants_agree(monkeypatch):
+def test_stencil_variants_agree():
     """The TMA-plane kernel, the register-marching kernel and the one-thread-per-output cross-check
     kernel compute the same stage."""
     import paper_2509_00966_b200 as M
     c = W.get_config(1, nsteps=3)
     d = W.generate(c)
     outs = []
-    for variant in ("0", "1", "2"):
-        monkeypatch.setenv("MLMD_STENCIL", variant)
-        dom = make_domain(c, d)
+    for variant in (2, 1, 0):
+        dom = make_domain(c, d, options=[(M.OPT_STENCIL, variant)])
         dom.propagate(3, c.dt, d["A"])
         outs.append(dom.get_orbitals())
         dom.close()
@@ -263,6 +265,58 @@ def test_device_pointers_and_torch_tensors():
     host.close()
 
 
+def test_borrowed_psi_buffer_is_updated_in_place():
+    """MLMD_BORROW_PSI: the handle adopts the caller's device Psi, every step updates that buffer in
+    place, and the results are bit-equal to a handle that copies; the workspace is one Psi buffer smaller."""
+    import torch
+    import paper_2509_00966_b200 as M
+    c = W.get_config(1, nsteps=3)                  # 64 orbitals: rows need no padding
+    d = W.generate(c)
+    own = make_domain(c, d, flags=M.KEEP_PSI0)
+    own.propagate(3, c.dt, d["A"])
+    expect, rho_expect, S_expect = own.get_orbitals(), own.density(), own.overlap(1)
+    ws_own = own.workspace_bytes
+    own.close()
+    buf = torch.from_numpy(d["psi"]).cuda()
+    dom = M.Domain(c.ndom, c.grid, c.h, c.norb, c.nproj, flags=M.BORROW_PSI | M.KEEP_PSI0)
+    assert ws_own - dom.workspace_bytes == c.ngrid * c.norb * 8      # no Psi copy in the workspace
+    dom.set_vloc(d["vloc"])
+    dom.set_projectors(d["beta"], d["D"])
+    with pytest.raises(M.MlmdError):
+        dom.set_orbitals(d["psi"], d["occ"])       # a host array cannot be borrowed
+    dom.set_orbitals(buf, d["occ"])
+    dom.propagate(3, c.dt, d["A"])
+    torch.cuda.synchronize()
+    assert np.array_equal(buf.cpu().numpy(), expect)            # the caller's buffer holds Psi(t)
+    assert np.array_equal(dom.get_orbitals(), expect) and np.array_equal(dom.density(), rho_expect)
+    assert np.array_equal(dom.overlap(1), S_expect)              # Psi(0) was snapshotted at set_orbitals
+    dom.close()
+    with pytest.raises(M.MlmdError) as e:
+        M.Domain(1, (16, 16, 16), (0.5, 0.5, 0.5), 8, 8, flags=M.BORROW_PSI)      # 8 orbitals: rows would need padding
+    assert e.value.code == M.api.ERR_SHAPE
+
+
+def test_projector_capacity_counts_real_rows_and_options_are_checked():
+    """include/mlmd.h: nproj_max counts REAL projector rows, a complex64 projector takes two."""
+    import paper_2509_00966_b200 as M
+    c = W.get_config(0)
+    d = W.generate(c)
+    dom = M.Domain(c.ndom, c.grid, c.h, c.norb, 8)
+    dom.set_projectors(d["beta"], d["D"])                                     # 8 real projectors fit 8 rows
+    bc = (d["beta"][..., :5] + 1j * d["beta"][..., :5]).astype(np.complex64)
+    with pytest.raises(M.MlmdError) as e:
+        dom.set_projectors(bc, d["D"][:, :5])                                 # 5 complex = 10 rows > 8
+    assert e.value.code == M.api.ERR_SHAPE
+    dom.set_projectors(np.ascontiguousarray(bc[..., :4]), d["D"][:, :4])      # 4 complex = 8 rows
+    for key, value in ((-1, 0), (M.api.OPT_KICK_NORM + 1, 0), (M.OPT_STENCIL, 3), (M.OPT_GRAPH, 2), (M.OPT_GEMM_PATH, -1)):
+        with pytest.raises(M.MlmdError) as e:
+            dom.set_option(key, value)
+        assert e.value.code == M.api.ERR_ARG
+    dom.set_option(M.OPT_GEMM_PATH, 1)
+    assert dom.gemm_path() == "simt"
+    dom.close()
+
+
 def test_gemm_modes():
     """FP64 accumulation is at least as close to the oracle as the default; the CUDA-core FP32 path
     and the TF32x1 rung meet the FP32-grade bar; the opt-in BF16 mode meets its stated 1e-3."""
@@ -317,7 +371,7 @@ def test_perovskite_domain_two_steps():
     check(run_both(c, d, 2, A=A, check_first=False))
 
 
-def test_cuda_graph_step_equals_eager_launches(monkeypatch):
+def test_cuda_graph_step_equals_eager_launches():
     """Small batches replay a CUDA graph of the step (device-side coefficient slot): same bits as the
     eager launches, with a field that changes every step and differs per domain."""
     c = W.get_config(0, ndom=2, nsteps=9)
@@ -326,9 +380,9 @@ def test_cuda_graph_step_equals_eager_launches(monkeypatch):
     A = 0.05 * rng.standard_normal((9, 2, 3))
     A[:, :, 1:] = 0.0
     outs, launches = [], []
-    for flag in ("1", "0"):
-        monkeypatch.setenv("MLMD_GRAPH", flag)
-        dom = make_domain(c, d)
+    import paper_2509_00966_b200 as M
+    for flag in (1, 0):
+        dom = make_domain(c, d, options=[(M.OPT_GRAPH, flag)])
         dom.propagate(9, c.dt, A)
         dom.propagate(5, c.dt, A[:5])          # second call reuses the captured graph
         outs.append((dom.get_orbitals(), dom.density()))
@@ -338,7 +392,7 @@ def test_cuda_graph_step_equals_eager_launches(monkeypatch):
     assert launches[0] > launches[1]            # + the coefficient-slot kernels of the graph
 
 
-def test_long_call_crosses_coefficient_upload_chunks(monkeypatch):
+def test_long_call_crosses_coefficient_upload_chunks():
     """One mlmd_propagate call of 600 steps (N_QD ~ 10^3 per MD step): the per-step coefficients are
     uploaded in chunks of 256 steps, so the call crosses two chunk boundaries, with and without the CUDA graph; the
     field changes every step and differs per domain.  Against the oracle, and graph == eager bit for bit."""
@@ -349,9 +403,9 @@ def test_long_call_crosses_coefficient_upload_chunks(monkeypatch):
     t = np.arange(600)[:, None, None] * c.dt
     A = 0.05 * np.sin(0.7 * t + rng.uniform(0, 6, (1, 2, 3)))
     outs = []
-    for flag in ("1", "0"):
-        monkeypatch.setenv("MLMD_GRAPH", flag)
-        dom = make_domain(c, d)
+    import paper_2509_00966_b200 as M
+    for flag in (1, 0):
+        dom = make_domain(c, d, options=[(M.OPT_GRAPH, flag)])
         dom.propagate(600, c.dt, A)
         outs.append((dom.get_orbitals(), dom.density()))
         dom.close()

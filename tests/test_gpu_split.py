@@ -160,7 +160,7 @@ def test_occupations_and_excited_electrons_after_the_pulse():
     dom.close()
 
 
-def test_split_cuda_graph_equals_eager_launches(monkeypatch):
+def test_split_cuda_graph_equals_eager_launches():
     """Small batches replay a CUDA graph of the split step too; switching between the two steppers on one handle
     re-captures.  Same bits as the eager launches."""
     c = W.get_config(0, ndom=2, nsteps=9)
@@ -168,9 +168,9 @@ def test_split_cuda_graph_equals_eager_launches(monkeypatch):
     rng = np.random.default_rng(12)
     A = 0.05 * rng.standard_normal((9, 2, 3))
     outs = []
-    for flag in ("1", "0"):
-        monkeypatch.setenv("MLMD_GRAPH", flag)
-        dom = make_domain(c, d)
+    import paper_2509_00966_b200 as M
+    for flag in (1, 0):
+        dom = make_domain(c, d, options=[(M.OPT_GRAPH, flag)])
         dom.propagate_split(9, c.dt, A)
         dom.propagate(6, c.dt, A[:6])
         dom.propagate_split(5, c.dt, A[:5])
@@ -212,15 +212,13 @@ def test_split_scissor_form_of_eq5():
     dom.close()
 
 
-def test_split_more_projector_rows_than_orbital_columns(monkeypatch):
+def test_split_more_projector_rows_than_orbital_columns():
     """ldp > 2 ld: the Gram-matrix identity for the norm after the second kick does not apply (its scratch is sized by
-    the psi columns), so the per-step norm pass runs; also forced on a normal shape with MLMD_KICK_IDENTITY=0."""
+    the psi columns), so the per-step norm pass runs; also forced on a normal shape with MLMD_OPT_KICK_NORM = 1."""
     import paper_2509_00966_b200 as M
     from oracle import ref
     rng = np.random.default_rng(5)
-    for grid, norb, nproj, env in (((8, 8, 8), 2, 40, None), ((16, 16, 16), 6, 5, "0")):
-        if env is not None:
-            monkeypatch.setenv("MLMD_KICK_IDENTITY", env)
+    for grid, norb, nproj, norm_pass in (((8, 8, 8), 2, 40, 0), ((16, 16, 16), 6, 5, 1)):
         ndom, h, dt, nsteps = 2, (0.5, 0.45, 0.4), 0.02, 4
         ngrid = int(np.prod(grid))
         psi = (rng.standard_normal((ndom, *grid, norb)) + 1j * rng.standard_normal((ndom, *grid, norb))).astype(np.complex64)
@@ -230,6 +228,7 @@ def test_split_more_projector_rows_than_orbital_columns(monkeypatch):
         D = rng.uniform(-2, 2, (ndom, nproj))
         A = rng.uniform(-0.2, 0.2, (nsteps, 1, 3))
         dom = M.Domain(ndom, grid, h, norb, nproj)
+        dom.set_option(M.OPT_KICK_NORM, norm_pass)
         dom.set_vloc(vloc)
         dom.set_orbitals(psi, occ)
         dom.set_projectors(beta, D)
