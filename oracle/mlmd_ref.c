@@ -50,9 +50,15 @@ typedef double complex zc;
 #define MLMD_REF_NO_KINETIC 1 /* oracle-internal switch for pin P6: drop -1/2 D2 - iA.D1 + 1/2|A|^2 */
 #define MLMD_REF_HORNER 2     /* pin P10: evaluate the same polynomial in Horner form */
 #define MLMD_REF_NO_LOCAL 4   /* split step (Eq. 2): drop the whole local part, out = V_NL u */
+#define MLMD_REF_ORDER2 8     /* the paper's own local discretisation ("nearest-neighbor mesh points", L283
+                               * "7-point star stencil"): 2nd-order central differences c2 = [1, -2, 1] / h^2,
+                               * c1 = [-1/2, 0, 1/2] / h instead of north_star's 4th-order ones */
 
 static const double C2[5] = {-1.0 / 12.0, 4.0 / 3.0, -5.0 / 2.0, 4.0 / 3.0, -1.0 / 12.0};
 static const double C1[5] = {1.0 / 12.0, -2.0 / 3.0, 0.0, 2.0 / 3.0, -1.0 / 12.0};
+/* 2nd order (7-point star), written on the same five offsets j = -2..2 */
+static const double C2_O2[5] = {0.0, 1.0, -2.0, 1.0, 0.0};
+static const double C1_O2[5] = {0.0, -0.5, 0.0, 0.5, 0.0};
 
 static int wrap(int i, int n) {
     i %= n;
@@ -77,6 +83,8 @@ int mlmd_ref_apply_h(int nx, int ny, int nz, double hx, double hy, double hz, in
     const double dv = hx * hy * hz;
     const double A2 = A[0] * A[0] + A[1] * A[1] + A[2] * A[2];
     const int kinetic = !(flags & MLMD_REF_NO_KINETIC);
+    const double *c2 = (flags & MLMD_REF_ORDER2) ? C2_O2 : C2;
+    const double *c1 = (flags & MLMD_REF_ORDER2) ? C1_O2 : C1;
 
     if (flags & MLMD_REF_NO_LOCAL) {
         for (size_t e = 0; e < (size_t)ngrid * norb; ++e) out[e] = 0.0;
@@ -96,7 +104,7 @@ int mlmd_ref_apply_h(int nx, int ny, int nz, double hx, double hy, double hz, in
                         int q3[3] = {i3[0], i3[1], i3[2]};
                         q3[d] = wrap(i3[d] + j, n3[d]);
                         const long rr = ((long)q3[0] * ny + q3[1]) * nz + q3[2];
-                        const zc coef = -0.5 * C2[j + 2] / (h[d] * h[d]) - I * A[d] * C1[j + 2] / h[d];
+                        const zc coef = -0.5 * c2[j + 2] / (h[d] * h[d]) - I * A[d] * c1[j + 2] / h[d];
                         for (int n = 0; n < norb; ++n) out[r * norb + n] += coef * u[rr * norb + n];
                     }
             }
@@ -413,6 +421,49 @@ int mlmd_ref_current(int ndom, int nx, int ny, int nz, double hx, double hy, dou
             free(plane);
             J[(size_t)dom * 3 + d] = acc;
         }
+    }
+    return 0;
+}
+
+/* Nonlocal (pseudopotential) part of the TDCDFT current of one batch ("GEMMification is applied to
+ * nonlocal correction in energy and electric current (TDCDFT), with the latter used in Maxwell's equations"; the paper
+ * prints no formula: reading D31 in DESIGN.md).  The velocity operator of a nonlocal potential is -i [r, V_NL]; with
+ * V_NL = dv sum_p |beta_p> D_p <beta_p| its expectation value is
+ *   J_d = sum_n f_n <psi_n| -i [r_d, V_NL] |psi_n> = 2 dv^2 sum_n f_n sum_p D_p Im( conj(G_dpn) C_pn ),
+ *   C_pn = sum_r conj(beta_p(r)) psi_n(r),   G_dpn = sum_r conj(rbeta_dp(r)) psi_n(r),   rbeta_dp(r) = (r - R_p)_d beta_p(r)
+ * ((r - R_p): position relative to the projector's centre, minimum image; a constant shift R_p commutes, so each term
+ * is the commutator with r itself).  The caller supplies the three arrays rbeta_d: [ndom][ngrid][nproj] each.
+ * J: [ndom][3]. */
+int mlmd_ref_current_nl(int ndom, long ngrid, int norb, int nproj, double dv, const zc *psi, const double *occ,
+                        const zc *beta, const zc *rbeta /* [3][ndom][ngrid][nproj] */, const double *D, double *J) {
+    for (int dom = 0; dom < ndom; ++dom) {
+        const zc *p = psi + (size_t)dom * ngrid * norb;
+        const zc *b = beta + (size_t)dom * ngrid * nproj;
+        zc *C = (zc *)calloc((size_t)nproj * norb, sizeof(zc));
+        zc *G = (zc *)calloc((size_t)nproj * norb, sizeof(zc));
+        if (!C || !G) {
+            free(C);
+            free(G);
+            return 5;
+        }
+        for (long r = 0; r < ngrid; ++r)
+            for (int q = 0; q < nproj; ++q)
+                for (int n = 0; n < norb; ++n) C[(size_t)q * norb + n] += conj(b[r * nproj + q]) * p[r * norb + n];
+        for (int d = 0; d < 3; ++d) {
+            const zc *rb = rbeta + ((size_t)d * ndom + dom) * ngrid * nproj;
+            memset(G, 0, (size_t)nproj * norb * sizeof(zc));
+            for (long r = 0; r < ngrid; ++r)
+                for (int q = 0; q < nproj; ++q)
+                    for (int n = 0; n < norb; ++n) G[(size_t)q * norb + n] += conj(rb[r * nproj + q]) * p[r * norb + n];
+            double acc = 0.0;
+            for (int n = 0; n < norb; ++n)
+                for (int q = 0; q < nproj; ++q)
+                    acc += occ[(size_t)dom * norb + n] * D[(size_t)dom * nproj + q] *
+                           cimag(conj(G[(size_t)q * norb + n]) * C[(size_t)q * norb + n]);
+            J[(size_t)dom * 3 + d] = 2.0 * dv * dv * acc;
+        }
+        free(C);
+        free(G);
     }
     return 0;
 }

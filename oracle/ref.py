@@ -17,6 +17,7 @@ from . import build as _build
 NO_KINETIC = 1
 HORNER = 2
 NO_LOCAL = 4
+ORDER2 = 8      # 2nd-order (7-point) stencil: the paper's own local discretisation (NEXT-3)
 
 _lib = None
 
@@ -43,6 +44,8 @@ def lib() -> ctypes.CDLL:
         _lib.mlmd_ref_energy_nl.restype = i
         _lib.mlmd_ref_current.argtypes = [i, i, i, i, d, d, d, i, p, p, p, i, p]
         _lib.mlmd_ref_current.restype = i
+        _lib.mlmd_ref_current_nl.argtypes = [i, l, i, i, d, p, p, p, p, p, p]
+        _lib.mlmd_ref_current_nl.restype = i
     return _lib
 
 
@@ -174,4 +177,20 @@ def current(psi, occ, A, h: Sequence[float]) -> np.ndarray:
     assert A.shape[0] in (1, ndom)
     J = np.empty((ndom, 3), dtype=np.float64)
     lib().mlmd_ref_current(ndom, nx, ny, nz, h[0], h[1], h[2], norb, _ptr(p), _ptr(_f64(occ)), _ptr(A), A.shape[0], _ptr(J))
+    return J
+
+
+def current_nl(psi, occ, beta, rbeta, D, dv: float) -> np.ndarray:
+    """Nonlocal part of the current: J[dom][d] = sum_n f_n <psi_n| -i [r_d, V_NL] |psi_n>.
+    rbeta: [3, ndom, ngrid, nproj] = (r - R_p)_d beta_p(r), supplied by the caller."""
+    p = _c128(psi)
+    ndom, nx, ny, nz, norb = p.shape
+    nproj = beta.shape[-1]
+    b = _c128(beta.reshape(ndom, -1, nproj))
+    rb = _c128(rbeta.reshape(3, ndom, -1, nproj))
+    J = np.empty((ndom, 3), dtype=np.float64)
+    rc = lib().mlmd_ref_current_nl(ndom, nx * ny * nz, norb, nproj, dv, _ptr(p), _ptr(_f64(occ)), _ptr(b), _ptr(rb),
+                                   _ptr(_f64(D)), _ptr(J))
+    if rc:
+        raise RuntimeError("mlmd_ref_current_nl failed: %d" % rc)
     return J

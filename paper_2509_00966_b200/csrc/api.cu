@@ -80,7 +80,8 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.psi0 = take((flags & MLMD_KEEP_PSI0) ? psi_b : 0);
     w.vloc = take(npts * sizeof(float));
     // + slack: the last 32-column TMA chunk of a row may read up to 128 B past the row
-    w.beta = take(npts * pl->ldp_max * sizeof(float) + 256);   // ONE FP32 copy: the kernels form hi / lo in shared memory
+    w.beta = take(npts * pl->ldp_max * sizeof(float) + 256);      // the projectors as given
+    w.beta_lo = take(npts * pl->ldp_max * sizeof(float) + 256);   // what a TF32 operand drops of them (back-application)
     w.dprime = take((size_t)ndom * pl->ldp_max * sizeof(float));
     w.occ = take((size_t)ndom * pl->ld * sizeof(float));
     w.rho = take(npts * sizeof(float));
@@ -352,6 +353,9 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
     // rows [P, ldp) of W are read (times zero columns of beta) by the K = 8 slabs of the back-application: a stale NaN
     // left there by an earlier projector set or a diverged run would poison psi
     CU(cudaMemsetAsync(h->what(), 0, 2 * (h->off.what_lo - h->off.what), h->stream));
+    int nl = 0;
+    CU(launch_tf32_remainder(h->stream, h->beta(), h->beta_lo(), rows * ldp, &nl));
+    h->launches += nl;
     CU(cudaStreamSynchronize(h->stream));   // dp is a temporary; host beta may be reused by the caller
     h->nproj = nproj; h->beta_complex = cplx; h->P = P; h->ldp = ldp; h->dmax = dmax;
     return MLMD_OK;
@@ -516,7 +520,7 @@ static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl, int nprod = -1) {
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     ProfScope ps(h, MLMD_K_BACK);
     if (use_tensor_cores(h))
-        CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->ldp, h->P, h->what(), h->what_lo(),
+        CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
                           (float *)out, 2 * h->ld, 2 * h->ld, h->prows, nprod, nl, &h->tmaps));
     else
         CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, h->what(), h->what_lo(),

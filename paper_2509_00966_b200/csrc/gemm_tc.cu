@@ -433,8 +433,10 @@ constexpr int P2_Y_BYTES = 7 * PJ_BK * 128;             // this CTA's half of th
 constexpr int P2_STAGE_BYTES = 2 * P2_A_BYTES + 2 * P2_Y_BYTES;   // 44 KB (3xTF32); one-product modes use half
 constexpr int P2_STAGES = 4;
 constexpr int P2_SMEM = P2_STAGES * P2_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 512;
-constexpr int P2_FWD = 4;                               // forwarding lanes of the peer's MMA warp
+constexpr int P2_FWD = 4;                               // forwarding lanes of the peer's MMA warp; must divide the stage count, so
+                                                        // that one lane sees all uses of a barrier in order (parity waits)
 
+static_assert(P2_STAGES % P2_FWD == 0, "one forwarding lane must see every use of a stage barrier in order");
 template <bool LO>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PJ_THREADS, 1)
 proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_y0,
@@ -840,20 +842,20 @@ back_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant_
 // TMA fills, cap the tensor pipe near 75 % (measured); this is what cta_group::2 exists for.
 // Per CTA: 128 x BN accumulator in TMEM (BN <= 448, BN % 64 == 0), UMMA pieces of N = 256 and BN - 256.
 //
-// beta is read from HBM ONCE as plain FP32: four converter warps per CTA (each takes every fourth stage) round the slab
-// to TF32 in place and write the exact remainder next to it, then tell the LEADER (whose single thread issues the
-// pair's UMMAs) with a cluster-scope arrive on its `conv` barrier: the beta_lo stream of round 1 (6.8 GB per launch at
-// configs[3]) is gone from HBM and from L2.
+// Operands of 3xTF32: the hi product reads the RAW FP32 beta slab (kind::tf32 ignores the 13 low mantissa bits, i.e.
+// uses beta truncated to TF32), the lo product the stored remainder beta - trunc(beta) (exact; written once by
+// mlmd_set_projectors).  Forming that remainder in shared memory instead (as the projection does) was built and
+// measured here in round 2: the leader's MMA thread then has to wait for a "slab converted" signal from BOTH CTAs
+// per K = 8 stage, and the kernel went from 9.3 to 11.3 ms at configs[3] although it read 6.8 GB less
+// (profiles/r2_negative_results.md), so this kernel keeps the second HBM stream.
 // =================================================================================================
 constexpr int B2_STAGES = 7;
 constexpr int B2_WH_BYTES = 7 * 1024;                  // this CTA's half of the W slab: <= 224 columns
 constexpr int B2_STAGE_BYTES = 2 * BK_A_BYTES + 2 * B2_WH_BYTES;
 constexpr int B2_SMEM = B2_STAGES * B2_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 512;
-constexpr int B2_CONV_WARPS = 4;
-constexpr int B2_THREADS = BK_THREADS + 32 * B2_CONV_WARPS;
 
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(B2_THREADS, 1)
-back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(BK_THREADS, 1)
+back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
                 const __grid_constant__ CUtensorMap map_w0h, const __grid_constant__ CUtensorMap map_w0l,
                 const __grid_constant__ CUtensorMap map_w1h, const __grid_constant__ CUtensorMap map_w1l,
                 const __grid_constant__ CUtensorMap map_out, const BackParams q) {
@@ -861,8 +863,8 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *stage = smem + B2_STAGES * B2_STAGE_BYTES;
     uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
-    uint64_t *full = bars, *empty = bars + B2_STAGES, *afull = bars + 2 * B2_STAGES, *conv = bars + 3 * B2_STAGES;
-    uint64_t *acc_full = bars + 4 * B2_STAGES, *acc_empty = acc_full + 1;
+    uint64_t *full = bars, *empty = bars + B2_STAGES;
+    uint64_t *acc_full = bars + 2 * B2_STAGES, *acc_empty = acc_full + 1;
     uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
     const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
     const int crank = (int)cluster_ctarank();
@@ -870,15 +872,14 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < B2_STAGES; ++s) {
-            mbar_init(&full[s], 1);     // used in the leader: its own expect_tx arrive; both CTAs' W bytes land on it
+            mbar_init(&full[s], 1);     // used in the leader: its own expect_tx arrive; both CTAs' TMA bytes land on it
             mbar_init(&empty[s], 1);    // the leader's tcgen05.commit, multicast to both CTAs
-            mbar_init(&afull[s], 1);    // LOCAL: this CTA's beta slab has landed (its converter warp waits here)
-            mbar_init(&conv[s], 2);     // used in the leader: one converter warp per CTA has split the slab
         }
         mbar_init(acc_full, 1);         // commit multicast
         mbar_init(acc_empty, 2);        // one elected epilogue thread per CTA (remote arrive on the leader)
         fence_barrier_init();
-        prefetch_tmap(&map_a);
+        prefetch_tmap(&map_ahi);
+        prefetch_tmap(&map_alo);
         prefetch_tmap(&map_w0h);
         prefetch_tmap(&map_w0l);
         prefetch_tmap(&map_out);
@@ -896,7 +897,7 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
     const bool need_lo = q.nprod >= 2, need_wlo = q.nprod == 3;   // as in back_tc_kernel
     const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;   // UMMA pieces (columns); per CTA n/2 of each
     const int h0 = n0 / 64, h1 = n1 / 64;                      // this CTA's 32-column chunks of each piece
-    const uint32_t w_bytes = (need_wlo ? 2u : 1u) * (uint32_t)(h0 + h1) * 1024;   // per CTA
+    const uint32_t cta_bytes = (need_lo ? 2u : 1u) * BK_A_BYTES + (need_wlo ? 2u : 1u) * (uint32_t)(h0 + h1) * 1024;
 
     if (warp == 0) {
         if (lane == 0) {
@@ -909,12 +910,12 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
                     const int s = it % B2_STAGES;
                     mbar_wait(&empty[s], ((it / B2_STAGES) & 1) ^ 1);
                     uint8_t *st = smem + s * B2_STAGE_BYTES;
-                    if (leader) mbar_expect_tx(&full[s], 2 * w_bytes);
-                    mbar_expect_tx(&afull[s], BK_A_BYTES);
+                    if (leader) mbar_expect_tx(&full[s], 2 * cta_bytes);
                     const int wrow = dom * q.prows + k * 8;
-                    tma_load_2d(st, &map_a, &afull[s], k * 8, row);          // raw beta slab, this CTA's barrier
+                    tma_load_2d_2cta(st, &map_ahi, &full[s], k * 8, row);
                     tma_load_3d_2cta(st + 2 * BK_A_BYTES, &map_w0h, &full[s], 0, wrow, ch0);
                     if (h1) tma_load_3d_2cta(st + 2 * BK_A_BYTES + h0 * 1024, &map_w1h, &full[s], 0, wrow, ch1);
+                    if (need_lo) tma_load_2d_2cta(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
                     if (need_wlo) {
                         tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES, &map_w0l, &full[s], 0, wrow, ch0);
                         if (h1)
@@ -934,7 +935,6 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
                 for (int k = 0; k < nk; ++k, ++it) {
                     const int s = it % B2_STAGES;
                     mbar_wait(&full[s], (it / B2_STAGES) & 1);
-                    mbar_wait(&conv[s], (it / B2_STAGES) & 1);
                     tc_fence_after();
                     const uint32_t st = smem_u32(smem + s * B2_STAGE_BYTES);
                     const uint64_t da = smem_desc(st, 16, 256, LAYOUT_SW32);
@@ -959,7 +959,7 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
                 umma_commit_2cta_mc(acc_full, (uint16_t)3);
             }
         }
-    } else if (warp < 2 + BK_EPI_WARPS) {
+    } else {
         const int quarter = warp % 4;
         const int er = quarter * 32 + lane;         // accumulator row of this thread
         int nu = 0, slot = 0;
@@ -981,22 +981,6 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_a,
             if (er == 0) mbar_arrive_remote(acc_empty, 0);   // this CTA's half of the accumulator is drained
         }
         if (er == 0) bulk_wait<0>();
-    } else {
-        // converter warps: warp j takes the stages it == j (mod B2_CONV_WARPS) of the CTA's stage sequence
-        const int cw = warp - (2 + BK_EPI_WARPS);
-        const int cmode = need_lo ? 0 : 1;
-        int it = 0;
-        for (int u = cl; u < total; u += ncl) {
-            for (int k = 0; k < nk; ++k, ++it) {
-                if (it % B2_CONV_WARPS != cw) continue;
-                const int s = it % B2_STAGES;
-                mbar_wait(&afull[s], (it / B2_STAGES) & 1);
-                convert_a_slab(smem + s * B2_STAGE_BYTES, lane, 32, cmode);
-                fence_proxy_async_smem();
-                __syncwarp();
-                if (lane == 0) mbar_arrive_remote(&conv[s], 0);
-            }
-        }
     }
     tc_fence_before();
     __syncthreads();
@@ -1107,7 +1091,7 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     return cudaGetLastError();
 }
 
-cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A, int lda, int P,
+cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A, const float *A_lo, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
                            int *nlaunch, TmapCache *cache) {
     static DeviceOnce attr_set;
@@ -1137,7 +1121,9 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     const int total = ndom * (int)((ngrid / 128 + 1) / 2) * q.ntile_n;   // cluster units (pairs of row tiles)
     const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
-    if (q.BN % 64 == 0 && !q.lowp) {
+    // CTA pairs for the modes that take beta as (raw, stored remainder): 3xTF32 and the staged mode's two products;
+    // one-product modes want beta ROUNDED (an unbiased operand), which the single-CTA kernel forms in shared memory
+    if (q.BN % 64 == 0 && !q.lowp && q.nprod >= 2 && A_lo) {
         static DeviceOnce attr2;
         if (!attr2.done()) {
             cudaError_t e = cudaFuncSetAttribute(back2_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, B2_SMEM);
@@ -1145,12 +1131,13 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
             attr2.mark();
         }
         const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;
-        CUtensorMap w0h, w0l, w1h, w1l;
+        CUtensorMap mal, w0h, w0l, w1h, w1l;
+        if (!make_k8_map(cache, &mal, A_lo, rows, lda, lda, 128)) return cudaErrorInvalidValue;
         if (!make_chunk_map(cache, &w0h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
         if (!make_chunk_map(cache, &w0l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
         if (!make_chunk_map(cache, &w1h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
         if (!make_chunk_map(cache, &w1l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
-        back2_tc_kernel<<<grid, B2_THREADS, B2_SMEM, st>>>(ma, w0h, w0l, w1h, w1l, mo, q);
+        back2_tc_kernel<<<grid, BK_THREADS, B2_SMEM, st>>>(ma, mal, w0h, w0l, w1h, w1l, mo, q);
         return cudaGetLastError();
     }
     const int chalf = (q.BN / 32 + 1) / 2;   // each CTA of a cluster fetches (and multicasts) half of the W chunks

@@ -178,19 +178,17 @@ cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld,
     return cudaGetLastError();
 }
 
-// In place: x -> hi = x rounded to the nearest TF32 value, lo = x - hi (exact in FP32, so hi + lo restores
-// x bit for bit).
-__global__ void split_tf32_kernel(float *__restrict__ x, float *__restrict__ lo, size_t n) {
+// lo = x - trunc_tf32(x): what a kind::tf32 tensor-core operand drops of x (it ignores the 13 low mantissa bits).
+// Exact in FP32.  The back-application reads (x, lo) as the operand pair of 3xTF32; x itself stays as given.
+__global__ void tf32_remainder_kernel(const float *__restrict__ x, float *__restrict__ lo, size_t n) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const float v = x[i];
-        const float hi = tf32_hi(v);
-        x[i] = hi;
-        lo[i] = v - hi;
+        lo[i] = v - __uint_as_float(__float_as_uint(v) & 0xffffe000u);
     }
 }
-cudaError_t launch_split_tf32(cudaStream_t st, float *x, float *lo, size_t n, int *nlaunch) {
+cudaError_t launch_tf32_remainder(cudaStream_t st, const float *x, float *lo, size_t n, int *nlaunch) {
     ++*nlaunch;
-    split_tf32_kernel<<<2368, 256, 0, st>>>(x, lo, n);
+    tf32_remainder_kernel<<<2368, 256, 0, st>>>(x, lo, n);
     return cudaGetLastError();
 }
 

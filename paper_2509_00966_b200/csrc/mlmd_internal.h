@@ -25,7 +25,7 @@ struct StepCoef {
 static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
-    size_t psi, ua, ub, psi0, vloc, beta, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
+    size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
         nrm, nrm_part, scl, occ_eff, avec, gram, total;
 };
 
@@ -125,7 +125,8 @@ struct mlmd_domain {
     float2 *ub() const { return (float2 *)(ws + off.ub); }
     float2 *psi0() const { return (float2 *)(ws + off.psi0); }
     float *vloc() const { return (float *)(ws + off.vloc); }
-    float *beta() const { return (float *)(ws + off.beta); }
+    float *beta() const { return (float *)(ws + off.beta); }          // the projectors as given (FP32)
+    float *beta_lo() const { return (float *)(ws + off.beta_lo); }    // beta - trunc_tf32(beta), exact (back-application)
     float *dprime() const { return (float *)(ws + off.dprime); }
     float *occ() const { return (float *)(ws + off.occ); }
     float *rho() const { return (float *)(ws + off.rho); }
@@ -206,7 +207,8 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
                            int chain /* 16-row stages per TMEM accumulation chain, 0 = whole slice */, int *nlaunch,
                            TmapCache *cache = nullptr);
-cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A /* raw FP32 */, int lda, int P,
+cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A /* raw FP32 */,
+                           const float *A_lo /* A - trunc_tf32(A), or NULL: formed in shared memory */, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
                            int *nlaunch, TmapCache *cache = nullptr);
 
@@ -221,8 +223,8 @@ cudaError_t launch_density(cudaStream_t st, int ndom, long ngrid, int ld, const 
 // S4 epilogue: S[dom][m][n] = dv * (sum over splits of the complex combination of Z)
 cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld, int prows, int nsplit,
                                     const float *zpart, float dv, float2 *S, int *nlaunch);
-// in place x -> hi (TF32-representable part), lo = x - hi (exact in FP32)
-cudaError_t launch_split_tf32(cudaStream_t st, float *x, float *lo, size_t n, int *nlaunch);
+// lo = x - (x with the 13 low mantissa bits cleared): the part of x a kind::tf32 operand drops (exact in FP32); x is kept
+cudaError_t launch_tf32_remainder(cudaStream_t st, const float *x, float *lo, size_t n, int *nlaunch);
 cudaError_t launch_max_abs(cudaStream_t st, const float *x, size_t n, int *flag_bits, int *nlaunch);
 cudaError_t launch_check_finite(cudaStream_t st, const float *x, size_t n, int *flag, int *nlaunch);
 // graph support: *counter = value;  and  cur[d] = all[*counter * ndom + d], ++*counter

@@ -23,13 +23,13 @@ HOOK int mlmd_debug_proj(int path, void *stream, int ndom, long ngrid, const flo
     return (int)e;
 }
 
-// Y[dom][r][c] += sum_p A[dom][r][p] * (W_hi + W_lo)[dom][p][c]   (A: plain FP32, split by the kernel)
-HOOK int mlmd_debug_back(int path, void *stream, int ndom, long ngrid, const float *A, int lda, int P,
+// Y[dom][r][c] += sum_p A[dom][r][p] * (W_hi + W_lo)[dom][p][c]   (A: plain FP32; A_lo = A - trunc_tf32(A) or NULL)
+HOOK int mlmd_debug_back(int path, void *stream, int ndom, long ngrid, const float *A, const float *A_lo, int lda, int P,
                     const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod) {
     int nl = 0;
     cudaError_t e;
     if (path == 1)
-        e = launch_back_tc((cudaStream_t)stream, ndom, ngrid, A, lda, P, W_hi, W_lo, Y, ldy, N, prows, nprod, &nl);
+        e = launch_back_tc((cudaStream_t)stream, ndom, ngrid, A, A_lo, lda, P, W_hi, W_lo, Y, ldy, N, prows, nprod, &nl);
     else
         e = launch_back_simt((cudaStream_t)stream, ndom, ngrid, A, nullptr, lda, P, W_hi, W_lo, Y, ldy, N, prows, false, &nl);
     if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);

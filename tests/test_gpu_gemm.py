@@ -21,7 +21,7 @@ def L():
     lib = ctypes.CDLL(M.api.TEST_LIB_PATH)
     i, p, l = ctypes.c_int, ctypes.c_void_p, ctypes.c_long
     lib.mlmd_debug_proj.argtypes = [i, p, i, l, p, p, i, i, p, i, i, p, i, i, i, i]
-    lib.mlmd_debug_back.argtypes = [i, p, i, l, p, i, i, p, p, p, i, i, i, i]
+    lib.mlmd_debug_back.argtypes = [i, p, i, l, p, p, i, i, p, p, p, i, i, i, i]
     return lib
 
 
@@ -55,7 +55,9 @@ def run_proj(L, path, ndom, ngrid, P, N, nsplit, nprod, chain, positive=False, s
     return float((Z - ref).abs().max() / ref.abs().max())
 
 
-def run_back(L, path, ndom, ngrid, P, N, nprod):
+def run_back(L, path, ndom, ngrid, P, N, nprod, stored_remainder=True):
+    """stored_remainder: hand the kernel A - trunc_tf32(A) as its second operand stream (the product path: CTA-pair
+    kernel); False: the single-CTA kernel forms the operand pair in shared memory."""
     import torch
     g = torch.Generator(device="cuda").manual_seed(4321)
     lda = (P + 7) // 8 * 8
@@ -67,8 +69,9 @@ def run_back(L, path, ndom, ngrid, P, N, nprod):
     Y0 = torch.randn(ndom, ngrid, N, device="cuda", generator=g)
     Y = Y0.clone()
     Wh, Wl = hi_lo(W)
-    rc = L.mlmd_debug_back(path, None, ndom, ngrid, A.data_ptr(), lda, P, Wh.data_ptr(), Wl.data_ptr(),
-                           Y.data_ptr(), N, N, prows, nprod)
+    Al = hi_lo(A)[1]
+    rc = L.mlmd_debug_back(path, None, ndom, ngrid, A.data_ptr(), Al.data_ptr() if stored_remainder else None, lda, P,
+                           Wh.data_ptr(), Wl.data_ptr(), Y.data_ptr(), N, N, prows, nprod)
     assert rc == 0
     ref = Y0.double() + torch.einsum("drp,dpc->drc", A.double(), W[:, :lda].double())
     return float((Y.double() - ref).abs().max() / ref.abs().max())
@@ -105,6 +108,7 @@ def test_projection_low_precision_rungs(L, nprod, tol):
 @pytest.mark.parametrize("ndom,ngrid,P,N", SHAPES)
 def test_back_application(L, ndom, ngrid, P, N):
     assert run_back(L, 1, ndom, ngrid, P, N, 3) < 6e-6
+    assert run_back(L, 1, ndom, ngrid, P, N, 3, stored_remainder=False) < 6e-6
     assert run_back(L, 1, ndom, ngrid, P, N, 1) < 3e-3
     assert run_back(L, 1, ndom, ngrid, P, N, 0) < 2e-2
 
