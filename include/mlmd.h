@@ -91,7 +91,12 @@ enum {
     MLMD_OPT_GEMM_PATH = 2, /* 0 (default): tcgen05 kernels when ngrid is a multiple of 128; 1: CUDA-core kernels        */
     MLMD_OPT_KICK_NORM = 3, /* mlmd_propagate_split, norm after the second kick: 0 (default) from the projector Gram
                              * matrix when it applies; 1: always by a pass over psi                                   */
-    MLMD_OPT_COUNT = 4
+    MLMD_OPT_FD_ORDER = 4,  /* order of the central finite differences of the kinetic and A.grad terms: 4 (default; north_star:
+                             * 13-point star) or 2 (the paper's own "7-point star stencil" on "nearest-neighbor mesh points",
+                             * PAPER.md L147, L283): c2 = [1, -2, 1] / h^2, c1 = [-1/2, 0, 1/2] / h.
+                             * mlmd_propagate, mlmd_propagate_split and mlmd_current follow it; the stability bound of
+                             * mlmd_propagate becomes dt [ 2 sum_d 1/h_d^2 + sum_d |A_d|/h_d + ... ]                    */
+    MLMD_OPT_COUNT = 5
 };
 
 /* Bytes of device workspace mlmd_domain_create needs for this shape (0 on invalid arguments).
@@ -171,9 +176,19 @@ MLMD_API int mlmd_occupations(mlmd_domain_t *h, double *f, double *n_exc, int wh
  *   in Hartree (the projection GEMM of the step + a reduction); double [ndom] at `where`; 0 when nproj = 0.
  * mlmd_current: J[dom][d] = sum_n f_n Re<psi_n| -i D1_d + A_d |psi_n>, D1 the 4th-order first difference of H,
  *   A: double [a_ndom][3] HOST (a_ndom = 1 or ndom), J: double [ndom][3] at `where`.  This is the current of
- *   h_loc's velocity operator; the nonlocal-pseudopotential term -i[r, V_NL] is not included (D30). */
+ *   h_loc's velocity operator; the nonlocal-pseudopotential term -i[r, V_NL] is mlmd_current_nl. */
 MLMD_API int mlmd_energy_nl(mlmd_domain_t *h, double *E, int where);
 MLMD_API int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int where);
+
+/* Nonlocal (pseudopotential) part of the current, the term PAPER.md L201 says is GEMMified (reading D31):
+ *     J_nl[dom][d] = sum_n f_n <psi_n| -i [r_d, V_NL] |psi_n> = 2 dv^2 sum_n f_n sum_p D_p Im( conj(G_dpn) C_pn ),
+ *     C_pn = sum_r conj(beta_p(r)) psi_n(r),  G_dpn = sum_r conj(rbeta_dp(r)) psi_n(r),  rbeta_dp(r) = (r - R_p)_d beta_p(r)
+ * i.e. the projection GEMM of the step against beta and against the three caller-supplied arrays rbeta_d (the paper's
+ * atom positions R_p are the caller's; a constant shift of r commutes with V_NL, so any centre per projector gives the
+ * commutator with r itself).  rbeta: [3][ndom][ngrid][nproj], same dtype as the beta given to mlmd_set_projectors, at
+ * `where_rbeta`; it is staged through a Psi-sized work buffer one direction at a time (nothing is kept).
+ * J: double [ndom][3] at `where`.  The total TDCDFT current is mlmd_current + mlmd_current_nl.  0 when nproj = 0. */
+MLMD_API int mlmd_current_nl(mlmd_domain_t *h, const void *rbeta, int where_rbeta, double *J, int where);
 
 /* Per-kernel-class timing of mlmd_propagate with CUDA events on the handle's stream (bench.py's
  * roofline numbers).  mlmd_profile(h, 1) starts recording (and clears earlier records),

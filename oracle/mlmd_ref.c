@@ -384,7 +384,8 @@ int mlmd_ref_energy_nl(int ndom, long ngrid, int norb, int nproj, double dv, con
  *   J_d = sum_n f_n Re <psi_n| -i D1_d + A_d |psi_n>,   D1_d = the 4th-order central first difference of H.
  * A: [a_ndom][3]; J: [ndom][3]. */
 int mlmd_ref_current(int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int norb, const zc *psi,
-                     const double *occ, const double *A, int a_ndom, double *J) {
+                     const double *occ, const double *A, int a_ndom, double *J, int flags /* MLMD_REF_ORDER2: 2nd-order D1 */) {
+    const double *c1 = (flags & MLMD_REF_ORDER2) ? C1_O2 : C1;
     const int n3[3] = {nx, ny, nz};
     const double h[3] = {hx, hy, hz};
     const long ngrid = (long)nx * ny * nz;
@@ -408,7 +409,7 @@ int mlmd_ref_current(int ndom, int nx, int ny, int nz, double hx, double hy, dou
                                 int q3[3] = {i3[0], i3[1], i3[2]};
                                 q3[d] = wrap(i3[d] + j, n3[d]);
                                 const long rr = ((long)q3[0] * ny + q3[1]) * nz + q3[2];
-                                g += C1[j + 2] / h[d] * p[rr * norb + n];
+                                g += c1[j + 2] / h[d] * p[rr * norb + n];
                             }
                             const zc u = p[r * norb + n];
                             acc += occ[(size_t)dom * norb + n] * dv * creal(conj(u) * (-I * g + Av[d] * u));

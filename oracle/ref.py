@@ -42,7 +42,7 @@ def lib() -> ctypes.CDLL:
         _lib.mlmd_ref_occupations.restype = i
         _lib.mlmd_ref_energy_nl.argtypes = [i, l, i, i, d, p, p, p, p, p]
         _lib.mlmd_ref_energy_nl.restype = i
-        _lib.mlmd_ref_current.argtypes = [i, i, i, i, d, d, d, i, p, p, p, i, p]
+        _lib.mlmd_ref_current.argtypes = [i, i, i, i, d, d, d, i, p, p, p, i, p, i]
         _lib.mlmd_ref_current.restype = i
         _lib.mlmd_ref_current_nl.argtypes = [i, l, i, i, d, p, p, p, p, p, p]
         _lib.mlmd_ref_current_nl.restype = i
@@ -169,14 +169,14 @@ def energy_nl(psi, occ, beta, D, dv: float) -> np.ndarray:
     return E
 
 
-def current(psi, occ, A, h: Sequence[float]) -> np.ndarray:
-    """J[dom][d] = sum_n f_n Re<psi_n| -i D1_d + A_d |psi_n>; A: [a_ndom, 3]."""
+def current(psi, occ, A, h: Sequence[float], flags: int = 0) -> np.ndarray:
+    """J[dom][d] = sum_n f_n Re<psi_n| -i D1_d + A_d |psi_n>; A: [a_ndom, 3]; flags=ORDER2: the 2nd-order D1."""
     p = _c128(psi)
     ndom, nx, ny, nz, norb = p.shape
     A = _f64(A).reshape(-1, 3)
     assert A.shape[0] in (1, ndom)
     J = np.empty((ndom, 3), dtype=np.float64)
-    lib().mlmd_ref_current(ndom, nx, ny, nz, h[0], h[1], h[2], norb, _ptr(p), _ptr(_f64(occ)), _ptr(A), A.shape[0], _ptr(J))
+    lib().mlmd_ref_current(ndom, nx, ny, nz, h[0], h[1], h[2], norb, _ptr(p), _ptr(_f64(occ)), _ptr(A), A.shape[0], _ptr(J), flags)
     return J
 
 

@@ -21,12 +21,12 @@ HOST, DEVICE = 0, 1
 BETA_REAL32, BETA_COMPLEX64 = 0, 1
 GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT, GEMM_FP32GRADE_STAGED = range(6)
 KEEP_PSI0, CHECK_FINITE, BORROW_PSI = 1, 2, 4
-OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM = range(4)
+OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM, OPT_FD_ORDER = range(5)
 
 EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",
     "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_set_option", "mlmd_propagate",
-    "mlmd_propagate_split", "mlmd_occupations", "mlmd_energy_nl", "mlmd_current",
+    "mlmd_propagate_split", "mlmd_occupations", "mlmd_energy_nl", "mlmd_current", "mlmd_current_nl",
     "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
 ]
 K_STENCIL, K_PROJ, K_BACK, K_GLUE, K_DENSITY, K_NLP, K_NORM = range(7)
@@ -68,6 +68,7 @@ def lib() -> ctypes.CDLL:
         L.mlmd_occupations.argtypes = [p, p, p, i]
         L.mlmd_energy_nl.argtypes = [p, p, i]
         L.mlmd_current.argtypes = [p, p, i, p, i]
+        L.mlmd_current_nl.argtypes = [p, p, i, p, i]
         L.mlmd_profile.argtypes = [p, i]
         L.mlmd_profile_read.argtypes = [p, i, ctypes.POINTER(d), ctypes.POINTER(ctypes.c_longlong)]
         L.mlmd_launch_count.argtypes = [p]
@@ -226,6 +227,15 @@ def mlmd_current(h, A, J):
     return J
 
 
+def mlmd_current_nl(h, rbeta, J):
+    """rbeta: [3, ndom, ngrid, nproj] = (r - R_p)_d beta_p(r), dtype of the projectors (numpy host array or CUDA tensor);
+    J: [ndom, 3] float64 (numpy host array or CUDA tensor)."""
+    pr, wr = _ptr_where(rbeta)
+    p, where = _ptr_where(J, np.dtype(np.float64))
+    _check(lib().mlmd_current_nl(h, pr, wr, p, where))
+    return J
+
+
 def mlmd_profile(h, enable: bool):
     _check(lib().mlmd_profile(h, 1 if enable else 0))
 
@@ -322,6 +332,9 @@ class Domain:
 
     def current(self, A):
         return mlmd_current(self.handle, A, np.empty((self.ndom, 3), dtype=np.float64))
+
+    def current_nl(self, rbeta):
+        return mlmd_current_nl(self.handle, rbeta, np.empty((self.ndom, 3), dtype=np.float64))
 
     def profile(self, enable=True):
         mlmd_profile(self.handle, enable)

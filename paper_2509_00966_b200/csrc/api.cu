@@ -153,6 +153,7 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     h->gemm_mode = MLMD_GEMM_FP32GRADE;
     for (int k = 0; k < MLMD_OPT_COUNT; ++k) h->opt[k] = 0;
     h->opt[MLMD_OPT_GRAPH] = 1;
+    h->opt[MLMD_OPT_FD_ORDER] = 4;
     h->psi_ptr = (flags & MLMD_BORROW_PSI) ? nullptr : (float2 *)(h->ws + pl.off.psi);
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
@@ -371,9 +372,13 @@ int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
 
 int mlmd_set_option(mlmd_domain_t *h, int key, int value) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_option: NULL handle");
-    static const int nvalues[MLMD_OPT_COUNT] = {2, 3, 2, 2};
+    static const int nvalues[MLMD_OPT_COUNT] = {2, 3, 2, 2, 0};
     if (key < 0 || key >= MLMD_OPT_COUNT) return fail(MLMD_ERR_ARG, "mlmd_set_option: unknown key %d", key);
-    if (value < 0 || value >= nvalues[key]) return fail(MLMD_ERR_ARG, "mlmd_set_option: key %d takes 0..%d, got %d", key, nvalues[key] - 1, value);
+    if (key == MLMD_OPT_FD_ORDER) {
+        if (value != 2 && value != 4) return fail(MLMD_ERR_ARG, "mlmd_set_option: MLMD_OPT_FD_ORDER takes 2 or 4, got %d", value);
+    } else if (value < 0 || value >= nvalues[key]) {
+        return fail(MLMD_ERR_ARG, "mlmd_set_option: key %d takes 0..%d, got %d", key, nvalues[key] - 1, value);
+    }
     drop_graph(h);      // a captured step bakes the kernel choice in
     h->opt[key] = value;
     return MLMD_OK;
@@ -446,11 +451,69 @@ int mlmd_current(mlmd_domain_t *h, const double *A, int a_ndom, double *J, int w
     double *jd = where == MLMD_DEVICE ? J : h->nrm(3);
     int nl = 0;
     CU(launch_current(h->stream, h->ndom, h->nx, h->ny, h->nz, h->hx, h->hy, h->hz, h->ld, h->psi(), h->occ(), a_dev, a_ndom,
-                      h->nrm_part(), (size_t)h->ndom * kNormSlabs * h->ld, jd, &nl));
+                      h->nrm_part(), (size_t)h->ndom * kNormSlabs * h->ld, jd, h->opt[MLMD_OPT_FD_ORDER], &nl));
     h->launches += nl;
     if (where == MLMD_HOST) {
         CU(cudaMemcpyAsync(J, jd, (size_t)h->ndom * 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
         CU(cudaStreamSynchronize(h->stream));
+    }
+    return MLMD_OK;
+}
+
+int mlmd_current_nl(mlmd_domain_t *h, const void *rbeta, int where_rbeta, double *J, int where) {
+    if (!h || !J) return fail(MLMD_ERR_ARG, "mlmd_current_nl: NULL argument");
+    if (bad_where(where) || bad_where(where_rbeta)) return fail(MLMD_ERR_ARG, "mlmd_current_nl: bad where");
+    if (!h->have_psi) return fail(MLMD_ERR_STATE, "mlmd_current_nl: no orbitals set");
+    double *jd = where == MLMD_DEVICE ? J : h->nrm(3);
+    int nl = 0;
+    if (h->nproj == 0) {
+        CU(cudaMemsetAsync(jd, 0, (size_t)h->ndom * 3 * sizeof(double), h->stream));
+    } else {
+        if (!rbeta) return fail(MLMD_ERR_ARG, "mlmd_current_nl: rbeta is NULL");
+        // scratch for one direction of rbeta in the layout of beta: the two Horner work buffers (free between steps)
+        const size_t rows = (size_t)h->ndom * h->ngrid;
+        const size_t need = rows * h->ldp * sizeof(float) + 256, have = h->off.psi0 - h->off.ua;
+        // the complex coefficient matrices C, G live in the Z / W scratch ([ndom][nproj][ld] float2 each)
+        if (need > have || (size_t)h->nproj * h->ld * sizeof(float2) > (size_t)h->prows * 2 * h->ld * sizeof(float))
+            return fail(MLMD_ERR_SHAPE, "mlmd_current_nl: %d projector rows need %zu bytes of staging, the work buffers hold %zu",
+                        h->P, need, have);
+        float *stage = (float *)h->ua();
+        float2 *cmat = (float2 *)h->z(), *gmat = (float2 *)h->what();
+        const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
+        // always FP32-grade (3xTF32 on tensor cores, or the CUDA-core path): it is a measurement
+        const bool tc = h->tc_ok && h->opt[MLMD_OPT_GEMM_PATH] == 0 && h->gemm_mode != MLMD_GEMM_FP64 && h->gemm_mode != MLMD_GEMM_FP32_SIMT;
+        const int nsplit = tc ? h->nsplit_tc : h->nsplit;
+        auto project = [&](const float *B, float2 *out) -> int {
+            if (tc)
+                CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, B, nullptr, h->ldp, h->P, (const float *)h->psi(), 2 * h->ld, 2 * h->ld,
+                                  h->zpart(), h->prows, nsplit, 3, kProjChain, &nl, &h->tmaps));
+            else
+                CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, B, nullptr, h->ldp, h->P, (const float *)h->psi(), 2 * h->ld, 2 * h->ld,
+                                    h->zpart(), h->prows, nsplit, fp64, &nl));
+            CU(launch_proj_coeff(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, nsplit, h->zpart(), out, &nl));
+            return MLMD_OK;
+        };
+        int rc = project(h->beta(), cmat);
+        if (rc) return rc;
+        const size_t elem = h->beta_complex ? sizeof(float2) : sizeof(float);
+        for (int d = 0; d < 3; ++d) {
+            const char *src = (const char *)rbeta + (size_t)d * rows * h->nproj * elem;
+            if (h->ldp != h->P) CU(cudaMemsetAsync(stage, 0, rows * h->ldp * sizeof(float), h->stream));
+            CU(cudaMemcpy2DAsync(stage, (size_t)h->ldp * sizeof(float), src, (size_t)h->P * sizeof(float), (size_t)h->P * sizeof(float),
+                                 rows, kind_in(where_rbeta), h->stream));
+            rc = project(stage, gmat);
+            if (rc) return rc;
+            CU(launch_current_nl(h->stream, h->ndom, h->nproj, h->ld, cmat, gmat, h->dprime(), h->occ(), h->dv, d, jd, &nl));
+        }
+        // the W scratch held G: rows of W beyond the projector count must be zero again for the back-application
+        CU(cudaMemsetAsync(h->what(), 0, 2 * (h->off.what_lo - h->off.what), h->stream));
+    }
+    h->launches += nl;
+    if (where == MLMD_HOST) {
+        CU(cudaMemcpyAsync(J, jd, (size_t)h->ndom * 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    } else if (where_rbeta == MLMD_HOST) {
+        CU(cudaStreamSynchronize(h->stream));   // the caller may reuse its host rbeta
     }
     return MLMD_OK;
 }
@@ -478,13 +541,17 @@ struct ProfScope {
 };
 
 static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
-    // SURVEY.md 8(a) S1; weights of the 4th-order central differences (north_star)
-    static const double c2[2] = {4.0 / 3.0, -1.0 / 12.0};   // j = 1, 2  (symmetric)
-    static const double c1[2] = {2.0 / 3.0, -1.0 / 12.0};   // j = +1, +2 (antisymmetric)
+    // SURVEY.md 8(a) S1; weights of the 4th-order central differences (north_star), or of the paper's own 2nd-order
+    // 7-point star (MLMD_OPT_FD_ORDER = 2) written on the same offsets with zero j = 2 weights
+    static const double c2_o4[2] = {4.0 / 3.0, -1.0 / 12.0}, c1_o4[2] = {2.0 / 3.0, -1.0 / 12.0};   // j = 1, 2
+    static const double c2_o2[2] = {1.0, 0.0}, c1_o2[2] = {0.5, 0.0};
+    const bool o2 = h->opt[MLMD_OPT_FD_ORDER] == 2;
+    const double *c2 = o2 ? c2_o2 : c2_o4, *c1 = o2 ? c1_o2 : c1_o4;
+    const double c2_0 = o2 ? -2.0 : -5.0 / 2.0;
     const double hh[3] = {h->hx, h->hy, h->hz};
     double centre = 0.5 * (A3[0] * A3[0] + A3[1] * A3[1] + A3[2] * A3[2]);
     for (int d = 0; d < 3; ++d) {
-        centre += -0.5 * (-5.0 / 2.0) / (hh[d] * hh[d]);
+        centre += -0.5 * c2_0 / (hh[d] * hh[d]);
         for (int j = 0; j < 2; ++j) {
             c->p[d][j] = (float)(-0.5 * c2[j] / (hh[d] * hh[d]));
             c->q[d][j] = (float)(A3[d] * c1[j] / hh[d]);
@@ -708,8 +775,10 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
         if (!std::isfinite(a[0]) || !std::isfinite(a[1]) || !std::isfinite(a[2]))
             return fail(MLMD_ERR_NONFINITE, "%s: A[%zu] is not finite", fn, i);
         yz = yz || a[1] != 0.0 || a[2] != 0.0;
-        const double b = (8.0 / 3.0) * (1 / (h->hx * h->hx) + 1 / (h->hy * h->hy) + 1 / (h->hz * h->hz)) +
-                         1.3722 * (fabs(a[0]) / h->hx + fabs(a[1]) / h->hy + fabs(a[2]) / h->hz) +
+        // maxima of the D2 / D1 symbols: 16/3 and 1.3722 (4th order), 4 and 1 (2nd order)
+        const bool o2 = h->opt[MLMD_OPT_FD_ORDER] == 2;
+        const double b = (o2 ? 2.0 : 8.0 / 3.0) * (1 / (h->hx * h->hx) + 1 / (h->hy * h->hy) + 1 / (h->hz * h->hz)) +
+                         (o2 ? 1.0 : 1.3722) * (fabs(a[0]) / h->hx + fabs(a[1]) / h->hy + fabs(a[2]) / h->hz) +
                          0.5 * (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) + h->vmax + (h->nproj && !split ? h->dmax : 0.0);
         bound = std::max(bound, b);
     }

@@ -450,6 +450,69 @@ cudaError_t launch_energy_nl(cudaStream_t st, int ndom, int nproj, int beta_comp
     return cudaGetLastError();
 }
 
+// ---- nonlocal part of the current (mlmd_current_nl, reading D31) ----
+// cmat[dom][p][n] = complex projection coefficient C_pn summed over the split-K slices in index order (real beta: row p
+// holds (Re, Im) pairs; complex beta: rows 2p, 2p+1 combine as in reduce_scale_kernel).
+__global__ void proj_coeff_kernel(int nproj, int beta_complex, int ld, int prows, int nsplit, const float *__restrict__ zpart,
+                                  float2 *__restrict__ cmat) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = blockIdx.y, dom = blockIdx.z;
+    if (n >= ld) return;
+    const int N = 2 * ld;
+    const float *zp = zpart + (size_t)dom * nsplit * prows * N;
+    const size_t slice = (size_t)prows * N;
+    float cre = 0.f, cim = 0.f;
+    for (int s = 0; s < nsplit; ++s) {
+        if (!beta_complex) {
+            const float2 v = *(const float2 *)(zp + s * slice + (size_t)p * N + 2 * n);
+            cre += v.x;
+            cim += v.y;
+        } else {
+            const float2 a = *(const float2 *)(zp + s * slice + (size_t)(2 * p) * N + 2 * n);
+            const float2 b = *(const float2 *)(zp + s * slice + (size_t)(2 * p + 1) * N + 2 * n);
+            cre += a.x + b.y;
+            cim += a.y - b.x;
+        }
+    }
+    cmat[((size_t)dom * nproj + p) * ld + n] = make_float2(cre, cim);
+}
+cudaError_t launch_proj_coeff(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows, int nsplit,
+                              const float *zpart, float2 *cmat, int *nlaunch) {
+    dim3 grid((ld + 127) / 128, nproj, ndom);
+    ++*nlaunch;
+    proj_coeff_kernel<<<grid, 128, 0, st>>>(nproj, beta_complex, ld, prows, nsplit, zpart, cmat);
+    return cudaGetLastError();
+}
+// J[dom][d] = 2 dv sum_n f_n sum_p D'_p Im( conj(G_pn) C_pn ),  D' = D dv;  one block per domain, FP64 sums in a fixed order
+__global__ void __launch_bounds__(256)
+current_nl_kernel(int nproj, int ld, const float2 *__restrict__ cmat, const float2 *__restrict__ gmat,
+                  const float *__restrict__ dprime, const float *__restrict__ occ, double dv, int d, double *__restrict__ J) {
+    const int dom = blockIdx.x;
+    double acc = 0.0;
+    for (int n = threadIdx.x; n < ld; n += blockDim.x) {
+        double an = 0.0;
+        for (int p = 0; p < nproj; ++p) {
+            const float2 c = cmat[((size_t)dom * nproj + p) * ld + n], g = gmat[((size_t)dom * nproj + p) * ld + n];
+            an += (double)dprime[(size_t)dom * nproj + p] * ((double)g.x * c.y - (double)g.y * c.x);
+        }
+        acc += (double)occ[(size_t)dom * ld + n] * an;
+    }
+    __shared__ double red[256];
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) J[(size_t)dom * 3 + d] = 2.0 * dv * red[0];
+}
+cudaError_t launch_current_nl(cudaStream_t st, int ndom, int nproj, int ld, const float2 *cmat, const float2 *gmat,
+                              const float *dprime, const float *occ, double dv, int d, double *J, int *nlaunch) {
+    ++*nlaunch;
+    current_nl_kernel<<<ndom, 256, 0, st>>>(nproj, ld, cmat, gmat, dprime, occ, dv, d, J);
+    return cudaGetLastError();
+}
+
 // Local current: part[dom][blk][0..2] = sum over the block's points and all orbitals of
 //   f_n * 2 * sum_{j=1,2} c1_j / h_d * Im( conj(psi(r)) psi(r + j e_d) )      (= f_n Im<psi|D1_d psi> restricted to r;
 //   the -j taps are the +j taps of the shifted sum, so only forward neighbours are read)
@@ -591,12 +654,12 @@ __global__ void current_final_kernel(int ndom, int nblk, int a_ndom, double dv, 
 }
 cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int ld,
                            const float2 *psi, const float *occ, const double *A_dev, int a_ndom, double *part,
-                           size_t part_doubles, double *J, int *nlaunch) {
+                           size_t part_doubles, double *J, int fd_order, int *nlaunch) {
     const long ngrid = (long)nx * ny * nz;
     const long max_blk = (long)(part_doubles / 4 / ndom);
     if (max_blk < 1) return cudaErrorInvalidValue;
-    // 2 c1_j / h_d with c1 = (2/3, -1/12): weights of the 4th-order first difference (north_star)
-    const float w1 = (float)(2.0 * 2.0 / 3.0), w2 = (float)(2.0 * -1.0 / 12.0);
+    // 2 c1_j / h_d: c1 = (2/3, -1/12), the 4th-order first difference (north_star), or (1/2, 0), the 2nd-order one
+    const float w1 = fd_order == 2 ? 1.0f : (float)(2.0 * 2.0 / 3.0), w2 = fd_order == 2 ? 0.f : (float)(2.0 * -1.0 / 12.0);
     if (ny % 8 == 0 && nz % 8 == 0) {
         const long tiles = (long)(ld / 8) * (ny / 8) * (nz / 8);
         int nxseg = 1;

@@ -180,6 +180,7 @@ bool stencil_tma_supported(const mlmd_domain *h);
 // value through the constant bank), NULL when coef[dom] differs per domain.
 cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const float2 *psi, float2 *out, const StepCoef *coef,
                                const StepCoef *coef_host, float tau, int *nlaunch, int norm_mode = 0, double *npart = nullptr);
+// (with MLMD_OPT_FD_ORDER = 2 it runs its radius-1 instantiation: same staging, the j = 2 taps neither loaded nor multiplied)
 // norm_mode 1 / 2: the pass also writes per-CTA partial sums of |w|^2 / |out|^2 per orbital into
 // npart[dom][slot][ld], slot < stencil_tma_norm_slots(h) (split step, reading D27)
 int stencil_tma_norm_slots(const mlmd_domain *h);
@@ -243,7 +244,13 @@ cudaError_t launch_energy_nl(cudaStream_t st, int ndom, int nproj, int beta_comp
                              const float *zpart, const float *dprime, const float *occ, double dv, double *E, int *nlaunch);
 cudaError_t launch_current(cudaStream_t st, int ndom, int nx, int ny, int nz, double hx, double hy, double hz, int ld,
                            const float2 *psi, const float *occ, const double *A_dev, int a_ndom, double *part,
-                           size_t part_doubles, double *J, int *nlaunch);
+                           size_t part_doubles, double *J, int fd_order, int *nlaunch);
+// nonlocal part of the current (reading D31): complex projection coefficients from the split-K partials, then
+// J[dom][d] = 2 dv sum_n f_n sum_p D'_p Im(conj(G_pn) C_pn)
+cudaError_t launch_proj_coeff(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows, int nsplit,
+                              const float *zpart, float2 *cmat, int *nlaunch);
+cudaError_t launch_current_nl(cudaStream_t st, int ndom, int nproj, int ld, const float2 *cmat, const float2 *gmat,
+                              const float *dprime, const float *occ, double dv, int d, double *J, int *nlaunch);
 cudaError_t launch_gram_reduce(cudaStream_t st, int ndom, int P, int ldg, int prows, int N, int nsplit, const float *zpart,
                                float *G, int accumulate, int *nlaunch);
 cudaError_t launch_kick_quad(cudaStream_t st, int ndom, int P, int ldg, int ld, int prows, const float *G, const float *what,

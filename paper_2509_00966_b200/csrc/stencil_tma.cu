@@ -84,7 +84,10 @@ __device__ __forceinline__ void pair_acc_real(float4 &acc, const float4 a, const
 
 // NORM (split step, reading D27): 1 = also sum |w|^2 of the CTA's own points per orbital, 2 = |out|^2;
 // one partial sum per (CTA, orbital), reduced in a fixed order, so the norms are reproducible.
-template <bool AYZ, bool PERDOM, int NORM>
+// R1: radius-1 instantiation for the paper's own 2nd-order / 7-point stencil (MLMD_OPT_FD_ORDER = 2;
+// SURVEY.md 8(f) NEXT-3): same staging and march, but the j = 2 taps are neither read from shared memory nor
+// multiplied (their coefficients are zero): 8 instead of 16 shared-memory loads per plane and thread.
+template <bool AYZ, bool PERDOM, int NORM, bool R1>
 __global__ void __launch_bounds__(S_THREADS, 1)
 stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_z,
                    const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_p,
@@ -211,19 +214,25 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         A2.z = fmaf(cen, u.z, A2.z);
         A2.w = fmaf(cen, u.w, A2.w);
         if (AYZ) pair_acc(A2, yp1, ym1, c.p[1][0], c.q[1][0]); else pair_acc_real(A2, yp1, ym1, c.p[1][0]);
-        if (AYZ) pair_acc(A2, yp2, ym2, c.p[1][1], c.q[1][1]); else pair_acc_real(A2, yp2, ym2, c.p[1][1]);
+        if (!R1) {
+            if (AYZ) pair_acc(A2, yp2, ym2, c.p[1][1], c.q[1][1]); else pair_acc_real(A2, yp2, ym2, c.p[1][1]);
+        }
         {
             const float4 p1 = lds4(buf + zp1), m1 = lds4(buf + zm1);
             if (AYZ) pair_acc(A2, p1, m1, c.p[2][0], c.q[2][0]); else pair_acc_real(A2, p1, m1, c.p[2][0]);
-            const float4 p2 = lds4(buf + zp2), m2 = lds4(buf + zm2);
-            if (AYZ) pair_acc(A2, p2, m2, c.p[2][1], c.q[2][1]); else pair_acc_real(A2, p2, m2, c.p[2][1]);
+            if (!R1) {
+                const float4 p2 = lds4(buf + zp2), m2 = lds4(buf + zm2);
+                if (AYZ) pair_acc(A2, p2, m2, c.p[2][1], c.q[2][1]); else pair_acc_real(A2, p2, m2, c.p[2][1]);
+            }
         }
         // x taps: u = w(plane q) is the +j neighbour of plane q-j (coefficient p_j - i q_j) and the -j
         // neighbour of plane q+j (coefficient p_j + i q_j)
         cmul_acc(A1, u, c.p[0][0], -c.q[0][0]);
         cmul_acc(A3, u, c.p[0][0], c.q[0][0]);
-        cmul_acc(A0, u, c.p[0][1], -c.q[0][1]);
-        cmul_acc(A4, u, c.p[0][1], c.q[0][1]);
+        if (!R1) {
+            cmul_acc(A0, u, c.p[0][1], -c.q[0][1]);
+            cmul_acc(A4, u, c.p[0][1], c.q[0][1]);
+        }
     };
     // One plane step.  A0..A4 / B0..B4 are the accumulators of planes q-2..q+2; the caller rotates the
     // names, so the ring costs no register moves.
@@ -247,8 +256,8 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         const uint32_t buf = sbase + k * S_PLANE;
         const bool own_plane = n >= 2 && n < nplanes - 2;
         {
-            const float4 rm2 = lds4(buf + oym2), rm1 = lds4(buf + oym1), r0 = lds4(buf + own), r1 = lds4(buf + own + 1024),
-                         r2 = lds4(buf + oyp2), r3 = lds4(buf + oyp3);
+            const float4 rm1 = lds4(buf + oym1), r0 = lds4(buf + own), r1 = lds4(buf + own + 1024), r2 = lds4(buf + oyp2);
+            const float4 rm2 = R1 ? zero4 : lds4(buf + oym2), r3 = R1 ? zero4 : lds4(buf + oyp3);
             point(buf, r0, r1, rm1, r2, rm2, ozm1, ozm2, ozp1, ozp2, c.centre + vA, own_plane, A0, A1, A2, A3, A4);
             point(buf, r1, r2, r0, r3, rm1, ozm1 + dzm1, ozm2 + dzm, ozp1 + dzp1, ozp2 + dzp, c.centre + vB, own_plane, B0, B1, B2,
                   B3, B4);
@@ -345,23 +354,23 @@ bool stencil_tma_supported(const mlmd_domain *h) {
 }
 
 namespace {
-template <int NORM>
+template <int NORM, bool R1>
 cudaError_t set_attrs() {
-    cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true, NORM>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
     return e;
 }
-template <int NORM>
+template <int NORM, bool R1>
 void launch_variant(bool yz, bool perdom, unsigned g, cudaStream_t st, const CUtensorMap &mc, const CUtensorMap &mz,
                     const CUtensorMap &my, const CUtensorMap &mp, const TmaStencilParams &P) {
     if (!perdom) {
-        if (yz) stencil_tma_kernel<true, false, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
-        else stencil_tma_kernel<false, false, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        if (yz) stencil_tma_kernel<true, false, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, false, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
     } else {
-        if (yz) stencil_tma_kernel<true, true, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
-        else stencil_tma_kernel<false, true, NORM><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        if (yz) stencil_tma_kernel<true, true, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, true, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
     }
 }
 }  // namespace
@@ -384,9 +393,12 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
                                const StepCoef *coef_host, float tau, int *nlaunch, int norm_mode, double *npart) {
     static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
     if (!attr_set.done()) {
-        cudaError_t e = set_attrs<0>();
-        if (e == cudaSuccess) e = set_attrs<1>();
-        if (e == cudaSuccess) e = set_attrs<2>();
+        cudaError_t e = set_attrs<0, false>();
+        if (e == cudaSuccess) e = set_attrs<1, false>();
+        if (e == cudaSuccess) e = set_attrs<2, false>();
+        if (e == cudaSuccess) e = set_attrs<0, true>();
+        if (e == cudaSuccess) e = set_attrs<1, true>();
+        if (e == cudaSuccess) e = set_attrs<2, true>();
         if (e != cudaSuccess) return e;
         attr_set.mark();
     }
@@ -422,9 +434,13 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
     ++*nlaunch;
     const unsigned g = (unsigned)grid;
     P.cval = coef_host ? *coef_host : StepCoef();
-    if (norm_mode == 1) launch_variant<1>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
-    else if (norm_mode == 2) launch_variant<2>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
-    else launch_variant<0>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    const bool r1 = h->opt[MLMD_OPT_FD_ORDER] == 2;
+    if (norm_mode == 1) r1 ? launch_variant<1, true>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
+                           : launch_variant<1, false>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    else if (norm_mode == 2) r1 ? launch_variant<2, true>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
+                                : launch_variant<2, false>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    else r1 ? launch_variant<0, true>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
+            : launch_variant<0, false>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
     return cudaGetLastError();
 }
 

@@ -102,6 +102,24 @@ def test_o2d_second_order_convergence_and_polynomial_exactness():
     assert np.abs(out[2:-2] - want[2:-2]).max() < 1e-11       # away from the periodic seam
 
 
+def test_o2e_plane_waves_carry_the_second_order_velocity():
+    """The local current with the 2nd-order first difference: D1 e^{ikx} = i sin(k h)/h e^{ikx}."""
+    grid, h = (12, 10, 16), (0.5, 0.45, 0.4)
+    box = [n * s for n, s in zip(grid, h)]
+    ax = [np.arange(n) * s for n, s in zip(grid, h)]
+    X, Y, Z = np.meshgrid(*ax, indexing="ij")
+    ms = [(1, 0, 0), (0, -2, 0), (2, -1, 4), (-5, 3, -7)]
+    f = np.array([[2.0, 1.0, 0.5, 1.5]])
+    A = np.array([[0.07, -0.04, 0.11]])
+    psi = np.zeros((1, *grid, len(ms)), dtype=np.complex128)
+    want = np.zeros(3)
+    for n, m in enumerate(ms):
+        k = [2 * np.pi * mi / b for mi, b in zip(m, box)]
+        psi[0, ..., n] = np.exp(1j * (k[0] * X + k[1] * Y + k[2] * Z)) / np.sqrt(np.prod(box))
+        want += f[0, n] * (np.array([np.sin(k[d] * h[d]) / h[d] for d in range(3)]) + A[0])
+    assert np.abs(ref.current(psi, f, A, h, flags=ref.ORDER2)[0] - want).max() < 1e-12
+
+
 # ---- NEXT-2: nonlocal part of the current --------------------------------------------------------------------
 def test_c1_dense_commutator_any_diagonal_position_operator():
     """<psi| -i [X_d, V_NL] |psi> with V_NL = dv B D B^H as a dense matrix and X_d ANY real diagonal matrix; the
