@@ -561,7 +561,15 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
     c->pad = 0.f;
 }
 
-static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl, int nprod = -1, int chain = -1) {
+// The step's first projection reads every psi row exactly once: on the CTA-pair kernel it can carry the density of
+// that state (S3) in its converter warps, so the separate 8 B/element pass over psi runs only once per call.
+static bool density_rides_on_projection(const mlmd_domain *h) {
+    return h->nproj > 0 && use_tensor_cores(h) && h->gemm_mode == MLMD_GEMM_FP32GRADE &&
+           proj_tc_can_fuse_density(h->P, 2 * h->ld, 3);
+}
+
+static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl, int nprod = -1, int chain = -1,
+                            bool with_density = false) {
     // S2a + S2b: What = (-i tau) D' (beta^H w); nprod >= 0 overrides the mode's products per MAC (staged mode)
     if (nprod < 0) nprod = tc_nprod(h);
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
@@ -571,7 +579,8 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl,
         ProfScope ps(h, MLMD_K_PROJ);
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
-                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, chain > 0 ? chain : proj_chain(nprod), nl, &h->tmaps));
+                              2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, chain > 0 ? chain : proj_chain(nprod), nl, &h->tmaps,
+                              with_density ? h->rho() : nullptr, h->occ()));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
@@ -598,7 +607,11 @@ static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl, int nprod = -1) {
 // One Taylor-4 time step on h->stream: four Horner stages (projection, glue, fused stencil pass,
 // back-application) and the density.  coef: this step's device coefficients [ndom];
 // coef_host: the same set on the host when it is identical for all domains (constant-bank path), else NULL.
-static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, int *nl) {
+// last: the final step of a call.  Every step ends with rho of its result (north_star); when the density can ride on a
+// projection, the rho of step n is formed by the FIRST projection of step n + 1 (which reads that state anyway) and
+// only the last step of a call runs the separate density pass.
+static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *coef_host, double dt, bool last, int *nl) {
+    const bool fused_rho = density_rides_on_projection(h);
     // Horner form of sum_{m<=4} (-i dt H)^m/m!: w4 = psi, w_{k-1} = psi + (-i dt/k) H w_k
     const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
     float2 *dst[4] = {h->ua(), h->ub(), h->ua(), h->psi()};
@@ -614,7 +627,8 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
             // inner stages: their accumulation drift is damped like every other projection error (weights <= dt/2 E
             // ~ 0.05 of the outer stage's), so the chains are 1024 stages: one or two drains per K slice instead of one per 128 stages
             // the three inner stages of every tensor-core mode take the long chains (the products stay as the mode says)
-            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? kStagedProjNprod : -1, i < 3 ? kInnerChain : -1);
+            int rc = nonlocal_project(h, src[i], tau, nl, reduced ? kStagedProjNprod : -1, i < 3 ? kInnerChain : -1,
+                                      fused_rho && i == 0);
             if (rc) return rc;
         }
         {
@@ -626,6 +640,7 @@ static int enqueue_step(mlmd_domain *h, const StepCoef *coef, const StepCoef *co
             if (rc) return rc;
         }
     }
+    if (fused_rho && !last) return MLMD_OK;
     ProfScope ps(h, MLMD_K_DENSITY);
     CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), nl));
     return MLMD_OK;
@@ -647,7 +662,7 @@ static int capture_step(mlmd_domain *h, double dt, bool yz, bool split) {
     h->stream = h->gstream;
     cudaError_t e = launch_advance_coef(h->gstream, h->coef(), h->coef_cur(), h->step_counter(), h->ndom, &nl);
     int rc = e != cudaSuccess ? MLMD_ERR_CUDA
-             : split ? enqueue_split_step(h, h->coef_cur(), nullptr, dt, false, &nl) : enqueue_step(h, h->coef_cur(), nullptr, dt, &nl);
+             : split ? enqueue_split_step(h, h->coef_cur(), nullptr, dt, false, &nl) : enqueue_step(h, h->coef_cur(), nullptr, dt, false, &nl);
     h->stream = user;
     cudaError_t e2 = cudaStreamEndCapture(h->gstream, &graph);
     if (rc || e != cudaSuccess || e2 != cudaSuccess || !graph) {
@@ -784,13 +799,14 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
     }
     h->field_yz = yz;
     int nl = 0;
+    bool rho_flush = false;
     // Small problems are launch-bound (17 launches per step): after one eager step the step is captured
     // into a CUDA graph that reads its stencil coefficients from a device slot.
     const bool want_graph = h->graph_allowed && h->opt[MLMD_OPT_GRAPH] && !h->prof_on && nsteps >= 4 &&
                             (double)h->ndom * (double)h->ngrid * h->ld <= (double)(1 << 23);
     if (h->gexec && (h->g_dt != dt || h->g_yz != yz || h->g_split != split)) drop_graph(h);
     auto one_step = [&](const StepCoef *coef, const StepCoef *coef_host, bool last) {
-        return split ? enqueue_split_step(h, coef, coef_host, dt, last, &nl) : enqueue_step(h, coef, coef_host, dt, &nl);
+        return split ? enqueue_split_step(h, coef, coef_host, dt, last, &nl) : enqueue_step(h, coef, coef_host, dt, last, &nl);
     };
     {
         int rc = flush_split_scale(h, &nl);      // only after a split call that failed half-way
@@ -841,6 +857,8 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
                 CU(cudaEventRecord(h->gjoin, h->gstream));
                 CU(cudaStreamWaitEvent(h->stream, h->gjoin, 0));
                 if (split && h->nproj > 0) h->split_pending = true;   // every replayed split step defers its scale
+                // a replayed Taylor step leaves its rho to the next step's first projection: the call's last step has none
+                if (!split && s0 + ns == nsteps && density_rides_on_projection(h)) rho_flush = true;
             }
         }
         for (; s < ns; ++s) {
@@ -852,6 +870,10 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
     {
         int rc = flush_split_scale(h, &nl);      // graph replays end on a deferred scale
         if (rc) return rc;
+    }
+    if (rho_flush) {
+        ProfScope ps(h, MLMD_K_DENSITY);
+        CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ(), h->rho(), &nl));
     }
     h->launches += nl;
     if (nsteps > 0) h->rho_valid = true;

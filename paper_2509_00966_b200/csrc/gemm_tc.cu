@@ -185,6 +185,10 @@ constexpr int PJ_THREADS = 192;          // warp 0 TMA, warp 1 MMA, warps 2-5 co
 struct ProjParams {
     int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, chain, lowp, rn;
     float *zpart;
+    // fused density (S3 riding on the step's first projection): rho[dom][r] += sum_n occ[dom][n] |Y[r][n]|^2 over this
+    // CTA's columns of the psi tile it holds anyway; NULL = off
+    float *rho;
+    const float *occ;
 };
 
 // LO = true: stages hold hi and lo tiles of both operands (3xTF32), 3 stages; LO = false (one product per MAC):
@@ -609,6 +613,30 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                     } else {
                         // elementwise on the swizzled image: the lo tile has the same layout as the hi tile
                         float4 *yl = (float4 *)(st + YOFF + P2_Y_BYTES);
+                        if (q.rho) {
+                            // S3 fused: thread t always holds row (t >> 3) & 15 of every chunk (a chunk = 16 rows x 8 units of
+                            // 16 B) and, undoing the 32-byte-atom swizzle (atom index ^ row & 3), the same pair of orbitals
+                            // inside each chunk; the 8 threads of a row are neighbouring lanes.  One FP32 sum per (CTA, row),
+                            // added to rho by ONE atomic: two addends per row (the pair's two column halves), so the result
+                            // does not depend on their order (reading D22).
+                            const int r = (t >> 3) & 15, w = t & 7;
+                            const int pair_in_chunk = (((w >> 1) ^ (r & 3)) << 1) | (w & 1);
+                            const float2 *f2 = (const float2 *)(q.occ + (size_t)dom * (q.N / 2));
+                            float acc = 0.f;
+                            int j = 0;
+                            for (int i = t; i < ny4; i += 128, ++j) {
+                                float4 v = y4[i];
+                                const int gch = j < h0 ? nt * (q.BN / 32) + crank * h0 + j : nt * (q.BN / 32) + n0 / 32 + crank * h1 + (j - h0);
+                                const float2 ff = __ldg(f2 + gch * 8 + pair_in_chunk);
+                                acc = fmaf(ff.x, fmaf(v.x, v.x, v.y * v.y), acc);
+                                acc = fmaf(ff.y, fmaf(v.z, v.z, v.w * v.w), acc);
+                                yl[i] = split4(v);
+                            }
+                            acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+                            acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+                            acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+                            if (w == 0) atomicAdd(q.rho + (size_t)dom * q.ngrid + (size_t)kb * PJ_BK + r, acc);
+                        } else
                         for (int i = t; i < ny4; i += 128) {
                             float4 v = y4[i];
                             yl[i] = split4(v);   // the hi tile stays as loaded: kind::tf32 ignores the 13 low bits
@@ -1030,9 +1058,14 @@ int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
     return best;
 }
 
+bool proj_tc_can_fuse_density(int P, int N, int nprod) {
+    // one pair of CTAs sees every psi row exactly once, each CTA half of its columns: two addends per rho element
+    return nprod == 3 && N % 64 == 0 && N <= BK_MAXBN && P <= 256;
+}
+
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
-                           int chain, int *nlaunch, TmapCache *cache) {
+                           int chain, int *nlaunch, TmapCache *cache, float *rho, const float *occ) {
     static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
     if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
@@ -1057,6 +1090,14 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.lowp = nprod == 0 ? 1 : 0;     // nprod 0 = one product of BF16-rounded operands
     q.rn = nprod == 4 ? 1 : 0;       // nprod 4 = one product, psi rounded to the nearest TF32 in shared memory
     if (q.lowp || q.rn) q.nprod = 1;
+    q.rho = nullptr;
+    q.occ = occ;
+    if (rho) {
+        if (!(A_lo == nullptr && proj_tc_can_fuse_density(P, N, nprod)) || ldy != N) return cudaErrorInvalidValue;
+        cudaError_t e = cudaMemsetAsync(rho, 0, (size_t)ndom * ngrid * sizeof(float), st);
+        if (e != cudaSuccess) return e;
+        q.rho = rho;
+    }
     const uint64_t rows = (uint64_t)ndom * ngrid;
     CUtensorMap mz;
     if (!make_out_map(cache, &mz, zpart, (uint64_t)ndom * nsplit * prows, N, N)) return cudaErrorInvalidValue;

@@ -207,7 +207,11 @@ int tc_choose_nsplit(int ndom, long ngrid, int P, int N);
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
                            int chain /* 16-row stages per TMEM accumulation chain, 0 = whole slice */, int *nlaunch,
-                           TmapCache *cache = nullptr);
+                           TmapCache *cache = nullptr,
+                           float *rho = nullptr /* != NULL: also rho[dom][r] = sum_n occ[dom][n] |Y[r][n]|^2 (S3 fused) */,
+                           const float *occ = nullptr);
+// whether that projection can carry the density (CTA-pair kernel, one row tile of projectors, one column tile)
+bool proj_tc_can_fuse_density(int P, int N, int nprod);
 cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A /* raw FP32 */,
                            const float *A_lo /* A - trunc_tf32(A), or NULL: formed in shared memory */, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,

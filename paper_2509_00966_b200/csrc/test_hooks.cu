@@ -36,6 +36,22 @@ HOOK int mlmd_debug_back(int path, void *stream, int ndom, long ngrid, const flo
     return (int)e;
 }
 
+// The density formed inside the step's first projection (S3 riding on S2a) is overwritten by the separate pass at the
+// end of every call, so it cannot be seen through the C ABI: this hook runs that projection on the handle's current
+// psi and copies the rho it formed to rho_dev [ndom][ngrid] (device).  Returns a cudaError_t value, -1 if the shape
+// cannot carry the density.
+HOOK int mlmd_debug_fused_density(mlmd_domain_t *h, float *rho_dev) {
+    if (!h->tc_ok || !proj_tc_can_fuse_density(h->P, 2 * h->ld, 3) || h->nproj == 0) return -1;
+    int nl = 0;
+    cudaError_t e = launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)h->psi(), 2 * h->ld,
+                                   2 * h->ld, h->zpart(), h->prows, h->nsplit_tc, 3, 128, &nl, nullptr, h->rho(), h->occ());
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(rho_dev, h->rho(), (size_t)h->ndom * h->ngrid * sizeof(float), cudaMemcpyDeviceToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    h->rho_valid = false;
+    return (int)e;
+}
+
 HOOK int mlmd_debug_nsplit(int ndom, long ngrid, int P, int N) { return tc_choose_nsplit(ndom, ngrid, P, N); }
 
 }  // extern "C"

@@ -317,6 +317,48 @@ def test_projector_capacity_counts_real_rows_and_options_are_checked():
     dom.close()
 
 
+def test_density_riding_on_the_first_projection_random_occupations():
+    """On the CTA-pair projection the density of a step is formed by the next step's first projection (per-orbital
+    occupations looked up through the swizzled tile layout) and by the separate pass only at the end of a call:
+    random occupations, several steps in one call and step by step, CUDA graph on and off, against the oracle and
+    against each other."""
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    c = W.get_config(1, nsteps=6)
+    d = W.generate(c)
+    occ = np.random.default_rng(5).uniform(0, 2, d["occ"].shape)
+    A = W.laser_samples(c, nsteps=6, t0=0.9)
+    r, rho_ref = ref.propagate(d["psi"], occ, d["vloc"], d["beta"], d["D"], A, c.dt, c.h)
+    outs = []
+    for graph, chunks in ((0, [6]), (1, [6]), (0, [1, 2, 3]), (0, [1] * 6)):
+        dom = make_domain(c, dict(d, occ=occ), options=[(M.OPT_GRAPH, graph)])
+        assert dom.gemm_path() == "tcgen05"
+        done = 0
+        for n in chunks:
+            dom.propagate(n, c.dt, A[done:done + n])
+            done += n
+        outs.append((dom.get_orbitals(), dom.density()))
+        dom.close()
+        assert rho_err(outs[-1][1], rho_ref) <= TOL_RHO and orb_err(outs[-1][0], r) <= TOL_LAST
+    for o in outs[1:]:
+        assert np.array_equal(o[0], outs[0][0]) and np.array_equal(o[1], outs[0][1])
+    # the density formed INSIDE a projection is overwritten by the separate pass at the end of every call: a test hook
+    # (libmlmd_test.so) runs that projection on the current state and hands back the rho it formed
+    import ctypes
+    import torch
+    hook = ctypes.CDLL(M.api.TEST_LIB_PATH).mlmd_debug_fused_density
+    hook.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+    dom = make_domain(c, dict(d, occ=occ))
+    dom.propagate(2, c.dt, A[:2])
+    rho_fused = torch.empty((c.ndom, *c.grid), dtype=torch.float32, device="cuda")
+    assert hook(dom.handle, rho_fused.data_ptr()) == 0
+    r2, rho2 = ref.propagate(d["psi"], occ, d["vloc"], d["beta"], d["D"], A[:2], c.dt, c.h)
+    e_fused, e_pass = rho_err(rho_fused.cpu().numpy(), rho2), rho_err(dom.density(), rho2)
+    print("density: riding on the projection", e_fused, " separate pass", e_pass)
+    assert e_fused <= TOL_RHO and e_pass <= TOL_RHO
+    dom.close()
+
+
 def test_gemm_modes():
     """FP64 accumulation is at least as close to the oracle as the default; the CUDA-core FP32 path
     and the TF32x1 rung meet the FP32-grade bar; the opt-in BF16 mode meets its stated 1e-3."""
