@@ -87,7 +87,10 @@ __device__ __forceinline__ void pair_acc_real(float4 &acc, const float4 a, const
 // R1: radius-1 instantiation for the paper's own 2nd-order / 7-point stencil (MLMD_OPT_FD_ORDER = 2;
 // SURVEY.md 8(f) NEXT-3): same staging and march, but the j = 2 taps are neither read from shared memory nor
 // multiplied (their coefficients are zero): 8 instead of 16 shared-memory loads per plane and thread.
-template <bool AYZ, bool PERDOM, int NORM, bool R1>
+// SAMEBASE: the Horner base IS the stencil input (the k = 4 stage, w == psi): the base of the plane completed at step n
+// is read from the shared-memory copy of plane n - 2 that the march already holds, instead of being loaded a second
+// time.  That buffer is released two steps later than usual, so the prefetch distance is two planes instead of three.
+template <bool AYZ, bool PERDOM, int NORM, bool R1, bool SAMEBASE>
 __global__ void __launch_bounds__(S_THREADS, 1)
 stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_z,
                    const __grid_constant__ CUtensorMap map_y, const __grid_constant__ CUtensorMap map_p,
@@ -147,7 +150,7 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         const int xr = dom * P.nx + x;
         uint8_t *buf = smem + b * S_PLANE;
         const int po = n - 4;   // output plane completed by step n: its Horner base travels with plane n
-        const bool with_psi = po >= 0 && po < nout;
+        const bool with_psi = !SAMEBASE && po >= 0 && po < nout;
         mbar_expect_tx(&full[b], with_psi ? S_PLANE : S_PLANE_W);
         if (with_psi) tma_load_4d(buf + S_PLANE_W, &map_p, &full[b], chunk * 16, z0, y0, dom * P.nx + x0 + po);
         tma_load_4d(buf, &map_c, &full[b], chunk * 16, z0, y0, xr);
@@ -156,8 +159,9 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         tma_load_4d(buf + S_CENTER + 2 * S_STRIP, &map_y, &full[b], chunk * 16, z0, ylo, xr);
         tma_load_4d(buf + S_CENTER + 3 * S_STRIP, &map_y, &full[b], chunk * 16, z0, yhi, xr);
     };
+    constexpr int PF = SAMEBASE ? 2 : S_PF;
     if (tid == 0)
-        for (int n = 0; n < S_PF && n < nplanes; ++n) issue(n);
+        for (int n = 0; n < PF && n < nplanes; ++n) issue(n);
 
     // Byte offsets inside a plane buffer.  Point A = (ty, tz), point B = (ty + 1, tz), ty even: the six rows
     // ty-2 .. ty+3 at the own z serve as centre and y-neighbours of BOTH points (6 loads instead of 10); the
@@ -239,8 +243,8 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     auto step = [&](const int n, const int k, const int it, float4 &A0, float4 &A1, float4 &A2, float4 &A3, float4 &A4,
                     float4 &B0, float4 &B1, float4 &B2, float4 &B3, float4 &B4) {
         // n = 5 it + k: plane n lives in buffer k; its barrier phase is it & 1
-        if (tid == 0 && n + S_PF < nplanes) {
-            const int m = n + S_PF, bm = (k + S_PF) % S_NBUF, um = it + (k + S_PF) / S_NBUF;   // um-th use of buffer bm
+        if (tid == 0 && n + PF < nplanes) {
+            const int m = n + PF, bm = (k + PF) % S_NBUF, um = it + (k + PF) / S_NBUF;   // um-th use of buffer bm
             if (um >= 1) mbar_wait(&empty[bm], (um - 1) & 1);
             issue(m);
         }
@@ -264,7 +268,9 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         }
         // plane q-2 (output n - 4) is complete: out = psi + (-i tau) acc
         if (n >= 4) {
-            const float4 psA = lds4(buf + S_PLANE_W + own), psB = lds4(buf + S_PLANE_W + own + 1024);
+            // SAMEBASE: plane n - 2 lives in buffer (k + 3) % 5
+            const uint32_t pb = SAMEBASE ? sbase + ((k + 3) % S_NBUF) * S_PLANE : buf + S_PLANE_W;
+            const float4 psA = lds4(pb + own), psB = lds4(pb + own + 1024);
             const float4 oA = make_float4(fmaf(P.tau, A0.y, psA.x), fmaf(-P.tau, A0.x, psA.y), fmaf(P.tau, A0.w, psA.z),
                                           fmaf(-P.tau, A0.z, psA.w));
             const float4 oB = make_float4(fmaf(P.tau, B0.y, psB.x), fmaf(-P.tau, B0.x, psB.y), fmaf(P.tau, B0.w, psB.z),
@@ -280,7 +286,11 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             }
         }
         __syncwarp();
-        if (tid % 32 == 0) mbar_arrive(&empty[k]);
+        if (SAMEBASE) {
+            if (n >= 2 && tid % 32 == 0) mbar_arrive(&empty[(k + 3) % S_NBUF]);   // plane n - 2 has served as base
+        } else if (tid % 32 == 0) {
+            mbar_arrive(&empty[k]);
+        }
         A0 = zero4;
         B0 = zero4;
     };
@@ -354,24 +364,30 @@ bool stencil_tma_supported(const mlmd_domain *h) {
 }
 
 namespace {
-template <int NORM, bool R1>
+template <int NORM, bool R1, bool SB>
 cudaError_t set_attrs() {
-    cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true, NORM, R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(stencil_tma_kernel<false, false, NORM, R1, SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, false, NORM, R1, SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<false, true, NORM, R1, SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stencil_tma_kernel<true, true, NORM, R1, SB>, cudaFuncAttributeMaxDynamicSharedMemorySize, S_SMEM);
     return e;
 }
-template <int NORM, bool R1>
+template <int NORM, bool R1, bool SB>
 void launch_variant(bool yz, bool perdom, unsigned g, cudaStream_t st, const CUtensorMap &mc, const CUtensorMap &mz,
                     const CUtensorMap &my, const CUtensorMap &mp, const TmaStencilParams &P) {
     if (!perdom) {
-        if (yz) stencil_tma_kernel<true, false, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
-        else stencil_tma_kernel<false, false, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        if (yz) stencil_tma_kernel<true, false, NORM, R1, SB><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, false, NORM, R1, SB><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
     } else {
-        if (yz) stencil_tma_kernel<true, true, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
-        else stencil_tma_kernel<false, true, NORM, R1><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        if (yz) stencil_tma_kernel<true, true, NORM, R1, SB><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
+        else stencil_tma_kernel<false, true, NORM, R1, SB><<<g, S_THREADS, S_SMEM, st>>>(mc, mz, my, mp, P);
     }
+}
+template <int NORM, bool R1>
+void launch_variant2(bool same, bool yz, bool perdom, unsigned g, cudaStream_t st, const CUtensorMap &mc, const CUtensorMap &mz,
+                     const CUtensorMap &my, const CUtensorMap &mp, const TmaStencilParams &P) {
+    if (same) launch_variant<NORM, R1, true>(yz, perdom, g, st, mc, mz, my, mp, P);
+    else launch_variant<NORM, R1, false>(yz, perdom, g, st, mc, mz, my, mp, P);
 }
 }  // namespace
 
@@ -393,12 +409,18 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
                                const StepCoef *coef_host, float tau, int *nlaunch, int norm_mode, double *npart) {
     static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
     if (!attr_set.done()) {
-        cudaError_t e = set_attrs<0, false>();
-        if (e == cudaSuccess) e = set_attrs<1, false>();
-        if (e == cudaSuccess) e = set_attrs<2, false>();
-        if (e == cudaSuccess) e = set_attrs<0, true>();
-        if (e == cudaSuccess) e = set_attrs<1, true>();
-        if (e == cudaSuccess) e = set_attrs<2, true>();
+        cudaError_t e = set_attrs<0, false, false>();
+        if (e == cudaSuccess) e = set_attrs<1, false, false>();
+        if (e == cudaSuccess) e = set_attrs<2, false, false>();
+        if (e == cudaSuccess) e = set_attrs<0, true, false>();
+        if (e == cudaSuccess) e = set_attrs<1, true, false>();
+        if (e == cudaSuccess) e = set_attrs<2, true, false>();
+        if (e == cudaSuccess) e = set_attrs<0, false, true>();
+        if (e == cudaSuccess) e = set_attrs<1, false, true>();
+        if (e == cudaSuccess) e = set_attrs<2, false, true>();
+        if (e == cudaSuccess) e = set_attrs<0, true, true>();
+        if (e == cudaSuccess) e = set_attrs<1, true, true>();
+        if (e == cudaSuccess) e = set_attrs<2, true, true>();
         if (e != cudaSuccess) return e;
         attr_set.mark();
     }
@@ -435,12 +457,13 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
     const unsigned g = (unsigned)grid;
     P.cval = coef_host ? *coef_host : StepCoef();
     const bool r1 = h->opt[MLMD_OPT_FD_ORDER] == 2;
-    if (norm_mode == 1) r1 ? launch_variant<1, true>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
-                           : launch_variant<1, false>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
-    else if (norm_mode == 2) r1 ? launch_variant<2, true>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
-                                : launch_variant<2, false>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
-    else r1 ? launch_variant<0, true>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
-            : launch_variant<0, false>(h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    const bool same = (const void *)w == (const void *)psi;      // the k = 4 stage: the Horner base is the stencil input
+    if (norm_mode == 1) r1 ? launch_variant2<1, true>(same, h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
+                           : launch_variant2<1, false>(same, h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    else if (norm_mode == 2) r1 ? launch_variant2<2, true>(same, h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
+                                : launch_variant2<2, false>(same, h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
+    else r1 ? launch_variant2<0, true>(same, h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P)
+            : launch_variant2<0, false>(same, h->field_yz, !coef_host, g, h->stream, mc, mz, my, mp, P);
     return cudaGetLastError();
 }
 
