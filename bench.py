@@ -120,8 +120,9 @@ def ncu_traffic(c, kernel_class):
             "back": ["back2_tc_kernel", "back_tc_kernel"], "density": ["density_kernel"]}.get(kernel_class, [])
     src = "%s (ncu --set full at commit %s)" % (os.path.relpath(paths[-1], ROOT), j.get("commit", "?"))
     for name in pick:
-        if name in t:
-            return t[name], src
+        for key in t:
+            if key == name or key.startswith(name + "<"):
+                return t[key], src
     return None, None
 
 

@@ -182,6 +182,47 @@ constexpr int PJ_STAGE_BYTES = 2 * PJ_A_BYTES + 2 * PJ_Y_BYTES;
 constexpr int PJ_SMEM = PJ_STAGES * PJ_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int PJ_THREADS = 192;          // warp 0 TMA, warp 1 MMA, warps 2-5 convert + epilogue
 
+// Column tiles of the CTA-pair kernels: N / 64 units of 64 columns over ntile = ceil(N / 448) tiles: `wt` wide tiles of
+// `wu` units followed by narrow tiles of `nu` units.  A tile is issued as UMMA pieces of n0 = min(width, 256) and
+// n1 = width - n0 columns (each CTA of the pair stages h0 = n0 / 64 and h1 = n1 / 64 chunks); a 64-column piece costs
+// as much as a 128-column one (its MMAs are bound by the A-operand reads), so the split avoids them where it can:
+// configs[4], 1408 columns = 448 + 448 + 256 + 256, nothing padded.
+struct ColSplit {
+    int ntile, wt, wu, nu;
+};
+struct ColTile {
+    int start, width, n0, n1, h0, h1;
+};
+__host__ __device__ inline ColTile col_tile(const ColSplit cs, int nt) {
+    ColTile t;
+    t.width = (nt < cs.wt ? cs.wu : cs.nu) * 64;
+    t.start = (nt < cs.wt ? nt * cs.wu : cs.wt * cs.wu + (nt - cs.wt) * cs.nu) * 64;
+    t.n0 = t.width < 256 ? t.width : 256;
+    t.n1 = t.width - t.n0;
+    t.h0 = t.n0 / 64;
+    t.h1 = t.n1 / 64;
+    return t;
+}
+inline ColSplit choose_col_split(int N) {
+    const int units = N / 64, ntile = (N + 447) / 448;
+    auto piece = [](int n) { return n == 0 ? 0 : (n < 128 ? 128 : n); };
+    auto cost = [&](int u) { const int w = u * 64, n0 = w < 256 ? w : 256; return piece(n0) + piece(w - n0); };
+    ColSplit best{ntile, ntile, (units + ntile - 1) / ntile, (units + ntile - 1) / ntile};
+    long best_cost = -1;
+    for (int wt = 1; wt <= ntile; ++wt)
+        for (int wu = 1; wu <= 7; ++wu) {
+            const int left = units - wt * wu, nn = ntile - wt;
+            if (left < 0 || (nn == 0 ? left != 0 : (left % nn != 0 || left / nn > wu || left / nn < 1))) continue;
+            const int nu = nn ? left / nn : wu;
+            const long c = (long)wt * cost(wu) + (long)nn * cost(nu);
+            if (best_cost < 0 || c < best_cost) {
+                best_cost = c;
+                best = ColSplit{ntile, wt, wu, nu};
+            }
+        }
+    return best;
+}
+
 struct ProjParams {
     int ndom, ngrid, P, N, BN, ntile_m, ntile_n, nsplit, prows, nprod, conv_a, chain, lowp, rn;
     float *zpart;
@@ -189,6 +230,7 @@ struct ProjParams {
     // CTA's columns of the psi tile it holds anyway; NULL = off
     float *rho;
     const float *occ;
+    ColSplit cs;                 // column tiles of the CTA-pair kernel
 };
 
 // LO = true: stages hold hi and lo tiles of both operands (3xTF32), 3 stages; LO = false (one product per MAC):
@@ -441,10 +483,13 @@ constexpr int P2_FWD = 4;                               // forwarding lanes of t
                                                         // that one lane sees all uses of a barrier in order (parity waits)
 
 static_assert(P2_STAGES % P2_FWD == 0, "one forwarding lane must see every use of a stage barrier in order");
+
 template <bool LO>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PJ_THREADS, 1)
 proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_y0,
-                const __grid_constant__ CUtensorMap map_y1, const __grid_constant__ CUtensorMap map_z, const ProjParams q) {
+                const __grid_constant__ CUtensorMap map_y1, const __grid_constant__ CUtensorMap map_y0n,
+                const __grid_constant__ CUtensorMap map_y1n, const __grid_constant__ CUtensorMap map_z, const ProjParams q) {
+    // map_y0 / map_y1: boxes of the WIDE column tiles' two pieces, map_y0n / map_y1n: of the tiles one unit narrower
     constexpr int NST = LO ? P2_STAGES : 2 * P2_STAGES;
     constexpr int SB = LO ? P2_STAGE_BYTES : P2_STAGE_BYTES / 2;
     constexpr int YOFF = (LO ? 2 : 1) * P2_A_BYTES;
@@ -472,6 +517,8 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
         prefetch_tmap(&map_a);
         prefetch_tmap(&map_y0);
         prefetch_tmap(&map_y1);
+        prefetch_tmap(&map_y0n);
+        prefetch_tmap(&map_y1n);
         prefetch_tmap(&map_z);
     }
     if (warp == 1) tmem_alloc_2cta(tmem_slot, 512);
@@ -484,9 +531,6 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
     const int nkb = q.ngrid / PJ_BK;
     const int total = q.ndom * q.ntile_m * q.ntile_n * q.nsplit;   // pair units
     const bool need_lo = q.nprod == 3;
-    const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;        // UMMA pieces (columns); per CTA n/2 of each
-    const int h0 = n0 / 64, h1 = n1 / 64;                           // this CTA's 32-column chunks of each piece
-    const uint32_t tx_bytes = P2_A_BYTES + (uint32_t)(h0 + h1) * PJ_BK * 128;
 
     auto decode = [&](int u, int &dom, int &mt, int &nt, int &sp, int &kb0, int &kb1) {
         nt = u % q.ntile_n;
@@ -505,7 +549,12 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
             for (int u = cl; u < total; u += ncl) {
                 int dom, mt, nt, sp, kb0, kb1;
                 decode(u, dom, mt, nt, sp, kb0, kb1);
-                const int ch0 = nt * (q.BN / 32) + crank * h0, ch1 = nt * (q.BN / 32) + n0 / 32 + crank * h1;
+                const ColTile ct = col_tile(q.cs, nt);
+                const int h0 = ct.h0, h1 = ct.h1;
+                const int ch0 = ct.start / 32 + crank * h0, ch1 = ct.start / 32 + ct.n0 / 32 + crank * h1;
+                const bool narrow = nt >= q.cs.wt;
+                const CUtensorMap *my0 = narrow ? &map_y0n : &map_y0, *my1 = narrow ? &map_y1n : &map_y1;
+                const uint32_t tx_bytes = P2_A_BYTES + (uint32_t)(h0 + h1) * PJ_BK * 128;
                 for (int kb = kb0; kb < kb1; ++kb, ++it) {
                     const int s = it % NST;
                     mbar_wait(&empty[s], ((it / NST) & 1) ^ 1);
@@ -513,20 +562,22 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                     mbar_expect_tx(&full[s], tx_bytes);
                     const int row = dom * q.ngrid + kb * PJ_BK;
                     tma_load_3d(st, &map_a, &full[s], 0, row, mt * 8 + crank * 4);
-                    tma_load_3d(st + YOFF, &map_y0, &full[s], 0, row, ch0);
-                    if (h1) tma_load_3d(st + YOFF + h0 * (PJ_BK * 128), &map_y1, &full[s], 0, row, ch1);
+                    tma_load_3d(st + YOFF, my0, &full[s], 0, row, ch0);
+                    if (h1) tma_load_3d(st + YOFF + h0 * (PJ_BK * 128), my1, &full[s], 0, row, ch1);
                 }
             }
         }
     } else if (warp == 1) {
         if (leader) {
             if (lane == 0) {
-                const uint32_t id0 = instr_desc(FMT_TF32, 1, 1, 256, (uint32_t)n0);
-                const uint32_t id1 = instr_desc(FMT_TF32, 1, 1, 256, (uint32_t)(n1 ? n1 : 64));
                 int it = 0, nd = 0;   // nd: accumulator hand-overs (drains) so far
                 for (int u = cl; u < total; u += ncl) {
                     int dom, mt, nt, sp, kb0, kb1;
                     decode(u, dom, mt, nt, sp, kb0, kb1);
+                    const ColTile ct = col_tile(q.cs, nt);
+                    const int n0 = ct.n0, h0 = ct.h0, h1 = ct.h1;
+                    const uint32_t id0 = instr_desc(FMT_TF32, 1, 1, 256, (uint32_t)n0);
+                    const uint32_t id1 = instr_desc(FMT_TF32, 1, 1, 256, (uint32_t)(ct.n1 ? ct.n1 : 64));
                     for (int kb = kb0; kb < kb1; ++kb, ++it) {
                         const bool first = (kb - kb0) % q.chain == 0;
                         if (first) {
@@ -589,10 +640,12 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
         const int er = quarter * 32 + lane;   // TMEM lane = accumulator row of this thread; er == 0 leads the TMA stores
         uint64_t *done = leader ? conv : cdone;
         int it = 0, nd = 0, slot = 0;
-        const int ny4 = (h0 + h1) * PJ_BK * 8;    // float4 count of this CTA's psi tile
         for (int u = cl; u < total; u += ncl) {
             int dom, mt, nt, sp, kb0, kb1;
             decode(u, dom, mt, nt, sp, kb0, kb1);
+            const ColTile ct = col_tile(q.cs, nt);
+            const int n0 = ct.n0, h0 = ct.h0, h1 = ct.h1;
+            const int ny4 = (h0 + h1) * PJ_BK * 8;    // float4 count of this CTA's psi tile
             const bool rows_live = q.P - mt * 256 - crank * 128 > 0;
             for (int c0k = kb0; c0k < kb1; c0k += q.chain) {
                 const int c1k = min(c0k + q.chain, kb1);
@@ -626,7 +679,7 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                             int j = 0;
                             for (int i = t; i < ny4; i += 128, ++j) {
                                 float4 v = y4[i];
-                                const int gch = j < h0 ? nt * (q.BN / 32) + crank * h0 + j : nt * (q.BN / 32) + n0 / 32 + crank * h1 + (j - h0);
+                                const int gch = j < h0 ? ct.start / 32 + crank * h0 + j : ct.start / 32 + n0 / 32 + crank * h1 + (j - h0);
                                 const float2 ff = __ldg(f2 + gch * 8 + pair_in_chunk);
                                 acc = fmaf(ff.x, fmaf(v.x, v.x, v.y * v.y), acc);
                                 acc = fmaf(ff.y, fmaf(v.z, v.z, v.w * v.w), acc);
@@ -659,12 +712,12 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                 // the store of the slice's first chain must have landed before later chains add to it
                 if (add && c0k == kb0 + q.chain && er == 0) bulk_wait<0>();
                 const int zrow = (dom * q.nsplit + sp) * q.prows + mt * 256 + crank * 128;
-                for (int cb = 0; cb < q.BN / 32; ++cb) {
+                for (int cb = 0; cb < ct.width / 32; ++cb) {
                     uint32_t v[32];
                     tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
                     tmem_ld_wait();
-                    const int c0 = nt * q.BN + cb * 32;
-                    if (c0 < q.N && rows_live) epi_tile_out<2>(stage, slot, &map_z, c0, zrow, v, er, add);
+                    const int c0 = ct.start + cb * 32;
+                    if (rows_live) epi_tile_out<2>(stage, slot, &map_z, c0, zrow, v, er, add);
                 }
                 tc_fence_before();
                 named_bar_sync(EPI_BAR, 128);
@@ -702,6 +755,7 @@ constexpr int BK_THREADS = 64 + 32 * BK_EPI_WARPS;
 struct BackParams {
     int ndom, ngrid, P, N, BN, ntile_n, prows, nprod, ldy, lowp;
     float *Y;
+    ColSplit cs;                 // column tiles of the CTA-pair kernel
 };
 
 // beta arrives as ONE FP32 copy (raw); the operand pair of 3xTF32 is formed in shared memory:
@@ -886,7 +940,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(BK_THREADS, 1)
 back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_constant__ CUtensorMap map_alo,
                 const __grid_constant__ CUtensorMap map_w0h, const __grid_constant__ CUtensorMap map_w0l,
                 const __grid_constant__ CUtensorMap map_w1h, const __grid_constant__ CUtensorMap map_w1l,
+                const __grid_constant__ CUtensorMap map_n0h, const __grid_constant__ CUtensorMap map_n0l,
+                const __grid_constant__ CUtensorMap map_n1h, const __grid_constant__ CUtensorMap map_n1l,
                 const __grid_constant__ CUtensorMap map_out, const BackParams q) {
+    // column tiles as in the projection (col_tile): map_w* are the boxes of the wide tiles' two pieces (hi, lo),
+    // map_n* those of the tiles one 64-column unit narrower
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
     uint8_t *stage = smem + B2_STAGES * B2_STAGE_BYTES;
@@ -923,9 +981,6 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
     const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
     const int nk = (q.P + 7) / 8;
     const bool need_lo = q.nprod >= 2, need_wlo = q.nprod == 3;   // as in back_tc_kernel
-    const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;   // UMMA pieces (columns); per CTA n/2 of each
-    const int h0 = n0 / 64, h1 = n1 / 64;                      // this CTA's 32-column chunks of each piece
-    const uint32_t cta_bytes = (need_lo ? 2u : 1u) * BK_A_BYTES + (need_wlo ? 2u : 1u) * (uint32_t)(h0 + h1) * 1024;
 
     if (warp == 0) {
         if (lane == 0) {
@@ -933,7 +988,13 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
             for (int u = cl; u < total; u += ncl) {
                 const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
                 const int row = dom * q.ngrid + rt * 128;
-                const int ch0 = nt * (q.BN / 32) + crank * h0, ch1 = nt * (q.BN / 32) + n0 / 32 + crank * h1;
+                const ColTile ct = col_tile(q.cs, nt);
+                const int h0 = ct.h0, h1 = ct.h1;
+                const int ch0 = ct.start / 32 + crank * h0, ch1 = ct.start / 32 + ct.n0 / 32 + crank * h1;
+                const bool narrow = nt >= q.cs.wt;
+                const CUtensorMap *m0h = narrow ? &map_n0h : &map_w0h, *m0l = narrow ? &map_n0l : &map_w0l;
+                const CUtensorMap *m1h = narrow ? &map_n1h : &map_w1h, *m1l = narrow ? &map_n1l : &map_w1l;
+                const uint32_t cta_bytes = (need_lo ? 2u : 1u) * BK_A_BYTES + (need_wlo ? 2u : 1u) * (uint32_t)(h0 + h1) * 1024;
                 for (int k = 0; k < nk; ++k, ++it) {
                     const int s = it % B2_STAGES;
                     mbar_wait(&empty[s], ((it / B2_STAGES) & 1) ^ 1);
@@ -941,23 +1002,25 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
                     if (leader) mbar_expect_tx(&full[s], 2 * cta_bytes);
                     const int wrow = dom * q.prows + k * 8;
                     tma_load_2d_2cta(st, &map_ahi, &full[s], k * 8, row);
-                    tma_load_3d_2cta(st + 2 * BK_A_BYTES, &map_w0h, &full[s], 0, wrow, ch0);
-                    if (h1) tma_load_3d_2cta(st + 2 * BK_A_BYTES + h0 * 1024, &map_w1h, &full[s], 0, wrow, ch1);
+                    tma_load_3d_2cta(st + 2 * BK_A_BYTES, m0h, &full[s], 0, wrow, ch0);
+                    if (h1) tma_load_3d_2cta(st + 2 * BK_A_BYTES + h0 * 1024, m1h, &full[s], 0, wrow, ch1);
                     if (need_lo) tma_load_2d_2cta(st + BK_A_BYTES, &map_alo, &full[s], k * 8, row);
                     if (need_wlo) {
-                        tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES, &map_w0l, &full[s], 0, wrow, ch0);
+                        tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES, m0l, &full[s], 0, wrow, ch0);
                         if (h1)
-                            tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES + h0 * 1024, &map_w1l, &full[s], 0, wrow, ch1);
+                            tma_load_3d_2cta(st + 2 * BK_A_BYTES + B2_WH_BYTES + h0 * 1024, m1l, &full[s], 0, wrow, ch1);
                     }
                 }
             }
         }
     } else if (warp == 1) {
         if (lane == 0 && leader) {
-            const uint32_t id0 = instr_desc(FMT_TF32, 0, 1, 256, (uint32_t)n0);
-            const uint32_t id1 = instr_desc(FMT_TF32, 0, 1, 256, (uint32_t)(n1 ? n1 : 64));
             int it = 0, nu = 0;
             for (int u = cl; u < total; u += ncl, ++nu) {
+                const ColTile ct = col_tile(q.cs, u % q.ntile_n);
+                const int n0 = ct.n0, h0 = ct.h0, h1 = ct.h1;
+                const uint32_t id0 = instr_desc(FMT_TF32, 0, 1, 256, (uint32_t)n0);
+                const uint32_t id1 = instr_desc(FMT_TF32, 0, 1, 256, (uint32_t)(ct.n1 ? ct.n1 : 64));
                 mbar_wait(acc_empty, (nu & 1) ^ 1);
                 tc_fence_after();
                 for (int k = 0; k < nk; ++k, ++it) {
@@ -997,12 +1060,13 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
             const bool live = rt < nrt;
             mbar_wait(acc_full, nu & 1);
             tc_fence_after();
-            for (int cb = 0; cb < q.BN / 32; ++cb) {
+            const ColTile ct = col_tile(q.cs, nt);
+            for (int cb = 0; cb < ct.width / 32; ++cb) {
                 uint32_t v[32];
                 tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
                 tmem_ld_wait();
-                const int c0 = nt * q.BN + cb * 32;
-                if (c0 < q.N && live) epi_tile_out<2>(stage, slot, &map_out, c0, row0, v, er, true);
+                const int c0 = ct.start + cb * 32;
+                if (live) epi_tile_out<2>(stage, slot, &map_out, c0, row0, v, er, true);
             }
             tc_fence_before();
             named_bar_sync(EPI_BAR, 128);
@@ -1103,18 +1167,21 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     if (!make_out_map(cache, &mz, zpart, (uint64_t)ndom * nsplit * prows, N, N)) return cudaErrorInvalidValue;
     if (N % 64 == 0 && A_lo == nullptr) {
         // CTA pairs (cta_group::2): one pair per (domain, 256-row tile, column tile of <= 448, K slice)
-        q.ntile_n = (N + BK_MAXBN - 1) / BK_MAXBN;
-        q.BN = ((N + q.ntile_n - 1) / q.ntile_n + 63) / 64 * 64;
-        const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;
-        CUtensorMap ma, my0, my1;
+        q.cs = choose_col_split(N);
+        q.ntile_n = q.cs.ntile;
+        const ColTile wide = col_tile(q.cs, 0), narrow = col_tile(q.cs, q.ntile_n - 1);
+        q.BN = wide.width;
+        CUtensorMap ma, my0, my1, my0n, my1n;
         if (!make_chunk_map(cache, &ma, A_hi, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(cache, &my0, Y, rows, ldy, N / 32, PJ_BK, n0 / 64)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(cache, &my1, Y, rows, ldy, N / 32, PJ_BK, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &my0, Y, rows, ldy, N / 32, PJ_BK, wide.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &my1, Y, rows, ldy, N / 32, PJ_BK, wide.h1 ? wide.h1 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &my0n, Y, rows, ldy, N / 32, PJ_BK, narrow.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &my1n, Y, rows, ldy, N / 32, PJ_BK, narrow.h1 ? narrow.h1 : 1)) return cudaErrorInvalidValue;
         const int total = ndom * q.ntile_m * q.ntile_n * nsplit;
         const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
         ++*nlaunch;
-        if (q.nprod == 3) proj2_tc_kernel<true><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, mz, q);
-        else proj2_tc_kernel<false><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, mz, q);
+        if (q.nprod == 3) proj2_tc_kernel<true><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, my0n, my1n, mz, q);
+        else proj2_tc_kernel<false><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, my0n, my1n, mz, q);
         return cudaGetLastError();
     }
     q.ntile_n = proj_ntile_n(N);
@@ -1164,21 +1231,28 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     ++*nlaunch;
     // CTA pairs for the modes that take beta as (raw, stored remainder): 3xTF32 and the staged mode's two products;
     // one-product modes want beta ROUNDED (an unbiased operand), which the single-CTA kernel forms in shared memory
-    if (q.BN % 64 == 0 && !q.lowp && q.nprod >= 2 && A_lo) {
+    if (N % 64 == 0 && !q.lowp && q.nprod >= 2 && A_lo) {
         static DeviceOnce attr2;
         if (!attr2.done()) {
             cudaError_t e = cudaFuncSetAttribute(back2_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, B2_SMEM);
             if (e != cudaSuccess) return e;
             attr2.mark();
         }
-        const int n0 = q.BN < 256 ? q.BN : 256, n1 = q.BN - n0;
-        CUtensorMap mal, w0h, w0l, w1h, w1l;
+        q.cs = choose_col_split(N);
+        const ColTile wide = col_tile(q.cs, 0), narrow = col_tile(q.cs, q.ntile_n - 1);
+        q.BN = wide.width;
+        const uint64_t wrows = (uint64_t)ndom * prows;
+        CUtensorMap mal, w0h, w0l, w1h, w1l, n0h, n0l, n1h, n1l;
         if (!make_k8_map(cache, &mal, A_lo, rows, lda, lda, 128)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(cache, &w0h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(cache, &w0l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n0 / 64)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(cache, &w1h, W_hi, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
-        if (!make_chunk_map(cache, &w1l, W_lo, (uint64_t)ndom * prows, N, N / 32, 8, n1 ? n1 / 64 : 1)) return cudaErrorInvalidValue;
-        back2_tc_kernel<<<grid, BK_THREADS, B2_SMEM, st>>>(ma, mal, w0h, w0l, w1h, w1l, mo, q);
+        if (!make_chunk_map(cache, &w0h, W_hi, wrows, N, N / 32, 8, wide.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &w0l, W_lo, wrows, N, N / 32, 8, wide.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &w1h, W_hi, wrows, N, N / 32, 8, wide.h1 ? wide.h1 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &w1l, W_lo, wrows, N, N / 32, 8, wide.h1 ? wide.h1 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &n0h, W_hi, wrows, N, N / 32, 8, narrow.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &n0l, W_lo, wrows, N, N / 32, 8, narrow.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &n1h, W_hi, wrows, N, N / 32, 8, narrow.h1 ? narrow.h1 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk_map(cache, &n1l, W_lo, wrows, N, N / 32, 8, narrow.h1 ? narrow.h1 : 1)) return cudaErrorInvalidValue;
+        back2_tc_kernel<<<grid, BK_THREADS, B2_SMEM, st>>>(ma, mal, w0h, w0l, w1h, w1l, n0h, n0l, n1h, n1l, mo, q);
         return cudaGetLastError();
     }
     const int chalf = (q.BN / 32 + 1) / 2;   // each CTA of a cluster fetches (and multicasts) half of the W chunks
