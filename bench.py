@@ -35,11 +35,11 @@ CPU_STEPS = 8            # timed oracle steps of the cpu_baseline leg
 STEP_NAMES = {"taylor": "Taylor-4 (full H, north_star)", "split": "Eq. (2) split (half-kick, Taylor-4 of h_loc, half-kick)"}
 # tensor peak as a multiple of the measured dense BF16 peak (B200_PROFILING.md nominal ratios:
 # tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
-# the opt-in BF16-operand mode issues its single product on the TF32 pipe (BF16 values are TF32 values)
+# the opt-in low-precision mode stores beta and W as BF16 and issues tcgen05.mma.kind::f16: the BF16 peak itself
 TF32_OVER_BF16 = 1.1 / 2.25     # nominal dense peaks (B200_PROFILING.md): tf32 1.1 PF, bf16 2.25 PF
 # "staged" (MLMD_GEMM_FP32GRADE_STAGED, Taylor step): of the 8 GEMMs of a step the outermost 2 issue 3 products per MAC, the
 # inner projections 1 and the inner back-applications 2: (2 x 3 + 3 x 1 + 3 x 2) / 8 = 1.875 products on average
-TENSOR_RATIO = {"fp32grade": TF32_OVER_BF16 / 3.0, "tf32x1": TF32_OVER_BF16, "bf16": TF32_OVER_BF16,
+TENSOR_RATIO = {"fp32grade": TF32_OVER_BF16 / 3.0, "tf32x1": TF32_OVER_BF16, "bf16": 1.0,
                 "staged": TF32_OVER_BF16 / 1.875}
 FP32_ALU_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FMA lanes x 2 flop x max SM clock
 FP64_ALU_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12    # nominal 64 DFMA lanes per SM (guide: ~40 TF)

@@ -319,6 +319,25 @@ static void drop_graph(mlmd_domain *h) {
     }
 }
 
+// The second beta-sized buffer holds what the current GEMM mode reads next to the FP32 projectors: the remainder
+// beta - trunc_tf32(beta) (lo operand of the 3xTF32 back-application), or, in the opt-in low-precision mode, the BF16
+// copy of beta (2 bytes per element) that both kind::f16 GEMMs read INSTEAD of the FP32 array.
+static bool lowp_bf16_storage(const mlmd_domain *h) {
+    return h->gemm_mode == MLMD_GEMM_LOWP_BF16 && h->tc_ok && h->opt[MLMD_OPT_GEMM_PATH] == 0 && (2 * h->ld) % 64 == 0;
+}
+static int fill_beta_companion(mlmd_domain *h) {
+    if (h->nproj == 0) return MLMD_OK;
+    const size_t n = (size_t)h->ndom * h->ngrid * h->ldp;
+    int nl = 0;
+    if (lowp_bf16_storage(h)) CU(launch_to_bf16(h->stream, h->beta(), h->beta_lo(), n, &nl));
+    else CU(launch_tf32_remainder(h->stream, h->beta(), h->beta_lo(), n, &nl));
+    // W changes its storage type with the mode too (FP32 hi / lo pair, or one BF16 array): rows beyond the projector
+    // count must read as zeros in either view
+    CU(cudaMemsetAsync(h->what(), 0, 2 * (h->off.what_lo - h->off.what), h->stream));
+    h->launches += nl;
+    return MLMD_OK;
+}
+
 int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_dtype, const double *D, int where) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: NULL handle");
     if (nproj < 0) return fail(MLMD_ERR_ARG, "mlmd_set_projectors: nproj=%d", nproj);
@@ -354,11 +373,10 @@ int mlmd_set_projectors(mlmd_domain_t *h, int nproj, const void *beta, int beta_
     // rows [P, ldp) of W are read (times zero columns of beta) by the K = 8 slabs of the back-application: a stale NaN
     // left there by an earlier projector set or a diverged run would poison psi
     CU(cudaMemsetAsync(h->what(), 0, 2 * (h->off.what_lo - h->off.what), h->stream));
-    int nl = 0;
-    CU(launch_tf32_remainder(h->stream, h->beta(), h->beta_lo(), rows * ldp, &nl));
-    h->launches += nl;
-    CU(cudaStreamSynchronize(h->stream));   // dp is a temporary; host beta may be reused by the caller
     h->nproj = nproj; h->beta_complex = cplx; h->P = P; h->ldp = ldp; h->dmax = dmax;
+    int rc = fill_beta_companion(h);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(h->stream));   // dp is a temporary; host beta may be reused by the caller
     return MLMD_OK;
 }
 
@@ -366,7 +384,9 @@ int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: NULL handle");
     drop_graph(h);
     if (mode < MLMD_GEMM_FP32GRADE || mode > MLMD_GEMM_FP32GRADE_STAGED) return fail(MLMD_ERR_ARG, "mlmd_set_gemm_mode: bad mode %d", mode);
+    const bool was16 = lowp_bf16_storage(h);
     h->gemm_mode = mode;
+    if (was16 != lowp_bf16_storage(h)) return fill_beta_companion(h);
     return MLMD_OK;
 }
 
@@ -380,7 +400,9 @@ int mlmd_set_option(mlmd_domain_t *h, int key, int value) {
         return fail(MLMD_ERR_ARG, "mlmd_set_option: key %d takes 0..%d, got %d", key, nvalues[key] - 1, value);
     }
     drop_graph(h);      // a captured step bakes the kernel choice in
+    const bool was16 = lowp_bf16_storage(h);
     h->opt[key] = value;
+    if (was16 != lowp_bf16_storage(h)) return fill_beta_companion(h);
     return MLMD_OK;
 }
 
@@ -580,14 +602,15 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl,
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
                               2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, chain > 0 ? chain : proj_chain(nprod), nl, &h->tmaps,
-                              with_density ? h->rho() : nullptr, h->occ()));
+                              with_density ? h->rho() : nullptr, h->occ(), lowp_bf16_storage(h) ? h->beta_lo() : nullptr));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
     }
     ProfScope ps(h, MLMD_K_GLUE);
     CU(launch_reduce_scale(h->stream, h->ndom, h->nproj, h->beta_complex, h->ld, h->prows, nsplit, h->zpart(),
-                           h->dprime(), tau, h->what(), h->what_lo(), (tc && h->gemm_mode == MLMD_GEMM_LOWP_BF16) ? 1 : 0, nl));
+                           h->dprime(), tau, h->what(), h->what_lo(),
+                           (tc && h->gemm_mode == MLMD_GEMM_LOWP_BF16) ? (lowp_bf16_storage(h) ? 2 : 1) : 0, nl));
     return MLMD_OK;
 }
 
@@ -596,8 +619,9 @@ static int nonlocal_back(mlmd_domain *h, float2 *out, int *nl, int nprod = -1) {
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
     ProfScope ps(h, MLMD_K_BACK);
     if (use_tensor_cores(h))
-        CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), h->beta_lo(), h->ldp, h->P, h->what(), h->what_lo(),
-                          (float *)out, 2 * h->ld, 2 * h->ld, h->prows, nprod, nl, &h->tmaps));
+        CU(launch_back_tc(h->stream, h->ndom, h->ngrid, h->beta(), lowp_bf16_storage(h) ? nullptr : h->beta_lo(), h->ldp, h->P,
+                          h->what(), h->what_lo(), (float *)out, 2 * h->ld, 2 * h->ld, h->prows, nprod, nl, &h->tmaps,
+                          lowp_bf16_storage(h) ? h->beta_lo() : nullptr, lowp_bf16_storage(h) ? h->what() : nullptr));
     else
         CU(launch_back_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, h->what(), h->what_lo(),
                             (float *)out, 2 * h->ld, 2 * h->ld, h->prows, fp64, nl));

@@ -106,6 +106,39 @@ bool make_out_map(TmapCache *cache, CUtensorMap *m, const float *base, uint64_t 
     return cached_tmap(cache, k, m, [&](CUtensorMap *o) { return make_out_map_raw(o, base, rows, cols, pitch); });
 }
 
+// BF16 operands (opt-in low-precision mode).  MN-major tiles keep the 32-column chunk granularity of the FP32 path:
+// dims (32 bf16 = 64 B, rows, chunks of 32 columns), 64-byte swizzle = UMMA MN-major SWIZZLE_64B atoms (8 K-rows x 32
+// MN-elements), so a CTA of a pair can hold any number of chunks of a column tile.
+bool make_chunk16_map(TmapCache *cache, CUtensorMap *m, const void *base, uint64_t rows, uint64_t pitch, uint64_t nchunk,
+                      uint32_t box_rows, uint32_t box_chunks) {
+    const TmapKey k{5, base, rows, pitch, nchunk, 0, box_rows, box_chunks};
+    return cached_tmap(cache, k, m, [&](CUtensorMap *o) {
+        EncodeTiledFn f = encode_fn();
+        if (!f) return false;
+        cuuint64_t dims[3] = {32, rows, nchunk};
+        cuuint64_t strides[2] = {pitch * 2, 64};
+        cuuint32_t box[3] = {32, box_rows, box_chunks};
+        cuuint32_t es[3] = {1, 1, 1};
+        return f(o, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                 CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    });
+}
+// K-major BF16 slab: (cols, rows) view with a (64 bf16 = 128 B, box_rows) box in the 128-byte swizzle = UMMA K-major
+// SWIZZLE_128B (four K = 16 steps per row)
+bool make_k64_map(TmapCache *cache, CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, uint64_t pitch, uint32_t box_rows) {
+    const TmapKey k{6, base, rows, cols, pitch, 0, box_rows, 0};
+    return cached_tmap(cache, k, m, [&](CUtensorMap *o) {
+        EncodeTiledFn f = encode_fn();
+        if (!f) return false;
+        cuuint64_t dims[2] = {cols, rows};
+        cuuint64_t strides[1] = {pitch * 2};
+        cuuint32_t box[2] = {64, box_rows};
+        cuuint32_t es[2] = {1, 1};
+        return f(o, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, (void *)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                 CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    });
+}
+
 constexpr int EPI_TILE_BYTES = 128 * 128;   // one staging tile: 128 rows x 32 floats
 constexpr int EPI_BAR = 1;                  // named barrier of the 128 epilogue threads
 
@@ -165,6 +198,14 @@ __device__ __forceinline__ float bf16_round(float x) {
 }
 __device__ __forceinline__ float4 bf16_round4(const float4 v) {
     return make_float4(bf16_round(v.x), bf16_round(v.y), bf16_round(v.z), bf16_round(v.w));
+}
+
+// two floats -> packed BF16 pair (round-to-nearest-even), low half = first
+__device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
+    uint32_t ua = __float_as_uint(a), ub = __float_as_uint(b);
+    ua += 0x7fffu + ((ua >> 16) & 1u);
+    ub += 0x7fffu + ((ub >> 16) & 1u);
+    return (ua >> 16) | (ub & 0xffff0000u);
 }
 
 // =================================================================================================
@@ -736,6 +777,207 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
 }
 
 // =================================================================================================
+// Opt-in low-precision projection (PAPER.md L207, L239 float_to_BF16; L296): BF16 x BF16 -> FP32 on CTA pairs with
+// tcgen05.mma.kind::f16 (K = 16 per instruction: one instruction per 16-row stage and column piece).  beta is read as
+// its stored BF16 copy (2 bytes per element instead of round 1's 8); psi arrives as FP32 (its only copy) and the
+// converter warps of each CTA write its BF16 image, re-laid-out from the FP32 tile's 32-byte-atom swizzle to the
+// 64-byte swizzle of a BF16 MN-major operand, next to it.  Same unit / chain / handshake structure as proj2_tc_kernel.
+// =================================================================================================
+constexpr int PH_A_BYTES = 4 * PJ_BK * 64;              // this CTA's 128 projector rows: 4 chunks of [16 r x 32 p] BF16
+constexpr int PH_Y16_BYTES = 7 * PJ_BK * 64;            // BF16 image of this CTA's half of the psi tile
+constexpr int PH_STAGE_BYTES = 4096 + P2_Y_BYTES + 7168;     // beta16 (4 KB) + psi FP32 staging (14 KB) + psi16 (7 KB)
+constexpr int PH_STAGES = 7;
+constexpr int PH_FWD = PH_STAGES;                       // one forwarding lane per stage
+constexpr int PH_SMEM = PH_STAGES * PH_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 512;
+static_assert(PH_A_BYTES == 4096 && PH_Y16_BYTES == 7168, "stage carving");
+static_assert(PH_SMEM <= 232448, "shared memory of proj2h_tc_kernel");
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PJ_THREADS, 1)
+proj2h_tc_kernel(const __grid_constant__ CUtensorMap map_a16, const __grid_constant__ CUtensorMap map_y0,
+                 const __grid_constant__ CUtensorMap map_y1, const __grid_constant__ CUtensorMap map_y0n,
+                 const __grid_constant__ CUtensorMap map_y1n, const __grid_constant__ CUtensorMap map_z, const ProjParams q) {
+    constexpr int NST = PH_STAGES, SB = PH_STAGE_BYTES, YOFF = PH_A_BYTES, Y16OFF = PH_A_BYTES + P2_Y_BYTES;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *stage = smem + NST * SB;
+    uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
+    uint64_t *full = bars, *empty = bars + NST, *conv = bars + 2 * NST, *cdone = bars + 3 * NST;
+    uint64_t *acc_full = bars + 4 * NST, *acc_empty = acc_full + 1;
+    uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const int crank = (int)cluster_ctarank();
+    const bool leader = crank == 0;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], 1);
+            mbar_init(&conv[s], 128 + 1);
+            mbar_init(&cdone[s], 128);
+        }
+        mbar_init(acc_full, 1);
+        mbar_init(acc_empty, 2);
+        fence_barrier_init();
+        prefetch_tmap(&map_a16);
+        prefetch_tmap(&map_y0);
+        prefetch_tmap(&map_y1);
+        prefetch_tmap(&map_z);
+    }
+    if (warp == 1) tmem_alloc_2cta(tmem_slot, 512);
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
+    const int nkb = q.ngrid / PJ_BK;
+    const int total = q.ndom * q.ntile_m * q.ntile_n * q.nsplit;
+
+    auto decode = [&](int u, int &dom, int &mt, int &nt, int &sp, int &kb0, int &kb1) {
+        nt = u % q.ntile_n;
+        u /= q.ntile_n;
+        sp = u % q.nsplit;
+        u /= q.nsplit;
+        mt = u % q.ntile_m;
+        dom = u / q.ntile_m;
+        kb0 = (int)((long)nkb * sp / q.nsplit);
+        kb1 = (int)((long)nkb * (sp + 1) / q.nsplit);
+    };
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int it = 0;
+            for (int u = cl; u < total; u += ncl) {
+                int dom, mt, nt, sp, kb0, kb1;
+                decode(u, dom, mt, nt, sp, kb0, kb1);
+                const ColTile ct = col_tile(q.cs, nt);
+                const int h0 = ct.h0, h1 = ct.h1;
+                const int ch0 = ct.start / 32 + crank * h0, ch1 = ct.start / 32 + ct.n0 / 32 + crank * h1;
+                const bool narrow = nt >= q.cs.wt;
+                const CUtensorMap *my0 = narrow ? &map_y0n : &map_y0, *my1 = narrow ? &map_y1n : &map_y1;
+                const uint32_t tx_bytes = PH_A_BYTES + (uint32_t)(h0 + h1) * PJ_BK * 128;
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    const int s = it % NST;
+                    mbar_wait(&empty[s], ((it / NST) & 1) ^ 1);
+                    uint8_t *st = smem + s * SB;
+                    mbar_expect_tx(&full[s], tx_bytes);
+                    const int row = dom * q.ngrid + kb * PJ_BK;
+                    tma_load_3d(st, &map_a16, &full[s], 0, row, mt * 8 + crank * 4);
+                    tma_load_3d(st + YOFF, my0, &full[s], 0, row, ch0);
+                    if (h1) tma_load_3d(st + YOFF + h0 * (PJ_BK * 128), my1, &full[s], 0, row, ch1);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (leader) {
+            if (lane == 0) {
+                int it = 0, nd = 0;
+                for (int u = cl; u < total; u += ncl) {
+                    int dom, mt, nt, sp, kb0, kb1;
+                    decode(u, dom, mt, nt, sp, kb0, kb1);
+                    const ColTile ct = col_tile(q.cs, nt);
+                    const uint32_t id0 = instr_desc(FMT_BF16, 1, 1, 256, (uint32_t)ct.n0);
+                    const uint32_t id1 = instr_desc(FMT_BF16, 1, 1, 256, (uint32_t)(ct.n1 ? ct.n1 : 64));
+                    for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                        const bool first = (kb - kb0) % q.chain == 0;
+                        if (first) {
+                            mbar_wait(acc_empty, (nd & 1) ^ 1);
+                            tc_fence_after();
+                        }
+                        const int s = it % NST;
+                        mbar_wait(&conv[s], (it / NST) & 1);
+                        tc_fence_after();
+                        const uint32_t st = smem_u32(smem + s * SB);
+                        // MN-major BF16 chunks of [16 rows x 64 B]: chunk stride 1024, 8-row group stride 512
+                        const uint64_t da = smem_desc(st, PJ_BK * 64, 512, LAYOUT_SW64);
+                        const uint64_t dy0 = smem_desc(st + Y16OFF, PJ_BK * 64, 512, LAYOUT_SW64);
+                        umma_f16_2cta(tmem, da, dy0, id0, first ? 0u : 1u);
+                        if (ct.h1) {
+                            const uint64_t dy1 = smem_desc(st + Y16OFF + ct.h0 * (PJ_BK * 64), PJ_BK * 64, 512, LAYOUT_SW64);
+                            umma_f16_2cta(tmem + ct.n0, da, dy1, id1, first ? 0u : 1u);
+                        }
+                        umma_commit_2cta_mc(&empty[s], (uint16_t)3);
+                        if ((kb - kb0 + 1) % q.chain == 0 || kb + 1 == kb1) {
+                            umma_commit_2cta_mc(acc_full, (uint16_t)3);
+                            ++nd;
+                        }
+                    }
+                }
+            }
+        } else if (lane < PH_FWD) {
+            int it = 0;
+            for (int u = cl; u < total; u += ncl) {
+                int dom, mt, nt, sp, kb0, kb1;
+                decode(u, dom, mt, nt, sp, kb0, kb1);
+                for (int kb = kb0; kb < kb1; ++kb, ++it) {
+                    if (it % PH_FWD != lane) continue;
+                    const int s = it % NST;
+                    mbar_wait(&cdone[s], (it / NST) & 1);
+                    mbar_arrive_remote(&conv[s], 0);
+                }
+            }
+        }
+    } else {
+        const int t = threadIdx.x - 64;
+        const int quarter = warp % 4;
+        const int er = quarter * 32 + lane;
+        uint64_t *done = leader ? conv : cdone;
+        // thread t holds row r, 16-byte unit w of every FP32 chunk; logical float column c of that unit (32-byte-atom
+        // swizzle undone); its four BF16 go to row r of the BF16 chunk at bytes 2c .. 2c + 7, 16-byte units swizzled by
+        // (r >> 1) & 3 (64-byte swizzle)
+        const int r = (t >> 3) & 15, w = t & 7;
+        const int c = (((w >> 1) ^ (r & 3)) << 3) | ((w & 1) << 2);
+        const uint32_t dst_off = (uint32_t)(r * 64 + ((((c >> 3) ^ ((r >> 1) & 3))) << 4) + ((c >> 2) & 1) * 8);
+        int it = 0, nd = 0, slot = 0;
+        for (int u = cl; u < total; u += ncl) {
+            int dom, mt, nt, sp, kb0, kb1;
+            decode(u, dom, mt, nt, sp, kb0, kb1);
+            const ColTile ct = col_tile(q.cs, nt);
+            const int nch = ct.h0 + ct.h1;
+            const bool rows_live = q.P - mt * 256 - crank * 128 > 0;
+            for (int c0k = kb0; c0k < kb1; c0k += q.chain) {
+                const int c1k = min(c0k + q.chain, kb1);
+                for (int kb = c0k; kb < c1k; ++kb, ++it) {
+                    const int s = it % NST;
+                    mbar_wait(&full[s], (it / NST) & 1);
+                    uint8_t *st = smem + s * SB;
+                    const float4 *y4 = (const float4 *)(st + YOFF);
+                    const uint32_t y16 = smem_u32(st + Y16OFF) + dst_off;
+                    for (int j = 0; j < nch; ++j) {
+                        const float4 v = y4[j * 128 + t];
+                        sts2(y16 + j * (PJ_BK * 64), pack_bf16(v.x, v.y), pack_bf16(v.z, v.w));
+                    }
+                    fence_proxy_async_smem();
+                    mbar_arrive(&done[s]);
+                }
+                mbar_wait(acc_full, nd & 1);
+                ++nd;
+                tc_fence_after();
+                const bool add = c0k > kb0;
+                if (add && c0k == kb0 + q.chain && er == 0) bulk_wait<0>();
+                const int zrow = (dom * q.nsplit + sp) * q.prows + mt * 256 + crank * 128;
+                for (int cb = 0; cb < ct.width / 32; ++cb) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
+                    tmem_ld_wait();
+                    if (rows_live) epi_tile_out<2>(stage, slot, &map_z, ct.start + cb * 32, zrow, v, er, add);
+                }
+                tc_fence_before();
+                named_bar_sync(EPI_BAR, 128);
+                if (er == 0) mbar_arrive_remote(acc_empty, 0);
+            }
+        }
+        if (er == 0) bulk_wait<0>();
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc_2cta(tmem, 512);
+    }
+}
+
+// =================================================================================================
 // Back-application: Y[r][c] += sum_p A[r][p] * W[p][c].
 // CTA tile: 128 grid points x BN <= 448 columns (TMEM accumulator), K pipeline of 8 projector rows.
 // CTAs run as clusters of two on neighbouring row tiles: the W slab of a stage is the same for both, so
@@ -1083,6 +1325,148 @@ back2_tc_kernel(const __grid_constant__ CUtensorMap map_ahi, const __grid_consta
     }
 }
 
+// =================================================================================================
+// Opt-in low-precision back-application on CTA pairs: Y[r][c] += sum_p A16[r][p] * W16[p][c], BF16 x BF16 -> FP32
+// (tcgen05.mma.kind::f16).  beta is read as its stored BF16 copy (K-major [128 rows x 64 p] slabs, 128-byte swizzle,
+// four K = 16 steps per slab), W as the BF16 array the glue kernel wrote (MN-major 32-column chunks, 64-byte
+// swizzle).  With a sixth of the MMA work of 3xTF32 the kernel is bound by its HBM traffic (beta 2 bytes per element,
+// Y read-modify-write) and by the epilogue, which is the one of back2_tc_kernel.
+// =================================================================================================
+constexpr int BH_KB = 64;                               // projector rows per stage
+constexpr int BH_A_BYTES = 128 * 128;                   // [128 rows x 64 BF16]
+constexpr int BH_W_BYTES = 7 * BH_KB * 64;              // this CTA's half of the W slab: <= 224 columns
+constexpr int BH_STAGE_BYTES = BH_A_BYTES + BH_W_BYTES; // 44 KB
+constexpr int BH_STAGES = 4;
+constexpr int BH_SMEM = BH_STAGES * BH_STAGE_BYTES + 2 * EPI_TILE_BYTES + 1024 + 512;
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(BK_THREADS, 1)
+back2h_tc_kernel(const __grid_constant__ CUtensorMap map_a16, const __grid_constant__ CUtensorMap map_w0,
+                 const __grid_constant__ CUtensorMap map_w1, const __grid_constant__ CUtensorMap map_n0,
+                 const __grid_constant__ CUtensorMap map_n1, const __grid_constant__ CUtensorMap map_out, const BackParams q) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t *stage = smem + BH_STAGES * BH_STAGE_BYTES;
+    uint64_t *bars = (uint64_t *)(stage + 2 * EPI_TILE_BYTES);
+    uint64_t *full = bars, *empty = bars + BH_STAGES;
+    uint64_t *acc_full = bars + 2 * BH_STAGES, *acc_empty = acc_full + 1;
+    uint32_t *tmem_slot = (uint32_t *)(acc_empty + 1);
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    const int crank = (int)cluster_ctarank();
+    const bool leader = crank == 0;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < BH_STAGES; ++s) {
+            mbar_init(&full[s], 1);     // used in the leader: its own expect_tx arrive; both CTAs' TMA bytes land on it
+            mbar_init(&empty[s], 1);    // the leader's tcgen05.commit, multicast to both CTAs
+        }
+        mbar_init(acc_full, 1);
+        mbar_init(acc_empty, 2);
+        fence_barrier_init();
+        prefetch_tmap(&map_a16);
+        prefetch_tmap(&map_w0);
+        prefetch_tmap(&map_w1);
+        prefetch_tmap(&map_out);
+    }
+    if (warp == 1) tmem_alloc_2cta(tmem_slot, 512);
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const int nrt = q.ngrid / 128, nrp = (nrt + 1) / 2;
+    const int total = q.ndom * nrp * q.ntile_n;
+    const int ncl = gridDim.x / 2, cl = blockIdx.x / 2;
+    const int nk = (q.P + BH_KB - 1) / BH_KB;      // columns of beta16 / rows of W16 past P are zero (out-of-bounds fill / memset)
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int it = 0;
+            for (int u = cl; u < total; u += ncl) {
+                const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
+                const int row = dom * q.ngrid + rt * 128;
+                const ColTile ct = col_tile(q.cs, nt);
+                const int h0 = ct.h0, h1 = ct.h1;
+                const int ch0 = ct.start / 32 + crank * h0, ch1 = ct.start / 32 + ct.n0 / 32 + crank * h1;
+                const bool narrow = nt >= q.cs.wt;
+                const CUtensorMap *m0 = narrow ? &map_n0 : &map_w0, *m1 = narrow ? &map_n1 : &map_w1;
+                const uint32_t cta_bytes = BH_A_BYTES + (uint32_t)(h0 + h1) * BH_KB * 64;
+                for (int k = 0; k < nk; ++k, ++it) {
+                    const int s = it % BH_STAGES;
+                    mbar_wait(&empty[s], ((it / BH_STAGES) & 1) ^ 1);
+                    uint8_t *st = smem + s * BH_STAGE_BYTES;
+                    if (leader) mbar_expect_tx(&full[s], 2 * cta_bytes);
+                    const int wrow = dom * q.prows + k * BH_KB;
+                    tma_load_2d_2cta(st, &map_a16, &full[s], k * BH_KB, row);
+                    tma_load_3d_2cta(st + BH_A_BYTES, m0, &full[s], 0, wrow, ch0);
+                    if (h1) tma_load_3d_2cta(st + BH_A_BYTES + h0 * (BH_KB * 64), m1, &full[s], 0, wrow, ch1);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0 && leader) {
+            int it = 0, nu = 0;
+            for (int u = cl; u < total; u += ncl, ++nu) {
+                const ColTile ct = col_tile(q.cs, u % q.ntile_n);
+                const uint32_t id0 = instr_desc(FMT_BF16, 0, 1, 256, (uint32_t)ct.n0);
+                const uint32_t id1 = instr_desc(FMT_BF16, 0, 1, 256, (uint32_t)(ct.n1 ? ct.n1 : 64));
+                mbar_wait(acc_empty, (nu & 1) ^ 1);
+                tc_fence_after();
+                for (int k = 0; k < nk; ++k, ++it) {
+                    const int s = it % BH_STAGES;
+                    mbar_wait(&full[s], (it / BH_STAGES) & 1);
+                    tc_fence_after();
+                    const uint32_t st = smem_u32(smem + s * BH_STAGE_BYTES);
+                    const uint32_t wb = st + BH_A_BYTES;
+#pragma unroll
+                    for (int k16 = 0; k16 < BH_KB / 16; ++k16) {
+                        const uint32_t acc = (k > 0 || k16 > 0) ? 1u : 0u;
+                        // A: K-major, 128-byte rows, 8-row atoms of 1024 B; a K = 16 step is 32 B further along the row
+                        const uint64_t da = smem_desc(st + k16 * 32, 16, 1024, LAYOUT_SW128);
+                        // W: MN-major chunks of [64 rows x 64 B] (chunk stride 4096), 8-row groups of 512 B; 16 rows per step
+                        const uint64_t dw0 = smem_desc(wb + k16 * 1024, BH_KB * 64, 512, LAYOUT_SW64);
+                        umma_f16_2cta(tmem, da, dw0, id0, acc);
+                        if (ct.h1) {
+                            const uint64_t dw1 = smem_desc(wb + ct.h0 * (BH_KB * 64) + k16 * 1024, BH_KB * 64, 512, LAYOUT_SW64);
+                            umma_f16_2cta(tmem + ct.n0, da, dw1, id1, acc);
+                        }
+                    }
+                    umma_commit_2cta_mc(&empty[s], (uint16_t)3);
+                }
+                umma_commit_2cta_mc(acc_full, (uint16_t)3);
+            }
+        }
+    } else {
+        const int quarter = warp % 4;
+        const int er = quarter * 32 + lane;
+        int nu = 0, slot = 0;
+        for (int u = cl; u < total; u += ncl, ++nu) {
+            const int nt = u % q.ntile_n, rt = 2 * ((u / q.ntile_n) % nrp) + crank, dom = u / (q.ntile_n * nrp);
+            const int row0 = dom * q.ngrid + rt * 128;
+            const bool live = rt < nrt;
+            const ColTile ct = col_tile(q.cs, nt);
+            mbar_wait(acc_full, nu & 1);
+            tc_fence_after();
+            for (int cb = 0; cb < ct.width / 32; ++cb) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(quarter * 32) << 16) + cb * 32, v);
+                tmem_ld_wait();
+                if (live) epi_tile_out<2>(stage, slot, &map_out, ct.start + cb * 32, row0, v, er, true);
+            }
+            tc_fence_before();
+            named_bar_sync(EPI_BAR, 128);
+            if (er == 0) mbar_arrive_remote(acc_empty, 0);
+        }
+        if (er == 0) bulk_wait<0>();
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc_2cta(tmem, 512);
+    }
+}
+
 // column tiles of the projection: <= 224 columns each.  (An odd count leaves one CTA of the last cluster
 // without a tile; rounding up to an even count of narrower tiles measured slower on configs[4].)
 int proj_ntile_n(int N) { return (N + PJ_MAXBN - 1) / PJ_MAXBN; }
@@ -1129,13 +1513,14 @@ bool proj_tc_can_fuse_density(int P, int N, int nprod) {
 
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
                            const float *Y, int ldy, int N, float *zpart, int prows, int nsplit, int nprod,
-                           int chain, int *nlaunch, TmapCache *cache, float *rho, const float *occ) {
+                           int chain, int *nlaunch, TmapCache *cache, float *rho, const float *occ, const void *A16) {
     static DeviceOnce attr_set;      // the opt-in shared-memory size is a per-device function attribute
     if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(proj_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(proj_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, PJ_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(proj2_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(proj2_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(proj2h_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PH_SMEM);
         if (e != cudaSuccess) return e;
         attr_set.mark();
     }
@@ -1180,6 +1565,13 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
         const int total = ndom * q.ntile_m * q.ntile_n * nsplit;
         const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
         ++*nlaunch;
+        if (q.lowp && A16) {
+            // low-precision mode proper: beta from its BF16 copy, kind::f16 MMAs
+            CUtensorMap ma16;
+            if (!make_chunk16_map(cache, &ma16, A16, rows, lda, (lda + 31) / 32, PJ_BK, 4)) return cudaErrorInvalidValue;
+            proj2h_tc_kernel<<<grid, PJ_THREADS, PH_SMEM, st>>>(ma16, my0, my1, my0n, my1n, mz, q);
+            return cudaGetLastError();
+        }
         if (q.nprod == 3) proj2_tc_kernel<true><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, my0n, my1n, mz, q);
         else proj2_tc_kernel<false><<<grid, PJ_THREADS, P2_SMEM, st>>>(ma, my0, my1, my0n, my1n, mz, q);
         return cudaGetLastError();
@@ -1201,10 +1593,11 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
 
 cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A, const float *A_lo, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
-                           int *nlaunch, TmapCache *cache) {
+                           int *nlaunch, TmapCache *cache, const void *A16, const void *W16) {
     static DeviceOnce attr_set;
     if (!attr_set.done()) {
         cudaError_t e = cudaFuncSetAttribute(back_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, BK_SMEM);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(back2h_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, BH_SMEM);
         if (e != cudaSuccess) return e;
         attr_set.mark();
     }
@@ -1229,6 +1622,20 @@ cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     const int total = ndom * (int)((ngrid / 128 + 1) / 2) * q.ntile_n;   // cluster units (pairs of row tiles)
     const int grid = 2 * (total < num_sms() / 2 ? total : num_sms() / 2);
     ++*nlaunch;
+    if (q.lowp && A16 && W16 && N % 64 == 0) {
+        // low-precision mode proper: BF16 copies of beta and W, kind::f16 MMAs on CTA pairs
+        q.cs = choose_col_split(N);
+        const ColTile wide = col_tile(q.cs, 0), narrow = col_tile(q.cs, q.ntile_n - 1);
+        const uint64_t wrows = (uint64_t)ndom * prows;
+        CUtensorMap ma16, w0, w1, n0m, n1m;
+        if (!make_k64_map(cache, &ma16, A16, rows, lda, lda, 128)) return cudaErrorInvalidValue;
+        if (!make_chunk16_map(cache, &w0, W16, wrows, N, N / 32, BH_KB, wide.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk16_map(cache, &w1, W16, wrows, N, N / 32, BH_KB, wide.h1 ? wide.h1 : 1)) return cudaErrorInvalidValue;
+        if (!make_chunk16_map(cache, &n0m, W16, wrows, N, N / 32, BH_KB, narrow.h0)) return cudaErrorInvalidValue;
+        if (!make_chunk16_map(cache, &n1m, W16, wrows, N, N / 32, BH_KB, narrow.h1 ? narrow.h1 : 1)) return cudaErrorInvalidValue;
+        back2h_tc_kernel<<<grid, BK_THREADS, BH_SMEM, st>>>(ma16, w0, w1, n0m, n1m, mo, q);
+        return cudaGetLastError();
+    }
     // CTA pairs for the modes that take beta as (raw, stored remainder): 3xTF32 and the staged mode's two products;
     // one-product modes want beta ROUNDED (an unbiased operand), which the single-CTA kernel forms in shared memory
     if (N % 64 == 0 && !q.lowp && q.nprod >= 2 && A_lo) {

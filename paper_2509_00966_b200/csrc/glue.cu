@@ -55,6 +55,19 @@ __global__ void reduce_scale_kernel(int nproj, int beta_complex, int ld, int pro
     // low-precision mode: W rounded to BF16 (round-to-nearest-even), no remainder
     const float wre_h = lowp ? bf16_rne(wre) : tf32_hi(wre), wim_h = lowp ? bf16_rne(wim) : tf32_hi(wim);
     const float wre_l = lowp ? 0.f : wre - wre_h, wim_l = lowp ? 0.f : wim - wim_h;
+    if (lowp == 2) {
+        // low-precision mode proper: W as a BF16 array [dom][prows][N] (the kind::f16 back-application reads it by TMA)
+        unsigned short *w16 = (unsigned short *)what + (size_t)dom * prows * N;
+        const unsigned short re = (unsigned short)(__float_as_uint(wre_h) >> 16), im = (unsigned short)(__float_as_uint(wim_h) >> 16);
+        const unsigned short nim = (unsigned short)(im ^ 0x8000u);
+        if (!beta_complex) {
+            *(ushort2 *)(w16 + (size_t)p * N + 2 * n) = make_ushort2(re, im);
+        } else {
+            *(ushort2 *)(w16 + (size_t)(2 * p) * N + 2 * n) = make_ushort2(re, im);
+            *(ushort2 *)(w16 + (size_t)(2 * p + 1) * N + 2 * n) = make_ushort2(nim, re);
+        }
+        return;
+    }
     float *wd = what + (size_t)dom * prows * N;
     float *wl = what_lo + (size_t)dom * prows * N;
     if (!beta_complex) {
@@ -175,6 +188,17 @@ cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld,
     dim3 grid((norb + 127) / 128, norb, ndom);
     ++*nlaunch;
     overlap_epilogue_kernel<<<grid, 128, 0, st>>>(norb, ld, prows, nsplit, zpart, dv, S);
+    return cudaGetLastError();
+}
+
+// y = x rounded to BF16 (nearest even): the stored low-precision copy of the projectors (PAPER.md L239 float_to_BF16)
+__global__ void to_bf16_kernel(const float *__restrict__ x, unsigned short *__restrict__ y, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        y[i] = (unsigned short)(__float_as_uint(bf16_rne(x[i])) >> 16);
+}
+cudaError_t launch_to_bf16(cudaStream_t st, const float *x, void *y, size_t n, int *nlaunch) {
+    ++*nlaunch;
+    to_bf16_kernel<<<2368, 256, 0, st>>>(x, (unsigned short *)y, n);
     return cudaGetLastError();
 }
 

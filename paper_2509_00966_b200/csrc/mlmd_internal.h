@@ -209,25 +209,30 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
                            int chain /* 16-row stages per TMEM accumulation chain, 0 = whole slice */, int *nlaunch,
                            TmapCache *cache = nullptr,
                            float *rho = nullptr /* != NULL: also rho[dom][r] = sum_n occ[dom][n] |Y[r][n]|^2 (S3 fused) */,
-                           const float *occ = nullptr);
+                           const float *occ = nullptr,
+                           const void *A16 = nullptr /* nprod == 0: BF16 copy of A [rows][lda] -> kind::f16 kernel */);
 // whether that projection can carry the density (CTA-pair kernel, one row tile of projectors, one column tile)
 bool proj_tc_can_fuse_density(int P, int N, int nprod);
 cudaError_t launch_back_tc(cudaStream_t st, int ndom, long ngrid, const float *A /* raw FP32 */,
                            const float *A_lo /* A - trunc_tf32(A), or NULL: formed in shared memory */, int lda, int P,
                            const float *W_hi, const float *W_lo, float *Y, int ldy, int N, int prows, int nprod,
-                           int *nlaunch, TmapCache *cache = nullptr);
+                           int *nlaunch, TmapCache *cache = nullptr,
+                           const void *A16 = nullptr, const void *W16 = nullptr /* nprod == 0: BF16 copies -> kind::f16 kernel */);
 
 // ---- glue.cu ---------------------------------------------------------------------------------
 // S2b: reduce split-K partials in fixed order and build What = (-i tau) D' C in real-GEMM form.
 cudaError_t launch_reduce_scale(cudaStream_t st, int ndom, int nproj, int beta_complex, int ld, int prows,
                                 int nsplit, const float *zpart, const float *dprime, float tau,
-                                float *what, float *what_lo, int lowp /* round W to BF16 */, int *nlaunch);
+                                float *what, float *what_lo, int lowp /* 1: round W to BF16 in FP32 containers; 2: write W as a
+                                BF16 array [prows][2 ld] into `what` */, int *nlaunch);
 // S3: rho[dom][r] = sum_n occ[dom][n] |psi[dom][r][n]|^2
 cudaError_t launch_density(cudaStream_t st, int ndom, long ngrid, int ld, const float2 *psi, const float *occ,
                            float *rho, int *nlaunch);
 // S4 epilogue: S[dom][m][n] = dv * (sum over splits of the complex combination of Z)
 cudaError_t launch_overlap_epilogue(cudaStream_t st, int ndom, int norb, int ld, int prows, int nsplit,
                                     const float *zpart, float dv, float2 *S, int *nlaunch);
+// y (BF16, round-to-nearest-even) = x
+cudaError_t launch_to_bf16(cudaStream_t st, const float *x, void *y, size_t n, int *nlaunch);
 // lo = x - (x with the 13 low mantissa bits cleared): the part of x a kind::tf32 operand drops (exact in FP32); x is kept
 cudaError_t launch_tf32_remainder(cudaStream_t st, const float *x, float *lo, size_t n, int *nlaunch);
 cudaError_t launch_max_abs(cudaStream_t st, const float *x, size_t n, int *flag_bits, int *nlaunch);
