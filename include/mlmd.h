@@ -207,6 +207,25 @@ MLMD_API int mlmd_gemm_path(const mlmd_domain_t *h);
 /* Number of kernels the library launched on this handle since create (bench.py's gpu_launches). */
 MLMD_API long long mlmd_launch_count(const mlmd_domain_t *h);
 
+/* Squared norms of all orbitals WITHOUT a handle, a workspace or any allocation, for callers that cannot call
+ * cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it):
+ *     norm2[dom][n] = dv * sum_r |psi[dom][r][n]|^2
+ * (the per-orbital norms that the kick of PAPER.md Eq. (2) L138 divides by, reading D27; the diagonal of mlmd_overlap's
+ * Gram matrix; sum_n f_n norm2[n] = the electron count of the density).  Same kernel pair as the split step's norm pass,
+ * but its per-slab FP64 partial sums live in a file-scope device array of MLMD_STATIC_SCRATCH_BYTES that every GPU
+ * loading the library holds until the process exits, instead of in a caller workspace.
+ *   psi     DEVICE, complex64 [ndom][ngrid][ld], orbital index fastest (ld = row pitch in complex elements; padded
+ *           columns are summed like any other)           norm2   DEVICE, double [ndom][ld]
+ *   stream  cudaStream_t the two kernels are enqueued on (NULL = default stream); the call is asynchronous
+ * Limit: ndom * 64 * ld * 8 bytes <= MLMD_STATIC_SCRATCH_BYTES (configs[3], 64 x 224, fits), ndom <= 65535; anything
+ * larger -> MLMD_ERR_SHAPE with the sizes in mlmd_last_error().  Host pointers -> MLMD_ERR_ARG.  Calls no cudaMalloc,
+ * cudaFree or allocating library routine.  All calls share the one array: calls that overlap on the GPU (two streams)
+ * race on it - serialise them on one stream.  Nothing needs clearing between calls (every partial sum that is read has
+ * been written by the same call). */
+#define MLMD_STATIC_SCRATCH_BYTES (8u << 20)
+MLMD_API int mlmd_orbital_norms_static(const void *psi_c64, int ndom, long long ngrid, int ld, double dv, double *norm2,
+                                       void *stream);
+
 /* Thread-local description of the last failure in this thread; never NULL. */
 MLMD_API const char *mlmd_last_error(void);
 

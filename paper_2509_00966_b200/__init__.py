@@ -22,6 +22,7 @@ from .api import (  # noqa: F401
     mlmd_propagate_split,
     mlmd_density,
     mlmd_overlap,
+    mlmd_orbital_norms_static,
     mlmd_occupations,
     mlmd_energy_nl,
     mlmd_current,

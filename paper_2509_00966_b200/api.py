@@ -27,7 +27,7 @@ EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",
     "mlmd_get_orbitals", "mlmd_set_vloc", "mlmd_set_projectors", "mlmd_set_gemm_mode", "mlmd_set_option", "mlmd_propagate",
     "mlmd_propagate_split", "mlmd_occupations", "mlmd_energy_nl", "mlmd_current", "mlmd_current_nl",
-    "mlmd_density", "mlmd_overlap", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
+    "mlmd_density", "mlmd_overlap", "mlmd_orbital_norms_static", "mlmd_launch_count", "mlmd_last_error", "mlmd_profile", "mlmd_profile_read", "mlmd_gemm_path",
 ]
 K_STENCIL, K_PROJ, K_BACK, K_GLUE, K_DENSITY, K_NLP, K_NORM = range(7)
 KERNEL_CLASSES = ["stencil", "proj", "back", "glue", "density", "nlp", "norm"]
@@ -65,6 +65,7 @@ def lib() -> ctypes.CDLL:
         L.mlmd_propagate_split.argtypes = [p, i, d, p, i]
         L.mlmd_density.argtypes = [p, p, i]
         L.mlmd_overlap.argtypes = [p, i, p, i]
+        L.mlmd_orbital_norms_static.argtypes = [p, i, ctypes.c_longlong, i, d, p, p]
         L.mlmd_occupations.argtypes = [p, p, p, i]
         L.mlmd_energy_nl.argtypes = [p, p, i]
         L.mlmd_current.argtypes = [p, p, i, p, i]
@@ -199,6 +200,19 @@ def mlmd_density(h, out):
 def mlmd_overlap(h, which, out):
     p, where = _ptr_where(out, np.dtype(np.complex64))
     _check(lib().mlmd_overlap(h, which, p, where))
+    return out
+
+
+def mlmd_orbital_norms_static(psi, dv, out, stream_ptr=0):
+    """norm2[dom][n] = dv sum_r |psi[dom][r][n]|^2 with no handle, workspace or allocation (include/mlmd.h).
+    psi: CUDA tensor complex64 [ndom, ngrid, ld]; out: CUDA tensor float64 [ndom, ld] (the caller's); returns out."""
+    if psi.dim() != 3 or tuple(out.shape) != (psi.shape[0], psi.shape[2]):
+        raise ValueError("psi must be [ndom, ngrid, ld] and out [ndom, ld]")
+    pp, wp = _ptr_where(psi, np.dtype(np.complex64))
+    po, wo = _ptr_where(out, np.dtype(np.float64))
+    if wp != DEVICE or wo != DEVICE:
+        raise ValueError("psi and out must be CUDA tensors")
+    _check(lib().mlmd_orbital_norms_static(pp, psi.shape[0], psi.shape[1], psi.shape[2], float(dv), po, ctypes.c_void_p(stream_ptr)))
     return out
 
 

@@ -35,6 +35,16 @@ static int fail(int code, const char *fmt, ...) {
     va_end(ap);
     return code;
 }
+// the same for the library's other translation units (noalloc.cu)
+namespace mlmd {
+int set_error(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+}  // namespace mlmd
 #define CU(call)                                                                                    \
     do {                                                                                            \
         cudaError_t e__ = (call);                                                                   \

@@ -52,6 +52,15 @@ HOOK int mlmd_debug_fused_density(mlmd_domain_t *h, float *rho_dev) {
     return (int)e;
 }
 
+// The split step's norm pass as the library runs it, with its partial sums in CALLER scratch part[ndom][64][ld] (device):
+// out[dom][c] = sum_r |psi[dom][r][c]|^2 (no dv).  The existing path that mlmd_orbital_norms_static is checked against.
+HOOK int mlmd_debug_colnorm2(void *stream, int ndom, long ngrid, int ld, const void *psi, double *part, double *out) {
+    int nl = 0;
+    cudaError_t e = launch_colnorm2((cudaStream_t)stream, ndom, ngrid, ld, (const float2 *)psi, part, out, &nl);
+    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+    return (int)e;
+}
+
 HOOK int mlmd_debug_nsplit(int ndom, long ngrid, int P, int N) { return tc_choose_nsplit(ndom, ngrid, P, N); }
 
 }  // extern "C"
