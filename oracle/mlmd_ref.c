@@ -252,8 +252,75 @@ int mlmd_ref_propagate(int ndom, int nx, int ny, int nz, double hx, double hy, d
  *        K psi_n = (psi_n - i dt/2 v_nl psi_n) * ||psi_n|| / ||psi_n - i dt/2 v_nl psi_n||.
  *   D28: exp(-i dt h_loc) is the same 4th-order Taylor sum as the full-H step, applied to h_loc
  *        alone (the paper's own local solver is only named, L147; NEXT-3).
- * kick_only != 0 skips the local propagator (pin S3).
+ * kick_only is a bit mask: 1 skips the local propagator (pin S3); 2 evaluates exp(-i dt h_loc) by the paper's own
+ * block-diagonal split-operator solver on 2nd-order differences (reading D33) instead of the Taylor sum.
  */
+/* ---- the paper's own local solver: block-diagonal split-operator (reading D33) ----
+ *
+ * PAPER.md L147 (A.5): exp(-i dt h_loc) is evaluated by "data-parallel local Hamiltonian-dynamics solvers that perform
+ * uniform operations on nearest-neighbor mesh points: (1) a block-diagonal split-operator solver for electronic wave
+ * functions [41]" (Richardson 1991); L283: "7-point star stencil (on which local computation is based)".  The paper
+ * prints no formula; reading D33 restates the published space-splitting scheme on the operator of reading D32:
+ *
+ *   h_loc = sum_d T_d + V_loc + 1/2|A|^2,   (T_d u)_j = a_d u_j + b_d u_{j+1} + conj(b_d) u_{j-1}   (periodic in j),
+ *   a_d = 1/h_d^2,  b_d = -1/(2 h_d^2) - i A_d/(2 h_d)        (-1/2 D2 - i A.D1 with 2nd-order central differences)
+ *   T_d = E_d + O_d:  E_d couples the pairs (j, j+1) with j even, O_d those with j odd (the last pair wraps: n_d even);
+ *   on its pair each is the 2 x 2 block [[a_d/2, b_d], [conj(b_d), a_d/2]], whose exponential is closed-form:
+ *   exp(-i tau block) = e^{-i tau a_d/2} [[cos(tau|b|), -i u sin(tau|b|)], [-i conj(u) sin(tau|b|), cos(tau|b|)]], u = b/|b|
+ *
+ *   U_loc(dt) = P(dt/2)  S_x S_y S_z  P(dt/2),   S_d = e^{-i dt/2 E_d} e^{-i dt O_d} e^{-i dt/2 E_d},
+ *   P(tau) = exp(-i tau (V_loc(r) + 1/2|A|^2))  (a phase per grid point).
+ * Every factor is unitary (any dt), the product is symmetric (S_x, S_y, S_z act along different axes and commute), so
+ * U_loc(-dt) U_loc(dt) = 1 and the error per step is O(dt^3).  Returns 2 if an axis has an odd number of points.
+ * Pins: tests/test_oracle_richardson_pins.py (dense expm of every factor, E + O = the pinned 2nd-order operator,
+ * unitarity for any dt, time reversal, order of convergence).
+ */
+static void pair_sweep(zc *p, int nx, int ny, int nz, int norb, int axis, int parity, double tau, double a, zc b) {
+    const int n[3] = {nx, ny, nz};
+    const long stride[3] = {(long)ny * nz * norb, (long)nz * norb, (long)norb};
+    const double mb = cabs(b);
+    const zc u = b / mb;
+    const double c = cos(tau * mb), s = sin(tau * mb);
+    const zc ph = cexp(-I * tau * a * 0.5);
+    const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
+    for (int j = parity; j < n[axis]; j += 2) {
+        const int jn = (j + 1) % n[axis];
+        for (int i1 = 0; i1 < n[o1]; ++i1)
+            for (int i2 = 0; i2 < n[o2]; ++i2) {
+                zc *q0 = p + j * stride[axis] + i1 * stride[o1] + i2 * stride[o2];
+                zc *q1 = p + jn * stride[axis] + i1 * stride[o1] + i2 * stride[o2];
+                for (int m = 0; m < norb; ++m) {
+                    const zc v0 = q0[m], v1 = q1[m];
+                    q0[m] = ph * (c * v0 - I * u * s * v1);
+                    q1[m] = ph * (-I * conj(u) * s * v0 + c * v1);
+                }
+            }
+    }
+}
+
+int mlmd_ref_local_richardson(int nx, int ny, int nz, double hx, double hy, double hz, int norb, zc *psi,
+                              const double *vloc, const double *Av, double dt) {
+    if (nx % 2 || ny % 2 || nz % 2) return 2;
+    const long ngrid = (long)nx * ny * nz;
+    const double hh[3] = {hx, hy, hz};
+    const double a2 = 0.5 * (Av[0] * Av[0] + Av[1] * Av[1] + Av[2] * Av[2]);
+    for (int half = 0; half < 2; ++half) {
+        for (long r = 0; r < ngrid; ++r) {
+            const zc f = cexp(-I * (0.5 * dt) * (vloc[r] + a2));
+            for (int m = 0; m < norb; ++m) psi[r * norb + m] *= f;
+        }
+        if (half == 1) break;
+        for (int d = 0; d < 3; ++d) {
+            const double a = 1.0 / (hh[d] * hh[d]);
+            const zc b = -0.5 / (hh[d] * hh[d]) - I * Av[d] / (2.0 * hh[d]);
+            pair_sweep(psi, nx, ny, nz, norb, d, 0, 0.5 * dt, a, b);
+            pair_sweep(psi, nx, ny, nz, norb, d, 1, dt, a, b);
+            pair_sweep(psi, nx, ny, nz, norb, d, 0, 0.5 * dt, a, b);
+        }
+    }
+    return 0;
+}
+
 static double col_norm2(const zc *u, long ngrid, int norb, int n) {
     double s = 0.0;
     for (long r = 0; r < ngrid; ++r) {
@@ -302,7 +369,10 @@ int mlmd_ref_propagate_split(int ndom, int nx, int ny, int nz, double hx, double
         for (int step = 0; step < nsteps && !rc; ++step) {
             const double *Av = A + ((size_t)step * a_ndom + (a_ndom == 1 ? 0 : dom)) * 3;
             if (nproj > 0) rc = half_kick(nx, ny, nz, hx, hy, hz, norb, nproj, p, hphi, v, b, d, Av, dt);
-            if (!kick_only && !rc) {
+            if (!(kick_only & 1) && (kick_only & 2) && !rc) {
+                /* reading D33: the paper's own local solver (block-diagonal split-operator, 2nd-order differences) */
+                rc = mlmd_ref_local_richardson(nx, ny, nz, hx, hy, hz, norb, p, v, Av, dt);
+            } else if (!(kick_only & 1) && !rc) {
                 /* phi_0 = psi; phi_m = (-i dt/m) h_loc phi_{m-1}; psi_new = sum_{m=0..4} phi_m */
                 memcpy(phi, p, ne * sizeof(zc));
                 memcpy(acc, p, ne * sizeof(zc));

@@ -38,6 +38,8 @@ def lib() -> ctypes.CDLL:
         _lib.mlmd_ref_propagate.restype = i
         _lib.mlmd_ref_propagate_split.argtypes = [i, i, i, i, d, d, d, i, i, p, p, p, p, p, i, d, p, i, p, i]
         _lib.mlmd_ref_propagate_split.restype = i
+        _lib.mlmd_ref_local_richardson.argtypes = [i, i, i, d, d, d, i, p, p, p, d]
+        _lib.mlmd_ref_local_richardson.restype = i
         _lib.mlmd_ref_occupations.argtypes = [i, i, p, p, p, p]
         _lib.mlmd_ref_occupations.restype = i
         _lib.mlmd_ref_energy_nl.argtypes = [i, l, i, i, d, p, p, p, p, p]
@@ -106,9 +108,11 @@ def propagate(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], nsteps:
 
 
 def propagate_split(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], nsteps: Optional[int] = None,
-                    kick_only: bool = False) -> Tuple[np.ndarray, np.ndarray]:
-    """nsteps steps of the paper's literal Eq. (2): half-kick, Taylor-4 of h_loc, half-kick.
-    Same arguments and return values as ``propagate``."""
+                    kick_only: bool = False, local: str = "taylor") -> Tuple[np.ndarray, np.ndarray]:
+    """nsteps steps of the paper's literal Eq. (2): half-kick, exp(-i dt h_loc), half-kick.  local = "taylor": the
+    4th-order Taylor sum on 4th-order differences (reading D28); "richardson": the paper's own block-diagonal
+    split-operator solver on 2nd-order differences (reading D33).  Same arguments and return values as ``propagate``."""
+    assert local in ("taylor", "richardson")
     p = _c128(psi).copy()
     ndom, nx, ny, nz, norb = p.shape
     vloc = _f64(vloc)
@@ -123,10 +127,21 @@ def propagate_split(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], n
     rho = np.empty((ndom, nx, ny, nz), dtype=np.float64)
     rc = lib().mlmd_ref_propagate_split(ndom, nx, ny, nz, h[0], h[1], h[2], norb, nproj, _ptr(p), _ptr(occ),
                                         _ptr(vloc), _ptr(b), _ptr(dd), nsteps, dt, _ptr(A), A.shape[1], _ptr(rho),
-                                        1 if kick_only else 0)
+                                        (1 if kick_only else 0) | (2 if local == "richardson" else 0))
     if rc:
         raise RuntimeError("mlmd_ref_propagate_split failed: %d" % rc)
     return p, rho
+
+
+def local_richardson(psi, vloc, A, dt: float, h: Sequence[float]) -> np.ndarray:
+    """One application of U_loc(dt) of reading D33 to psi [nx, ny, nz, norb] (one domain); A: [3]."""
+    p = _c128(psi).copy()
+    nx, ny, nz, norb = p.shape
+    v, a = _f64(vloc), _f64(A)
+    rc = lib().mlmd_ref_local_richardson(nx, ny, nz, h[0], h[1], h[2], norb, _ptr(p), _ptr(v), _ptr(a), dt)
+    if rc:
+        raise RuntimeError("mlmd_ref_local_richardson failed: %d" % rc)
+    return p
 
 
 def density(psi, occ) -> np.ndarray:
