@@ -96,7 +96,14 @@ enum {
                              * PAPER.md L147, L283): c2 = [1, -2, 1] / h^2, c1 = [-1/2, 0, 1/2] / h.
                              * mlmd_propagate, mlmd_propagate_split and mlmd_current follow it; the stability bound of
                              * mlmd_propagate becomes dt [ 2 sum_d 1/h_d^2 + sum_d |A_d|/h_d + ... ]                    */
-    MLMD_OPT_COUNT = 5
+    MLMD_OPT_LOCAL_SOLVER = 5, /* how mlmd_propagate_split evaluates exp(-i dt h_loc) in Eq. (2): 0 (default) the 4th-order
+                             * Taylor sum on the differences MLMD_OPT_FD_ORDER selects (reading D28); 1 the paper's own
+                             * "block-diagonal split-operator solver" (ref. [41]; reading
+                             * D33): space splitting of the 2nd-order (7-point) operator into 2 x 2 nearest-neighbour blocks,
+                             * exp(-i dt/2 (V + 1/2|A|^2)) prod_d [even(dt/2) odd(dt) even(dt/2)] exp(-i dt/2 (V + 1/2|A|^2)):
+                             * unitary for any dt, time-reversible, O(dt^3) per step.  Needs even nx, ny, nz (<= 256 each),
+                             * else MLMD_ERR_SHAPE.  mlmd_propagate (Taylor-4 of the full H) ignores it.               */
+    MLMD_OPT_COUNT = 6
 };
 
 /* Bytes of device workspace mlmd_domain_create needs for this shape (0 on invalid arguments).

@@ -36,6 +36,6 @@ from .api import (  # noqa: F401
     HOST, DEVICE, BETA_REAL32, BETA_COMPLEX64,
     GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT, GEMM_FP32GRADE_STAGED,
     KEEP_PSI0, CHECK_FINITE, BORROW_PSI,
-    OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM, OPT_FD_ORDER,
+    OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM, OPT_FD_ORDER, OPT_LOCAL_SOLVER,
     OK, WARN_UNSTABLE,
 )

@@ -21,7 +21,7 @@ HOST, DEVICE = 0, 1
 BETA_REAL32, BETA_COMPLEX64 = 0, 1
 GEMM_FP32GRADE, GEMM_FP64, GEMM_LOWP_BF16, GEMM_TF32X1, GEMM_FP32_SIMT, GEMM_FP32GRADE_STAGED = range(6)
 KEEP_PSI0, CHECK_FINITE, BORROW_PSI = 1, 2, 4
-OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM, OPT_FD_ORDER = range(5)
+OPT_GRAPH, OPT_STENCIL, OPT_GEMM_PATH, OPT_KICK_NORM, OPT_FD_ORDER, OPT_LOCAL_SOLVER = range(6)
 
 EXPORTED_SYMBOLS = [
     "mlmd_workspace_bytes", "mlmd_domain_create", "mlmd_domain_destroy", "mlmd_set_orbitals",

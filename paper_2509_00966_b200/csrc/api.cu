@@ -164,6 +164,7 @@ int mlmd_domain_create(mlmd_domain_t **out, int ndom, int nx, int ny, int nz, do
     for (int k = 0; k < MLMD_OPT_COUNT; ++k) h->opt[k] = 0;
     h->opt[MLMD_OPT_GRAPH] = 1;
     h->opt[MLMD_OPT_FD_ORDER] = 4;
+    h->coef_o2 = false;
     h->psi_ptr = (flags & MLMD_BORROW_PSI) ? nullptr : (float2 *)(h->ws + pl.off.psi);
     h->have_psi = h->have_vloc = h->have_occ = false; h->field_yz = false; h->rho_valid = false;
     h->vmax = h->dmax = 0.0; h->launches = 0;
@@ -402,7 +403,7 @@ int mlmd_set_gemm_mode(mlmd_domain_t *h, int mode) {
 
 int mlmd_set_option(mlmd_domain_t *h, int key, int value) {
     if (!h) return fail(MLMD_ERR_ARG, "mlmd_set_option: NULL handle");
-    static const int nvalues[MLMD_OPT_COUNT] = {2, 3, 2, 2, 0};
+    static const int nvalues[MLMD_OPT_COUNT] = {2, 3, 2, 2, 0, 2};
     if (key < 0 || key >= MLMD_OPT_COUNT) return fail(MLMD_ERR_ARG, "mlmd_set_option: unknown key %d", key);
     if (key == MLMD_OPT_FD_ORDER) {
         if (value != 2 && value != 4) return fail(MLMD_ERR_ARG, "mlmd_set_option: MLMD_OPT_FD_ORDER takes 2 or 4, got %d", value);
@@ -577,7 +578,7 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
     // 7-point star (MLMD_OPT_FD_ORDER = 2) written on the same offsets with zero j = 2 weights
     static const double c2_o4[2] = {4.0 / 3.0, -1.0 / 12.0}, c1_o4[2] = {2.0 / 3.0, -1.0 / 12.0};   // j = 1, 2
     static const double c2_o2[2] = {1.0, 0.0}, c1_o2[2] = {0.5, 0.0};
-    const bool o2 = h->opt[MLMD_OPT_FD_ORDER] == 2;
+    const bool o2 = h->opt[MLMD_OPT_FD_ORDER] == 2 || h->coef_o2;
     const double *c2 = o2 ? c2_o2 : c2_o4, *c1 = o2 ? c1_o2 : c1_o4;
     const double c2_0 = o2 ? -2.0 : -5.0 / 2.0;
     const double hh[3] = {h->hx, h->hy, h->hz};
@@ -744,6 +745,22 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         int rc = kick_only();
         if (rc) return rc;
     }
+    if (h->opt[MLMD_OPT_LOCAL_SOLVER] == 1) {
+        // the paper's own local solver (reading D33): three in-place passes of 2 x 2 nearest-neighbour rotations; the
+        // squared norms before and after it (the kicks' normalisation, reading D27) are measured by the norm pass
+        if (kicks) {
+            int rc = norm2(1);
+            if (rc) return rc;
+        }
+        {
+            ProfScope ps(h, MLMD_K_STENCIL);
+            CU(launch_richardson(h, h->psi(), coef, dt, nl));
+        }
+        if (kicks) {
+            int rc = norm2(2);
+            if (rc) return rc;
+        }
+    } else {
     // Taylor-4 of h_loc (Horner form).  With kicks, the first stage also sums |psi_a|^2 (its input) and the last
     // |psi_c|^2 (its output) per orbital: the norms ride on passes that read or write those arrays anyway.
     const float2 *src[4] = {h->psi(), h->ua(), h->ub(), h->ua()};
@@ -756,6 +773,7 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
                                          h->nrm(i == 0 ? 1 : 2), nl));
         else
             CU(launch_stencil_stage(h, src[i], h->psi(), dst[i], coef, coef_host, tau, nl));
+    }
     }
     if (!kicks) {
         ProfScope ps(h, MLMD_K_DENSITY);
@@ -817,6 +835,13 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
     if (!h->have_psi || !h->have_vloc) return fail(MLMD_ERR_STATE, "%s: call mlmd_set_orbitals and mlmd_set_vloc first", fn);
     // a-priori stability bound of Taylor-4 (reading D14): dt * |lambda|max(H) <= 2 sqrt(2); in the split step the
     // Taylor sum acts on h_loc only and the normalised kick is stable for any dt |D|
+    // the paper's own local solver (MLMD_OPT_LOCAL_SOLVER = 1, reading D33) works on the 2nd-order operator whatever
+    // MLMD_OPT_FD_ORDER says, pairs neighbouring points on every periodic axis and is unitary for any dt
+    const bool rich = split && h->opt[MLMD_OPT_LOCAL_SOLVER] == 1;
+    if (rich && !richardson_supported(h))
+        return fail(MLMD_ERR_SHAPE, "%s: the split-operator local solver needs even nx, ny, nz (<= 256 each), got %d x %d x %d", fn,
+                    h->nx, h->ny, h->nz);
+    h->coef_o2 = rich;
     bool yz = false;
     double bound = 0.0;
     for (size_t i = 0; i < (size_t)nsteps * a_ndom; ++i) {
@@ -829,7 +854,7 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
         const double b = (o2 ? 2.0 : 8.0 / 3.0) * (1 / (h->hx * h->hx) + 1 / (h->hy * h->hy) + 1 / (h->hz * h->hz)) +
                          (o2 ? 1.0 : 1.3722) * (fabs(a[0]) / h->hx + fabs(a[1]) / h->hy + fabs(a[2]) / h->hz) +
                          0.5 * (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) + h->vmax + (h->nproj && !split ? h->dmax : 0.0);
-        bound = std::max(bound, b);
+        bound = std::max(bound, rich ? 0.0 : b);
     }
     h->field_yz = yz;
     int nl = 0;

@@ -93,6 +93,7 @@ struct mlmd_domain {
     bool tc_ok;                 // shape and device allow the tcgen05 GEMM kernels
     int gemm_mode;
     int opt[MLMD_OPT_COUNT];    // mlmd_set_option values
+    bool coef_o2;               // the call in flight takes 2nd-order weights whatever MLMD_OPT_FD_ORDER says (split-operator solver)
     float2 *psi_ptr;            // Psi: inside the workspace, or the caller's buffer (MLMD_BORROW_PSI)
     mutable mlmd::TmapCache tmaps;
     bool have_psi, have_vloc, have_occ, rho_valid;
@@ -184,6 +185,12 @@ cudaError_t launch_stencil_tma(const mlmd_domain *h, const float2 *w, const floa
 // norm_mode 1 / 2: the pass also writes per-CTA partial sums of |w|^2 / |out|^2 per orbital into
 // npart[dom][slot][ld], slot < stencil_tma_norm_slots(h) (split step, reading D27)
 int stencil_tma_norm_slots(const mlmd_domain *h);
+
+// ---- richardson.cu ---------------------------------------------------------------------------
+// The paper's own local solver (MLMD_OPT_LOCAL_SOLVER = 1; reading D33): psi <- U_loc(dt) psi in place, three passes
+// (one per axis); coef: this step's device coefficients [ndom] with the 2nd-order weights.
+bool richardson_supported(const mlmd_domain *h);
+cudaError_t launch_richardson(const mlmd_domain *h, float2 *psi, const StepCoef *coef, double dt, int *nlaunch);
 
 // ---- gemm_simt.cu ----------------------------------------------------------------------------
 // Projection (S2a): zpart[dom][s][p][c] = sum_{r in slice s} B[dom][r][p] * Y[dom][r][c]
