@@ -32,7 +32,10 @@ PAPER_CONTEXT = {
 }
 MODE_NAMES = {"fp32grade": 0, "fp64": 1, "bf16": 2, "tf32x1": 3, "simt": 4, "staged": 5}
 CPU_STEPS = 8            # timed oracle steps of the cpu_baseline leg
-STEP_NAMES = {"taylor": "Taylor-4 (full H, north_star)", "split": "Eq. (2) split (half-kick, Taylor-4 of h_loc, half-kick)"}
+STEP_NAMES = {"taylor": "Taylor-4 (full H, north_star)", "split": "Eq. (2) split (half-kick, Taylor-4 of h_loc, half-kick)",
+              "richardson": "Eq. (2) split with the paper's own local solver (half-kick, block-diagonal split-operator on the "
+                            "7-point operator, half-kick)"}
+SPLIT_STEPS = ("split", "richardson")
 # tensor peak as a multiple of the measured dense BF16 peak (B200_PROFILING.md nominal ratios:
 # tf32 1.1 PF vs bf16 2.25 PF); 3xTF32 issues three TF32 MMAs per product.
 # the opt-in low-precision mode stores beta and W as BF16 and issues tcgen05.mma.kind::f16: the BF16 peak itself
@@ -95,9 +98,10 @@ def algorithmic(c, gemm_real=True, step="taylor"):
     CALL for the incoming norms and one 16 B/element rescaling pass per CALL are not counted: inside a call psi stays
     un-normalised and the density takes the scale through the occupations)."""
     elems = c.ndom * c.ngrid * c.norb
-    stage_bytes = [16, 24, 24, 24]
-    split = step == "split"
-    density_b, norm_b, ngemm = (8, 0, 4) if split else (8, 0, 8)
+    # "richardson": three in-place passes (one per axis) and the two norm passes around them
+    stage_bytes = [16, 16, 16] if step == "richardson" else [16, 24, 24, 24]
+    split = step in SPLIT_STEPS
+    density_b, norm_b, ngemm = (8, 16 if step == "richardson" else 0, 4) if split else (8, 0, 8)
     bytes_step = elems * (sum(stage_bytes) + density_b + norm_b) + c.ndom * c.ngrid * (4 * 4 + 4)
     gemm_flops_each = (2 if gemm_real else 4) * 2.0 * c.ndom * c.ngrid * c.nproj * c.norb   # one GEMM batch
     return {"elems": elems, "bytes_step": bytes_step, "stencil_bytes": [elems * b for b in stage_bytes],
@@ -135,7 +139,11 @@ def sample_for_oracle(c, d, norb_sample):
 
 def time_oracle(c, s, A, steps, warmup, step="taylor"):
     from oracle import ref
-    prop = ref.propagate_split if step == "split" else ref.propagate
+    if step == "richardson":
+        def prop(*a):
+            return ref.propagate_split(*a, local="richardson")
+    else:
+        prop = ref.propagate_split if step == "split" else ref.propagate
     for _ in range(warmup):
         prop(s["psi"], s["occ"], s["vloc"], s["beta"], s["D"], A[:1], c.dt, c.h)
     t0 = time.perf_counter()
@@ -252,7 +260,9 @@ def main():
     dom.set_orbitals(psi_dev, occ)
     del beta_dev
     stream = dom.stream
-    propagate = dom.propagate_split if args.step == "split" else dom.propagate
+    propagate = dom.propagate_split if args.step in SPLIT_STEPS else dom.propagate
+    if args.step == "richardson":
+        dom.set_option(M.OPT_LOCAL_SOLVER, 1)
     flush = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device=dev) if alg["elems"] * 8 < 4e8 else None
 
     def barrier():
@@ -329,7 +339,7 @@ def main():
         e2e = {"value": electrons * K / sec, "unit": "electron-steps/s", "h2d_bytes_per_step": int(vnp.nbytes + 24),
                "d2h_bytes_per_step": int(rnp.nbytes), "ms_per_step": sec / K * 1e3,
                "what": "per step: mlmd_set_vloc(host pinned) + %s(1, A host) + mlmd_density(host pinned); " % (
-                   "mlmd_propagate_split" if args.step == "split" else "mlmd_propagate") +
+                   "mlmd_propagate_split" if args.step in SPLIT_STEPS else "mlmd_propagate") +
                        "Psi stays device-resident as in the paper's shadow dynamics (L130-132, L145)"}
 
     # ---- on-request observables (NEXT rows of SURVEY.md 8(f)): device time of one call each, CUDA events
@@ -386,7 +396,7 @@ def main():
 
     # ---- roofline of the dominant kernel class and of the whole step
     mode = args.gemm_mode
-    if mode == "staged" and args.step == "split":
+    if mode == "staged" and args.step in SPLIT_STEPS:
         mode = "fp32grade"      # the staged mode only changes mlmd_propagate's inner Horner stages
     tensor_peak_sus = peaks["bf16_sustained"] * TENSOR_RATIO.get(mode, TENSOR_RATIO["fp32grade"])
     tensor_peak_burst = peaks["bf16_burst"] * TENSOR_RATIO.get(mode, TENSOR_RATIO["fp32grade"])
@@ -396,7 +406,8 @@ def main():
         avg = kms / n
         entry = {"ms_total": kms, "launches": n, "ms_avg": avg, "share": kms / total_kernel_ms}
         if name == "stencil":
-            b = sum(alg["stencil_bytes"]) / 4.0
+            # the Taylor forms time one Horner stage per profiling scope, the split-operator solver its three passes together
+            b = sum(alg["stencil_bytes"]) / (1.0 if args.step == "richardson" else 4.0)
             entry.update(bound="hbm", achieved=b / (avg * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
         elif name == "density":
             entry.update(bound="hbm", achieved=alg["density_bytes"] / (avg * 1e-3) / 1e9, peak=peaks["hbm_gbs"], unit="GB/s")
@@ -429,7 +440,7 @@ def main():
                  "definition": "max(stencil+density%s bytes / HBM peak, real-beta GEMM flops / tensor peak of the GEMM mode); "
                                "t_sum / frac_of_sum: the same two terms added, the bound for kernels that do not overlap "
                                "(at the power cap overlap buys little: DESIGN.md section 8)" % (
-                     "+norm" if args.step == "split" else "")}
+                     "+norm" if args.step in SPLIT_STEPS else "")}
 
     cpu = None
     if world > 1:
@@ -441,7 +452,7 @@ def main():
         v, sec_step, cores, el = time_oracle(c, s, W.laser_samples(c, nsteps=CPU_STEPS, t0=0.9), steps=CPU_STEPS, warmup=1, step=args.step)
         cpu = {"value": v, "unit": "electron-steps/s", "cores": cores, "kind": "oracle", "s_per_step": sec_step,
                "sample": "domain 0, first %d of %d orbitals (%g electrons), all %d projectors, %d timed %s steps" % (
-                   s["psi"].shape[-1], c.norb, el, c.nproj, CPU_STEPS, "Eq. (2) split" if args.step == "split" else "Taylor-4")}
+                   s["psi"].shape[-1], c.norb, el, c.nproj, CPU_STEPS, "Eq. (2) split" if args.step in SPLIT_STEPS else "Taylor-4")}
 
     line = {
         "metric": "electron-steps/s", "value": value, "unit": "electron-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,

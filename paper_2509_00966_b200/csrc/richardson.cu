@@ -13,9 +13,9 @@
 // EVEN pair (2p, 2p+1) of its line for one float4 (two orbitals), so the two even sweeps are register-only; for the odd sweep
 // the even points go through shared memory once (thread p rotates its point 2p+1 with point 2p+2 of thread p+1; the last
 // pair wraps, which is why every axis needs an even number of points).  Eight float4 lanes per line keep every access a full
-// 128-byte line whatever the axis.  The rotation constants are computed in FP64 per thread and applied as hi + lo pairs of
-// floats: a rounded (cos, sin) pair is off the unit circle by ~6e-8, the SAME factor on every point in every sweep, which
-// would be a coherent norm drift of ~5e-7 per step; with the pair the remaining error is the FP32 rounding of the products.
+// 128-byte line whatever the axis.  The rotation constants are computed in FP64 by one thread per line; a rounded (cos, sin)
+// pair is off the unit circle by ~6e-8, the SAME factor on every point in every sweep: the last pass divides the product of
+// the nine factors out again (see make_rot), so what remains is the FP32 rounding of the products.
 #include "mlmd_internal.h"
 
 namespace mlmd {
@@ -37,102 +37,149 @@ struct RichParams {
     long sdom;                // float4 per domain
     int lanes;                // float4 per grid point
     int ngroups;              // lanes / R_LG
-    long nlines;              // ndom * n1 * n2 * ngroups
+    int nlines;               // ndom * n1 * n2 * ngroups
     int nlb;                  // lines per block
+    long pa, p1, p2, pdom;    // the same strides in grid points (index into V_loc)
 };
 
-struct Rot {                  // (c, wr + i wi) = (cos, -i u sin) as hi + lo floats
-    float c, cl, wr, wrl, wi, wil;
+struct Rot {                  // (c, wr + i wi) = (cos, -i u sin), rounded to float
+    float c, wr, wi;
 };
-__device__ __forceinline__ Rot make_rot(double theta, double ur, double ui) {
+// The rounded triple is sqrt(c^2 + wr^2 + wi^2) times an exactly unitary 2 x 2 matrix (its off-diagonal entries are each
+// other's negated conjugates bit for bit): that factor, ~1 +- 6e-8 and the SAME on every pair in every sweep, is returned
+// through *scale so that the last pass can take the product of all nine out again (in FP64) instead of letting it
+// accumulate as a coherent norm drift of ~5e-7 per step.
+__device__ __forceinline__ Rot make_rot(double theta, double ur, double ui, double *scale) {
     double s, c;
     sincos(theta, &s, &c);
-    const double wr = s * ui, wi = -s * ur;     // -i (ur + i ui) s
     Rot r;
     r.c = (float)c;
-    r.cl = (float)(c - (double)r.c);
-    r.wr = (float)wr;
-    r.wrl = (float)(wr - (double)r.wr);
-    r.wi = (float)wi;
-    r.wil = (float)(wi - (double)r.wi);
+    r.wr = (float)(s * ui);        // -i (ur + i ui) s
+    r.wi = (float)(-s * ur);
+    *scale *= sqrt((double)r.c * r.c + (double)r.wr * r.wr + (double)r.wi * r.wi);
     return r;
 }
-// one complex number: c * a + (wr + i wi) * b, every constant as hi + lo
-__device__ __forceinline__ float2 rot1(const Rot &r, float ax, float ay, float bx, float by, bool conj_w) {
-    // upper row: w = (wr, wi); lower row: w' = -i conj(u) s = (-wr, wi)
-    const float wr = conj_w ? -r.wr : r.wr, wrl = conj_w ? -r.wrl : r.wrl;
-    float lo = fmaf(r.cl, ax, fmaf(wrl, bx, -r.wil * by));
-    float x = fmaf(r.c, ax, fmaf(wr, bx, fmaf(-r.wi, by, lo)));
-    float lo2 = fmaf(r.cl, ay, fmaf(wrl, by, r.wil * bx));
-    float y = fmaf(r.c, ay, fmaf(wr, by, fmaf(r.wi, bx, lo2)));
-    return make_float2(x, y);
-}
-// (a, b) <- R (a, b) for both complex numbers of the float4s; a is the lower-index point of the pair
+// (a, b) <- R (a, b) for both complex numbers of the float4s; a is the lower-index point of the pair:
+// a' = c a + w b, b' = w' a + c b with w = (wr, wi), w' = -i conj(u) s = (-wr, wi)
 __device__ __forceinline__ void rotate(const Rot &r, float4 &a, float4 &b) {
-    const float2 a0 = rot1(r, a.x, a.y, b.x, b.y, false), a1 = rot1(r, a.z, a.w, b.z, b.w, false);
-    const float2 b0 = rot1(r, b.x, b.y, a.x, a.y, true), b1 = rot1(r, b.z, b.w, a.z, a.w, true);
-    a = make_float4(a0.x, a0.y, a1.x, a1.y);
-    b = make_float4(b0.x, b0.y, b1.x, b1.y);
+    const float4 x = a, y = b;
+    a.x = fmaf(r.c, x.x, fmaf(r.wr, y.x, -r.wi * y.y));
+    a.y = fmaf(r.c, x.y, fmaf(r.wr, y.y, r.wi * y.x));
+    a.z = fmaf(r.c, x.z, fmaf(r.wr, y.z, -r.wi * y.w));
+    a.w = fmaf(r.c, x.w, fmaf(r.wr, y.w, r.wi * y.z));
+    b.x = fmaf(r.c, y.x, fmaf(-r.wr, x.x, -r.wi * x.y));
+    b.y = fmaf(r.c, y.y, fmaf(-r.wr, x.y, r.wi * x.x));
+    b.z = fmaf(r.c, y.z, fmaf(-r.wr, x.z, -r.wi * x.w));
+    b.w = fmaf(r.c, y.w, fmaf(-r.wr, x.w, r.wi * x.z));
 }
 __device__ __forceinline__ float4 phase4(const float4 v, float cs, float sn) {
     return make_float4(v.x * cs - v.y * sn, v.x * sn + v.y * cs, v.z * cs - v.w * sn, v.z * sn + v.w * cs);
 }
 
-template <bool PHASE_IN, bool PHASE_OUT>
+struct LineConst {
+    Rot half, full;
+    float unscale;            // PHASE_OUT: 1 / (product of the nine sweeps' scale factors)
+};
+
+// LPT: float4 lanes per thread (2 when the lane count allows: the index arithmetic and the phases are shared)
+template <bool PHASE_IN, bool PHASE_OUT, int LPT>
 __global__ void __launch_bounds__(1024) richardson_axis_kernel(const RichParams P) {
-    extern __shared__ float4 ev[];      // [nlb][n / 2][R_LG]: the even points of every line of the block
+    extern __shared__ float4 ev[];      // [nlb][n / 2][LPT * R_LG]: the even points of every line of the block
+    constexpr int LW = LPT * R_LG;      // float4 per line and point
     const int np = P.n / 2;
     const int tid = threadIdx.x;
     const int l = tid % R_LG, p = (tid / R_LG) % np, ql = tid / (R_LG * np);
-    long line = (long)blockIdx.x * P.nlb + ql;
+    int line = (int)blockIdx.x * P.nlb + ql;
     const bool live = line < P.nlines;
     if (!live) line = P.nlines - 1;     // keeps the barriers uniform; nothing is stored
-    const int g = (int)(line % P.ngroups);
-    long rest = line / P.ngroups;
-    const int i2 = (int)(rest % P.n2);
+    const int g = line % P.ngroups;
+    int rest = line / P.ngroups;
+    const int i2 = rest % P.n2;
     rest /= P.n2;
-    const int i1 = (int)(rest % P.n1);
-    const int dom = (int)(rest / P.n1);
-    const long base = (long)dom * P.sdom + i1 * P.s1 + i2 * P.s2 + g * R_LG + l;
+    const int i1 = rest % P.n1;
+    const int dom = rest / P.n1;
+    const long base = (long)dom * P.sdom + i1 * P.s1 + i2 * P.s2 + g * LW + l;
     const long ad0 = base + (long)(2 * p) * P.sa, ad1 = ad0 + P.sa;
+    const long gp0 = (long)dom * P.pdom + i1 * P.p1 + i2 * P.p2 + (long)(2 * p) * P.pa, gp1 = gp0 + P.pa;
 
-    const StepCoef c = P.coef[dom];
-    const double bp = (double)c.p[P.axis][0], bq = (double)c.q[P.axis][0];      // b = bp - i bq
-    const double mb = sqrt(bp * bp + bq * bq);
-    const double ur = bp / mb, ui = -bq / mb;
-    const Rot rh = make_rot(0.5 * P.dt * mb, ur, ui), rf = make_rot(P.dt * mb, ur, ui);
+    // constants of this line's domain: FP64, by one thread per line (B200 has little FP64 throughput)
+    LineConst *lc = (LineConst *)(ev + (size_t)P.nlb * np * LW);
+    const float centre = P.coef[dom].centre;
+    if (p == 0 && l == 0) {
+        const StepCoef c = P.coef[dom];
+        double sc_all = 1.0;
+        LineConst k;
+        for (int d = 0; d < 3; ++d) {
+            if (!PHASE_OUT && d != P.axis) continue;
+            const double bp = (double)c.p[d][0], bq = (double)c.q[d][0];      // b = bp - i bq
+            const double mb = sqrt(bp * bp + bq * bq);
+            const double ur = bp / mb, ui = -bq / mb;
+            double sc = 1.0;
+            const Rot h = make_rot(0.5 * P.dt * mb, ur, ui, &sc);
+            sc *= sc;                                                         // two half sweeps
+            const Rot f = make_rot(P.dt * mb, ur, ui, &sc);
+            sc_all *= sc;
+            if (d == P.axis) {
+                k.half = h;
+                k.full = f;
+            }
+        }
+        k.unscale = (float)(1.0 / sc_all);
+        lc[ql] = k;
+    }
+    __syncthreads();
+    const Rot rh = lc[ql].half, rf = lc[ql].full;
 
-    float4 u0 = P.psi[ad0], u1 = P.psi[ad1];
+    float4 u0[LPT], u1[LPT];
+#pragma unroll
+    for (int k = 0; k < LPT; ++k) {
+        u0[k] = P.psi[ad0 + k * R_LG];
+        u1[k] = P.psi[ad1 + k * R_LG];
+    }
     float cs0 = 1.f, sn0 = 0.f, cs1 = 1.f, sn1 = 0.f;
     if (PHASE_IN || PHASE_OUT) {
         const float half = (float)(-0.5 * P.dt);
-        sincosf(half * (P.vloc[ad0 / P.lanes] + c.centre), &sn0, &cs0);
-        sincosf(half * (P.vloc[ad1 / P.lanes] + c.centre), &sn1, &cs1);
+        sincosf(half * (P.vloc[gp0] + centre), &sn0, &cs0);
+        sincosf(half * (P.vloc[gp1] + centre), &sn1, &cs1);
     }
-    if (PHASE_IN) {
-        u0 = phase4(u0, cs0, sn0);
-        u1 = phase4(u1, cs1, sn1);
-    }
-    rotate(rh, u0, u1);                                   // even pairs, dt/2
-    float4 *mine = ev + ((size_t)ql * np + p) * R_LG + l;
-    float4 *next = ev + ((size_t)ql * np + (p + 1 == np ? 0 : p + 1)) * R_LG + l;
-    *mine = u0;
-    __syncthreads();
-    {
-        float4 w = *next;                                 // point 2p + 2 (periodic)
-        rotate(rf, u1, w);                                // odd pairs, dt
-        *next = w;
+    float4 *mine = ev + ((size_t)ql * np + p) * LW + l;
+    float4 *next = ev + ((size_t)ql * np + (p + 1 == np ? 0 : p + 1)) * LW + l;
+#pragma unroll
+    for (int k = 0; k < LPT; ++k) {
+        if (PHASE_IN) {
+            u0[k] = phase4(u0[k], cs0, sn0);
+            u1[k] = phase4(u1[k], cs1, sn1);
+        }
+        rotate(rh, u0[k], u1[k]);                         // even pairs, dt/2
+        mine[k * R_LG] = u0[k];
     }
     __syncthreads();
-    u0 = *mine;
-    rotate(rh, u0, u1);                                   // even pairs, dt/2
+#pragma unroll
+    for (int k = 0; k < LPT; ++k) {
+        float4 w = next[k * R_LG];                        // point 2p + 2 (periodic)
+        rotate(rf, u1[k], w);                             // odd pairs, dt
+        next[k * R_LG] = w;
+    }
+    __syncthreads();
     if (PHASE_OUT) {
-        u0 = phase4(u0, cs0, sn0);
-        u1 = phase4(u1, cs1, sn1);
+        const float us = lc[ql].unscale;
+        cs0 *= us;
+        sn0 *= us;
+        cs1 *= us;
+        sn1 *= us;
     }
-    if (live) {
-        P.psi[ad0] = u0;
-        P.psi[ad1] = u1;
+#pragma unroll
+    for (int k = 0; k < LPT; ++k) {
+        u0[k] = mine[k * R_LG];
+        rotate(rh, u0[k], u1[k]);                         // even pairs, dt/2
+        if (PHASE_OUT) {
+            u0[k] = phase4(u0[k], cs0, sn0);
+            u1[k] = phase4(u1[k], cs1, sn1);
+        }
+        if (live) {
+            P.psi[ad0 + k * R_LG] = u0[k];
+            P.psi[ad1 + k * R_LG] = u1[k];
+        }
     }
 }
 
@@ -168,18 +215,30 @@ cudaError_t launch_richardson(const mlmd_domain *h, float2 *psi, const StepCoef 
         P.s2 = stride[o2];
         P.sdom = (long)h->ngrid * lanes;
         P.lanes = lanes;
-        P.ngroups = lanes / R_LG;
-        P.nlines = (long)h->ndom * P.n1 * P.n2 * P.ngroups;
+        const int lpt = lanes % (2 * R_LG) == 0 ? 2 : 1;
+        P.ngroups = lanes / (lpt * R_LG);
+        const long nlines = (long)h->ndom * P.n1 * P.n2 * P.ngroups;
+        if (nlines > 0x7fffffffL) return cudaErrorInvalidConfiguration;
+        P.nlines = (int)nlines;
+        P.pa = stride[d] / lanes;
+        P.p1 = stride[o1] / lanes;
+        P.p2 = stride[o2] / lanes;
+        P.pdom = h->ngrid;
         const int tpl = (P.n / 2) * R_LG;                 // threads per line
         P.nlb = tpl >= 256 ? 1 : 256 / tpl;
-        const long blocks = (P.nlines + P.nlb - 1) / P.nlb;
-        if (blocks > 0x7fffffffL) return cudaErrorInvalidConfiguration;
-        const size_t smem = (size_t)P.nlb * (P.n / 2) * R_LG * sizeof(float4);
+        const long blocks = (nlines + P.nlb - 1) / P.nlb;
+        const size_t smem = (size_t)P.nlb * (P.n / 2) * lpt * R_LG * sizeof(float4) + (size_t)P.nlb * sizeof(LineConst);
         const dim3 grid((unsigned)blocks), block((unsigned)(tpl * P.nlb));
         ++*nlaunch;
-        if (k == 0) richardson_axis_kernel<true, false><<<grid, block, smem, h->stream>>>(P);
-        else if (k == 2) richardson_axis_kernel<false, true><<<grid, block, smem, h->stream>>>(P);
-        else richardson_axis_kernel<false, false><<<grid, block, smem, h->stream>>>(P);
+        if (lpt == 2) {
+            if (k == 0) richardson_axis_kernel<true, false, 2><<<grid, block, smem, h->stream>>>(P);
+            else if (k == 2) richardson_axis_kernel<false, true, 2><<<grid, block, smem, h->stream>>>(P);
+            else richardson_axis_kernel<false, false, 2><<<grid, block, smem, h->stream>>>(P);
+        } else {
+            if (k == 0) richardson_axis_kernel<true, false, 1><<<grid, block, smem, h->stream>>>(P);
+            else if (k == 2) richardson_axis_kernel<false, true, 1><<<grid, block, smem, h->stream>>>(P);
+            else richardson_axis_kernel<false, false, 1><<<grid, block, smem, h->stream>>>(P);
+        }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
