@@ -50,14 +50,18 @@ def load_batch(c, keep):
     return psi_dev, beta_dev, vloc, occ, D, kept
 
 
-def oracle_states(c, k, dd, orbs, A, steps, split=False):
+def oracle_states(c, k, dd, orbs, A, steps, split=False, local="taylor"):
     """Oracle state of orbitals `orbs` (None = all) of domain k after each step count in `steps` (ascending):
     {n: (psi complex128 [nx,ny,nz,len(orbs)], rho of those orbitals)}; one pass, continued from state to state."""
     from oracle import ref
-    key = (c.cfg, k, None if orbs is None else tuple(orbs), tuple(steps), split)
+    key = (c.cfg, k, None if orbs is None else tuple(orbs), tuple(steps), split, local)
     if key in _oracle_cache:
         return _oracle_cache[key]
-    prop = ref.propagate_split if split else ref.propagate
+    if split and local != "taylor":
+        def prop(*a):
+            return ref.propagate_split(*a, local=local)
+    else:
+        prop = ref.propagate_split if split else ref.propagate
     sel = slice(None) if orbs is None else list(orbs)
     psi = np.ascontiguousarray(dd["psi"][None][..., sel])
     occ = np.ascontiguousarray(dd["occ"][None][:, sel])
@@ -74,7 +78,7 @@ def orb_errs(g, r):
     return np.sqrt((np.abs(g - r) ** 2).sum(axis=(0, 1, 2)) / (np.abs(r) ** 2).sum(axis=(0, 1, 2)))
 
 
-def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, tol=None, label=None):
+def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, tol=None, label=None, local="taylor"):
     """whole: the domain compared in full after each step count of `whole_steps`; sample: {domain: [orbitals]}
     compared after step 1 and step nsteps."""
     import torch
@@ -92,6 +96,8 @@ def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, to
     del beta_dev
     assert dom.gemm_path() == "tcgen05"
     prop = dom.propagate_split if split else dom.propagate
+    if local == "richardson":
+        dom.set_option(M.OPT_LOCAL_SOLVER, 1)      # Eq. (2) with the paper's own split-operator local solver (reading D33)
     out = torch.empty_like(psi_dev)
     rho = torch.empty((c.ndom, *c.grid), dtype=torch.float32, device=psi_dev.device)
     errs = {}
@@ -103,7 +109,7 @@ def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, to
         M.mlmd_density(dom.handle, rho)
         worst = 0.0
         if n in whole_steps:
-            r, rho_ref = oracle_states(c, whole, kept[whole], None, A, sorted(whole_steps), split)[n]
+            r, rho_ref = oracle_states(c, whole, kept[whole], None, A, sorted(whole_steps), split, local)[n]
             worst = float(orb_errs(out[whole].cpu().numpy(), r).max())
             errs["rho_" + tag] = float(np.abs(rho[whole].cpu().numpy() - rho_ref).max() / rho_ref.max())
             G = dom.overlap(0)[whole]
@@ -111,7 +117,7 @@ def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, to
             errs["gram_" + tag] = float(np.abs(G - G_ref).max())
         if n in (1, nsteps):
             for k, orbs in sample.items():
-                r, _ = oracle_states(c, k, kept[k], orbs, A, sorted(set([1, nsteps])), split)[n]
+                r, _ = oracle_states(c, k, kept[k], orbs, A, sorted(set([1, nsteps])), split, local)[n]
                 worst = max(worst, float(orb_errs(out[k][..., list(orbs)].cpu().numpy(), r).max()))
         errs[tag] = worst
         # electron count of rho against the GPU's own orbitals on EVERY domain (sum rule)
@@ -121,7 +127,7 @@ def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, to
                               for k in range(c.ndom)])
         errs["electrons_" + tag] = float(((ne_gpu - ne_own).abs() / ne_own).max().item())
     dom.close()
-    label = label or "configs[%d] %s mode=%s" % (cfg, "split" if split else "taylor", mode)
+    label = label or "configs[%d] %s mode=%s" % (cfg, ("split/" + local) if split else "taylor", mode)
     MEASURED.append((label, errs))
     print(label, errs)
     for key, v in errs.items():
@@ -183,6 +189,13 @@ def test_config3_two_runs_are_bit_identical():
 
 def test_config3_full_batch_split_step():
     run_full(3, whole=17, whole_steps=[1], sample={63: [3, 113, 223]}, nsteps=2, split=True)
+
+
+def test_config3_full_batch_split_operator_local_solver_10_steps():
+    """The paper's literal algorithm at the benchmarked size (`bench.py --step richardson`): Eq. (2) with the block-diagonal
+    split-operator local solver on the 7-point operator, 10 steps, a whole domain and samples in the first / last domain."""
+    run_full(3, whole=29, whole_steps=[1, 10], sample={0: SAMPLE_224, 63: [3, 113, 223]}, nsteps=10, split=True,
+             local="richardson")
 
 
 def test_config4_full_batch_10_steps_complex64():
