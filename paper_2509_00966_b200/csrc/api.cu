@@ -109,6 +109,7 @@ static bool make_plan(int ndom, int nx, int ny, int nz, int norb, int nproj_max,
     w.occ_eff = take((size_t)ndom * pl->ld * sizeof(float));
     w.avec = take((size_t)ndom * 3 * sizeof(double));
     w.gram = take((size_t)ndom * pl->ldp_max * pl->ldp_max * sizeof(float));
+    w.rich = take((size_t)ndom * 3 * 8 * sizeof(float));
     w.total = o;
     return true;
 }

@@ -26,7 +26,7 @@ static_assert(sizeof(StepCoef) == 56, "StepCoef layout");
 
 struct Workspace {              // byte offsets into the caller's workspace
     size_t psi, ua, ub, psi0, vloc, beta, beta_lo, dprime, occ, rho, z, what, what_lo, zpart, coef, coef_cur, flag,
-        nrm, nrm_part, scl, occ_eff, avec, gram, total;
+        nrm, nrm_part, scl, occ_eff, avec, gram, rich, total;
 };
 
 // Tensor maps are pure functions of (base pointer, shape, box): encoded once per distinct key and kept in the
@@ -137,6 +137,7 @@ struct mlmd_domain {
     float *zpart() const { return (float *)(ws + off.zpart); }
     mlmd::StepCoef *coef() const { return (mlmd::StepCoef *)(ws + off.coef); }
     mlmd::StepCoef *coef_cur() const { return (mlmd::StepCoef *)(ws + off.coef_cur); }
+    float *rich() const { return (float *)(ws + off.rich); }     // split-operator solver: [ndom][3][8] rotation constants of the step
     int *step_counter() const { return (int *)(ws + off.flag + 64); }
     int *flag() const { return (int *)(ws + off.flag); }
     // split step (Eq. 2): squared orbital norms [4][ndom][ld] (input, after kick 1, after Taylor, after kick 2)

@@ -13,9 +13,10 @@
 // EVEN pair (2p, 2p+1) of its line for one float4 (two orbitals), so the two even sweeps are register-only; for the odd sweep
 // the even points go through shared memory once (thread p rotates its point 2p+1 with point 2p+2 of thread p+1; the last
 // pair wraps, which is why every axis needs an even number of points).  Eight float4 lanes per line keep every access a full
-// 128-byte line whatever the axis.  The rotation constants are computed in FP64 by one thread per line; a rounded (cos, sin)
-// pair is off the unit circle by ~6e-8, the SAME factor on every point in every sweep: the last pass divides the product of
-// the nine factors out again (see make_rot), so what remains is the FP32 rounding of the products.
+// 128-byte line whatever the axis.  The rotation constants of a step are computed in FP64 by a one-block kernel ahead of the
+// three passes (from the step's device-resident StepCoef, so a CUDA graph replays them); a rounded (cos, sin) pair is off the
+// unit circle by ~6e-8, the SAME factor on every point in every sweep: the last pass takes the product of the nine factors out
+// again (see make_rot), so what remains is the FP32 rounding of the products.
 #include "mlmd_internal.h"
 
 namespace mlmd {
@@ -24,8 +25,10 @@ namespace {
 
 constexpr int R_LG = 8;       // float4 lanes per line and thread group: 128 bytes
 
+struct AxisConst;
 struct RichParams {
     float4 *psi;
+    const AxisConst *consts;  // [ndom][3], written by richardson_consts_kernel for this step
     const float *vloc;
     const StepCoef *coef;     // [ndom], 2nd-order weights (fill_coef with the 7-point star)
     double dt;
@@ -45,10 +48,17 @@ struct RichParams {
 struct Rot {                  // (c, wr + i wi) = (cos, -i u sin), rounded to float
     float c, wr, wi;
 };
+struct AxisConst {            // one per (domain, axis) and step: 8 floats in the handle's workspace
+    Rot half, full;
+    float excess;             // axis 0 only: 1 / (product of the nine sweeps' scale factors) - 1
+    float pad;
+};
+static_assert(sizeof(AxisConst) == 32, "AxisConst layout");
+
 // The rounded triple is sqrt(c^2 + wr^2 + wi^2) times an exactly unitary 2 x 2 matrix (its off-diagonal entries are each
-// other's negated conjugates bit for bit): that factor, ~1 +- 6e-8 and the SAME on every pair in every sweep, is returned
-// through *scale so that the last pass can take the product of all nine out again (in FP64) instead of letting it
-// accumulate as a coherent norm drift of ~5e-7 per step.
+// other's negated conjugates bit for bit): that factor, 1 +- 6e-8 and the SAME on every pair in every sweep, would be a
+// coherent norm drift.  The constants kernel returns the product of all nine factors (FP64) as `excess` = 1/product - 1
+// (a number of size 1e-7 kept to 24 bits), and the last pass multiplies by 1 + excess.
 __device__ __forceinline__ Rot make_rot(double theta, double ur, double ui, double *scale) {
     double s, c;
     sincos(theta, &s, &c);
@@ -59,6 +69,30 @@ __device__ __forceinline__ Rot make_rot(double theta, double ur, double ui, doub
     *scale *= sqrt((double)r.c * r.c + (double)r.wr * r.wr + (double)r.wi * r.wi);
     return r;
 }
+// One thread per domain: the constants of the step for the three axes, in FP64, once per step instead of once per thread
+// block (B200 has little FP64 throughput: with every thread computing them the three passes took twice as long).
+__global__ void richardson_consts_kernel(const StepCoef *__restrict__ coef, double dt, int ndom, AxisConst *__restrict__ out) {
+    const int dom = blockIdx.x * blockDim.x + threadIdx.x;
+    if (dom >= ndom) return;
+    const StepCoef c = coef[dom];
+    double sc_all = 1.0;
+    AxisConst k[3];
+    for (int d = 0; d < 3; ++d) {
+        const double bp = (double)c.p[d][0], bq = (double)c.q[d][0];      // b = bp - i bq
+        const double mb = sqrt(bp * bp + bq * bq);
+        const double ur = bp / mb, ui = -bq / mb;
+        double sc = 1.0;
+        k[d].half = make_rot(0.5 * dt * mb, ur, ui, &sc);
+        sc *= sc;                                                         // two half sweeps
+        k[d].full = make_rot(dt * mb, ur, ui, &sc);
+        sc_all *= sc;
+        k[d].excess = 0.f;
+        k[d].pad = 0.f;
+    }
+    k[0].excess = (float)(1.0 / sc_all - 1.0);
+    for (int d = 0; d < 3; ++d) out[dom * 3 + d] = k[d];
+}
+
 // (a, b) <- R (a, b) for both complex numbers of the float4s; a is the lower-index point of the pair:
 // a' = c a + w b, b' = w' a + c b with w = (wr, wi), w' = -i conj(u) s = (-wr, wi)
 __device__ __forceinline__ void rotate(const Rot &r, float4 &a, float4 &b) {
@@ -72,14 +106,11 @@ __device__ __forceinline__ void rotate(const Rot &r, float4 &a, float4 &b) {
     b.z = fmaf(r.c, y.z, fmaf(-r.wr, x.z, -r.wi * x.w));
     b.w = fmaf(r.c, y.w, fmaf(-r.wr, x.w, r.wi * x.z));
 }
-__device__ __forceinline__ float4 phase4(const float4 v, float cs, float sn) {
-    return make_float4(v.x * cs - v.y * sn, v.x * sn + v.y * cs, v.z * cs - v.w * sn, v.z * sn + v.w * cs);
+// v (cs + i sn) (1 + ex)
+__device__ __forceinline__ float4 phase4(const float4 v, float cs, float sn, float ex) {
+    const float4 p = make_float4(v.x * cs - v.y * sn, v.x * sn + v.y * cs, v.z * cs - v.w * sn, v.z * sn + v.w * cs);
+    return make_float4(fmaf(ex, p.x, p.x), fmaf(ex, p.y, p.y), fmaf(ex, p.z, p.z), fmaf(ex, p.w, p.w));
 }
-
-struct LineConst {
-    Rot half, full;
-    float unscale;            // PHASE_OUT: 1 / (product of the nine sweeps' scale factors)
-};
 
 // LPT: float4 lanes per thread (2 when the lane count allows: the index arithmetic and the phases are shared)
 template <bool PHASE_IN, bool PHASE_OUT, int LPT>
@@ -102,53 +133,29 @@ __global__ void __launch_bounds__(1024) richardson_axis_kernel(const RichParams 
     const long ad0 = base + (long)(2 * p) * P.sa, ad1 = ad0 + P.sa;
     const long gp0 = (long)dom * P.pdom + i1 * P.p1 + i2 * P.p2 + (long)(2 * p) * P.pa, gp1 = gp0 + P.pa;
 
-    // constants of this line's domain: FP64, by one thread per line (B200 has little FP64 throughput)
-    LineConst *lc = (LineConst *)(ev + (size_t)P.nlb * np * LW);
-    const float centre = P.coef[dom].centre;
-    if (p == 0 && l == 0) {
-        const StepCoef c = P.coef[dom];
-        double sc_all = 1.0;
-        LineConst k;
-        for (int d = 0; d < 3; ++d) {
-            if (!PHASE_OUT && d != P.axis) continue;
-            const double bp = (double)c.p[d][0], bq = (double)c.q[d][0];      // b = bp - i bq
-            const double mb = sqrt(bp * bp + bq * bq);
-            const double ur = bp / mb, ui = -bq / mb;
-            double sc = 1.0;
-            const Rot h = make_rot(0.5 * P.dt * mb, ur, ui, &sc);
-            sc *= sc;                                                         // two half sweeps
-            const Rot f = make_rot(P.dt * mb, ur, ui, &sc);
-            sc_all *= sc;
-            if (d == P.axis) {
-                k.half = h;
-                k.full = f;
-            }
-        }
-        k.unscale = (float)(1.0 / sc_all);
-        lc[ql] = k;
-    }
-    __syncthreads();
-    const Rot rh = lc[ql].half, rf = lc[ql].full;
-
     float4 u0[LPT], u1[LPT];
 #pragma unroll
     for (int k = 0; k < LPT; ++k) {
         u0[k] = P.psi[ad0 + k * R_LG];
         u1[k] = P.psi[ad1 + k * R_LG];
     }
-    float cs0 = 1.f, sn0 = 0.f, cs1 = 1.f, sn1 = 0.f;
+    const AxisConst ac = P.consts[dom * 3 + P.axis];
+    const Rot rh = ac.half, rf = ac.full;
+    float cs0 = 1.f, sn0 = 0.f, cs1 = 1.f, sn1 = 0.f, ex = 0.f;
     if (PHASE_IN || PHASE_OUT) {
+        const float centre = P.coef[dom].centre;
         const float half = (float)(-0.5 * P.dt);
         sincosf(half * (P.vloc[gp0] + centre), &sn0, &cs0);
         sincosf(half * (P.vloc[gp1] + centre), &sn1, &cs1);
+        if (PHASE_OUT) ex = P.consts[dom * 3].excess;
     }
     float4 *mine = ev + ((size_t)ql * np + p) * LW + l;
     float4 *next = ev + ((size_t)ql * np + (p + 1 == np ? 0 : p + 1)) * LW + l;
 #pragma unroll
     for (int k = 0; k < LPT; ++k) {
         if (PHASE_IN) {
-            u0[k] = phase4(u0[k], cs0, sn0);
-            u1[k] = phase4(u1[k], cs1, sn1);
+            u0[k] = phase4(u0[k], cs0, sn0, 0.f);
+            u1[k] = phase4(u1[k], cs1, sn1, 0.f);
         }
         rotate(rh, u0[k], u1[k]);                         // even pairs, dt/2
         mine[k * R_LG] = u0[k];
@@ -161,20 +168,13 @@ __global__ void __launch_bounds__(1024) richardson_axis_kernel(const RichParams 
         next[k * R_LG] = w;
     }
     __syncthreads();
-    if (PHASE_OUT) {
-        const float us = lc[ql].unscale;
-        cs0 *= us;
-        sn0 *= us;
-        cs1 *= us;
-        sn1 *= us;
-    }
 #pragma unroll
     for (int k = 0; k < LPT; ++k) {
         u0[k] = mine[k * R_LG];
         rotate(rh, u0[k], u1[k]);                         // even pairs, dt/2
         if (PHASE_OUT) {
-            u0[k] = phase4(u0[k], cs0, sn0);
-            u1[k] = phase4(u1[k], cs1, sn1);
+            u0[k] = phase4(u0[k], cs0, sn0, ex);
+            u1[k] = phase4(u1[k], cs1, sn1, ex);
         }
         if (live) {
             P.psi[ad0 + k * R_LG] = u0[k];
@@ -192,17 +192,21 @@ bool richardson_supported(const mlmd_domain *h) {
     return h->ld % 16 == 0;     // lanes = ld / 2 float4 per point, a multiple of R_LG
 }
 
-// psi <- U_loc(dt) psi in place: three launches (z with the leading phase, y, x with the trailing phase).
+// psi <- U_loc(dt) psi in place: the constants kernel and three passes (z with the leading phase, y, x with the trailing phase).
 cudaError_t launch_richardson(const mlmd_domain *h, float2 *psi, const StepCoef *coef, double dt, int *nlaunch) {
     if (!richardson_supported(h)) return cudaErrorInvalidValue;
     const int lanes = h->ld / 2;
     const int n[3] = {h->nx, h->ny, h->nz};
     const long stride[3] = {(long)h->ny * h->nz * lanes, (long)h->nz * lanes, (long)lanes};
     static const int order[3] = {2, 1, 0};
+    AxisConst *consts = (AxisConst *)h->rich();
+    ++*nlaunch;
+    richardson_consts_kernel<<<(h->ndom + 63) / 64, 64, 0, h->stream>>>(coef, dt, h->ndom, consts);
     for (int k = 0; k < 3; ++k) {
         const int d = order[k], o1 = (d + 1) % 3, o2 = (d + 2) % 3;
         RichParams P;
         P.psi = (float4 *)psi;
+        P.consts = consts;
         P.vloc = h->vloc();
         P.coef = coef;
         P.dt = dt;
@@ -227,7 +231,7 @@ cudaError_t launch_richardson(const mlmd_domain *h, float2 *psi, const StepCoef 
         const int tpl = (P.n / 2) * R_LG;                 // threads per line
         P.nlb = tpl >= 256 ? 1 : 256 / tpl;
         const long blocks = (nlines + P.nlb - 1) / P.nlb;
-        const size_t smem = (size_t)P.nlb * (P.n / 2) * lpt * R_LG * sizeof(float4) + (size_t)P.nlb * sizeof(LineConst);
+        const size_t smem = (size_t)P.nlb * (P.n / 2) * lpt * R_LG * sizeof(float4);
         const dim3 grid((unsigned)blocks), block((unsigned)(tpl * P.nlb));
         ++*nlaunch;
         if (lpt == 2) {
