@@ -747,8 +747,10 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         if (rc) return rc;
     }
     if (h->opt[MLMD_OPT_LOCAL_SOLVER] == 1) {
-        // the paper's own local solver (reading D33): three in-place passes of 2 x 2 nearest-neighbour rotations; the
-        // squared norms before and after it (the kicks' normalisation, reading D27) are measured by the norm pass
+        // the paper's own local solver (reading D33): three in-place passes of 2 x 2 nearest-neighbour rotations.  The
+        // squared norms the kicks' normalisation needs (reading D27): before the solver by the norm pass; after it they are
+        // the same numbers, because U_loc is unitary by construction (in the oracle to 1e-16; here the passes' FP32 rounding
+        // moves a norm by ~1e-7, and handing the second kick the norm BEFORE the solver takes that noise out again)
         if (kicks) {
             int rc = norm2(1);
             if (rc) return rc;
@@ -757,10 +759,8 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
             ProfScope ps(h, MLMD_K_STENCIL);
             CU(launch_richardson(h, h->psi(), coef, dt, nl));
         }
-        if (kicks) {
-            int rc = norm2(2);
-            if (rc) return rc;
-        }
+        if (kicks)
+            CU(cudaMemcpyAsync(h->nrm(2), h->nrm(1), (size_t)h->ndom * h->ld * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
     } else {
     // Taylor-4 of h_loc (Horner form).  With kicks, the first stage also sums |psi_a|^2 (its input) and the last
     // |psi_c|^2 (its output) per orbital: the norms ride on passes that read or write those arrays anyway.
