@@ -189,6 +189,89 @@ def workload_config(c, args):
         "working set may fit L2: a 256 MB buffer is written between timed repetitions"}
 
 
+def power_probe(c, dom, psi_dev, occ, vloc, A, dev):
+    """--power: what 1000 W buy for each operation (profiles/r*_power_per_kernel.md).  One operation at a time is launched back
+    to back for ~3 s while a host thread samples NVML power and clocks every 20 ms; the second half of the samples is averaged.
+    Returns a list of rows.  Uses the public API only (the back-application alone is the step minus the rest)."""
+    import torch
+    import pynvml
+    import paper_2509_00966_b200 as M
+    pynvml.nvmlInit()
+    H = pynvml.nvmlDeviceGetHandleByIndex(dev.index or 0)
+    rows = []
+
+    def run(name, fn, seconds=3.0):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(dom.stream)
+        fn()
+        e1.record(dom.stream)
+        torch.cuda.synchronize()
+        n = max(2, int(seconds * 1e3 / max(e0.elapsed_time(e1), 1e-3)))
+        samples, stop = [], threading.Event()
+
+        def sample():
+            while not stop.is_set():
+                samples.append((pynvml.nvmlDeviceGetPowerUsage(H) / 1e3, pynvml.nvmlDeviceGetClockInfo(H, pynvml.NVML_CLOCK_SM)))
+                stop.wait(0.02)
+        th = threading.Thread(target=sample, daemon=True)
+        th.start()
+        e0.record(dom.stream)
+        for _ in range(n):
+            fn()
+        e1.record(dom.stream)
+        torch.cuda.synchronize()
+        stop.set()
+        th.join(timeout=5)
+        half = samples[len(samples) // 2:] or [(0.0, 0.0)]
+        w = float(np.mean([x[0] for x in half]))
+        ms = e0.elapsed_time(e1) / n
+        rows.append({"operation": name, "ms_per_launch": ms, "watt": w, "sm_mhz": float(np.median([x[1] for x in half])),
+                     "joule_per_launch": w * ms * 1e-3, "launches": n, "samples": len(samples)})
+        time.sleep(1.0)
+
+    time.sleep(2.0)
+    rows.append({"operation": "idle", "watt": pynvml.nvmlDeviceGetPowerUsage(H) / 1e3})
+    with torch.cuda.stream(dom.stream):
+        a = torch.empty(1 << 30, dtype=torch.bfloat16, device=dev)
+        b = torch.empty_like(a)
+        run("torch copy, 2 GiB read + 2 GiB written", lambda: b.copy_(a))
+        del a, b
+        x = torch.randn(8192, 8192, device=dev, dtype=torch.bfloat16)
+        y = torch.randn(8192, 8192, device=dev, dtype=torch.bfloat16)
+        run("cuBLAS bf16 8192^3", lambda: torch.matmul(x, y))
+        xf, yf = x.float(), y.float()
+        torch.backends.cuda.matmul.allow_tf32 = True
+        run("cuBLAS tf32 8192^3", lambda: torch.matmul(xf, yf))
+        del x, y, xf, yf
+    torch.cuda.empty_cache()
+    dom.set_orbitals(psi_dev, occ)
+    run("one Taylor-4 step of the whole batch (mlmd_propagate, 3xTF32)", lambda: dom.propagate(1, c.dt, A[:1]), 5.0)
+    E = torch.empty(c.ndom, dtype=torch.float64, device=dev)
+    run("projection, 3xTF32 (mlmd_energy_nl: proj2_tc_kernel + a reduction)", lambda: M.mlmd_energy_nl(dom.handle, E))
+    dom.set_gemm_mode(M.GEMM_FP32GRADE_STAGED)
+    run("the same step, staged mode", lambda: dom.propagate(1, c.dt, A[:1]), 5.0)
+    dom.set_gemm_mode(M.GEMM_LOWP_BF16)
+    run("the same step, low-precision (BF16) mode", lambda: dom.propagate(1, c.dt, A[:1]), 5.0)
+    dom.set_gemm_mode(M.GEMM_FP32GRADE)
+    dom.set_orbitals(psi_dev, occ)
+    run("Eq. (2) step, Taylor local solver (mlmd_propagate_split)", lambda: dom.propagate_split(1, c.dt, A[:1]), 4.0)
+    dom.set_option(M.OPT_LOCAL_SOLVER, 1)
+    run("Eq. (2) step, split-operator local solver", lambda: dom.propagate_split(1, c.dt, A[:1]), 4.0)
+    dom.set_option(M.OPT_LOCAL_SOLVER, 0)
+    # the local part alone: a second handle without projectors (four stencil passes + the density pass per step)
+    loc = M.Domain(c.ndom, c.grid, c.h, c.norb, 0, device=str(dev), stream=dom.stream)
+    loc.set_vloc(vloc)
+    loc.set_projectors(None, None)
+    loc.set_orbitals(psi_dev, occ)
+    run("four stencil passes + the density pass (a handle without projectors)", lambda: loc.propagate(1, c.dt, A[:1]))
+    loc.set_option(M.OPT_LOCAL_SOLVER, 1)
+    run("three split-operator passes + the density pass (the same handle)", lambda: loc.propagate_split(1, c.dt, A[:1]))
+    loc.close()
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -205,6 +288,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-observables", action="store_true")
     ap.add_argument("--no-staged", action="store_true", help="skip the extra timing of the same steps in the staged GEMM mode")
+    ap.add_argument("--power", action="store_true",
+                    help="instead of the bench line: board power / SM clock / energy per launch of each operation looping alone (NVML)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -269,6 +354,11 @@ def main():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.power:
+        if rank == 0:
+            print(json.dumps({"power_probe": power_probe(c, dom, psi_dev, occ, vloc, A, dev), "config": workload_config(c, args)}))
+        return
 
     # ---- warm-up (W steps), then EXACTLY K timed steps in one mlmd_propagate call
     if Wm > 0:
