@@ -603,7 +603,7 @@ static bool density_rides_on_projection(const mlmd_domain *h) {
 }
 
 static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl, int nprod = -1, int chain = -1,
-                            bool with_density = false) {
+                            bool with_density = false, const float *density_occ = nullptr) {
     // S2a + S2b: What = (-i tau) D' (beta^H w); nprod >= 0 overrides the mode's products per MAC (staged mode)
     if (nprod < 0) nprod = tc_nprod(h);
     const bool fp64 = h->gemm_mode == MLMD_GEMM_FP64;
@@ -614,7 +614,8 @@ static int nonlocal_project(mlmd_domain *h, const float2 *w, float tau, int *nl,
         if (tc)
             CU(launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
                               2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, nprod, chain > 0 ? chain : proj_chain(nprod), nl, &h->tmaps,
-                              with_density ? h->rho() : nullptr, h->occ(), lowp_bf16_storage(h) ? h->beta_lo() : nullptr));
+                              with_density ? h->rho() : nullptr, density_occ ? density_occ : h->occ(),
+                              lowp_bf16_storage(h) ? h->beta_lo() : nullptr));
         else
             CU(launch_proj_simt(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)w,
                                 2 * h->ld, 2 * h->ld, h->zpart(), h->prows, nsplit, fp64, nl));
@@ -738,8 +739,12 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         if (!rc) rc = nonlocal_back(h, h->psi(), nl);
         return rc ? rc : norm2(which);
     };
+    // S3 inside a call: the density of the state a step starts from (= the result of the previous step: psi in memory
+    // times the pending scale, i.e. occupations occ_eff = f scl^2) rides on the first kick's projection, which reads that
+    // state anyway (reading R4, as in the Taylor step); the separate density pass runs for other shapes / modes only
+    const bool fused_rho = kicks && density_rides_on_projection(h);
     auto kick_only = [&]() -> int {              // psi += (-i dt/2) V_NL psi
-        int rc = nonlocal_project(h, h->psi(), (float)(0.5 * dt), nl);
+        int rc = nonlocal_project(h, h->psi(), (float)(0.5 * dt), nl, -1, -1, fused_rho, h->occ_eff());
         return rc ? rc : nonlocal_back(h, h->psi(), nl);
     };
     if (kicks) {
@@ -811,9 +816,10 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         ProfScope ps(h, MLMD_K_GLUE);
         CU(launch_occ_eff(h->stream, h->ndom * h->ld, h->occ(), h->scl(), h->occ_eff(), nl));
     }
+    h->split_pending = true;
+    if (fused_rho) return MLMD_OK;      // the next step's first projection forms this step's rho; a call ends on a flush
     ProfScope ps(h, MLMD_K_DENSITY);
     CU(launch_density(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->occ_eff(), h->rho(), nl));
-    h->split_pending = true;
     return MLMD_OK;
 }
 
@@ -886,6 +892,8 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
     if (split && nsteps > 0 && h->nproj > 0) {      // squared norms of the incoming orbitals (reading D27)
         ProfScope ps(h, MLMD_K_NORM);
         CU(launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->nrm_part(), h->nrm(0), &nl));
+        // the incoming state carries no pending scale: its density (riding on the first kick's projection) takes occ itself
+        CU(cudaMemcpyAsync(h->occ_eff(), h->occ(), (size_t)h->ndom * h->ld * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
     }
     CU(cudaEventSynchronize(h->coef_uploaded));   // an earlier call's upload has left the pinned staging buffer
     for (int s0 = 0; s0 < nsteps; s0 += kCoefCapacity) {
