@@ -98,10 +98,10 @@ def algorithmic(c, gemm_real=True, step="taylor"):
     CALL for the incoming norms and one 16 B/element rescaling pass per CALL are not counted: inside a call psi stays
     un-normalised and the density takes the scale through the occupations)."""
     elems = c.ndom * c.ngrid * c.norb
-    # "richardson": three in-place passes (one per axis) and the norm pass ahead of them
+    # "richardson": three in-place passes (one per axis); no per-step norm pass either (norms from the projector Gram matrix)
     stage_bytes = [16, 16, 16] if step == "richardson" else [16, 24, 24, 24]
     split = step in SPLIT_STEPS
-    density_b, norm_b, ngemm = (8, 8 if step == "richardson" else 0, 4) if split else (8, 0, 8)
+    density_b, norm_b, ngemm = (8, 0, 4) if split else (8, 0, 8)
     bytes_step = elems * (sum(stage_bytes) + density_b + norm_b) + c.ndom * c.ngrid * (4 * 4 + 4)
     gemm_flops_each = (2 if gemm_real else 4) * 2.0 * c.ndom * c.ngrid * c.nproj * c.norb   # one GEMM batch
     return {"elems": elems, "bytes_step": bytes_step, "stencil_bytes": [elems * b for b in stage_bytes],

@@ -747,16 +747,32 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
         int rc = nonlocal_project(h, h->psi(), (float)(0.5 * dt), nl, -1, -1, fused_rho, h->occ_eff());
         return rc ? rc : nonlocal_back(h, h->psi(), nl);
     };
-    if (kicks) {
+    const bool rich = h->opt[MLMD_OPT_LOCAL_SOLVER] == 1;
+    // split-operator solver: ||psi_a||^2 after the first kick from the identity the second kick uses (below), with the
+    // squared norms of the state in memory at the start of the step, which nrm(3) holds (the previous step's ||psi_d||^2,
+    // or the incoming norms at the start of a call)
+    const bool quad_a = kicks && rich && h->gram_valid;
+    if (quad_a) {
+        int rc = nonlocal_project(h, h->psi(), (float)(0.5 * dt), nl, -1, -1, fused_rho, h->occ_eff());
+        if (rc) return rc;
+        {
+            ProfScope ps(h, MLMD_K_GLUE);
+            CU(launch_kick_quad(h->stream, h->ndom, h->P, h->ldg, h->ld, h->prows, h->gram(), h->what(), h->what_lo(), h->nrm(3),
+                                h->nrm(1), nl));
+        }
+        rc = nonlocal_back(h, h->psi(), nl);
+        if (rc) return rc;
+    } else if (kicks) {
         int rc = kick_only();
         if (rc) return rc;
     }
-    if (h->opt[MLMD_OPT_LOCAL_SOLVER] == 1) {
+    if (rich) {
         // the paper's own local solver (reading D33): three in-place passes of 2 x 2 nearest-neighbour rotations.  The
         // squared norms the kicks' normalisation needs (reading D27): before the solver by the norm pass; after it they are
         // the same numbers, because U_loc is unitary by construction (in the oracle to 1e-16; here the passes' FP32 rounding
-        // moves a norm by ~1e-7, and handing the second kick the norm BEFORE the solver takes that noise out again)
-        if (kicks) {
+        // moves a norm by ~1e-7, and handing the second kick the norm BEFORE the solver takes that noise out again).
+        // With the projector Gram matrix at hand (quad_a) the norm before the solver needs no pass over psi either
+        if (kicks && !quad_a) {
             int rc = norm2(1);
             if (rc) return rc;
         }
@@ -894,6 +910,8 @@ static int propagate_impl(mlmd_domain_t *h, int nsteps, double dt, const double 
         CU(launch_colnorm2(h->stream, h->ndom, h->ngrid, h->ld, h->psi(), h->nrm_part(), h->nrm(0), &nl));
         // the incoming state carries no pending scale: its density (riding on the first kick's projection) takes occ itself
         CU(cudaMemcpyAsync(h->occ_eff(), h->occ(), (size_t)h->ndom * h->ld * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+        // nrm(3) = squared norms of the state in memory at the start of a step (enqueue_split_step, quad_a)
+        CU(cudaMemcpyAsync(h->nrm(3), h->nrm(0), (size_t)h->ndom * h->ld * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
     }
     CU(cudaEventSynchronize(h->coef_uploaded));   // an earlier call's upload has left the pinned staging buffer
     for (int s0 = 0; s0 < nsteps; s0 += kCoefCapacity) {
