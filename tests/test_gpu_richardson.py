@@ -122,3 +122,28 @@ def test_richardson_rejects_an_odd_axis_and_leaves_the_taylor_path_alone():
     dom.set_option(M.OPT_LOCAL_SOLVER, 0)
     assert dom.propagate_split(1, 0.02, np.zeros((1, 1, 3))) == M.OK
     dom.close()
+
+
+@pytest.mark.parametrize("kick_norm,lowp", [(1, False), (0, True)])
+def test_richardson_other_norm_path_and_low_precision_mode(kick_norm, lowp):
+    """MLMD_OPT_KICK_NORM = 1 (every norm by a pass over psi: the path shapes without a usable projector Gram matrix take) and
+    the opt-in low-precision GEMM mode (1e-3; the density then comes from the separate pass) around the same local solver,
+    on one configs[2] domain (tcgen05 kicks); the occupations afterwards follow the oracle's overlap."""
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    from test_gpu_parity import TOL_LOWP
+    c = W.get_config(2, ndom=1, nsteps=3)
+    d = W.generate(c)
+    A = W.laser_samples(c, nsteps=3, t0=0.9)
+    dom = make_domain(c, d, flags=M.KEEP_PSI0, mode=M.GEMM_LOWP_BF16 if lowp else None)
+    dom.set_option(M.OPT_LOCAL_SOLVER, 1)
+    dom.set_option(M.OPT_KICK_NORM, kick_norm)
+    dom.propagate_split(3, c.dt, A)
+    r, rho_ref = ref.propagate_split(d["psi"], d["occ"], d["vloc"], d["beta"], d["D"], A, c.dt, c.h, local="richardson")
+    tol_psi, tol_rho = (TOL_LOWP, TOL_LOWP) if lowp else (TOL_LAST, TOL_RHO)
+    assert orb_err(dom.get_orbitals(), r) <= tol_psi
+    assert rho_err(dom.density(), rho_ref) <= tol_rho
+    f, nexc = dom.occupations()
+    f_ref, _ = ref.occupations(ref.overlap(d["psi"], r, c.dv), d["occ"])
+    assert np.abs(f - f_ref).max() <= (1e-3 if lowp else 1e-5) * d["occ"].max()
+    dom.close()
