@@ -78,3 +78,25 @@ def test_gemm_mode_enum_matches_header():
                     "GEMM_FP32GRADE_STAGED": 5}
     for name, value in enum.items():
         assert getattr(api, name) == value
+
+
+def test_option_enum_matches_header_and_split_steps_are_accounted():
+    """The binding's option keys are the header's enum values, and bench.py's accounting knows the three step forms."""
+    import re
+    sys.path.insert(0, ROOT)
+    from paper_2509_00966_b200 import api
+    import bench
+    import workloads as W
+    text = open(os.path.join(ROOT, "include", "mlmd.h")).read()
+    enum = dict((m.group(1), int(m.group(2))) for m in re.finditer(r"MLMD_(OPT_\w+)\s*=\s*(\d+)", text))
+    assert enum == {"OPT_GRAPH": 0, "OPT_STENCIL": 1, "OPT_GEMM_PATH": 2, "OPT_KICK_NORM": 3, "OPT_FD_ORDER": 4,
+                    "OPT_LOCAL_SOLVER": 5, "OPT_COUNT": 6}
+    for name, value in enum.items():
+        if name != "OPT_COUNT":
+            assert getattr(api, name) == value
+    c = W.get_config(3)
+    elems = 64 * 48 ** 3 * 224
+    taylor, split, rich = (bench.algorithmic(c, step=s) for s in ("taylor", "split", "richardson"))
+    assert split["gemm_flops_step"] * 2 == taylor["gemm_flops_step"] == rich["gemm_flops_step"] * 2   # two V_NL applications, not four
+    assert split["bytes_step"] == taylor["bytes_step"]                       # four Horner stages of h_loc + the density
+    assert rich["bytes_step"] == elems * (3 * 16 + 8) + 64 * 48 ** 3 * 20     # three in-place passes + the density
