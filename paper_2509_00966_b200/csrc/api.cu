@@ -769,7 +769,7 @@ static int enqueue_split_step(mlmd_domain *h, const StepCoef *coef, const StepCo
     if (rich) {
         // the paper's own local solver (reading D33): three in-place passes of 2 x 2 nearest-neighbour rotations.  The
         // squared norms the kicks' normalisation needs (reading D27): before the solver by the norm pass; after it they are
-        // the same numbers, because U_loc is unitary by construction (in the oracle to 1e-16; here the passes' FP32 rounding
+        // the same numbers, because U_loc is unitary by construction (exactly so in exact arithmetic; here the passes' FP32 rounding
         // moves a norm by ~1e-7, and handing the second kick the norm BEFORE the solver takes that noise out again).
         // With the projector Gram matrix at hand (quad_a) the norm before the solver needs no pass over psi either
         if (kicks && !quad_a) {
