@@ -253,7 +253,8 @@ int mlmd_ref_propagate(int ndom, int nx, int ny, int nz, double hx, double hy, d
  *   D28: exp(-i dt h_loc) is the same 4th-order Taylor sum as the full-H step, applied to h_loc
  *        alone (the paper's own local solver is only named, L147; NEXT-3).
  * kick_only is a bit mask: 1 skips the local propagator (pin S3); 2 evaluates exp(-i dt h_loc) by the paper's own
- * block-diagonal split-operator solver on 2nd-order differences (reading D33) instead of the Taylor sum.
+ * block-diagonal split-operator solver on 2nd-order differences (reading D33) instead of the Taylor sum; 4 takes the
+ * Taylor sum on the 2nd-order (7-point) differences of reading D32 instead of the 4th-order ones.
  */
 /* ---- the paper's own local solver: block-diagonal split-operator (reading D33) ----
  *
@@ -377,7 +378,8 @@ int mlmd_ref_propagate_split(int ndom, int nx, int ny, int nz, double hx, double
                 memcpy(phi, p, ne * sizeof(zc));
                 memcpy(acc, p, ne * sizeof(zc));
                 for (int m = 1; m <= 4 && !rc; ++m) {
-                    rc = mlmd_ref_apply_h(nx, ny, nz, hx, hy, hz, norb, 0, phi, hphi, v, NULL, NULL, Av, 0);
+                    rc = mlmd_ref_apply_h(nx, ny, nz, hx, hy, hz, norb, 0, phi, hphi, v, NULL, NULL, Av,
+                                          (kick_only & 4) ? MLMD_REF_ORDER2 : 0);
                     const zc f = -I * dt / (double)m;
                     for (size_t e = 0; e < ne; ++e) {
                         phi[e] = f * hphi[e];

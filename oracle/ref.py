@@ -108,11 +108,12 @@ def propagate(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], nsteps:
 
 
 def propagate_split(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], nsteps: Optional[int] = None,
-                    kick_only: bool = False, local: str = "taylor") -> Tuple[np.ndarray, np.ndarray]:
+                    kick_only: bool = False, local: str = "taylor", order: int = 4) -> Tuple[np.ndarray, np.ndarray]:
     """nsteps steps of the paper's literal Eq. (2): half-kick, exp(-i dt h_loc), half-kick.  local = "taylor": the
     4th-order Taylor sum on 4th-order differences (reading D28); "richardson": the paper's own block-diagonal
-    split-operator solver on 2nd-order differences (reading D33).  Same arguments and return values as ``propagate``."""
-    assert local in ("taylor", "richardson")
+    split-operator solver on 2nd-order differences (reading D33).  order = 2: the Taylor sum on the 2nd-order (7-point)
+    differences of reading D32.  Same arguments and return values as ``propagate``."""
+    assert local in ("taylor", "richardson") and order in (2, 4)
     p = _c128(psi).copy()
     ndom, nx, ny, nz, norb = p.shape
     vloc = _f64(vloc)
@@ -127,7 +128,7 @@ def propagate_split(psi, occ, vloc, beta, D, A, dt: float, h: Sequence[float], n
     rho = np.empty((ndom, nx, ny, nz), dtype=np.float64)
     rc = lib().mlmd_ref_propagate_split(ndom, nx, ny, nz, h[0], h[1], h[2], norb, nproj, _ptr(p), _ptr(occ),
                                         _ptr(vloc), _ptr(b), _ptr(dd), nsteps, dt, _ptr(A), A.shape[1], _ptr(rho),
-                                        (1 if kick_only else 0) | (2 if local == "richardson" else 0))
+                                        (1 if kick_only else 0) | (2 if local == "richardson" else 0) | (4 if order == 2 else 0))
     if rc:
         raise RuntimeError("mlmd_ref_propagate_split failed: %d" % rc)
     return p, rho

@@ -169,3 +169,35 @@ def test_c3_real_orbitals_and_real_projectors_carry_no_nonlocal_current():
     X = RNG.uniform(-2, 2, (3, 1, ngrid, 1))
     J = ref.current_nl(psi, np.array([[2.0, 1.0]]), beta, X * beta[None], RNG.uniform(-1, 1, (1, 3)), dv)
     assert np.abs(J).max() < 1e-12
+
+
+def test_o2f_eq2_step_on_second_order_differences_from_dense_matrices():
+    """O2f: mlmd_ref_propagate_split(order=2) = kick, Taylor-4 of the dense 2nd-order h_loc (Vandermonde-solved weights), kick:
+    the order switch reaches the local propagator of the Eq. (2) step and nothing else."""
+    from oracle import ref
+    from test_oracle_pins import rand_c, rel
+    grid, h, dt, nsteps = (5, 6, 5), (0.5, 0.4, 0.45), 0.04, 2
+    ngrid, dv = int(np.prod(grid)), float(np.prod(h))
+    psi = rand_c(1, *grid, 3)
+    vloc = RNG.uniform(-1, 0.5, (1, *grid))
+    beta = rand_c(1, ngrid, 4) * 0.6
+    D = RNG.uniform(-2, 2, (1, 4))
+    A = RNG.uniform(-0.2, 0.2, (nsteps, 1, 3))
+    out, _ = ref.propagate_split(psi, np.full((1, 3), 2.0), vloc, beta, D, A, dt, h, order=2)
+    x = psi[0].reshape(ngrid, 3).astype(np.complex128)
+    V = dv * (beta[0] * D[0][None, :]) @ beta[0].conj().T
+
+    def kick(y):
+        z = y - 0.5j * dt * (V @ y)
+        return z * (np.linalg.norm(y, axis=0) / np.linalg.norm(z, axis=0))[None, :]
+    for n in range(nsteps):
+        x = kick(x)
+        z = -1j * dt * dense_h_order2(grid, h, vloc[0], A[n, 0])
+        term, acc = x.copy(), x.copy()
+        for m in range(1, 5):
+            term = z @ term / m
+            acc = acc + term
+        x = kick(acc)
+    assert rel(out[0].reshape(ngrid, 3), x) < 1e-12
+    o4, _ = ref.propagate_split(psi, np.full((1, 3), 2.0), vloc, beta, D, A, dt, h)
+    assert rel(o4, out) > 1e-4          # the 4th-order step is a different operator
