@@ -151,9 +151,8 @@ def test_second_order_stencil_plane_waves_and_field_components():
 
 def test_second_order_stencil_perovskite_domain_and_split_step():
     """One configs[2] domain (48^3: the TMA kernel's radius-1 instantiation with the tcgen05 GEMMs), Taylor and the
-    literal Eq. (2) split step.  (The oracle's split step has no order switch: with nproj = 0 the split step is the
-    Taylor step, which pins the stencil of mlmd_propagate_split; with projectors the two GPU steppers are compared
-    through their common limit instead.)"""
+    literal Eq. (2) split step (through its nproj = 0 limit, where it is the Taylor step, and with projectors against the
+    oracle's order switch)."""
     import paper_2509_00966_b200 as M
     from oracle import ref
     c = W.get_config(2, ndom=1, nsteps=3)
@@ -172,3 +171,9 @@ def test_second_order_stencil_perovskite_domain_and_split_step():
     r0, _ = ref.propagate(d["psi"], d["occ"], d["vloc"], None, None, A, c.dt, c.h, flags=ref.ORDER2)
     assert orb_err(nop.get_orbitals(), r0) <= TOL_LAST
     nop.close()
+    # the Eq. (2) step with projectors on the 7-point operator against the oracle's own order switch (pin O2f)
+    sp = make_domain(c, d, options=[(M.OPT_FD_ORDER, 2)])
+    sp.propagate_split(3, c.dt, A)
+    rs, rho_s = ref.propagate_split(d["psi"], d["occ"], d["vloc"], d["beta"], d["D"], A, c.dt, c.h, order=2)
+    assert orb_err(sp.get_orbitals(), rs) <= TOL_LAST and rho_err(sp.density(), rho_s) <= TOL_RHO
+    sp.close()
