@@ -89,8 +89,9 @@ enum {
     MLMD_OPT_STENCIL = 1,   /* 0 (default): TMA-staged kernel when ny, nz are multiples of 16, else the fallbacks;
                              * 1: register-marching kernel; 2: one-thread-per-output kernel (cross-checks)            */
     MLMD_OPT_GEMM_PATH = 2, /* 0 (default): tcgen05 kernels when ngrid is a multiple of 128; 1: CUDA-core kernels        */
-    MLMD_OPT_KICK_NORM = 3, /* mlmd_propagate_split, norm after the second kick: 0 (default) from the projector Gram
-                             * matrix when it applies; 1: always by a pass over psi                                   */
+    MLMD_OPT_KICK_NORM = 3, /* mlmd_propagate_split, norm after the second kick (and, with MLMD_OPT_LOCAL_SOLVER = 1, after
+                             * the first): 0 (default) from the projector Gram matrix when it applies; 1: always by a pass
+                             * over psi                                                                               */
     MLMD_OPT_FD_ORDER = 4,  /* order of the central finite differences of the kinetic and A.grad terms: 4 (default; north_star:
                              * 13-point star) or 2 (the paper's own "7-point star stencil" on "nearest-neighbor mesh points",
                              * PAPER.md L147, L283): c2 = [1, -2, 1] / h^2, c1 = [-1/2, 0, 1/2] / h.
@@ -157,7 +158,10 @@ MLMD_API int mlmd_propagate(mlmd_domain_t *h, int nsteps, double dt, const doubl
  * a second half-kick.  With beta = Psi(0) (MLMD_BETA_COMPLEX64) and D_p = const this V_NL is the nonlocal
  * correction of Eq. (5) L199 with delta = -i dt/2 D dv.  Two V_NL applications per step instead of four.
  * Arguments, density and return values as mlmd_propagate; the stability bound leaves out max|D| (the
- * normalised kick is stable for any dt |D|).  With nproj = 0 it is the same map as mlmd_propagate. */
+ * normalised kick is stable for any dt |D|).  With nproj = 0 it is the same map as mlmd_propagate.
+ * With MLMD_OPT_LOCAL_SOLVER = 1 the middle factor is the paper's own block-diagonal split-operator solver on the
+ * 7-point operator (reading D33) instead of the Taylor sum: unitary for any dt (no stability
+ * warning), needs even nx, ny, nz (else MLMD_ERR_SHAPE). */
 MLMD_API int mlmd_propagate_split(mlmd_domain_t *h, int nsteps, double dt, const double *A, int a_ndom);
 
 /* rho(r) = sum_n f_n |psi_n(r)|^2 of the current state, float [ndom][nx][ny][nz] at `where`. */
