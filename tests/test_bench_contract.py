@@ -88,7 +88,7 @@ def test_option_enum_matches_header_and_split_steps_are_accounted():
     import bench
     import workloads as W
     text = open(os.path.join(ROOT, "include", "mlmd.h")).read()
-    enum = dict((m.group(1), int(m.group(2))) for m in re.finditer(r"MLMD_(OPT_\w+)\s*=\s*(\d+)", text))
+    enum = dict((m.group(1), int(m.group(2))) for m in re.finditer(r"^\s+MLMD_(OPT_\w+)\s*=\s*(\d+)", text, re.M))
     assert enum == {"OPT_GRAPH": 0, "OPT_STENCIL": 1, "OPT_GEMM_PATH": 2, "OPT_KICK_NORM": 3, "OPT_FD_ORDER": 4,
                     "OPT_LOCAL_SOLVER": 5, "OPT_COUNT": 6}
     for name, value in enum.items():
