@@ -10,10 +10,10 @@
 // up to e^{-i dt sum_d a_d} per step: they ride in P, whose argument is then V_loc + the `centre` of the 2nd-order StepCoef).
 //
 // One pass per axis, in place (16 B per element and pass: 48 B per step against 88 B for the Taylor sum): a thread owns the
-// EVEN pair (2p, 2p+1) of its line for one float4 (two orbitals), so the two even sweeps are register-only; for the odd sweep
-// the even points go through shared memory once (thread p rotates its point 2p+1 with point 2p+2 of thread p+1; the last
-// pair wraps, which is why every axis needs an even number of points).  Eight float4 lanes per line keep every access a full
-// 128-byte line whatever the axis.  The rotation constants of a step are computed in FP64 by a one-block kernel ahead of the
+// EVEN pair (2p, 2p+1) of its line for one or two float4 (two or four orbitals), so the two even sweeps are register-only; for
+// the odd sweep the even points go through shared memory once (thread p rotates its point 2p+1 with point 2p+2 of thread p+1;
+// the last pair wraps, which is why every axis needs an even number of points).  Eight threads side by side on a point keep
+// every access a full 128-byte line (two of them with two float4 per thread) whatever the axis.  The rotation constants of a step are computed in FP64 by a one-block kernel ahead of the
 // three passes (from the step's device-resident StepCoef, so a CUDA graph replays them); a rounded (cos, sin) pair is off the
 // unit circle by ~6e-8, the SAME factor on every point in every sweep: the last pass takes the product of the nine factors out
 // again (see make_rot), so what remains is the FP32 rounding of the products.
