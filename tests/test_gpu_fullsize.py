@@ -30,23 +30,36 @@ _oracle_cache = {}
 MEASURED = []          # (label, errors) of every run: printed at the end of the module (copied to profiles/)
 
 
+_batch_cache = {}      # cfg -> (psi_dev, beta_dev, vloc, occ, D): a batch is generated once per session, not once per test
+_domain_cache = {}     # (cfg, k) -> host copy of one generated domain
+
+
 def load_batch(c, keep):
-    """The whole batch on the device, generated domain by domain as bench.py does; host copies of `keep` only."""
+    """The whole batch on the device, generated domain by domain as bench.py does; host copies of `keep` only.
+    The device tensors are shared by the tests of this module (nothing writes to them: the library copies what
+    mlmd_set_orbitals / mlmd_set_projectors are given) and released by the module's last test."""
     import torch
-    dev = torch.device("cuda", 0)
-    psi_dev = torch.empty((c.ndom, *c.grid, c.norb), dtype=torch.complex64, device=dev)
-    beta_dev = torch.empty((c.ndom, c.ngrid, c.nproj), dtype=torch.float32, device=dev)
-    vloc = np.empty((c.ndom, *c.grid), dtype=np.float32)
-    occ = np.empty((c.ndom, c.norb))
-    D = np.empty((c.ndom, c.nproj))
+    if c.cfg not in _batch_cache:
+        dev = torch.device("cuda", 0)
+        psi_dev = torch.empty((c.ndom, *c.grid, c.norb), dtype=torch.complex64, device=dev)
+        beta_dev = torch.empty((c.ndom, c.ngrid, c.nproj), dtype=torch.float32, device=dev)
+        vloc = np.empty((c.ndom, *c.grid), dtype=np.float32)
+        occ = np.empty((c.ndom, c.norb))
+        D = np.empty((c.ndom, c.nproj))
+        with ThreadPoolExecutor(max_workers=max(1, min(8, (os.cpu_count() or 2) // 2))) as ex:
+            for k, dd in enumerate(ex.map(lambda k: W.generate_domain(c, k), range(c.ndom))):
+                psi_dev[k].copy_(torch.from_numpy(dd["psi"]))
+                beta_dev[k].copy_(torch.from_numpy(dd["beta"]))
+                vloc[k], occ[k], D[k] = dd["vloc"], dd["occ"], dd["D"]
+                if k in keep:
+                    _domain_cache[(c.cfg, k)] = dd
+        _batch_cache[c.cfg] = (psi_dev, beta_dev, vloc, occ, D)
+    psi_dev, beta_dev, vloc, occ, D = _batch_cache[c.cfg]
     kept = {}
-    with ThreadPoolExecutor(max_workers=max(1, min(8, (os.cpu_count() or 2) // 2))) as ex:
-        for k, dd in enumerate(ex.map(lambda k: W.generate_domain(c, k), range(c.ndom))):
-            psi_dev[k].copy_(torch.from_numpy(dd["psi"]))
-            beta_dev[k].copy_(torch.from_numpy(dd["beta"]))
-            vloc[k], occ[k], D[k] = dd["vloc"], dd["occ"], dd["D"]
-            if k in keep:
-                kept[k] = dd
+    for k in keep:
+        if (c.cfg, k) not in _domain_cache:
+            _domain_cache[(c.cfg, k)] = W.generate_domain(c, k)
+        kept[k] = _domain_cache[(c.cfg, k)]
     return psi_dev, beta_dev, vloc, occ, D, kept
 
 
@@ -113,7 +126,10 @@ def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, to
             worst = float(orb_errs(out[whole].cpu().numpy(), r).max())
             errs["rho_" + tag] = float(np.abs(rho[whole].cpu().numpy() - rho_ref).max() / rho_ref.max())
             G = dom.overlap(0)[whole]
-            G_ref = ref.overlap(r[None], r[None], c.dv)[0]
+            gkey = (c.cfg, whole, n, split, local, "gram")     # the oracle's Gram matrix of that state: once per session
+            if gkey not in _oracle_cache:
+                _oracle_cache[gkey] = ref.overlap(r[None], r[None], c.dv)[0]
+            G_ref = _oracle_cache[gkey]
             errs["gram_" + tag] = float(np.abs(G - G_ref).max())
         if n in (1, nsteps):
             for k, orbs in sample.items():
@@ -222,6 +238,12 @@ def test_config3_full_batch_staged_mode_as_benchmarked():
 
 
 def test_zz_print_measured_errors():
-    """Not a check: prints the table of measured errors of this module's runs (copied into profiles/)."""
+    """Not a check: prints the table of measured errors of this module's runs (copied into profiles/) and releases the
+    batches this module kept on the device."""
+    import torch
     for label, errs in MEASURED:
         print("| %s | %s |" % (label, " | ".join("%s %.3e" % kv for kv in sorted(errs.items()))))
+    _batch_cache.clear()
+    _domain_cache.clear()
+    _oracle_cache.clear()
+    torch.cuda.empty_cache()
