@@ -10,7 +10,7 @@ runs on exactly the data it is compared on):
   * scattered (domain, orbital) samples in other domains - first and last domain of the batch, orbitals in every
     column tile of the GEMMs - after the first and the last step.
 configs[4] (696 orbitals, 64^3, 810 projectors: 80 s of oracle time per step and domain) takes the whole domain for
-the first step (orbitals, density, Gram) and 48 orbitals spread over all column tiles for the 10 steps.
+the first step (orbitals, density, Gram) and 25 orbitals spread over all column tiles (every tile edge) for the 10 steps.
 On every domain the electron count of rho is checked against the GPU's own orbitals (a sum rule, not parity).
 Tolerances are north_star's: 1e-5 after one step, 1e-4 after the last, density 1e-4, Gram 1e-5; 1e-3 for all of
 them in the low-precision mode.  Oracle results are cached per (config, domain, orbitals, steps) within the session.
@@ -164,7 +164,7 @@ def run_full(cfg, whole, whole_steps, sample, nsteps, split=False, mode=None, to
 # orbitals in every 224-column (112-orbital) tile of the projection and at the tile edges
 SAMPLE_224 = [0, 1, 111, 112, 223]
 # configs[4]: 696 orbitals = 1392 columns -> 7 column tiles of 224 columns (112 orbitals, the last one ragged)
-SAMPLE_696 = sorted(set([0, 1, 111, 112, 223, 224, 335, 336, 447, 448, 559, 560, 671, 672, 695] + list(range(5, 696, 21))))
+SAMPLE_696 = sorted(set([0, 1, 111, 112, 223, 224, 335, 336, 447, 448, 559, 560, 671, 672, 695] + list(range(5, 696, 70))))
 
 
 def test_config2_full_batch_20_steps():
