@@ -598,7 +598,9 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
 // The step's first projection reads every psi row exactly once: on the CTA-pair kernel it can carry the density of
 // that state (S3) in its converter warps, so the separate 8 B/element pass over psi runs only once per call.
 static bool density_rides_on_projection(const mlmd_domain *h) {
-    return h->nproj > 0 && use_tensor_cores(h) && h->gemm_mode == MLMD_GEMM_FP32GRADE &&
+    // (the staged mode's first projection of a step takes one product of rounded operands: it carries the density too)
+    return h->nproj > 0 && use_tensor_cores(h) &&
+           (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED) &&
            proj_tc_can_fuse_density(h->P, 2 * h->ld, 3);
 }
 

@@ -702,7 +702,27 @@ proj2_tc_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant
                         for (int i = t; i < P2_A_BYTES / 16; i += 128) a4[i] = bf16_round4(a4[i]);
                     } else if (!LO) {
                         for (int i = t; i < P2_A_BYTES / 16; i += 128) a4[i] = tf32_rn4(a4[i]);
-                        if (q.rn)
+                        if (q.rn && q.rho) {
+                            // S3 fused, as in the three-product branch below (same tile layout, same thread -> row / orbital map):
+                            // the density is summed from the values as loaded, then psi is rounded in place
+                            const int r = (t >> 3) & 15, w = t & 7;
+                            const int pair_in_chunk = (((w >> 1) ^ (r & 3)) << 1) | (w & 1);
+                            const float2 *f2 = (const float2 *)(q.occ + (size_t)dom * (q.N / 2));
+                            float acc = 0.f;
+                            int j = 0;
+                            for (int i = t; i < ny4; i += 128, ++j) {
+                                const float4 v = y4[i];
+                                const int gch = j < h0 ? ct.start / 32 + crank * h0 + j : ct.start / 32 + n0 / 32 + crank * h1 + (j - h0);
+                                const float2 ff = __ldg(f2 + gch * 8 + pair_in_chunk);
+                                acc = fmaf(ff.x, fmaf(v.x, v.x, v.y * v.y), acc);
+                                acc = fmaf(ff.y, fmaf(v.z, v.z, v.w * v.w), acc);
+                                y4[i] = tf32_rn4(v);
+                            }
+                            acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+                            acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+                            acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+                            if (w == 0) atomicAdd(q.rho + (size_t)dom * q.ngrid + (size_t)kb * PJ_BK + r, acc);
+                        } else if (q.rn)
                             for (int i = t; i < ny4; i += 128) y4[i] = tf32_rn4(y4[i]);
                     } else {
                         // elementwise on the swizzled image: the lo tile has the same layout as the hi tile
@@ -1508,7 +1528,7 @@ int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
 
 bool proj_tc_can_fuse_density(int P, int N, int nprod) {
     // one pair of CTAs sees every psi row exactly once, each CTA half of its columns: two addends per rho element
-    return nprod == 3 && N % 64 == 0 && N <= BK_MAXBN && P <= 256;
+    return (nprod == 3 || nprod == 4) && N % 64 == 0 && N <= BK_MAXBN && P <= 256;
 }
 
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,

@@ -136,3 +136,40 @@ def test_staged_cuda_graph_equals_eager_and_mode_switch_drops_the_graph():
     assert np.array_equal(dom.get_orbitals(), outs["1"][0])
     assert not np.array_equal(pure, outs["1"][0])
     dom.close()
+
+
+def test_staged_density_rides_on_the_one_product_projection():
+    """In the staged mode the step's first projection takes one product of rounded operands; it carries the density of the
+    previous step like the default mode's three-product projection does: random occupations, one call and step by step,
+    against the oracle and bit for bit against each other; the rho formed inside the projection through the test hook."""
+    import ctypes
+    import torch
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    from test_gpu_parity import TOL_LAST, TOL_RHO, make_domain, orb_err, rho_err
+    c = W.get_config(1, nsteps=6)
+    d = W.generate(c)
+    occ = np.random.default_rng(6).uniform(0, 2, d["occ"].shape)
+    A = W.laser_samples(c, nsteps=6, t0=0.9)
+    r, rho_ref = ref.propagate(d["psi"], occ, d["vloc"], d["beta"], d["D"], A, c.dt, c.h)
+    outs = []
+    for graph, chunks in ((0, [6]), (1, [6]), (0, [1, 2, 3])):
+        dom = make_domain(c, dict(d, occ=occ), mode=M.GEMM_FP32GRADE_STAGED, options=[(M.OPT_GRAPH, graph)])
+        done = 0
+        for n in chunks:
+            dom.propagate(n, c.dt, A[done:done + n])
+            done += n
+        outs.append((dom.get_orbitals(), dom.density()))
+        dom.close()
+        assert rho_err(outs[-1][1], rho_ref) <= TOL_RHO and orb_err(outs[-1][0], r) <= TOL_LAST
+    for o in outs[1:]:
+        assert np.array_equal(o[0], outs[0][0]) and np.array_equal(o[1], outs[0][1])
+    hook = ctypes.CDLL(M.api.TEST_LIB_PATH).mlmd_debug_fused_density_np
+    hook.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
+    dom = make_domain(c, dict(d, occ=occ), mode=M.GEMM_FP32GRADE_STAGED)
+    dom.propagate(2, c.dt, A[:2])
+    rho_fused = torch.empty((c.ndom, *c.grid), dtype=torch.float32, device="cuda")
+    assert hook(dom.handle, rho_fused.data_ptr(), 4) == 0
+    _, rho2 = ref.propagate(d["psi"], occ, d["vloc"], d["beta"], d["D"], A[:2], c.dt, c.h)
+    assert rho_err(rho_fused.cpu().numpy(), rho2) <= TOL_RHO and rho_err(dom.density(), rho2) <= TOL_RHO
+    dom.close()
