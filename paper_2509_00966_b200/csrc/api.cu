@@ -599,8 +599,9 @@ static void fill_coef(const mlmd_domain *h, const double *A3, StepCoef *c) {
 // that state (S3) in its converter warps, so the separate 8 B/element pass over psi runs only once per call.
 static bool density_rides_on_projection(const mlmd_domain *h) {
     // (the staged mode's first projection of a step takes one product of rounded operands: it carries the density too)
+    // and so does the low-precision mode's BF16 kernel (it sums the FP32 values it packs)
     return h->nproj > 0 && use_tensor_cores(h) &&
-           (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED) &&
+           (h->gemm_mode == MLMD_GEMM_FP32GRADE || h->gemm_mode == MLMD_GEMM_FP32GRADE_STAGED || lowp_bf16_storage(h)) &&
            proj_tc_can_fuse_density(h->P, 2 * h->ld, 3);
 }
 

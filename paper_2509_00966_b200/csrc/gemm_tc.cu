@@ -962,6 +962,26 @@ proj2h_tc_kernel(const __grid_constant__ CUtensorMap map_a16, const __grid_const
                     uint8_t *st = smem + s * SB;
                     const float4 *y4 = (const float4 *)(st + YOFF);
                     const uint32_t y16 = smem_u32(st + Y16OFF) + dst_off;
+                    if (q.rho) {
+                        // S3 fused, as in proj2_tc_kernel (same FP32 tile layout, same thread -> row / orbital map): the density
+                        // is summed from the FP32 values as loaded, before they are packed to BF16
+                        const int pair_in_chunk = (((w >> 1) ^ (r & 3)) << 1) | (w & 1);
+                        const float2 *f2 = (const float2 *)(q.occ + (size_t)dom * (q.N / 2));
+                        float acc = 0.f;
+                        for (int j = 0; j < nch; ++j) {
+                            const float4 v = y4[j * 128 + t];
+                            const int gch = j < ct.h0 ? ct.start / 32 + crank * ct.h0 + j
+                                                      : ct.start / 32 + ct.n0 / 32 + crank * ct.h1 + (j - ct.h0);
+                            const float2 ff = __ldg(f2 + gch * 8 + pair_in_chunk);
+                            acc = fmaf(ff.x, fmaf(v.x, v.x, v.y * v.y), acc);
+                            acc = fmaf(ff.y, fmaf(v.z, v.z, v.w * v.w), acc);
+                            sts2(y16 + j * (PJ_BK * 64), pack_bf16(v.x, v.y), pack_bf16(v.z, v.w));
+                        }
+                        acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+                        acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+                        acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+                        if (w == 0) atomicAdd(q.rho + (size_t)dom * q.ngrid + (size_t)kb * PJ_BK + r, acc);
+                    } else
                     for (int j = 0; j < nch; ++j) {
                         const float4 v = y4[j * 128 + t];
                         sts2(y16 + j * (PJ_BK * 64), pack_bf16(v.x, v.y), pack_bf16(v.z, v.w));
@@ -1528,7 +1548,8 @@ int tc_choose_nsplit(int ndom, long ngrid, int P, int N) {
 
 bool proj_tc_can_fuse_density(int P, int N, int nprod) {
     // one pair of CTAs sees every psi row exactly once, each CTA half of its columns: two addends per rho element
-    return (nprod == 3 || nprod == 4) && N % 64 == 0 && N <= BK_MAXBN && P <= 256;
+    // (nprod 0: the BF16 kind::f16 kernel, i.e. only with a BF16 copy of A)
+    return (nprod == 3 || nprod == 4 || nprod == 0) && N % 64 == 0 && N <= BK_MAXBN && P <= 256;
 }
 
 cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A_hi, const float *A_lo, int lda, int P,
@@ -1562,7 +1583,7 @@ cudaError_t launch_proj_tc(cudaStream_t st, int ndom, long ngrid, const float *A
     q.rho = nullptr;
     q.occ = occ;
     if (rho) {
-        if (!(A_lo == nullptr && proj_tc_can_fuse_density(P, N, nprod)) || ldy != N) return cudaErrorInvalidValue;
+        if (!(A_lo == nullptr && proj_tc_can_fuse_density(P, N, nprod)) || ldy != N || (nprod == 0 && !A16)) return cudaErrorInvalidValue;
         cudaError_t e = cudaMemsetAsync(rho, 0, (size_t)ndom * ngrid * sizeof(float), st);
         if (e != cudaSuccess) return e;
         q.rho = rho;

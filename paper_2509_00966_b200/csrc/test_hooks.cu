@@ -40,14 +40,16 @@ HOOK int mlmd_debug_back(int path, void *stream, int ndom, long ngrid, const flo
 // end of every call, so it cannot be seen through the C ABI: this hook runs that projection on the handle's current
 // psi and copies the rho it formed to rho_dev [ndom][ngrid] (device).  Returns a cudaError_t value, -1 if the shape
 // cannot carry the density.
-// nprod: 3 = the default mode's three-product projection, 4 = the staged mode's one-product projection of rounded operands.
+// nprod: 3 = the default mode's three-product projection, 4 = the staged mode's one-product projection of rounded operands,
+// 0 = the low-precision mode's BF16 projection (the handle must be in that mode: beta's BF16 copy lives in the remainder buffer).
 HOOK int mlmd_debug_fused_density_np(mlmd_domain_t *h, float *rho_dev, int nprod);
 HOOK int mlmd_debug_fused_density(mlmd_domain_t *h, float *rho_dev) { return mlmd_debug_fused_density_np(h, rho_dev, 3); }
 HOOK int mlmd_debug_fused_density_np(mlmd_domain_t *h, float *rho_dev, int nprod) {
     if (!h->tc_ok || !proj_tc_can_fuse_density(h->P, 2 * h->ld, nprod) || h->nproj == 0) return -1;
     int nl = 0;
     cudaError_t e = launch_proj_tc(h->stream, h->ndom, h->ngrid, h->beta(), nullptr, h->ldp, h->P, (const float *)h->psi(), 2 * h->ld,
-                                   2 * h->ld, h->zpart(), h->prows, h->nsplit_tc, nprod, 128, &nl, nullptr, h->rho(), h->occ());
+                                   2 * h->ld, h->zpart(), h->prows, h->nsplit_tc, nprod, 128, &nl, nullptr, h->rho(), h->occ(),
+                                   nprod == 0 && h->gemm_mode == MLMD_GEMM_LOWP_BF16 ? h->beta_lo() : nullptr);
     if (e == cudaSuccess)
         e = cudaMemcpyAsync(rho_dev, h->rho(), (size_t)h->ndom * h->ngrid * sizeof(float), cudaMemcpyDeviceToDevice, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);

@@ -127,7 +127,7 @@ def test_richardson_rejects_an_odd_axis_and_leaves_the_taylor_path_alone():
 @pytest.mark.parametrize("kick_norm,lowp", [(1, False), (0, True)])
 def test_richardson_other_norm_path_and_low_precision_mode(kick_norm, lowp):
     """MLMD_OPT_KICK_NORM = 1 (every norm by a pass over psi: the path shapes without a usable projector Gram matrix take) and
-    the opt-in low-precision GEMM mode (1e-3; the density then comes from the separate pass) around the same local solver,
+    the opt-in low-precision GEMM mode (1e-3) around the same local solver,
     on one configs[2] domain (tcgen05 kicks); the occupations afterwards follow the oracle's overlap."""
     import paper_2509_00966_b200 as M
     from oracle import ref

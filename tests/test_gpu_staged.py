@@ -173,3 +173,41 @@ def test_staged_density_rides_on_the_one_product_projection():
     _, rho2 = ref.propagate(d["psi"], occ, d["vloc"], d["beta"], d["D"], A[:2], c.dt, c.h)
     assert rho_err(rho_fused.cpu().numpy(), rho2) <= TOL_RHO and rho_err(dom.density(), rho2) <= TOL_RHO
     dom.close()
+
+
+def test_low_precision_mode_density_rides_on_the_bf16_projection():
+    """The same for MLMD_GEMM_LOWP_BF16: the BF16 projection kernel sums the density from the FP32 values it packs."""
+    import ctypes
+    import torch
+    import paper_2509_00966_b200 as M
+    from oracle import ref
+    from test_gpu_parity import TOL_LOWP, make_domain, orb_err, rho_err
+    c = W.get_config(1, nsteps=6)
+    d = W.generate(c)
+    occ = np.random.default_rng(7).uniform(0, 2, d["occ"].shape)
+    A = W.laser_samples(c, nsteps=6, t0=0.9)
+    r, rho_ref = ref.propagate(d["psi"], occ, d["vloc"], d["beta"], d["D"], A, c.dt, c.h)
+    outs = []
+    for graph, chunks in ((0, [6]), (1, [6]), (0, [1, 2, 3])):
+        dom = make_domain(c, dict(d, occ=occ), mode=M.GEMM_LOWP_BF16, options=[(M.OPT_GRAPH, graph)])
+        done = 0
+        for n in chunks:
+            dom.propagate(n, c.dt, A[done:done + n])
+            done += n
+        outs.append((dom.get_orbitals(), dom.density()))
+        dom.close()
+        assert rho_err(outs[-1][1], rho_ref) <= TOL_LOWP and orb_err(outs[-1][0], r) <= TOL_LOWP
+    for o in outs[1:]:
+        assert np.array_equal(o[0], outs[0][0]) and np.array_equal(o[1], outs[0][1])
+    hook = ctypes.CDLL(M.api.TEST_LIB_PATH).mlmd_debug_fused_density_np
+    hook.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
+    dom = make_domain(c, dict(d, occ=occ), mode=M.GEMM_LOWP_BF16)
+    dom.propagate(2, c.dt, A[:2])
+    rho_fused = torch.empty((c.ndom, *c.grid), dtype=torch.float32, device="cuda")
+    assert hook(dom.handle, rho_fused.data_ptr(), 0) == 0
+    rho_pass = dom.density()
+    _, rho2 = ref.propagate(d["psi"], occ, d["vloc"], d["beta"], d["D"], A[:2], c.dt, c.h)
+    assert rho_err(rho_fused.cpu().numpy(), rho2) <= TOL_LOWP
+    # the riding sum and the separate pass see the same FP32 state: they agree to FP32 summation order
+    assert rho_err(rho_fused.cpu().numpy(), rho_pass.astype(np.float64)) <= 1e-5
+    dom.close()
